@@ -1,0 +1,189 @@
+"""CPU ORACLE (test infrastructure only) -- ctypes front end of oracle/rpa_oracle.c.
+
+Only tests/, ``__graft_entry__.smoke()`` and bench.py's ``cpu_baseline`` / ``--impl reference`` legs may import
+this package.  It imports nothing from ``paper_1307_8052_b200`` and shares no code with the CUDA path.
+Every routine here is pinned by tests/test_oracle_pins.py; none is "parity unpinned".
+
+``Chi0Oracle`` strings the C routines together in the paper's order (Table 1 steps 5, 6, 8, 9, 11, 13;
+P:L149-162) with the same call shape as the library boundary, so a test can feed both the same arrays.
+"""
+from __future__ import annotations
+
+import ctypes as C
+
+import numpy as np
+
+from .build import build as _build
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(_build())
+        i32, f64, vp = C.c_int32, C.c_double, C.c_void_p
+        L.orc_num_threads.restype = i32
+        L.orc_volume.restype = f64
+        L.orc_volume.argtypes = [vp]
+        L.orc_sphere.restype = i32
+        L.orc_sphere.argtypes = [vp, vp, vp, f64, i32, vp, vp]
+        L.orc_K2.restype = None
+        L.orc_K2.argtypes = [vp, vp, i32, vp, vp]
+        for name in ("orc_pair_density_naive", "orc_pair_density_separable"):
+            f = getattr(L, name)
+            f.restype = None
+            f.argtypes = [vp, vp, i32, vp, i32, vp, vp]
+        L.orc_paw_add.restype = None
+        L.orc_paw_add.argtypes = [vp, vp, i32, vp, i32, vp, vp, i32, vp, vp, vp, vp]
+        L.orc_weights.restype = None
+        L.orc_weights.argtypes = [f64, f64, i32, vp, vp, i32, vp, vp]
+        L.orc_accumulate.restype = None
+        L.orc_accumulate.argtypes = [i32, i32, vp, i32, vp, f64, vp]
+        L.orc_chi0_from_S.restype = None
+        L.orc_chi0_from_S.argtypes = [C.c_int64, f64, vp, vp]
+        L.orc_ec_q.restype = i32
+        L.orc_ec_q.argtypes = [i32, i32, vp, vp, vp, vp, vp]
+        _lib = L
+    return _lib
+
+
+def _p(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def _c128(a):
+    return np.ascontiguousarray(a, dtype=np.complex128)
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _i32(a):
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+def num_threads() -> int:
+    return int(lib().orc_num_threads())
+
+
+def volume(cell) -> float:
+    return float(lib().orc_volume(_p(_f64(cell).reshape(9))))
+
+
+def sphere(grid, cell, q_red, ecut_ha):
+    """(g[ng,3] int32, K2[ng]) in ascending flat-FFT-index order."""
+    grid, cell, q = _i32(grid), _f64(cell).reshape(9), _f64(q_red)
+    ng = lib().orc_sphere(_p(grid), _p(cell), _p(q), float(ecut_ha), 0, None, None)
+    g = np.zeros((ng, 3), dtype=np.int32)
+    K2 = np.zeros(ng, dtype=np.float64)
+    lib().orc_sphere(_p(grid), _p(cell), _p(q), float(ecut_ha), ng, _p(g), _p(K2))
+    return g, K2
+
+
+def K2_of(cell, q_red, g):
+    g = _i32(g).reshape(-1, 3)
+    out = np.zeros(g.shape[0], dtype=np.float64)
+    lib().orc_K2(_p(_f64(cell).reshape(9)), _p(_f64(q_red)), g.shape[0], _p(g), _p(out))
+    return out
+
+
+def pair_density(grid, u_n, u_m, g, mode="separable"):
+    """ntilde[m][g] for one u_n against a stack u_m[n_m][N1][N2][N3]."""
+    grid = _i32(grid)
+    u_n, u_m, g = _c128(u_n), _c128(u_m), _i32(g).reshape(-1, 3)
+    N = int(np.prod(grid))
+    n_m = u_m.size // N
+    out = np.zeros((n_m, g.shape[0]), dtype=np.complex128)
+    fn = {"separable": lib().orc_pair_density_separable, "naive": lib().orc_pair_density_naive}[mode]
+    fn(_p(grid), _p(u_n), n_m, _p(u_m), g.shape[0], _p(g), _p(out))
+    return out
+
+
+def paw_add(cell, q_red, g, n_proj, P_n, P_m, Q, R_cart, n):
+    """In-place n[m][g] += PAW term; returns n."""
+    g = _i32(g).reshape(-1, 3)
+    n_proj = _i32(n_proj)
+    P_n, P_m, Q, R = _c128(P_n), _c128(P_m), _c128(Q), _f64(R_cart)
+    assert n.dtype == np.complex128 and n.flags.c_contiguous
+    n_m = n.shape[0]
+    lib().orc_paw_add(_p(_f64(cell).reshape(9)), _p(_f64(q_red)), g.shape[0], _p(g), n_proj.size, _p(n_proj), _p(P_n),
+                      n_m, _p(P_m), _p(Q), _p(R), _p(n))
+    return n
+
+
+def weights(eps_n, f_n, eps_m, f_m, omega):
+    eps_m, f_m, omega = _f64(eps_m), _f64(f_m), _f64(omega)
+    w = np.zeros((omega.size, eps_m.size), dtype=np.float64)
+    lib().orc_weights(float(eps_n), float(f_n), eps_m.size, _p(eps_m), _p(f_m), omega.size, _p(omega), _p(w))
+    return w
+
+
+def accumulate(S, n, w, kweight):
+    """S[nw][ng][ng] += kweight * sum_p w[iw][p] n[p][g] conj(n[p][g'])."""
+    n, w = _c128(n), _f64(w)
+    assert S.dtype == np.complex128 and S.flags.c_contiguous
+    lib().orc_accumulate(n.shape[1], n.shape[0], _p(n), w.shape[0], _p(w), float(kweight), _p(S))
+    return S
+
+
+def chi0_from_S(S, vol):
+    S = _c128(S)
+    out = np.empty_like(S)
+    lib().orc_chi0_from_S(S.size, float(vol), _p(S), _p(out))
+    return out
+
+
+def ec_q(chi0, v, omega_wt):
+    """(E_c(q), e_omega[nw]); raises if I - D chi0 D is not positive definite."""
+    chi0, v, wt = _c128(chi0), _f64(v), _f64(omega_wt)
+    nw, ng = chi0.shape[0], chi0.shape[1]
+    ec = C.c_double(0.0)
+    e = np.zeros(nw, dtype=np.float64)
+    st = lib().orc_ec_q(ng, nw, _p(chi0), _p(v), _p(wt), C.byref(ec), _p(e))
+    if st != 0:
+        raise FloatingPointError(f"I - v^1/2 chi0 v^1/2 not positive definite at omega index {-st - 1}")
+    return float(ec.value), e
+
+
+class Chi0Oracle:
+    """Same call shape as the library boundary (include/rpa_chi0.h), every step by the C oracle.
+
+    ``g`` may be given explicitly (a sampled sub-list of the sphere): chi0 restricted to those G is exactly the
+    chi0 of those G, because every element of Eq. 17 is an independent sum."""
+
+    def __init__(self, grid, cell, q_red, ecut_ha, omega, omega_wt=None, g=None, mode="separable"):
+        self.grid, self.cell, self.q = _i32(grid), _f64(cell).reshape(3, 3), _f64(q_red)
+        self.omega = _f64(omega)
+        self.omega_wt = None if omega_wt is None else _f64(omega_wt)
+        if g is None:
+            self.g, self.K2 = sphere(self.grid, self.cell, self.q, ecut_ha)
+        else:
+            self.g = _i32(g).reshape(-1, 3)
+            self.K2 = K2_of(self.cell, self.q, self.g)
+        self.ng = self.g.shape[0]
+        self.mode = mode
+        self.S = np.zeros((self.omega.size, self.ng, self.ng), dtype=np.complex128)
+        self.n_pairs = 0
+
+    def pair_densities(self, n, kd, n_proj=None, Q=None, R_cart=None):
+        """n_nm(g) of occupied band index n (row of kd.psi_occ) against all kd.psi_unocc: [m][g]."""
+        nt = pair_density(self.grid, kd.psi_occ[n], kd.psi_unocc, self.g, self.mode)
+        if n_proj is not None and len(n_proj) > 0:
+            paw_add(self.cell, self.q, self.g, n_proj, kd.P_occ[n], kd.P_unocc, Q, R_cart, nt)
+        return nt
+
+    def add_kpoint(self, kd, n_proj=None, Q=None, R_cart=None):
+        for n in range(kd.psi_occ.shape[0]):
+            nt = self.pair_densities(n, kd, n_proj, Q, R_cart)
+            w = weights(kd.eps_occ[n], kd.f_occ[n], kd.eps_unocc, kd.f_unocc, self.omega)
+            accumulate(self.S, nt, w, kd.kweight)
+            self.n_pairs += nt.shape[0]
+
+    def get(self, i_omega=None):
+        chi = chi0_from_S(self.S, volume(self.cell))
+        return chi if i_omega is None else chi[i_omega]
+
+    def ec_q(self, v):
+        return ec_q(self.get(), v, self.omega_wt)
