@@ -1,0 +1,141 @@
+/*
+ * rpa_chi0.h -- C ABI of the B200-native chi0 / RPA hot path (librpa_chi0.so).
+ *
+ * What it computes: the non-interacting density response chi0_GG'(q, i omega) of the RPA correlation energy
+ * in the PAW method, and the per-q energy integrand, as stated in the paper
+ * (P:Lnnn = /root/reference/PAPER.md line nnn):
+ *
+ *   pair density   ntilde_nm(G) = F[ conj(u_nk(r)) u_m,k+q(r) ]            Eq. 7 / Eq. 12
+ *   PAW correction n_nm(G) = ntilde_nm(G) + sum_a e^{-i(q+G).R_a} sum_ij conj(P^a_i,n) Q^a_ij(q+G) P^a_j,m
+ *                                                                           Eq. 6
+ *   accumulation   chi0(i w) = (2/Omega) sum_k wk sum_{n occ, m unocc} w_nm(w) n_nm(G) conj(n_nm(G'))
+ *                  w_nm(w) = 2 (f_n - f_m)(e_n - e_m) / (w^2 + (e_n - e_m)^2)   Eq. 3, 17, 18
+ *   energy         E_c(q) = (1/2pi) sum_i wt_i { ln det[1 - v chi0(i w_i)] + Tr[v chi0(i w_i)] }
+ *                                                                           Eq. 1-2
+ *
+ * Conventions: Hartree atomic units (bohr, Ha).  Grid N1 x N2 x N3, C order (index 3
+ * fastest).  cell = rows a1,a2,a3; B = 2 pi cell^-T; K_g = (q_red + g) B for integer g.  Orbitals are the
+ * cell-periodic parts u(r_j) on the grid, normalised (1/N) sum_j |u_j|^2 = 1.  complex128 is interleaved
+ * (re, im) doubles ("cdouble").  Every G-indexed array (Q, v_G, chi0 rows/cols) is ordered as
+ * rpa_chi0_gvectors() returns: ascending flat FFT index ((g1 mod N1) N2 + (g2 mod N2)) N3 + (g3 mod N3).
+ *
+ * Memory: "dev" pointers are CUDA device pointers (allocated by the caller, e.g. with PyTorch); "host"
+ * pointers are ordinary host memory.  The library allocates no device memory: everything it needs is carved
+ * from the caller's `workspace`.  All inputs are read-only and stay owned by the caller.
+ *
+ * Stream semantics: every call on a handle enqueues its work on the cudaStream_t given to rpa_chi0_create and
+ * may return before the device work finishes; device inputs must stay alive until the stream reaches that
+ * point.  Host input arrays are consumed before the call returns.  rpa_ec_q and rpa_chi0_sync block.
+ *
+ * Errors: every int-returning call gives 0 on success or a negative RPA_ERR_* code; rpa_last_error() holds
+ * a thread-local message.  Nothing is thrown across the ABI.  A handle is not thread-safe; distinct handles
+ * are independent.
+ */
+#ifndef RPA_CHI0_H
+#define RPA_CHI0_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define RPA_OK 0
+#define RPA_ERR_INVALID_ARG (-1)  /* null pointer, non-positive size, omega <= 0, i_omega out of range, |K_g| = 0 */
+#define RPA_ERR_UNSUPPORTED (-2)  /* q = 0 optical limit (out of scope, reading A13); unsupported grid */
+#define RPA_ERR_WORKSPACE (-3)    /* workspace too small or misaligned */
+#define RPA_ERR_CUDA (-4)         /* a CUDA runtime call or kernel launch failed */
+#define RPA_ERR_NOT_PD (-5)       /* 1 - v^1/2 chi0 v^1/2 not positive definite in rpa_ec_q */
+
+typedef struct rpa_chi0 rpa_chi0_t; /* opaque, owned by the library, freed by rpa_chi0_destroy */
+
+/*
+ * Bytes of device workspace rpa_chi0_create needs for this sphere (Table 1 step 6) and omega count.
+ * max_batch_pairs bounds how many (n,m) transitions are grouped into one batched pass (the paper's "Nu",
+ * Eq. 20); <= 0 picks the default (4096).  Results never depend on it beyond rounding order.
+ * max_proj_total bounds sum_a n_proj[a] of later rpa_chi0_add_kpoint calls (0: no PAW term will be used); it
+ * sizes the scratch of the PAW contraction (Table 1 steps 8-9).
+ * All pointers host.  Returns 0 on invalid arguments.
+ */
+size_t rpa_chi0_workspace_bytes(const int32_t grid[3], const double cell[9], const double q_red[3],
+                                double ecut_ha, int32_t n_omega, int32_t max_batch_pairs, int32_t max_proj_total);
+
+/*
+ * Create a handle for one q: builds the |q+G|^2/2 <= ecut_ha sphere (strict |g_i| < N_i/2), its index
+ * tables and the FFT twiddles, and zeroes the n_omega accumulators.
+ *   grid, cell, q_red, omega_ha[n_omega] (> 0), omega_wt[n_omega] (may be NULL if rpa_ec_q is not used): host.
+ *   workspace: dev, 256-byte aligned, at least rpa_chi0_workspace_bytes(...) bytes, must outlive the handle.
+ *   cuda_stream: a cudaStream_t (NULL = legacy default stream).
+ * q_red = 0 gives RPA_ERR_UNSUPPORTED; so does a grid length N2 or N3 with a prime factor other than 2, 3, 5, 7
+ * (N1 is unrestricted) or a grid so large that one z line per chunk does not fit shared memory.
+ */
+int rpa_chi0_create(rpa_chi0_t **out, const int32_t grid[3], const double cell[9], const double q_red[3],
+                    double ecut_ha, int32_t n_omega, const double *omega_ha, const double *omega_wt,
+                    int32_t max_batch_pairs, int32_t max_proj_total, void *workspace, size_t workspace_bytes,
+                    void *cuda_stream);
+
+/* Number of G vectors in the sphere. */
+int rpa_chi0_ng(const rpa_chi0_t *h, int32_t *ng);
+
+/* g[ng][3] (host, int32): the integer G vectors in the order of every G-indexed array; K2[ng] (host, may be
+ * NULL) = |q+G|^2 in bohr^-2. */
+int rpa_chi0_gvectors(const rpa_chi0_t *h, int32_t *g, double *K2);
+
+/*
+ * Add the transitions of one k-point (Table 1 steps 5, 6, 8, 9, 11):
+ *   S_w[G][G'] += kweight * sum_{n < n_occ, m < n_unocc} w_nm(w) n_nm(G) conj(n_nm(G'))   for every omega.
+ * All n_occ x n_unocc pairs are included (metallic / smeared occupations allowed, reading A12).
+ *   psi_occ   dev cdouble [n_occ][N1][N2][N3]     u_nk;      psi_unocc dev cdouble [n_unocc][N1][N2][N3]  u_m,k+q
+ *   eps_occ, f_occ host double [n_occ];  eps_unocc, f_unocc host double [n_unocc]   (Ha; f per spin in [0,1])
+ *   n_atoms, n_proj host int32 [n_atoms] (projectors per atom, may differ per atom);  n_atoms = 0: no PAW
+ *   P_occ dev cdouble [n_occ][sum n_proj] = <p~^a_i|psi~_nk>;  P_unocc dev cdouble [n_unocc][sum n_proj]
+ *   Q dev cdouble, per atom [n_i][n_i][ng] (i, j, G), atoms concatenated; atom-centred (no phase, reading A9)
+ *   R_cart host double [n_atoms][3], bohr.
+ * Additive and order-independent up to rounding: any split of bands or k-points over calls gives the same chi0.
+ */
+int rpa_chi0_add_kpoint(rpa_chi0_t *h, double kweight, int32_t n_occ, const void *psi_occ, int32_t n_unocc,
+                        const void *psi_unocc, const double *eps_occ, const double *eps_unocc, const double *f_occ,
+                        const double *f_unocc, int32_t n_atoms, const int32_t *n_proj, const void *P_occ,
+                        const void *P_unocc, const void *Q, const double *R_cart);
+
+/* chi0(i omega_i) = (2/Omega) S_i as a full Hermitian matrix, dev cdouble [ng][ng] row-major (Eq. 3 prefactor,
+ * P:L56; spin-paired, reading A3).  Stream-ordered; does not modify the accumulators. */
+int rpa_chi0_get(rpa_chi0_t *h, int32_t i_omega, void *chi0_out);
+
+/*
+ * E_c(q) = (1/2pi) sum_i wt_i e_i,  e_i = ln det(I - D chi0_i D) + Tr(D chi0_i D),  D = diag(sqrt(v_G))
+ * (Eq. 1-2 in the similar Hermitian form, reading A14), by an on-device blocked Cholesky.
+ *   v_G host double [ng] (> 0, e.g. 4 pi/|q+G|^2);  ec_ha host double[1];  e_omega host double [n_omega] or NULL.
+ * Blocks until done; leaves the accumulators untouched.  Needs omega_wt at create.  RPA_ERR_NOT_PD if a pivot <= 0.
+ */
+int rpa_ec_q(rpa_chi0_t *h, const double *v_G, double *ec_ha, double *e_omega);
+
+/* Zero the accumulators (start another q with the same sphere). */
+int rpa_chi0_reset(rpa_chi0_t *h);
+
+/* Block until all work enqueued on the handle's stream is done; reports asynchronous CUDA errors. */
+int rpa_chi0_sync(rpa_chi0_t *h);
+
+/*
+ * Per-stage device times (ms, CUDA events on the handle's stream) accumulated by rpa_chi0_add_kpoint while
+ * profiling is on: [0] pair product + 2-D FFT, [1] third-axis DFT + sphere gather, [2] PAW, [3] weights,
+ * [4] rank-K update; launches[5] = kernel launches per stage.  Turning profiling on adds event records only.
+ */
+int rpa_chi0_set_profiling(rpa_chi0_t *h, int32_t on);
+int rpa_chi0_stage_times(rpa_chi0_t *h, double ms[5], int64_t launches[5]);
+
+void rpa_chi0_destroy(rpa_chi0_t *h);
+
+/* Register-only DMMA issue-rate probe: runs `iters` dependent-free mma.sync.m8n8k4.f64 per warp on every SM and
+ * returns the achieved FP64 tensor TFLOP/s (the measured roofline denominator of the rank-K update).  The one
+ * call that allocates (and frees) 64 bytes of device memory itself: it has no handle and no workspace. */
+int rpa_probe_fp64_tensor_peak(void *cuda_stream, double *tflops);
+
+/* Thread-local message of the last error on this thread (static storage, never NULL). */
+const char *rpa_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RPA_CHI0_H */

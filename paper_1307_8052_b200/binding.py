@@ -1,0 +1,310 @@
+"""Thin Python binding of librpa_chi0.so (include/rpa_chi0.h): same names, argument marshalling only.
+
+PyTorch is used for device memory (the workspace and the caller's tensors) and for the CUDA stream; every step
+of the path runs in the library's kernels.  There is no CPU fallback: if the shared library is missing or no
+CUDA device is present, the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+from . import build as _build
+
+RPA_OK = 0
+RPA_ERR_INVALID_ARG = -1
+RPA_ERR_UNSUPPORTED = -2
+RPA_ERR_WORKSPACE = -3
+RPA_ERR_CUDA = -4
+RPA_ERR_NOT_PD = -5
+
+EXPORTS = (
+    "rpa_chi0_workspace_bytes", "rpa_chi0_create", "rpa_chi0_ng", "rpa_chi0_gvectors", "rpa_chi0_add_kpoint",
+    "rpa_chi0_get", "rpa_ec_q", "rpa_chi0_reset", "rpa_chi0_sync", "rpa_chi0_set_profiling", "rpa_chi0_stage_times",
+    "rpa_chi0_destroy", "rpa_probe_fp64_tensor_peak", "rpa_last_error",
+)
+
+STAGE_NAMES = ("pair_product_fft_yz", "fft_x_gather", "paw", "weights", "rank_k")
+
+
+class RpaError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"librpa_chi0 error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def library_path() -> str:
+    return _build.LIB
+
+
+def lib():
+    """Load librpa_chi0.so (building it first if nvcc is here and the sources are newer); raises if impossible."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    try:
+        path = _build.build()
+    except Exception as exc:  # no nvcc / compile error: never fall back to anything else
+        if not os.path.exists(_build.LIB):
+            raise ImportError(f"librpa_chi0.so is missing and could not be built: {exc}") from exc
+        path = _build.LIB
+    L = C.CDLL(path)
+    i32, i64, f64, vp, sz = C.c_int32, C.c_int64, C.c_double, C.c_void_p, C.c_size_t
+    L.rpa_chi0_workspace_bytes.restype = sz
+    L.rpa_chi0_workspace_bytes.argtypes = [vp, vp, vp, f64, i32, i32, i32]
+    L.rpa_chi0_create.restype = C.c_int
+    L.rpa_chi0_create.argtypes = [C.POINTER(vp), vp, vp, vp, f64, i32, vp, vp, i32, i32, vp, sz, vp]
+    L.rpa_chi0_ng.restype = C.c_int
+    L.rpa_chi0_ng.argtypes = [vp, C.POINTER(i32)]
+    L.rpa_chi0_gvectors.restype = C.c_int
+    L.rpa_chi0_gvectors.argtypes = [vp, vp, vp]
+    L.rpa_chi0_add_kpoint.restype = C.c_int
+    L.rpa_chi0_add_kpoint.argtypes = [vp, f64, i32, vp, i32, vp, vp, vp, vp, vp, i32, vp, vp, vp, vp, vp]
+    L.rpa_chi0_get.restype = C.c_int
+    L.rpa_chi0_get.argtypes = [vp, i32, vp]
+    L.rpa_ec_q.restype = C.c_int
+    L.rpa_ec_q.argtypes = [vp, vp, C.POINTER(f64), vp]
+    for name in ("rpa_chi0_reset", "rpa_chi0_sync"):
+        getattr(L, name).restype = C.c_int
+        getattr(L, name).argtypes = [vp]
+    L.rpa_chi0_set_profiling.restype = C.c_int
+    L.rpa_chi0_set_profiling.argtypes = [vp, i32]
+    L.rpa_chi0_stage_times.restype = C.c_int
+    L.rpa_chi0_stage_times.argtypes = [vp, vp, vp]
+    L.rpa_chi0_destroy.restype = None
+    L.rpa_chi0_destroy.argtypes = [vp]
+    L.rpa_probe_fp64_tensor_peak.restype = C.c_int
+    L.rpa_probe_fp64_tensor_peak.argtypes = [vp, C.POINTER(f64)]
+    L.rpa_last_error.restype = C.c_char_p
+    L.rpa_last_error.argtypes = []
+    _ = i64
+    _lib = L
+    return L
+
+
+def _check(rc: int):
+    if rc != RPA_OK:
+        raise RpaError(rc, lib().rpa_last_error().decode("utf-8", "replace"))
+
+
+def rpa_last_error() -> str:
+    return lib().rpa_last_error().decode("utf-8", "replace")
+
+
+def _np(a, dtype):
+    return np.ascontiguousarray(a, dtype=dtype)
+
+
+def _hp(a) -> C.c_void_p:
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_1307_8052_b200 needs a CUDA device (there is no CPU fallback)")
+    return torch
+
+
+def _dev_ptr(t, name: str, dtype, device) -> C.c_void_p:
+    torch = _torch()
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError(f"{name} must be a CUDA tensor")
+    if t.dtype != dtype:
+        raise TypeError(f"{name} must have dtype {dtype}, got {t.dtype}")
+    if not t.is_contiguous():
+        raise ValueError(f"{name} must be contiguous")
+    if t.device != device:
+        raise ValueError(f"{name} is on {t.device}, the handle on {device}")
+    return C.c_void_p(t.data_ptr())
+
+
+class Handle:
+    """Owns the opaque rpa_chi0_t* and the torch-allocated workspace it lives in."""
+
+    def __init__(self, ptr, workspace, device, stream, grid, n_omega):
+        self.ptr, self.workspace, self.device, self.stream = ptr, workspace, device, stream
+        self.grid, self.n_omega = tuple(int(x) for x in grid), int(n_omega)
+        self._ng = None
+
+    @property
+    def ng(self) -> int:
+        if self._ng is None:
+            self._ng = rpa_chi0_ng(self)
+        return self._ng
+
+    def close(self):
+        if self.ptr:
+            lib().rpa_chi0_destroy(self.ptr)
+            self.ptr = None
+            self.workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def rpa_chi0_workspace_bytes(grid, cell, q_red, ecut_ha, n_omega, max_batch_pairs=0, max_proj_total=0) -> int:
+    g, c, q = _np(grid, np.int32), _np(cell, np.float64).reshape(9), _np(q_red, np.float64)
+    n = int(lib().rpa_chi0_workspace_bytes(_hp(g), _hp(c), _hp(q), float(ecut_ha), int(n_omega), int(max_batch_pairs),
+                                           int(max_proj_total)))
+    if n == 0:
+        raise RpaError(RPA_ERR_INVALID_ARG, rpa_last_error())
+    return n
+
+
+def rpa_chi0_create(grid, cell, q_red, ecut_ha, omega_ha, omega_wt=None, max_batch_pairs=0, max_proj_total=0,
+                    device="cuda:0", stream=None) -> Handle:
+    torch = _torch()
+    device = torch.device(device)
+    if device.index is None:
+        device = torch.device("cuda", torch.cuda.current_device())
+    g, c, q = _np(grid, np.int32), _np(cell, np.float64).reshape(9), _np(q_red, np.float64)
+    om = _np(omega_ha, np.float64)
+    wt = None if omega_wt is None else _np(omega_wt, np.float64)
+    nbytes = rpa_chi0_workspace_bytes(g, c, q, ecut_ha, om.size, max_batch_pairs, max_proj_total)
+    with torch.cuda.device(device):
+        ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=device)
+        off = (-ws.data_ptr()) % 256
+        if stream is None:
+            stream = torch.cuda.current_stream(device)
+        out = C.c_void_p()
+        rc = lib().rpa_chi0_create(C.byref(out), _hp(g), _hp(c), _hp(q), float(ecut_ha), int(om.size), _hp(om),
+                                   None if wt is None else _hp(wt), int(max_batch_pairs), int(max_proj_total),
+                                   C.c_void_p(ws.data_ptr() + off), C.c_size_t(nbytes), C.c_void_p(stream.cuda_stream))
+    _check(rc)
+    return Handle(out, ws, device, stream, g, om.size)
+
+
+def rpa_chi0_ng(h: Handle) -> int:
+    n = C.c_int32()
+    _check(lib().rpa_chi0_ng(h.ptr, C.byref(n)))
+    return int(n.value)
+
+
+def rpa_chi0_gvectors(h: Handle):
+    ng = h.ng
+    g = np.zeros((ng, 3), dtype=np.int32)
+    K2 = np.zeros(ng, dtype=np.float64)
+    _check(lib().rpa_chi0_gvectors(h.ptr, _hp(g), _hp(K2)))
+    return g, K2
+
+
+def rpa_chi0_add_kpoint(h: Handle, kweight, psi_occ, psi_unocc, eps_occ, eps_unocc, f_occ, f_unocc,
+                        n_proj: Optional[Sequence[int]] = None, P_occ=None, P_unocc=None, Q=None, R_cart=None):
+    """psi_*, P_*, Q: CUDA complex128 tensors (layouts of include/rpa_chi0.h); eps_*, f_*, n_proj, R_cart: host."""
+    torch = _torch()
+    c128 = torch.complex128
+    N = int(np.prod(h.grid))
+    n_occ = int(psi_occ.shape[0]) if psi_occ.numel() else 0
+    n_unocc = int(psi_unocc.shape[0]) if psi_unocc.numel() else 0
+    if n_occ and psi_occ.numel() != n_occ * N:
+        raise ValueError("psi_occ must be [n_occ][N1][N2][N3]")
+    if n_unocc and psi_unocc.numel() != n_unocc * N:
+        raise ValueError("psi_unocc must be [n_unocc][N1][N2][N3]")
+    eo, eu = _np(eps_occ, np.float64), _np(eps_unocc, np.float64)
+    fo, fu = _np(f_occ, np.float64), _np(f_unocc, np.float64)
+    if eo.size != n_occ or fo.size != n_occ or eu.size != n_unocc or fu.size != n_unocc:
+        raise ValueError("eps/f lengths must match the band counts")
+    n_atoms = 0 if n_proj is None else len(n_proj)
+    if n_atoms:
+        npj = _np(n_proj, np.int32)
+        ptot = int(npj.sum())
+        R = _np(R_cart, np.float64).reshape(-1)
+        if R.size != 3 * n_atoms:
+            raise ValueError("R_cart must be [n_atoms][3]")
+        if P_occ.numel() != n_occ * ptot or P_unocc.numel() != n_unocc * ptot:
+            raise ValueError("P_occ / P_unocc must be [bands][sum n_proj]")
+        if Q.numel() != int((npj.astype(np.int64) ** 2).sum()) * h.ng:
+            raise ValueError("Q must hold sum_a n_a^2 * ng elements")
+        args = (int(n_atoms), _hp(npj), _dev_ptr(P_occ, "P_occ", c128, h.device) if n_occ else None,
+                _dev_ptr(P_unocc, "P_unocc", c128, h.device) if n_unocc else None, _dev_ptr(Q, "Q", c128, h.device), _hp(R))
+    else:
+        args = (0, None, None, None, None, None)
+    rc = lib().rpa_chi0_add_kpoint(
+        h.ptr, float(kweight), n_occ, _dev_ptr(psi_occ, "psi_occ", c128, h.device) if n_occ else None, n_unocc,
+        _dev_ptr(psi_unocc, "psi_unocc", c128, h.device) if n_unocc else None, _hp(eo), _hp(eu), _hp(fo), _hp(fu), *args)
+    _check(rc)
+
+
+def rpa_chi0_get(h: Handle, i_omega: int, out=None):
+    torch = _torch()
+    ng = h.ng
+    if out is None:
+        out = torch.empty((ng, ng), dtype=torch.complex128, device=h.device)
+    elif tuple(out.shape) != (ng, ng):
+        raise ValueError("out must be [ng][ng]")
+    _check(lib().rpa_chi0_get(h.ptr, int(i_omega), _dev_ptr(out, "out", torch.complex128, h.device)))
+    return out
+
+
+def rpa_ec_q(h: Handle, v_G):
+    v = _np(v_G, np.float64)
+    if v.size != h.ng:
+        raise ValueError("v_G must have ng entries")
+    ec = C.c_double(0.0)
+    e = np.zeros(h.n_omega, dtype=np.float64)
+    _check(lib().rpa_ec_q(h.ptr, _hp(v), C.byref(ec), _hp(e)))
+    return float(ec.value), e
+
+
+def rpa_chi0_reset(h: Handle):
+    _check(lib().rpa_chi0_reset(h.ptr))
+
+
+def rpa_chi0_sync(h: Handle):
+    _check(lib().rpa_chi0_sync(h.ptr))
+
+
+def rpa_chi0_set_profiling(h: Handle, on: bool):
+    _check(lib().rpa_chi0_set_profiling(h.ptr, 1 if on else 0))
+
+
+def rpa_chi0_stage_times(h: Handle):
+    ms = np.zeros(5, dtype=np.float64)
+    n = np.zeros(5, dtype=np.int64)
+    _check(lib().rpa_chi0_stage_times(h.ptr, _hp(ms), _hp(n)))
+    return ms, n
+
+
+def rpa_chi0_destroy(h: Handle):
+    h.close()
+
+
+def rpa_probe_fp64_tensor_peak(device="cuda:0") -> float:
+    torch = _torch()
+    with torch.cuda.device(torch.device(device)):
+        t = C.c_double(0.0)
+        _check(lib().rpa_probe_fp64_tensor_peak(C.c_void_p(torch.cuda.current_stream().cuda_stream), C.byref(t)))
+    return float(t.value)
+
+
+# ---- host-buffer convenience on top of the calls above (the end-to-end path bench.py times) ------------------
+
+def add_kpoint_host(h: Handle, kd, n_proj=None, Q_dev=None, R_cart=None, pinned=None):
+    """Copy one k-point's host arrays (workload.KPointData) to the device and add it.  `pinned` may hold
+    pre-pinned host tensors keyed like the KPointData fields; returns the bytes copied host->device."""
+    torch = _torch()
+
+    def up(name):
+        src = pinned[name] if pinned is not None else torch.from_numpy(getattr(kd, name))
+        return src.to(h.device, non_blocking=True)
+
+    psi_o, psi_u = up("psi_occ"), up("psi_unocc")
+    nbytes = psi_o.numel() * 16 + psi_u.numel() * 16
+    if n_proj is not None and len(n_proj):
+        P_o, P_u = up("P_occ"), up("P_unocc")
+        nbytes += P_o.numel() * 16 + P_u.numel() * 16
+    else:
+        P_o = P_u = None
+    rpa_chi0_add_kpoint(h, kd.kweight, psi_o, psi_u, kd.eps_occ, kd.eps_unocc, kd.f_occ, kd.f_unocc, n_proj, P_o, P_u,
+                        Q_dev, R_cart)
+    return nbytes

@@ -1,0 +1,38 @@
+"""Compile the CUDA library in-tree: paper_1307_8052_b200/librpa_chi0.so (sm_100a only, nvcc cross-compiles
+without a GPU).  Run as ``python -m paper_1307_8052_b200.build [--force]``."""
+import os
+import subprocess
+import sys
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(HERE, "csrc")
+LIB = os.path.join(HERE, "librpa_chi0.so")
+SOURCES = ["rpa_chi0.cu"]
+HEADERS = ["common.cuh", "fft.cuh", "pair_density.cuh", "paw.cuh", "rank_k.cuh", "energy.cuh",
+           os.path.join("..", "..", "include", "rpa_chi0.h")]
+NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC",
+              "-shared", "-Xptxas", "-v", "-diag-suppress", "20011,20013,20014,20015"]
+
+
+def _stale() -> bool:
+    if not os.path.exists(LIB):
+        return True
+    t = os.path.getmtime(LIB)
+    return any(os.path.getmtime(os.path.join(CSRC, f)) > t for f in SOURCES + HEADERS)
+
+
+def build(force: bool = False, verbose: bool = False) -> str:
+    if not force and not _stale():
+        return LIB
+    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    cmd = [nvcc] + NVCC_FLAGS + ["-o", LIB] + [os.path.join(CSRC, f) for f in SOURCES]
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    if verbose or r.returncode != 0:
+        sys.stderr.write(r.stdout + r.stderr)
+    if r.returncode != 0:
+        raise RuntimeError("nvcc failed building librpa_chi0.so")
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force="--force" in sys.argv, verbose=True))

@@ -1,0 +1,181 @@
+// Transition weights (Eq. 18, in the real form of BASELINE.json north_star) and the weighted Hermitian
+// rank-K update for every imaginary frequency (Eq. 17 / Eq. 20; Table 1 step 11):
+//   S_w[g][g'] += sum_{p < K} w[w][p] n_p(g) conj(n_p(g')),      g >= g' only (one triangle).
+//
+// FP64 tensor cores: the only native FP64 MMA on sm_100a is DMMA.8x8x4 (mma.sync.m8n8k4.f64).  The complex
+// product is taken in its real view: with k = 2p + c (c = 0: re, 1: im),
+//   Re S[g][g'] = sum_k  A[g][k] B[k][g'],   A[g][2p+c]  = w_p (re, im) n_p(g),   B[2p+c][g'] = (re, im) n_p(g')
+//   Im S[g][g'] = sum_k A'[g][k] B[k][g'],   A'[g][2p+c] = w_p (im, -re) n_p(g)
+// so one staged N tile feeds both; A and A' are the same shared-memory words read with c and c^1.  The N buffer is
+// pair-major ([p][g], g contiguous) exactly as the sphere gather writes it: a DMMA fragment is then 2 pair rows x
+// 8 consecutive complex numbers = 2 x 128 B, conflict-free with a row pitch = 128 (mod 256) bytes.
+//
+// One CTA = one 64 x 64 complex tile of the lower triangle x 2 frequencies (warps 0-3: first, 4-7: second; each
+// warp a 32 x 32 complex sub-tile = 4 x 4 x {Re,Im} DMMA accumulators = 128 registers).  K is streamed in chunks
+// of 16 pairs through a 4-stage ring filled by the TMA engine (cp.async.bulk, one 1 KB row per copy) and
+// tracked with full/empty mbarriers.  Both frequencies share the staged rows; only the weights differ.
+#pragma once
+#include "common.cuh"
+
+namespace rk {
+constexpr int T = 64;        // tile edge (complex elements)
+constexpr int KC = 16;       // pairs per stage
+constexpr int STAGES = 4;
+constexpr int NW = 2;        // frequencies per CTA
+constexpr int THREADS = 256;
+constexpr int PITCH = T * 16 + 128;              // bytes per pair row in shared memory
+constexpr int TILE_BYTES = KC * PITCH;           // 18432
+constexpr int W_BYTES = NW * KC * 8;             // 256
+constexpr int STAGE_BYTES = 2 * TILE_BYTES + W_BYTES;
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 2 * STAGES * 8;
+}  // namespace rk
+
+// w[iw*ldw + p] = kweight * 2 (f_n - f_m)(e_n - e_m) / (omega_iw^2 + (e_n - e_m)^2) for p < K, 0 for K <= p < Kpad.
+__global__ void weights_kernel(double *__restrict__ w, int64_t ldw, int K, int Kpad, const double *__restrict__ omega,
+                               int n_omega, const double *__restrict__ eps_occ, const double *__restrict__ f_occ,
+                               const double *__restrict__ eps_unocc, const double *__restrict__ f_unocc, int n0,
+                               int mlen, int m0, double kweight) {
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    const int iw = blockIdx.y;
+    if (p >= Kpad || iw >= n_omega) return;
+    double val = 0.0;
+    if (p < K) {
+        const int n = n0 + p / mlen, m = m0 + p % mlen;
+        const double de = eps_occ[n] - eps_unocc[m];
+        const double om = omega[iw];
+        val = kweight * (2.0 * (f_occ[n] - f_unocc[m]) * de / (om * om + de * de));
+    }
+    w[(size_t)iw * ldw + p] = val;
+}
+
+// Nb[Kpad][ldn] (rows >= K are zero), w[n_omega][ldw], S[n_omega][ng][ldS] (lower triangle accumulated).
+// Kpad % KC == 0.  grid = (ntiles_lower, ceil(n_omega / 2)).
+__global__ void __launch_bounds__(rk::THREADS, 1)
+rank_k_kernel(const cd *__restrict__ Nb, int64_t ldn, int Kpad, const double *__restrict__ w, int64_t ldw,
+              cd *__restrict__ S, int64_t ldS, int64_t strideS, int ng, int n_omega) {
+    using namespace rk;
+    extern __shared__ __align__(128) unsigned char rk_smem[];
+    uint64_t *full = reinterpret_cast<uint64_t *>(rk_smem + STAGES * STAGE_BYTES);
+    uint64_t *empty = full + STAGES;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    // lower-triangle tile (ti >= tj) from the linear index
+    const int t = blockIdx.x;
+    int ti = (int)((sqrt(8.0 * (double)t + 1.0) - 1.0) * 0.5);
+    while ((ti + 1) * (ti + 2) / 2 <= t) ti++;
+    while (ti * (ti + 1) / 2 > t) ti--;
+    const int tj = t - ti * (ti + 1) / 2;
+    const int row0 = ti * T, col0 = tj * T;
+    const int om0 = blockIdx.y * NW;
+    const int n_om = min(NW, n_omega - om0);
+    const uint32_t rowbytes = (uint32_t)min(T, ng - row0) * 16u, colbytes = (uint32_t)min(T, ng - col0) * 16u;
+    const uint32_t stage_tx = KC * (rowbytes + colbytes) + (uint32_t)n_om * KC * 8u;
+
+    // zero the ring once so that the never-copied tail columns of edge tiles hold finite numbers
+    for (int i = tid; i < STAGES * STAGE_BYTES / 16; i += THREADS)
+        reinterpret_cast<double2 *>(rk_smem)[i] = make_double2(0.0, 0.0);
+    if (tid == 0) {
+        for (int s = 0; s < STAGES; s++) {
+            mbar_init(&full[s], 1);
+            mbar_init(&empty[s], THREADS / 32);
+        }
+        mbar_fence_init();
+    }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    __syncthreads();
+
+    const int nk = Kpad / KC;
+    auto issue = [&](int it) {  // warp 0 only
+        const int s = it % STAGES;
+        unsigned char *st = rk_smem + s * STAGE_BYTES;
+        if (lane == 0) mbar_arrive_expect_tx(&full[s], stage_tx);
+        __syncwarp();
+        const size_t krow = (size_t)it * KC + (lane & 15);
+        if (lane < 16) bulk_g2s(st + lane * PITCH, Nb + krow * ldn + row0, rowbytes, &full[s]);
+        else bulk_g2s(st + TILE_BYTES + (lane - 16) * PITCH, Nb + krow * ldn + col0, colbytes, &full[s]);
+        if (lane < n_om)
+            bulk_g2s(st + 2 * TILE_BYTES + lane * KC * 8, w + (size_t)(om0 + lane) * ldw + (size_t)it * KC, KC * 8,
+                     &full[s]);
+    };
+    if (warp == 0)
+        for (int it = 0; it < STAGES - 1 && it < nk; it++) issue(it);
+
+    const int g = lane >> 2, kq = lane & 3, pp = kq >> 1, c = kq & 1;
+    const int wsel = warp >> 2, quad = warp & 3;
+    const int rowoff = (quad >> 1) * 32, coloff = (quad & 1) * 32;
+    // a warp whose sub-tile lies strictly above the diagonal, or whose frequency does not exist, only keeps the
+    // barriers moving
+    const bool active = (wsel < n_om) && !(ti == tj && coloff > rowoff);
+
+    double re[4][4][2], im[4][4][2];
+#pragma unroll
+    for (int mi = 0; mi < 4; mi++)
+#pragma unroll
+        for (int ni = 0; ni < 4; ni++) re[mi][ni][0] = re[mi][ni][1] = im[mi][ni][0] = im[mi][ni][1] = 0.0;
+
+    const uint32_t a_off = pp * PITCH + (rowoff + g) * 16;
+    const uint32_t b_off = TILE_BYTES + pp * PITCH + (coloff + g) * 16 + c * 8;
+    const uint32_t w_off = 2 * TILE_BYTES + (wsel * KC + pp) * 8;
+
+    for (int it = 0; it < nk; it++) {
+        if (warp == 0) {
+            const int nx = it + STAGES - 1;
+            if (nx < nk) {
+                if (nx >= STAGES) mbar_wait(&empty[nx % STAGES], ((nx / STAGES) - 1) & 1);
+                issue(nx);
+            }
+        }
+        const int s = it % STAGES;
+        mbar_wait(&full[s], (it / STAGES) & 1);
+        if (active) {
+            const unsigned char *st = rk_smem + s * STAGE_BYTES;
+#pragma unroll
+            for (int ks = 0; ks < KC / 2; ks++) {
+                const uint32_t ko = ks * 2 * PITCH;
+                const double wv = *reinterpret_cast<const double *>(st + w_off + ks * 16);
+                const double swv = c ? -wv : wv;
+                double a[4], a2[4], b[4];
+#pragma unroll
+                for (int mi = 0; mi < 4; mi++) {
+                    const unsigned char *ap = st + a_off + ko + mi * 128;
+                    a[mi] = wv * *reinterpret_cast<const double *>(ap + c * 8);
+                    a2[mi] = swv * *reinterpret_cast<const double *>(ap + (c ^ 1) * 8);
+                }
+#pragma unroll
+                for (int ni = 0; ni < 4; ni++) b[ni] = *reinterpret_cast<const double *>(st + b_off + ko + ni * 128);
+#pragma unroll
+                for (int mi = 0; mi < 4; mi++)
+#pragma unroll
+                    for (int ni = 0; ni < 4; ni++) {
+                        dmma(re[mi][ni][0], re[mi][ni][1], a[mi], b[ni]);
+                        dmma(im[mi][ni][0], im[mi][ni][1], a2[mi], b[ni]);
+                    }
+            }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty[s]);
+    }
+
+    if (!active) return;
+    cd *Sw = S + (size_t)(om0 + wsel) * strideS;
+#pragma unroll
+    for (int mi = 0; mi < 4; mi++) {
+        const int r = row0 + rowoff + mi * 8 + g;
+        if (r >= ng) continue;
+#pragma unroll
+        for (int ni = 0; ni < 4; ni++) {
+            const int cc = col0 + coloff + ni * 8 + 2 * kq;
+#pragma unroll
+            for (int e = 0; e < 2; e++) {
+                const int col = cc + e;
+                if (col < ng && col <= r) {
+                    cd *ptr = Sw + (size_t)r * ldS + col;
+                    cd v = *ptr;
+                    v.x += re[mi][ni][e];
+                    v.y += im[mi][ni][e];
+                    *ptr = v;
+                }
+            }
+        }
+    }
+}

@@ -1,0 +1,93 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+
+Tolerances are BASELINE.json north_star's: chi0 relative Frobenius error <= 1e-10 per frequency, E_c(q)
+relative error <= 1e-9.  All tests need a B200 (``-m gpu``)."""
+import numpy as np
+import pytest
+
+from paper_1307_8052_b200 import workload as W
+from tests.parity_util import gpu_run, oracle_run, rel_fro
+
+pytestmark = pytest.mark.gpu
+
+CHI_TOL = 1e-10
+EC_TOL = 1e-9
+
+
+def _compare(cfg, kds, use_paw=True, max_batch_pairs=0):
+    chi_g, ec_g, g_g, K2_g = gpu_run(cfg, kds, use_paw, max_batch_pairs)
+    chi_o, ec_o, g_o, K2_o = oracle_run(cfg, kds, use_paw)
+    assert g_g.shape == g_o.shape and (g_g == g_o).all(), "sphere / ordering differs"
+    assert np.allclose(K2_g, K2_o, rtol=1e-13)
+    for i in range(cfg.n_omega):
+        err = rel_fro(chi_g[i], chi_o[i])
+        assert err <= CHI_TOL, f"omega {i}: rel Frobenius error {err:.3e}"
+    assert abs(ec_g[0] - ec_o[0]) <= EC_TOL * abs(ec_o[0]), (ec_g[0], ec_o[0])
+    assert np.allclose(ec_g[1], ec_o[1], rtol=EC_TOL, atol=0)
+    return chi_g
+
+
+def test_tiny_skewed_cell_ragged(tiny_cfg):
+    """6x4x8 grid, skewed cell, 2x5 bands, 3 frequencies, 2 atoms x 3 projectors: every tail is ragged."""
+    _compare(tiny_cfg, [W.kpoint(tiny_cfg, 0)])
+
+
+def test_config0_toy_full():
+    cfg = W.CONFIGS[0]
+    chi = _compare(cfg, [W.kpoint(cfg, 0)])
+    for i in range(cfg.n_omega):  # Hermitian by construction, negative semidefinite on the imaginary axis
+        assert np.array_equal(chi[i], chi[i].conj().T)
+        assert np.linalg.eigvalsh(chi[i]).max() <= 1e-13 * np.abs(chi[i]).max()
+
+
+def test_config0_no_paw():
+    cfg = W.CONFIGS[0]
+    _compare(cfg, [W.kpoint(cfg, 0)], use_paw=False)
+
+
+@pytest.mark.parametrize("batch", [16, 48, 100])
+def test_batch_size_invariance(batch):
+    """Results must not depend on the internal grouping of transitions (the paper's Nu)."""
+    cfg = W.CONFIGS[0]
+    kds = [W.kpoint(cfg, 0)]
+    a, _, _, _ = gpu_run(cfg, kds, True, 0, want_ec=False)
+    b, _, _, _ = gpu_run(cfg, kds, True, batch, want_ec=False)
+    for i in range(cfg.n_omega):
+        assert rel_fro(b[i], a[i]) <= 1e-12
+
+
+def test_additivity_over_calls():
+    """Splitting bands over several add_kpoint calls gives the same chi0."""
+    cfg = W.CONFIGS[0]
+    full = [W.kpoint(cfg, 0)]
+    parts = [W.kpoint(cfg, 0, occ=[0, 1], unocc=range(0, 11)), W.kpoint(cfg, 0, occ=[0, 1], unocc=range(11, 28)),
+             W.kpoint(cfg, 0, occ=[2, 3])]
+    a, _, _, _ = gpu_run(cfg, full, True, 0, want_ec=False)
+    b, _, _, _ = gpu_run(cfg, parts, True, 0, want_ec=False)
+    for i in range(cfg.n_omega):
+        assert rel_fro(b[i], a[i]) <= 1e-12
+
+
+@pytest.mark.parametrize("grid,q", [((12, 10, 14), (0.25, 0.0, 0.5)), ((9, 15, 7), (0.1, 0.2, -0.3)),
+                                    ((8, 1, 6), (0.5, 0.0, 0.0)), ((5, 6, 1), (0.0, 0.25, 0.0))])
+def test_mixed_radix_grids(grid, q):
+    """Grid lengths with factors 2, 3, 5, 7 and degenerate axes of length 1."""
+    cell = np.array([[6.0, 0.2, 0.0], [0.1, 5.0, 0.3], [0.0, -0.2, 7.0]])
+    cfg = W.custom_config(200 + sum(grid), cell, grid, q, n_occ=3, n_unocc=7, ng_target=12, n_omega=4, n_atoms=2,
+                          n_proj_per_atom=2, orb_ecut_ha=2.0)
+    _compare(cfg, [W.kpoint(cfg, 0)])
+
+
+def test_config2_bulk_two_kpoints_slice():
+    """24^3 fcc grid, nG = 401 (ragged 64-tile tail), 16 frequencies, 3 atoms x 8 projectors; 2 k-points,
+    3 occupied x 45 unoccupied bands each."""
+    cfg = W.CONFIGS[2]
+    kds = [W.kpoint(cfg, k, occ=[0, 3, 7], unocc=range(0, 300, 7)[:45]) for k in (0, 1)]
+    _compare(cfg, kds)
+
+
+def test_config1_molecule_slice():
+    """56x60x64 grid (radices 7, 5, 3), nG = 1200, 2 occupied x 37 unoccupied bands."""
+    cfg = W.CONFIGS[1]
+    kds = [W.kpoint(cfg, 0, occ=[0, 11], unocc=range(0, 600, 16)[:37])]
+    _compare(cfg, kds)
