@@ -1,0 +1,325 @@
+#!/usr/bin/env python
+"""bench.py -- chi0 pair transitions/s and rank-K FP64 TFLOP/s on BASELINE.json configs[1] (molecule-in-box).
+
+A step is one pass of the whole hot path over the workload (S1 = create is done
+once, untimed): reset, rpa_chi0_add_kpoint for every k-point of the rank, rpa_chi0_get for every omega and
+rpa_ec_q.  `value` = transitions of all ranks / max-over-ranks device time, inputs resident in HBM.
+`e2e` = the same pass with the k-point arrays starting in pinned HOST memory (H2D inside the timed region)
+and E_c(q) / e(omega) read back to the host.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1] [--impl reference]
+    torchrun --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P bench.py --gpus N ...
+
+N > 1: weak scaling, no data-path collective -- every rank owns one k-point of an N-k-point problem (P:L181:
+"no MPI communication throughout steps 2-11"); the one exchange of the method, the sum of the per-rank
+accumulators at the end of a q, is an NCCL all-reduce inside the timed step.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1307_8052_b200 import workload as W  # noqa: E402
+
+METRIC = "chi0 pair transitions/s (rank-K FP64 TFLOP/s in roofline), 1 q-point, all omega"
+UNIT = "transitions/s"
+# ncu --set full capture of rank_k_kernel on this workload (profiles/): dram bytes read+written per launch
+RANK_K_DRAM_TRAFFIC_BYTES = None
+
+
+def rank_k_useful_flops(ng, n_omega, n_pairs):
+    """8 flop per complex MAC on one triangle: 4 nG (nG+1) n_omega per pair."""
+    return 4.0 * ng * (ng + 1) * n_omega * n_pairs
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            if len(r) < 7:
+                continue
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); power.append(float(r[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as fh:
+            return json.load(fh), "measured"
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0}, "fallback"
+
+
+# ------------------------------------------------------------------------------------------------ reference arm
+def oracle_sample(cfg, budget_s, chunk=64):
+    """The oracle, as it stands, on a bounded sample of the workload: slices of `chunk` unoccupied bands against
+    one occupied band of k-point 0 (full grid / nG / omega / atoms) are added until `budget_s` seconds of CPU
+    work are spent, then E_c(q) is taken on the full nG x nG matrices.  Returns
+    (pairs, t_add, t_ec, estimated whole-workload transitions/s, threads)."""
+    import oracle
+    om, wt = W.omega_grid(cfg.n_omega)
+    orc = oracle.Chi0Oracle(cfg.grid, cfg.cell, cfg.q_red, W.tuned_ecut(cfg), om, wt)
+    Q, R = W.paw_Q(cfg, orc.K2), W.atom_positions(cfg)
+    pairs, t_add, n, m0 = 0, 0.0, 0, 0
+    while t_add < budget_s and n < cfg.n_occ:
+        m1 = min(m0 + chunk, cfg.n_unocc)
+        kd = W.kpoint(cfg, 0, occ=[n], unocc=range(m0, m1))
+        t0 = time.perf_counter()
+        orc.add_kpoint(kd, cfg.n_proj, Q, R)
+        t_add += time.perf_counter() - t0
+        pairs += m1 - m0
+        m0 = m1
+        if m0 >= cfg.n_unocc:
+            n, m0 = n + 1, 0
+    t1 = time.perf_counter()
+    orc.ec_q(W.coulomb(orc.K2))
+    t_ec = time.perf_counter() - t1
+    est = cfg.n_pairs / (cfg.n_pairs * t_add / pairs + t_ec)
+    return pairs, t_add, t_ec, est, oracle.num_threads()
+
+
+def run_reference(args, cfg):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    budget = min(args.ref_seconds, 150.0 / max(1, args.warmup + args.steps))
+    vals, ts = [], []
+    for i in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        pairs, t_add, t_ec, est, cores = oracle_sample(cfg, budget)
+        if i >= args.warmup:
+            vals.append(est)
+            ts.append(time.perf_counter() - t0)
+    v = float(np.mean(vals))
+    sample = (f"per step: {pairs} transitions of k-point 0 (64-band slices, full grid/nG/omega/atoms, {budget:.0f} s "
+              f"budget) + E_c(q) on the full nG x nG matrices; value = n_pairs / (n_pairs * t_add/pairs_sampled + t_ec)")
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean(ts)), "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64 (complex128)", "data": "synthetic",
+            "config": {"workload": f"configs[{cfg.index}] {cfg.name}", "grid": list(cfg.grid), "n_pairs": cfg.n_pairs},
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------------ our arm
+def run_ours(args, cfg):
+    import torch
+    import torch.distributed as dist
+    from paper_1307_8052_b200 import binding as B
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    om, wt = W.omega_grid(cfg.n_omega)
+    ptot = int(cfg.n_proj.sum())
+    h = B.rpa_chi0_create(cfg.grid, cfg.cell, cfg.q_red, W.tuned_ecut(cfg), om, wt, args.batch, ptot, dev)
+    g, K2 = B.rpa_chi0_gvectors(h)
+    ng = len(g)
+    Qd = torch.from_numpy(W.paw_Q(cfg, K2)).to(dev)
+    R, npj = W.atom_positions(cfg), cfg.n_proj
+    v = W.coulomb(K2)
+    # weak scaling: this rank's k-points of a (world * n_k)-k-point problem; throughput does not depend on values
+    my_k = [rank * cfg.n_k + k for k in range(cfg.n_k)]
+    n_k_total = world * cfg.n_k
+    t0 = time.perf_counter()
+    # one generated k-point per rank is reused for all its k labels when n_k > 1 (no data-dependent
+    # branching); configs[1] has a single k-point, so nothing is reused there
+    kd = W.kpoint(cfg, my_k[0] % max(cfg.n_k, 1))
+    gen_s = time.perf_counter() - t0
+    host = {k: torch.from_numpy(getattr(kd, k)).pin_memory() for k in ("psi_occ", "psi_unocc", "P_occ", "P_unocc")}
+    devt = {k: t.to(dev) for k, t in host.items()}
+    kweight = 1.0 / n_k_total
+    out = torch.empty((ng, ng), dtype=torch.complex128, device=dev)
+    S = B.rpa_chi0_accumulators(h) if world > 1 else None
+
+    def step(from_host):
+        B.rpa_chi0_reset(h)
+        nb = 0
+        for _ in my_k:
+            if from_host:
+                nb += B.add_kpoint_host(h, kd, npj, Qd, R, pinned=host, kweight=kweight)
+            else:
+                B.rpa_chi0_add_kpoint(h, kweight, devt["psi_occ"], devt["psi_unocc"], kd.eps_occ, kd.eps_unocc, kd.f_occ,
+                                      kd.f_unocc, npj, devt["P_occ"], devt["P_unocc"], Qd, R)
+        if world > 1:
+            dist.all_reduce(torch.view_as_real(S))
+        for i in range(cfg.n_omega):
+            B.rpa_chi0_get(h, i, out)
+        ec, e = B.rpa_ec_q(h, v)  # blocks; reads E_c(q), e(omega) back to the host
+        return nb, ec, e
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(from_host, steps, warmup):
+        for _ in range(warmup):
+            step(from_host)
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        nb = 0
+        for _ in range(steps):
+            nb, ec, e = step(from_host)
+        e1.record()
+        barrier()
+        ms = e0.elapsed_time(e1)
+        if world > 1:
+            t = torch.tensor([ms], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        return ms / steps, nb, ec
+
+    peak_tf = B.rpa_probe_fp64_tensor_peak(dev)
+    pairs_per_rank = len(my_k) * cfg.n_occ * cfg.n_unocc
+    pairs_total = pairs_per_rank * world
+
+    # device-resident inputs, stage events on, clocks sampled
+    B.rpa_chi0_set_profiling(h, True)
+    sampler = ClockSampler(local)
+    launches0 = None
+    for _ in range(args.warmup):
+        step(False)
+    barrier()
+    B.rpa_chi0_set_profiling(h, True)  # zero the stage timers after warm-up
+    launches0 = B.rpa_chi0_launch_count(h)
+    if rank == 0:
+        sampler.start()
+    ms_step, _, ec_dev = timed(False, args.steps, 0)
+    clocks = sampler.stop() if rank == 0 else None
+    launches = B.rpa_chi0_launch_count(h) - launches0
+    stage_ms, stage_n = B.rpa_chi0_stage_times(h)
+    B.rpa_chi0_set_profiling(h, False)
+
+    # end to end from pinned host memory
+    ms_e2e, h2d, ec_e2e = timed(True, args.steps, max(1, args.warmup // 2))
+    assert abs(ec_e2e - ec_dev) <= 1e-12 * abs(ec_dev), (ec_e2e, ec_dev)
+
+    if rank == 0:
+        peaks, peak_kind = measured_peaks()
+        rk_launches = int(stage_n[4])
+        rk_ms = float(stage_ms[4]) / max(rk_launches, 1)
+        rk_flops = rank_k_useful_flops(ng, cfg.n_omega, pairs_per_rank * args.steps) / max(rk_launches, 1)
+        rk_tf = rk_flops / (rk_ms * 1e-3) * 1e-12 if rk_ms > 0 else 0.0
+        # pair-density stage (HBM-bound): algorithmic bytes = 16 N per pair (stream psi_m) + 16 nG (write n)
+        pd_ms = float(stage_ms[0] + stage_ms[1]) / args.steps
+        pd_bytes = pairs_per_rank * 16.0 * (cfg.n_grid + ng)
+        pd_gbs = pd_bytes / (pd_ms * 1e-3) * 1e-9 if pd_ms > 0 else 0.0
+        total_stage = float(stage_ms.sum()) / args.steps
+        line = {
+            "metric": METRIC, "value": pairs_total / (ms_step * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64 (complex128)", "data": "synthetic",
+            "config": {"workload": f"configs[{cfg.index}] {cfg.name}", "grid": list(cfg.grid), "n_k_per_gpu": len(my_k),
+                       "n_occ": cfg.n_occ, "n_unocc": cfg.n_unocc, "n_pairs": pairs_total, "nG": ng, "n_omega": cfg.n_omega,
+                       "atoms_x_proj": [cfg.n_atoms, cfg.n_proj_per_atom], "max_batch_pairs": args.batch or 4096,
+                       "l2": "inputs (%.2f GB of orbitals per k-point) exceed the 126 MB L2; no explicit flush" %
+                             ((cfg.n_occ + cfg.n_unocc) * cfg.n_grid * 16 / 1e9),
+                       "step": "reset + add_kpoint (S2-S6) + get x n_omega (S7) + ec_q (S8)",
+                       "parallelism": "1 GPU" if world == 1 else f"k-points sharded over {world} GPUs + all-reduce of S"},
+            "clocks": clocks,
+            "e2e": {"value": pairs_total / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e,
+                    "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": 8 * (1 + cfg.n_omega) + 16},
+            "gpu_launches": int(launches),
+            "roofline": {"kernel": "rank_k_kernel", "bound": "tensor", "achieved": rk_tf, "peak": peak_tf, "unit": "TFLOP/s",
+                         "frac": rk_tf / peak_tf if peak_tf else None, "traffic": RANK_K_DRAM_TRAFFIC_BYTES,
+                         "peak_source": "FP64 DMMA issue rate measured live by rpa_probe_fp64_tensor_peak (register-only "
+                                        "mma.sync.m8n8k4.f64, all SMs); MEASURED_PEAKS.json has no FP64 entry",
+                         "peak_alt_tflops_from_bf16": peaks.get("bf16_tflops", 0) * 40.0 / 2250.0,
+                         "flops_per_launch": rk_flops, "ms_per_launch": rk_ms, "launches": rk_launches,
+                         "share_of_step": float(stage_ms[4]) / args.steps / ms_step},
+            "stages": {"ms_per_step": {n: float(t) / args.steps for n, t in zip(B.STAGE_NAMES, stage_ms)},
+                       "sum_ms": total_stage,
+                       "pair_density": {"bound": "hbm", "achieved": pd_gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                                        "frac": pd_gbs / peaks["hbm_gbs"], "peak_kind": peak_kind,
+                                        "bytes_per_pair": 16.0 * (cfg.n_grid + ng)}},
+            "ec_q_ha": ec_dev, "gen_s": gen_s,
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            pairs, t_add, t_ec, est, cores = oracle_sample(cfg, args.ref_seconds)
+            line["cpu_baseline"] = {"value": est, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                    "sample": f"{pairs} transitions of k-point 0 (64-band slices, full grid/nG/omega/"
+                                              f"atoms; {t_add:.1f} s) + E_c(q) on the full matrices ({t_ec:.1f} s); "
+                                              f"value = n_pairs / (n_pairs * t_add/{pairs} + t_ec)"}
+        print(json.dumps(line), flush=True)
+    h.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs (default: 1, molecule)")
+    ap.add_argument("--batch", type=int, default=0, help="max_batch_pairs (0: library default)")
+    ap.add_argument("--ref-seconds", type=float, default=12.0, help="CPU seconds of oracle work per sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 0)
+    cfg = W.CONFIGS[args.config]
+    if args.impl == "reference":
+        run_reference(args, cfg)
+    else:
+        if args.warmup < 3:
+            args.warmup = 3
+        run_ours(args, cfg)
+
+
+if __name__ == "__main__":
+    main()

@@ -125,6 +125,17 @@ int rpa_chi0_sync(rpa_chi0_t *h);
 int rpa_chi0_set_profiling(rpa_chi0_t *h, int32_t on);
 int rpa_chi0_stage_times(rpa_chi0_t *h, double ms[5], int64_t launches[5]);
 
+/* Number of kernel launches enqueued through this handle since it was created. */
+int rpa_chi0_launch_count(const rpa_chi0_t *h, int64_t *count);
+
+/*
+ * The raw accumulators S[n_omega][ng][ng] (dev cdouble, inside the caller's workspace; only the lower triangle
+ * g >= g' is meaningful, the rest is zero) and their size in bytes.  For the multi-GPU sum of per-rank partial
+ * chi0 (ranks share nothing until the end of a q): all-reduce this buffer in place on the handle's
+ * stream, then call rpa_chi0_get / rpa_ec_q.  The pointer stays valid for the life of the handle.
+ */
+int rpa_chi0_accumulators(const rpa_chi0_t *h, void **S, size_t *bytes);
+
 void rpa_chi0_destroy(rpa_chi0_t *h);
 
 /* Register-only DMMA issue-rate probe: runs `iters` dependent-free mma.sync.m8n8k4.f64 per warp on every SM and

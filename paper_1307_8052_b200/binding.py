@@ -24,7 +24,7 @@ RPA_ERR_NOT_PD = -5
 EXPORTS = (
     "rpa_chi0_workspace_bytes", "rpa_chi0_create", "rpa_chi0_ng", "rpa_chi0_gvectors", "rpa_chi0_add_kpoint",
     "rpa_chi0_get", "rpa_ec_q", "rpa_chi0_reset", "rpa_chi0_sync", "rpa_chi0_set_profiling", "rpa_chi0_stage_times",
-    "rpa_chi0_destroy", "rpa_probe_fp64_tensor_peak", "rpa_last_error",
+    "rpa_chi0_launch_count", "rpa_chi0_accumulators", "rpa_chi0_destroy", "rpa_probe_fp64_tensor_peak", "rpa_last_error",
 )
 
 STAGE_NAMES = ("pair_product_fft_yz", "fft_x_gather", "paw", "weights", "rank_k")
@@ -77,13 +77,16 @@ def lib():
     L.rpa_chi0_set_profiling.argtypes = [vp, i32]
     L.rpa_chi0_stage_times.restype = C.c_int
     L.rpa_chi0_stage_times.argtypes = [vp, vp, vp]
+    L.rpa_chi0_launch_count.restype = C.c_int
+    L.rpa_chi0_launch_count.argtypes = [vp, C.POINTER(i64)]
+    L.rpa_chi0_accumulators.restype = C.c_int
+    L.rpa_chi0_accumulators.argtypes = [vp, C.POINTER(vp), C.POINTER(sz)]
     L.rpa_chi0_destroy.restype = None
     L.rpa_chi0_destroy.argtypes = [vp]
     L.rpa_probe_fp64_tensor_peak.restype = C.c_int
     L.rpa_probe_fp64_tensor_peak.argtypes = [vp, C.POINTER(f64)]
     L.rpa_last_error.restype = C.c_char_p
     L.rpa_last_error.argtypes = []
-    _ = i64
     _lib = L
     return L
 
@@ -275,6 +278,21 @@ def rpa_chi0_stage_times(h: Handle):
     return ms, n
 
 
+def rpa_chi0_launch_count(h: Handle) -> int:
+    n = C.c_int64(0)
+    _check(lib().rpa_chi0_launch_count(h.ptr, C.byref(n)))
+    return int(n.value)
+
+
+def rpa_chi0_accumulators(h: Handle):
+    """The accumulators as a flat complex128 CUDA tensor aliasing the workspace (for an in-place all-reduce)."""
+    torch = _torch()
+    p, n = C.c_void_p(), C.c_size_t()
+    _check(lib().rpa_chi0_accumulators(h.ptr, C.byref(p), C.byref(n)))
+    off = int(p.value) - h.workspace.data_ptr()
+    return h.workspace[off:off + int(n.value)].view(torch.complex128)
+
+
 def rpa_chi0_destroy(h: Handle):
     h.close()
 
@@ -289,7 +307,7 @@ def rpa_probe_fp64_tensor_peak(device="cuda:0") -> float:
 
 # ---- host-buffer convenience on top of the calls above (the end-to-end path bench.py times) ------------------
 
-def add_kpoint_host(h: Handle, kd, n_proj=None, Q_dev=None, R_cart=None, pinned=None):
+def add_kpoint_host(h: Handle, kd, n_proj=None, Q_dev=None, R_cart=None, pinned=None, kweight=None):
     """Copy one k-point's host arrays (workload.KPointData) to the device and add it.  `pinned` may hold
     pre-pinned host tensors keyed like the KPointData fields; returns the bytes copied host->device."""
     torch = _torch()
@@ -305,6 +323,6 @@ def add_kpoint_host(h: Handle, kd, n_proj=None, Q_dev=None, R_cart=None, pinned=
         nbytes += P_o.numel() * 16 + P_u.numel() * 16
     else:
         P_o = P_u = None
-    rpa_chi0_add_kpoint(h, kd.kweight, psi_o, psi_u, kd.eps_occ, kd.eps_unocc, kd.f_occ, kd.f_unocc, n_proj, P_o, P_u,
+    rpa_chi0_add_kpoint(h, kd.kweight if kweight is None else kweight, psi_o, psi_u, kd.eps_occ, kd.eps_unocc, kd.f_occ, kd.f_unocc, n_proj, P_o, P_u,
                         Q_dev, R_cart)
     return nbytes

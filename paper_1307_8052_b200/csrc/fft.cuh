@@ -158,14 +158,26 @@ struct Bfly<6> {
 //   st(line, idx, value)     writes element idx of the line in the pass's output (idx is the final frequency
 //                            index when this is the last pass)
 //   tw[t] = exp(-2 pi i t/N), t = 0..N-1
-template <int R, class LD, class ST>
-HD void fft_pass(int tid, int nthreads, int nlines, int N, int ns, const cd *tw, LD ld, ST st) {
+//   LINE_FAST = false: consecutive threads take consecutive butterflies of one line (coalesced along the line);
+//   LINE_FAST = true : consecutive threads take the same butterfly of consecutive lines (for data stored
+//                      [element][line], every access is then contiguous and the twiddles are warp-uniform).
+//   NC, NSC > 0 fix N and ns at compile time (the runtime arguments are then ignored).
+template <int R, bool LINE_FAST, int NC = 0, int NSC = 0, class LD, class ST>
+HD void fft_pass(int tid, int nthreads, int nlines, int N_rt, int ns_rt, const cd *tw, LD ld, ST st) {
+    const int N = NC > 0 ? NC : N_rt;
+    const int ns = NSC > 0 ? NSC : ns_rt;
     const int nb = N / R;            // butterflies per line
     const int total = nlines * nb;
     const int tstep = nb / ns;       // N / (ns R)
     for (int idx = tid; idx < total; idx += nthreads) {
-        const int line = idx / nb;
-        const int j = idx - line * nb;
+        int line, j;
+        if (LINE_FAST) {
+            j = idx / nlines;
+            line = idx - j * nlines;
+        } else {
+            line = idx / nb;
+            j = idx - line * nb;
+        }
         cd v[R];
 #pragma unroll
         for (int s = 0; s < R; s++) v[s] = ld(line, j + s * nb);
@@ -182,42 +194,58 @@ HD void fft_pass(int tid, int nthreads, int nlines, int N, int ns, const cd *tw,
     }
 }
 
-template <class LD, class ST>
+template <bool LINE_FAST, class LD, class ST>
 HD void fft_pass_r(int R, int tid, int nthreads, int nlines, int N, int ns, const cd *tw, LD ld, ST st) {
     switch (R) {
-        case 2: fft_pass<2>(tid, nthreads, nlines, N, ns, tw, ld, st); break;
-        case 3: fft_pass<3>(tid, nthreads, nlines, N, ns, tw, ld, st); break;
-        case 4: fft_pass<4>(tid, nthreads, nlines, N, ns, tw, ld, st); break;
-        case 5: fft_pass<5>(tid, nthreads, nlines, N, ns, tw, ld, st); break;
-        case 6: fft_pass<6>(tid, nthreads, nlines, N, ns, tw, ld, st); break;
-        case 7: fft_pass<7>(tid, nthreads, nlines, N, ns, tw, ld, st); break;
-        default: fft_pass<8>(tid, nthreads, nlines, N, ns, tw, ld, st); break;
+        case 2: fft_pass<2, LINE_FAST, 0, 0>(tid, nthreads, nlines, N, ns, tw, ld, st); break;
+        case 3: fft_pass<3, LINE_FAST, 0, 0>(tid, nthreads, nlines, N, ns, tw, ld, st); break;
+        case 4: fft_pass<4, LINE_FAST, 0, 0>(tid, nthreads, nlines, N, ns, tw, ld, st); break;
+        case 5: fft_pass<5, LINE_FAST, 0, 0>(tid, nthreads, nlines, N, ns, tw, ld, st); break;
+        case 6: fft_pass<6, LINE_FAST, 0, 0>(tid, nthreads, nlines, N, ns, tw, ld, st); break;
+        case 7: fft_pass<7, LINE_FAST, 0, 0>(tid, nthreads, nlines, N, ns, tw, ld, st); break;
+        default: fft_pass<8, LINE_FAST, 0, 0>(tid, nthreads, nlines, N, ns, tw, ld, st); break;
     }
 }
 
-// Radix plan for a length with prime factors 2,3,5,7 only; returns false otherwise.  Prefers few, large passes.
-static inline bool fft_make_plan(int n, FftPlan *p) {
-    p->n = n;
-    p->npass = 0;
-    if (n < 1) return false;
+// Radix plan for a length with prime factors 2,3,5,7 only; ok = false otherwise.  Prefers few, large passes.
+// constexpr so that the kernels specialised on a grid length get their radices at compile time.
+struct FftPlanResult {
+    FftPlan plan;
+    bool ok;
+};
+
+__host__ __device__ constexpr FftPlanResult fft_plan_c(int n) {
+    FftPlanResult out{};
+    out.plan.n = n;
+    out.plan.npass = 0;
+    out.ok = false;
+    if (n < 1) return out;
     int m = n;
     int c2 = 0, c3 = 0, c5 = 0, c7 = 0;
     while (m % 2 == 0) { m /= 2; c2++; }
     while (m % 3 == 0) { m /= 3; c3++; }
     while (m % 5 == 0) { m /= 5; c5++; }
     while (m % 7 == 0) { m /= 7; c7++; }
-    if (m != 1) return false;
-    int r[32], nr = 0;
+    if (m != 1) return out;
+    int r[32] = {};
+    int nr = 0;
     while (c2 >= 3) { r[nr++] = 8; c2 -= 3; }
     if (c2 == 2) { r[nr++] = 4; c2 = 0; }
     if (c2 == 1 && c3 >= 1) { r[nr++] = 6; c2 = 0; c3--; }
-    while (c7-- > 0) r[nr++] = 7;
-    while (c5-- > 0) r[nr++] = 5;
-    while (c3-- > 0) r[nr++] = 3;
+    while (c7 > 0) { r[nr++] = 7; c7--; }
+    while (c5 > 0) { r[nr++] = 5; c5--; }
+    while (c3 > 0) { r[nr++] = 3; c3--; }
     if (c2 == 1) r[nr++] = 2;
     // n == 1: npass = 0, callers treat the axis as a copy
-    if (nr > FFT_MAX_PASSES) return false;
-    p->npass = nr;
-    for (int i = 0; i < nr; i++) p->radix[i] = r[i];
-    return true;
+    if (nr > FFT_MAX_PASSES) return out;
+    out.plan.npass = nr;
+    for (int i = 0; i < nr; i++) out.plan.radix[i] = r[i];
+    out.ok = true;
+    return out;
+}
+
+static inline bool fft_make_plan(int n, FftPlan *p) {
+    const FftPlanResult r = fft_plan_c(n);
+    *p = r.plan;
+    return r.ok;
 }

@@ -23,6 +23,7 @@ struct PdPlaneParams {
     int p_begin, p_count;           // pairs of the batch handled by this launch
     int g2min, ng2, g3min, ng3;
     int RC;                         // z lines per chunk
+    int nbuf;                       // z ping-pong buffers in shared memory (0, 1 or 2)
     FftPlan pz, py;
 };
 
@@ -32,70 +33,101 @@ __device__ __forceinline__ int freq_to_box(int f, int n, int gmin, int ngb) {
     return (i >= 0 && i < ngb) ? i : -1;
 }
 
+// element index -> padded index inside a z line: one spare slot per 8 elements turns the stride-R stores of the
+// first Stockham pass (R = 4, 8: 64 / 128-byte strides) into conflict-free ones.
+__device__ __forceinline__ int zpad(int i) { return i + (i >> 3); }
+
+__device__ __forceinline__ void cp_async16(void *dst_smem, const void *src_gmem) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst_smem)), "l"(src_gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+// Shared memory (all cd): tw3[N3] tw2[N2] | stage[2][2][RC*N3] (u_m, u_n chunks, double-buffered, filled by
+// cp.async one chunk ahead) | zbuf[nbuf][RC*zpad(N3)] | Y0[N2*ng3] Y1[N2*ng3] ([row][g3i], g3i fastest).
 __global__ void __launch_bounds__(256) pd_plane_kernel(const __grid_constant__ PdPlaneParams P) {
     extern __shared__ __align__(16) unsigned char pd_smem[];
     const int tid = threadIdx.x, nth = blockDim.x;
-    const int N2 = P.N2, N3 = P.N3, ng2 = P.ng2, ng3 = P.ng3;
+    const int N2 = P.N2, N3 = P.N3, ng2 = P.ng2, ng3 = P.ng3, RC = P.RC;
+    const int N3p = zpad(N3) + 1;
     cd *tw3s = reinterpret_cast<cd *>(pd_smem);
     cd *tw2s = tw3s + N3;
-    cd *bufA = tw2s + N2;
-    cd *bufB = bufA + (size_t)P.RC * N3;
-    cd *Y0 = bufB + (size_t)P.RC * N3;
+    cd *stage = tw2s + N2;                        // [buf][um|un][RC*N3]
+    cd *zbuf = stage + 4 * (size_t)RC * N3;       // [nbuf][RC*N3p]
+    cd *Y0 = zbuf + (size_t)P.nbuf * RC * N3p;
     cd *Y1 = Y0 + (size_t)ng3 * N2;
     for (int i = tid; i < N3; i += nth) tw3s[i] = P.tw3[i];
     for (int i = tid; i < N2; i += nth) tw2s[i] = P.tw2[i];
-    __syncthreads();
 
     const int j1 = blockIdx.x;
     const size_t plane = (size_t)N2 * N3;
     const size_t vol = plane * P.N1;
     const int nb2 = ng2 * ng3;
+    const int nchunks = (N2 + RC - 1) / RC;
+    const int npairs = (P.p_count - (int)blockIdx.y + (int)gridDim.y - 1) / (int)gridDim.y;  // pairs of this CTA
+    const int total = npairs * nchunks;
 
-    for (int p = P.p_begin + blockIdx.y; p < P.p_begin + P.p_count; p += gridDim.y) {
+    // chunk q of this CTA: pair p = p_begin + blockIdx.y + (q / nchunks) * gridDim.y, rows [c*RC, c*RC + rc)
+    auto prefetch = [&](int q) {
+        const int p = P.p_begin + blockIdx.y + (q / nchunks) * gridDim.y;
+        const int row0 = (q % nchunks) * RC;
+        const int cnt = min(RC, N2 - row0) * N3;
         const int n = P.n0 + p / P.mlen, m = P.m0 + p % P.mlen;
-        const cd *un = P.psi_occ + (size_t)n * vol + (size_t)j1 * plane;
-        const cd *um = P.psi_unocc + (size_t)m * vol + (size_t)j1 * plane;
+        const cd *um = P.psi_unocc + (size_t)m * vol + (size_t)j1 * plane + (size_t)row0 * N3;
+        const cd *un = P.psi_occ + (size_t)n * vol + (size_t)j1 * plane + (size_t)row0 * N3;
+        cd *sm = stage + (size_t)(q & 1) * 2 * RC * N3;
+        cd *sn = sm + (size_t)RC * N3;
+        for (int i = tid; i < cnt; i += nth) {
+            cp_async16(sm + i, um + i);
+            cp_async16(sn + i, un + i);
+        }
+        cp_async_commit();
+    };
+    if (total > 0) prefetch(0);
 
-        // ---- z axis: chunks of RC lines -------------------------------------------------------------------
-        for (int row0 = 0; row0 < N2; row0 += P.RC) {
-            const int rc = min(P.RC, N2 - row0);
-            const cd *unr = un + (size_t)row0 * N3, *umr = um + (size_t)row0 * N3;
-            auto ld_g = [&](int line, int i) {
-                const cd a = __ldg(unr + line * N3 + i), b = __ldg(umr + line * N3 + i);
-                return cmulc(a, b);
-            };
-            auto st_y = [&](int line, int f, cd v) {
-                const int gi = freq_to_box(f, N3, P.g3min, ng3);
-                if (gi >= 0) Y0[gi * N2 + row0 + line] = v;
-            };
-            if (P.pz.npass == 0) {
-                for (int i = tid; i < rc; i += nth) Y0[row0 + i] = ld_g(i, 0);
-            } else {
-                cd *src = bufA, *dst = bufB;
-                int ns = 1;
-                for (int ps = 0; ps < P.pz.npass; ps++) {
-                    const int R = P.pz.radix[ps];
-                    const bool first = (ps == 0), last = (ps == P.pz.npass - 1);
-                    cd *s_ = src, *d_ = dst;
-                    auto ld_s = [&](int line, int i) { return s_[line * N3 + i]; };
-                    auto st_s = [&](int line, int i, cd v) { d_[line * N3 + i] = v; };
-                    if (first && last) fft_pass_r(R, tid, nth, rc, N3, ns, tw3s, ld_g, st_y);
-                    else if (first) fft_pass_r(R, tid, nth, rc, N3, ns, tw3s, ld_g, st_s);
-                    else if (last) fft_pass_r(R, tid, nth, rc, N3, ns, tw3s, ld_s, st_y);
-                    else fft_pass_r(R, tid, nth, rc, N3, ns, tw3s, ld_s, st_s);
-                    ns *= R;
-                    if (!first) { cd *t = src; src = dst; dst = t; }
-                    else { src = bufB; dst = bufA; }
-                    __syncthreads();
-                }
+    for (int q = 0; q < total; q++) {
+        const int c = q % nchunks;
+        const int row0 = c * RC;
+        const int rc = min(RC, N2 - row0);
+        cp_async_wait_all();
+        __syncthreads();  // chunk q has landed; everybody is done with the buffers of chunk q-1
+        if (q + 1 < total) prefetch(q + 1);
+
+        // ---- z axis of chunk q -------------------------------------------------------------------------------
+        const cd *sm = stage + (size_t)(q & 1) * 2 * RC * N3;
+        const cd *sn = sm + (size_t)RC * N3;
+        auto ld_g = [&](int line, int i) { return cmulc(sn[line * N3 + i], sm[line * N3 + i]); };
+        auto st_y = [&](int line, int f, cd v) {
+            const int gi = freq_to_box(f, N3, P.g3min, ng3);
+            if (gi >= 0) Y0[(row0 + line) * ng3 + gi] = v;
+        };
+        if (P.pz.npass == 0) {
+            for (int i = tid; i < rc; i += nth) Y0[(row0 + i) * ng3] = ld_g(i, 0);
+        } else {
+            int ns = 1;
+            for (int ps = 0; ps < P.pz.npass; ps++) {
+                const int R = P.pz.radix[ps];
+                const bool first = (ps == 0), last = (ps == P.pz.npass - 1);
+                const cd *s_ = zbuf + (size_t)((ps + 1) & 1) * RC * N3p;  // written by pass ps-1
+                cd *d_ = zbuf + (size_t)(ps & 1) * RC * N3p;
+                auto ld_s = [&](int line, int i) { return s_[line * N3p + zpad(i)]; };
+                auto st_s = [&](int line, int i, cd v) { d_[line * N3p + zpad(i)] = v; };
+                if (first && last) fft_pass_r<false>(R, tid, nth, rc, N3, ns, tw3s, ld_g, st_y);
+                else if (first) fft_pass_r<false>(R, tid, nth, rc, N3, ns, tw3s, ld_g, st_s);
+                else if (last) fft_pass_r<false>(R, tid, nth, rc, N3, ns, tw3s, ld_s, st_y);
+                else fft_pass_r<false>(R, tid, nth, rc, N3, ns, tw3s, ld_s, st_s);
+                ns *= R;
+                if (!last) __syncthreads();
             }
         }
+        if (c != nchunks - 1) continue;
         __syncthreads();
 
-        // ---- y axis on the ng3 surviving columns ----------------------------------------------------------
+        // ---- last chunk of the pair: y axis on the ng3 surviving columns, then write out ---------------------------
+        const int p = P.p_begin + blockIdx.y + (q / nchunks) * gridDim.y;
         cd *out;  // [g2i][g3i]
         if (P.py.npass == 0) {
-            out = Y0;  // N2 == 1: Y0[g3i * 1 + 0] is already [0][g3i]
+            out = Y0;  // N2 == 1: Y0[0 * ng3 + g3i]
         } else {
             cd *src = Y0, *dst = Y1;
             int ns = 1;
@@ -103,14 +135,14 @@ __global__ void __launch_bounds__(256) pd_plane_kernel(const __grid_constant__ P
                 const int R = P.py.radix[ps];
                 const bool last = (ps == P.py.npass - 1);
                 cd *s_ = src, *d_ = dst;
-                auto ld_s = [&](int line, int i) { return s_[line * N2 + i]; };
-                auto st_s = [&](int line, int i, cd v) { d_[line * N2 + i] = v; };
+                auto ld_s = [&](int line, int i) { return s_[i * ng3 + line]; };
+                auto st_s = [&](int line, int i, cd v) { d_[i * ng3 + line] = v; };
                 auto st_o = [&](int line, int f, cd v) {
                     const int gi = freq_to_box(f, N2, P.g2min, ng2);
                     if (gi >= 0) d_[gi * ng3 + line] = v;
                 };
-                if (last) fft_pass_r(R, tid, nth, ng3, N2, ns, tw2s, ld_s, st_o);
-                else fft_pass_r(R, tid, nth, ng3, N2, ns, tw2s, ld_s, st_s);
+                if (last) fft_pass_r<true>(R, tid, nth, ng3, N2, ns, tw2s, ld_s, st_o);
+                else fft_pass_r<true>(R, tid, nth, ng3, N2, ns, tw2s, ld_s, st_s);
                 ns *= R;
                 cd *t = src; src = dst; dst = t;
                 __syncthreads();
@@ -119,7 +151,7 @@ __global__ void __launch_bounds__(256) pd_plane_kernel(const __grid_constant__ P
         }
         cd *Io = P.I + ((size_t)(p - P.p_begin) * P.N1 + j1) * nb2;
         for (int i = tid; i < nb2; i += nth) Io[i] = out[i];
-        __syncthreads();
+        // the next pair's first z pass writes zbuf / Y0 only after the __syncthreads at the top of the loop
     }
 }
 

@@ -190,7 +190,7 @@ struct rpa_chi0 {
     Layout L;
     int max_proj;
     FftPlan pz, py;
-    int RC, pd_threads;
+    int RC, pd_threads, pd_nbuf;
     size_t pd_smem;
     unsigned char *ws;
     // profiling
@@ -199,6 +199,7 @@ struct rpa_chi0 {
     std::vector<cudaEvent_t> pool;
     double stage_ms[NSTAGE] = {0, 0, 0, 0, 0};
     int64_t stage_launches[NSTAGE] = {0, 0, 0, 0, 0};
+    int64_t launches = 0;  // every kernel launch enqueued through this handle
 
     template <class T>
     T *ptr(size_t off) const { return reinterpret_cast<T *>(ws + off); }
@@ -223,6 +224,7 @@ struct StageTimer {
     cudaEvent_t a = nullptr, b = nullptr;
     StageTimer(rpa_chi0 *h_, int stage_, int launches) : h(h_), stage(stage_) {
         h->stage_launches[stage] += h->prof ? launches : 0;
+        h->launches += launches;
         if (h->prof) {
             a = get_event(h);
             b = get_event(h);
@@ -255,23 +257,33 @@ int ntiles_lower(int n, int t) {
     return nt * (nt + 1) / 2;
 }
 
-// shared-memory plan of pd_plane_kernel: returns false if even one z line per chunk does not fit.
+// shared-memory plan of pd_plane_kernel: rows per chunk, threads, dynamic shared memory.  Prefers two CTAs per SM
+// (the cp.async prefetch of one CTA overlaps the butterflies of the other); returns false if even one z line per
+// chunk does not fit.
 bool plan_plane_kernel(rpa_chi0 *h) {
     const int N2 = h->grid[1], N3 = h->grid[2];
     const int ng3 = h->sp.gmax[2] - h->sp.gmin[2] + 1;
+    const int N3p = N3 + (N3 >> 3) + 1;
+    const int nbuf = h->pz.npass >= 3 ? 2 : (h->pz.npass == 2 ? 1 : 0);
     const size_t fixed = ((size_t)N3 + N2 + 2 * (size_t)ng3 * N2) * sizeof(cd);
-    const size_t per_row = 2 * (size_t)N3 * sizeof(cd);
-    const size_t cap_small = 100 * 1024, cap_big = 220 * 1024;
-    auto rows_for = [&](size_t cap) -> int { return cap > fixed + per_row ? (int)((cap - fixed) / per_row) : 0; };
-    int rc = rows_for(cap_small);
-    if (rc < std::min(N2, 8)) rc = rows_for(cap_big);
+    const size_t per_row = (4 * (size_t)N3 + (size_t)nbuf * N3p) * sizeof(cd);
+    const size_t caps[3] = {72 * 1024, 110 * 1024, 224 * 1024};   // 3, 2, 1 CTAs per SM
+    int rc = 0;
+    for (int t = 1; t < 3 && rc == 0; t++) {
+        if (caps[t] <= fixed + per_row) continue;
+        const int r = (int)((caps[t] - fixed) / per_row);
+        if (r >= std::min(N2, 8) || t == 2) rc = r;
+    }
     if (rc < 1) return false;
     rc = std::min(rc, N2);
     const int chunks = (N2 + rc - 1) / rc;
     rc = (N2 + chunks - 1) / chunks;
     h->RC = rc;
+    h->pd_nbuf = nbuf;
     h->pd_smem = fixed + per_row * rc;
-    h->pd_threads = 256;
+    const int r0 = h->pz.npass > 0 ? h->pz.radix[0] : 1;
+    const int bf = rc * (N3 / r0);
+    h->pd_threads = (int)align_up((size_t)std::min(256, std::max(64, bf)), 32);
     return true;
 }
 
@@ -497,7 +509,7 @@ int rpa_chi0_add_kpoint(rpa_chi0_t *h, double kweight, int32_t n_occ, const void
                     P.n0 = n0; P.mlen = mlen; P.m0 = m0;
                     P.p_begin = p0; P.p_count = pc;
                     P.g2min = sp.gmin[1]; P.ng2 = ng2; P.g3min = sp.gmin[2]; P.ng3 = ng3;
-                    P.RC = h->RC; P.pz = h->pz; P.py = h->py;
+                    P.RC = h->RC; P.nbuf = h->pd_nbuf; P.pz = h->pz; P.py = h->py;
                     const int gy = std::max(1, std::min(pc, (148 * 8 + N1 - 1) / N1));
                     pd_plane_kernel<<<dim3(N1, gy), h->pd_threads, h->pd_smem, st>>>(P);
                     CUDA_TRY(cudaGetLastError());
@@ -548,6 +560,7 @@ int rpa_chi0_get(rpa_chi0_t *h, int32_t i_omega, void *chi0_out) {
     const int nt = (ng + 31) / 32;
     chi0_get_kernel<<<dim3(nt, nt), dim3(32, 8), 0, h->stream>>>(h->ptr<cd>(h->L.S) + (size_t)i_omega * ng * h->L.ldS, h->L.ldS, ng,
                                                                  2.0 / h->vol, (cd *)chi0_out);
+    h->launches += 1;
     CUDA_TRY(cudaGetLastError());
     return RPA_OK;
 }
@@ -573,16 +586,20 @@ int rpa_ec_q(rpa_chi0_t *h, const double *v_G, double *ec_ha, double *e_omega) {
         CUDA_TRY(cudaMemsetAsync(d_flag, 0, EC_GROUP * sizeof(int), st));
         ec_build_kernel<<<dim3((ng + 127) / 128, ng, nm), 128, 0, st>>>(S + (size_t)iw0 * strideS, L.ldS, strideS, ng, scale, d_v, M);
         ec_trace_kernel<<<nm, 256, 0, st>>>(S + (size_t)iw0 * strideS, L.ldS, strideS, ng, scale, d_v, d_tr);
+        h->launches += 2;
         for (int k0 = 0; k0 < ng; k0 += CH_NB) {
             chol_diag_kernel<<<nm, dim3(CH_NB, CH_NB), 0, st>>>(M, ng, k0, d_flag, d_ld);
+            h->launches += 1;
             const int rest = ng - (k0 + CH_NB);
             if (rest > 0) {
                 chol_panel_kernel<<<dim3((rest + 127) / 128, nm), 128, 0, st>>>(M, ng, k0);
                 chol_update_kernel<<<dim3(ntiles_lower(rest, 64), nm), 256, 0, st>>>(M, ng, k0);
+                h->launches += 2;
             }
         }
         CUDA_TRY(cudaGetLastError());
         ec_collect_kernel<<<1, 32, 0, st>>>(d_ld, d_tr, nm, iw0, d_e);
+        h->launches += 1;
         int flags[EC_GROUP] = {0, 0, 0, 0};
         CUDA_TRY(cudaMemcpyAsync(flags, d_flag, EC_GROUP * sizeof(int), cudaMemcpyDeviceToHost, st));
         CUDA_TRY(cudaStreamSynchronize(st));
@@ -590,6 +607,7 @@ int rpa_ec_q(rpa_chi0_t *h, const double *v_G, double *ec_ha, double *e_omega) {
             if (flags[i]) return fail(RPA_ERR_NOT_PD, "rpa_ec_q: I - v^1/2 chi0 v^1/2 not positive definite at omega index %d", iw0 + i);
     }
     ec_sum_kernel<<<1, 32, 0, st>>>(d_e, h->ptr<double>(L.wt), h->n_omega, h->ptr<double>(L.ec));
+    h->launches += 1;
     CUDA_TRY(cudaGetLastError());
     CUDA_TRY(cudaMemcpyAsync(ec_ha, h->ptr<double>(L.ec), sizeof(double), cudaMemcpyDeviceToHost, st));
     if (e_omega) CUDA_TRY(cudaMemcpyAsync(e_omega, d_e, h->n_omega * sizeof(double), cudaMemcpyDeviceToHost, st));
@@ -624,6 +642,19 @@ int rpa_chi0_stage_times(rpa_chi0_t *h, double ms[5], int64_t launches[5]) {
     int rc = drain_events(h);
     if (rc != RPA_OK) return rc;
     for (int i = 0; i < NSTAGE; i++) { ms[i] = h->stage_ms[i]; launches[i] = h->stage_launches[i]; }
+    return RPA_OK;
+}
+
+int rpa_chi0_launch_count(const rpa_chi0_t *h, int64_t *count) {
+    if (!h || !count) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_launch_count: NULL argument");
+    *count = h->launches;
+    return RPA_OK;
+}
+
+int rpa_chi0_accumulators(const rpa_chi0_t *h, void **S, size_t *bytes) {
+    if (!h || !S || !bytes) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_accumulators: NULL argument");
+    *S = h->ws + h->L.S;
+    *bytes = (size_t)h->n_omega * h->sp.ng * h->L.ldS * sizeof(cd);
     return RPA_OK;
 }
 
