@@ -8,7 +8,8 @@
 //   Im S[g][g'] = sum_k A'[g][k] B[k][g'],   A'[g][2p+c] = w_p (im, -re) n_p(g)
 // so one staged N tile feeds both; A and A' are the same shared-memory words read with c and c^1.  The N buffer is
 // pair-major ([p][g], g contiguous) exactly as the sphere gather writes it: a DMMA fragment is then 2 pair rows x
-// 8 consecutive complex numbers = 2 x 128 B, conflict-free with a row pitch = 128 (mod 256) bytes.
+// 8 consecutive complex numbers = 2 x 128 B.  An LDS.64 is served per half-warp (4 g values x 2 pair rows x 16 B):
+// with a row pitch = 64 (mod 128) bytes the two pair rows of a half-warp fall in different bank halves.
 //
 // One CTA = one 64 x 64 complex tile of the lower triangle x 2 frequencies (warps 0-3: first, 4-7: second; each
 // warp a 32 x 32 complex sub-tile = 4 x 4 x {Re,Im} DMMA accumulators = 128 registers).  K is streamed in chunks
@@ -23,8 +24,8 @@ constexpr int KC = 16;       // pairs per stage
 constexpr int STAGES = 4;
 constexpr int NW = 2;        // frequencies per CTA
 constexpr int THREADS = 256;
-constexpr int PITCH = T * 16 + 128;              // bytes per pair row in shared memory
-constexpr int TILE_BYTES = KC * PITCH;           // 18432
+constexpr int PITCH = T * 16 + 64;               // bytes per pair row in shared memory (= 64 mod 128, see below)
+constexpr int TILE_BYTES = KC * PITCH;           // 17408
 constexpr int W_BYTES = NW * KC * 8;             // 256
 constexpr int STAGE_BYTES = 2 * TILE_BYTES + W_BYTES;
 constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 2 * STAGES * 8;

@@ -191,6 +191,7 @@ struct rpa_chi0 {
     int max_proj;
     FftPlan pz, py;
     int RC, pd_threads, pd_nbuf;
+    PdPlaneKernel pd_kernel = nullptr;
     size_t pd_smem;
     unsigned char *ws;
     // profiling
@@ -257,15 +258,32 @@ int ntiles_lower(int n, int t) {
     return nt * (nt + 1) / 2;
 }
 
-// shared-memory plan of pd_plane_kernel: rows per chunk, threads, dynamic shared memory.  Prefers two CTAs per SM
-// (the cp.async prefetch of one CTA overlaps the butterflies of the other); returns false if even one z line per
-// chunk does not fit.
+// Launch plan of the plane kernel: rows per chunk, threads, dynamic shared memory.
+//  fast path (grid lengths known at build time): one butterfly per thread per pass, so threads = RC * max_nb <= 256;
+//  several CTAs per SM (shared memory is small: no staging).
+//  run-time path: cp.async staging, two CTAs per SM preferred.
+// Returns false if even one z line per chunk does not fit.
 bool plan_plane_kernel(rpa_chi0 *h) {
     const int N2 = h->grid[1], N3 = h->grid[2];
     const int ng3 = h->sp.gmax[2] - h->sp.gmin[2] + 1;
     const int N3p = N3 + (N3 >> 3) + 1;
     const int nbuf = h->pz.npass >= 3 ? 2 : (h->pz.npass == 2 ? 1 : 0);
-    const size_t fixed = ((size_t)N3 + N2 + 2 * (size_t)ng3 * N2) * sizeof(cd);
+    h->pd_nbuf = nbuf;
+    const PdPlaneChoice ch = pd_plane_pick(N2, N3);
+    h->pd_kernel = ch.kernel;
+    const size_t ysz = (size_t)ng3 * N2;
+    if (ch.fast) {
+        int rc = std::max(1, std::min(N2, ch.max_threads / ch.max_nb));
+        const int chunks = (N2 + rc - 1) / rc;
+        rc = (N2 + chunks - 1) / chunks;
+        const size_t zsz = (size_t)nbuf * rc * N3p;
+        const size_t elems = (size_t)N2 + zsz + ysz + (ysz <= zsz ? 0 : ysz);
+        h->RC = rc;
+        h->pd_smem = elems * sizeof(cd);
+        h->pd_threads = (int)align_up((size_t)std::max(32, rc * ch.max_nb), 32);
+        return h->pd_smem <= 220 * 1024 && h->pd_threads <= ch.max_threads;
+    }
+    const size_t fixed = ((size_t)N3 + N2 + 2 * ysz) * sizeof(cd);
     const size_t per_row = (4 * (size_t)N3 + (size_t)nbuf * N3p) * sizeof(cd);
     const size_t caps[3] = {72 * 1024, 110 * 1024, 224 * 1024};   // 3, 2, 1 CTAs per SM
     int rc = 0;
@@ -279,7 +297,6 @@ bool plan_plane_kernel(rpa_chi0 *h) {
     const int chunks = (N2 + rc - 1) / rc;
     rc = (N2 + chunks - 1) / chunks;
     h->RC = rc;
-    h->pd_nbuf = nbuf;
     h->pd_smem = fixed + per_row * rc;
     const int r0 = h->pz.npass > 0 ? h->pz.radix[0] : 1;
     const int bf = rc * (N3 / r0);
@@ -370,7 +387,7 @@ int rpa_chi0_create(rpa_chi0_t **out, const int32_t grid[3], const double cell[9
         }                                                                                       \
     } while (0)
 
-    CREATE_TRY(cudaFuncSetAttribute(pd_plane_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->pd_smem));
+    CREATE_TRY(cudaFuncSetAttribute(h->pd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->pd_smem));
     CREATE_TRY(cudaFuncSetAttribute(rank_k_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, rk::SMEM_BYTES));
 
     // tables: twiddles in extended precision, box -> sphere map
@@ -511,7 +528,7 @@ int rpa_chi0_add_kpoint(rpa_chi0_t *h, double kweight, int32_t n_occ, const void
                     P.g2min = sp.gmin[1]; P.ng2 = ng2; P.g3min = sp.gmin[2]; P.ng3 = ng3;
                     P.RC = h->RC; P.nbuf = h->pd_nbuf; P.pz = h->pz; P.py = h->py;
                     const int gy = std::max(1, std::min(pc, (148 * 8 + N1 - 1) / N1));
-                    pd_plane_kernel<<<dim3(N1, gy), h->pd_threads, h->pd_smem, st>>>(P);
+                    h->pd_kernel<<<dim3(N1, gy), h->pd_threads, h->pd_smem, st>>>(P);
                     CUDA_TRY(cudaGetLastError());
                 }
                 {
