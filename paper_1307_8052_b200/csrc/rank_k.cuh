@@ -13,17 +13,19 @@
 //
 // One CTA = one 64 x 64 complex tile of the lower triangle x 2 frequencies (warps 0-3: first, 4-7: second; each
 // warp a 32 x 32 complex sub-tile = 4 x 4 x {Re,Im} DMMA accumulators = 128 registers).  K is streamed in chunks
-// of 16 pairs through a 4-stage ring filled by the TMA engine (cp.async.bulk, one 1 KB row per copy) and
-// tracked with full/empty mbarriers.  Both frequencies share the staged rows; only the weights differ.
+// of 16 pairs through a 5-stage ring filled by a dedicated producer warp through the TMA engine (cp.async.bulk, one
+// 1 KB row per copy) and tracked with full/empty mbarriers.  Both frequencies share the staged rows; only the
+// weights differ, and they multiply the column operand (4 DMUL per 32 DMMA).
 #pragma once
 #include "common.cuh"
 
 namespace rk {
 constexpr int T = 64;        // tile edge (complex elements)
 constexpr int KC = 16;       // pairs per stage
-constexpr int STAGES = 4;
+constexpr int STAGES = 5;
 constexpr int NW = 2;        // frequencies per CTA
-constexpr int THREADS = 256;
+constexpr int CONSUMER_WARPS = 8;
+constexpr int THREADS = (CONSUMER_WARPS + 1) * 32;   // warp 8 is the TMA producer
 constexpr int PITCH = T * 16 + 64;               // bytes per pair row in shared memory (= 64 mod 128, see below)
 constexpr int TILE_BYTES = KC * PITCH;           // 17408
 constexpr int W_BYTES = NW * KC * 8;             // 256
@@ -78,7 +80,7 @@ rank_k_kernel(const cd *__restrict__ Nb, int64_t ldn, int Kpad, const double *__
     if (tid == 0) {
         for (int s = 0; s < STAGES; s++) {
             mbar_init(&full[s], 1);
-            mbar_init(&empty[s], THREADS / 32);
+            mbar_init(&empty[s], CONSUMER_WARPS);
         }
         mbar_fence_init();
     }
@@ -86,20 +88,23 @@ rank_k_kernel(const cd *__restrict__ Nb, int64_t ldn, int Kpad, const double *__
     __syncthreads();
 
     const int nk = Kpad / KC;
-    auto issue = [&](int it) {  // warp 0 only
-        const int s = it % STAGES;
-        unsigned char *st = rk_smem + s * STAGE_BYTES;
-        if (lane == 0) mbar_arrive_expect_tx(&full[s], stage_tx);
-        __syncwarp();
-        const size_t krow = (size_t)it * KC + (lane & 15);
-        if (lane < 16) bulk_g2s(st + lane * PITCH, Nb + krow * ldn + row0, rowbytes, &full[s]);
-        else bulk_g2s(st + TILE_BYTES + (lane - 16) * PITCH, Nb + krow * ldn + col0, colbytes, &full[s]);
-        if (lane < n_om)
-            bulk_g2s(st + 2 * TILE_BYTES + lane * KC * 8, w + (size_t)(om0 + lane) * ldw + (size_t)it * KC, KC * 8,
-                     &full[s]);
-    };
-    if (warp == 0)
-        for (int it = 0; it < STAGES - 1 && it < nk; it++) issue(it);
+    if (warp == CONSUMER_WARPS) {
+        // ---- producer warp: keeps the ring full, never touches the tensor pipe -------------------------------
+        for (int it = 0; it < nk; it++) {
+            const int s = it % STAGES;
+            if (it >= STAGES) mbar_wait(&empty[s], ((it / STAGES) - 1) & 1);
+            unsigned char *st = rk_smem + s * STAGE_BYTES;
+            if (lane == 0) mbar_arrive_expect_tx(&full[s], stage_tx);
+            __syncwarp();
+            const size_t krow = (size_t)it * KC + (lane & 15);
+            if (lane < 16) bulk_g2s(st + lane * PITCH, Nb + krow * ldn + row0, rowbytes, &full[s]);
+            else bulk_g2s(st + TILE_BYTES + (lane - 16) * PITCH, Nb + krow * ldn + col0, colbytes, &full[s]);
+            if (lane < n_om)
+                bulk_g2s(st + 2 * TILE_BYTES + lane * KC * 8, w + (size_t)(om0 + lane) * ldw + (size_t)it * KC, KC * 8,
+                         &full[s]);
+        }
+        return;
+    }
 
     const int g = lane >> 2, kq = lane & 3, pp = kq >> 1, c = kq & 1;
     const int wsel = warp >> 2, quad = warp & 3;
@@ -117,15 +122,9 @@ rank_k_kernel(const cd *__restrict__ Nb, int64_t ldn, int Kpad, const double *__
     const uint32_t a_off = pp * PITCH + (rowoff + g) * 16;
     const uint32_t b_off = TILE_BYTES + pp * PITCH + (coloff + g) * 16 + c * 8;
     const uint32_t w_off = 2 * TILE_BYTES + (wsel * KC + pp) * 8;
+    const uint32_t sign_hi = (uint32_t)c << 31;   // A'[2p+1] = -re: flip the sign bit on odd k lanes (ALU pipe, not FP64)
 
     for (int it = 0; it < nk; it++) {
-        if (warp == 0) {
-            const int nx = it + STAGES - 1;
-            if (nx < nk) {
-                if (nx >= STAGES) mbar_wait(&empty[nx % STAGES], ((nx / STAGES) - 1) & 1);
-                issue(nx);
-            }
-        }
         const int s = it % STAGES;
         mbar_wait(&full[s], (it / STAGES) & 1);
         if (active) {
@@ -133,17 +132,18 @@ rank_k_kernel(const cd *__restrict__ Nb, int64_t ldn, int Kpad, const double *__
 #pragma unroll
             for (int ks = 0; ks < KC / 2; ks++) {
                 const uint32_t ko = ks * 2 * PITCH;
+                // the weight multiplies the shared (column) operand: 4 DMUL per k-step instead of 8
                 const double wv = *reinterpret_cast<const double *>(st + w_off + ks * 16);
-                const double swv = c ? -wv : wv;
                 double a[4], a2[4], b[4];
 #pragma unroll
                 for (int mi = 0; mi < 4; mi++) {
                     const unsigned char *ap = st + a_off + ko + mi * 128;
-                    a[mi] = wv * *reinterpret_cast<const double *>(ap + c * 8);
-                    a2[mi] = swv * *reinterpret_cast<const double *>(ap + (c ^ 1) * 8);
+                    a[mi] = *reinterpret_cast<const double *>(ap + c * 8);
+                    const double o = *reinterpret_cast<const double *>(ap + (c ^ 1) * 8);
+                    a2[mi] = __hiloint2double(__double2hiint(o) ^ (int)sign_hi, __double2loint(o));
                 }
 #pragma unroll
-                for (int ni = 0; ni < 4; ni++) b[ni] = *reinterpret_cast<const double *>(st + b_off + ko + ni * 128);
+                for (int ni = 0; ni < 4; ni++) b[ni] = wv * *reinterpret_cast<const double *>(st + b_off + ko + ni * 128);
 #pragma unroll
                 for (int mi = 0; mi < 4; mi++)
 #pragma unroll
