@@ -153,6 +153,7 @@ def run_ours(args, cfg):
     import torch
     import torch.distributed as dist
     from paper_1307_8052_b200 import binding as B
+    from paper_1307_8052_b200 import sharding
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -194,7 +195,7 @@ def run_ours(args, cfg):
                 B.rpa_chi0_add_kpoint(h, kweight, devt["psi_occ"], devt["psi_unocc"], kd.eps_occ, kd.eps_unocc, kd.f_occ,
                                       kd.f_unocc, npj, devt["P_occ"], devt["P_unocc"], Qd, R)
         if world > 1:
-            dist.all_reduce(torch.view_as_real(S))
+            sharding.allreduce_accumulators(S)
         for i in range(cfg.n_omega):
             B.rpa_chi0_get(h, i, out)
         ec, e = B.rpa_ec_q(h, v)  # blocks; reads E_c(q), e(omega) back to the host
