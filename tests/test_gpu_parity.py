@@ -92,3 +92,66 @@ def test_config1_molecule_slice():
     cfg = W.CONFIGS[1]
     kds = [W.kpoint(cfg, 0, occ=[0, 11], unocc=range(0, 600, 16)[:37])]
     _compare(cfg, kds)
+
+
+def _big_config_slice(cfg, occ, unocc, n_sample, omegas=(0, 7, 15)):
+    """Configs 3 / 4 at full grid, nG, omega count and atoms, on a band slice (a full oracle run costs hours to a
+    day of CPU).  The oracle evaluates chi0 on a sampled sub-list of the sphere (every element of
+    Eq. 17 is an independent sum, so chi0 restricted to those G is exactly the chi0 of those G); the sample holds
+    the first / last G and both sides of several 64-tile boundaries.  E_c(q), which needs the whole matrix, is
+    checked against the eigenvalue route sum_i ln(1 - l_i) + l_i on the library's own chi0 (numpy eigvalsh)."""
+    import torch
+    from paper_1307_8052_b200 import binding as B
+    om, wt = W.omega_grid(cfg.n_omega)
+    ptot = int(cfg.n_proj.sum())
+    kds = [W.kpoint(cfg, k, occ=occ, unocc=unocc) for k in (0, 1)]
+    h = B.rpa_chi0_create(cfg.grid, cfg.cell, cfg.q_red, W.tuned_ecut(cfg), om, wt, 0, ptot, "cuda:0")
+    try:
+        g, K2 = B.rpa_chi0_gvectors(h)
+        ng = len(g)
+        rng = np.random.default_rng(7)
+        sel = set([0, 1, ng - 1, ng - 2, 63, 64, 65, 127, 128, (ng // 64) * 64 - 1, (ng // 64) * 64])
+        sel |= set(rng.choice(ng, n_sample - len(sel), replace=False).tolist())
+        sel = np.array(sorted(s for s in sel if 0 <= s < ng))
+        Qd = torch.from_numpy(W.paw_Q(cfg, K2)).to("cuda:0")
+        R = W.atom_positions(cfg)
+        for kd in kds:
+            B.add_kpoint_host(h, kd, cfg.n_proj, Qd, R)
+        seld = torch.from_numpy(sel).to("cuda:0")
+        chi_sel, chi_full = {}, {}
+        for i in omegas:
+            c = B.rpa_chi0_get(h, i)
+            chi_sel[i] = c[seld][:, seld].cpu().numpy()
+            if i in (omegas[0], omegas[-1]):
+                chi_full[i] = c.cpu().numpy()
+            del c
+        v = W.coulomb(K2)
+        ec, e = B.rpa_ec_q(h, v)
+    finally:
+        h.close()
+    chi_o, _, g_o, _ = oracle_run(cfg, kds, True, want_ec=False, g=g[sel])
+    for i in omegas:
+        err = rel_fro(chi_sel[i], chi_o[i])
+        assert err <= CHI_TOL, f"omega {i}: rel Frobenius error on the sampled G {err:.3e}"
+    d = np.sqrt(v)
+    for i, c in chi_full.items():
+        assert np.array_equal(c, c.conj().T)
+        lam = np.linalg.eigvalsh(d[:, None] * c * d[None, :])
+        assert lam.max() <= 1e-12 * np.abs(lam).max()          # negative semidefinite
+        want = float(np.sum(np.log1p(-lam) + lam))
+        assert abs(e[i] - want) <= 1e-9 * max(abs(want), np.abs(e).max() * 1e-3), (i, e[i], want)
+    assert np.isfinite(ec) and ec < 0.0
+
+
+def test_config3_slab_slice():
+    """40x40x168 grid (radices 8,7,3 / 8,5), nG = 3004, 16 omega, 10 atoms x 18 projectors, metallic smearing;
+    2 k-points x 3 occupied (lowest, middle, highest) x 23 unoccupied (strided, includes the band nearest mu)."""
+    cfg = W.CONFIGS[3]
+    _big_config_slice(cfg, occ=[0, 31, 63], unocc=list(range(0, 1500, 68))[:23], n_sample=160)
+
+
+def test_config4_large_slab_slice():
+    """48x48x192 grid, nG = 5001 (chi0 6.4 GB resident), 18 atoms x 18 projectors; 2 k-points x 2 occupied x 13
+    unoccupied."""
+    cfg = W.CONFIGS[4]
+    _big_config_slice(cfg, occ=[0, 119], unocc=list(range(0, 3000, 240))[:13], n_sample=120)
