@@ -29,8 +29,16 @@ constexpr int THREADS = (CONSUMER_WARPS + 1) * 32;   // warp 8 is the TMA produc
 constexpr int PITCH = T * 16 + 64;               // bytes per pair row in shared memory (= 64 mod 128, see below)
 constexpr int TILE_BYTES = KC * PITCH;           // 17408
 constexpr int W_BYTES = NW * KC * 8;             // 256
-constexpr int STAGE_BYTES = 2 * TILE_BYTES + W_BYTES;
-constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 2 * STAGES * 8;
+// SHARED_N = true : both frequencies of a CTA read the same N tiles (the chi0 accumulation), 5 stages.
+// SHARED_N = false: every frequency has its own N (the Cholesky trailing update of rpa_ec_q, where N is the
+//                   transposed panel of that frequency's matrix): two tile sets per stage, 3 stages.
+template <bool SHARED_N>
+struct Cfg {
+    static constexpr int NSTAGES = SHARED_N ? STAGES : 3;
+    static constexpr int TILE_SETS = SHARED_N ? 1 : NW;
+    static constexpr int STAGE_BYTES = 2 * TILE_SETS * TILE_BYTES + W_BYTES;
+    static constexpr int SMEM_BYTES = NSTAGES * STAGE_BYTES + 2 * NSTAGES * 8;
+};
 }  // namespace rk
 
 // w[iw*ldw + p] = kweight * 2 (f_n - f_m)(e_n - e_m) / (omega_iw^2 + (e_n - e_m)^2) for p < K, 0 for K <= p < Kpad.
@@ -51,12 +59,17 @@ __global__ void weights_kernel(double *__restrict__ w, int64_t ldw, int K, int K
     w[(size_t)iw * ldw + p] = val;
 }
 
-// Nb[Kpad][ldn] (rows >= K are zero), w[n_omega][ldw], S[n_omega][ng][ldS] (lower triangle accumulated).
-// Kpad % KC == 0.  grid = (ntiles_lower, ceil(n_omega / 2)).
+// Nb[Kpad][ldn] (rows >= K are zero; frequency iw reads Nb + iw*strideN, strideN = 0 when SHARED_N), w[n_omega][ldw],
+// S[n_omega][ng][ldS] (lower triangle accumulated).  Only rows / columns g >= g0 are touched (g0 % 1 == 0; tiles
+// start at g0).  Kpad % KC == 0.  grid = (ntiles_lower(ng - g0), ceil(n_omega / 2)).
+template <bool SHARED_N>
 __global__ void __launch_bounds__(rk::THREADS, 1)
-rank_k_kernel(const cd *__restrict__ Nb, int64_t ldn, int Kpad, const double *__restrict__ w, int64_t ldw,
-              cd *__restrict__ S, int64_t ldS, int64_t strideS, int ng, int n_omega) {
+rank_k_kernel(const cd *__restrict__ Nb, int64_t ldn, int64_t strideN, int Kpad, const double *__restrict__ w,
+              int64_t ldw, cd *__restrict__ S, int64_t ldS, int64_t strideS, int ng, int g0, int n_omega) {
     using namespace rk;
+    constexpr int STAGES = Cfg<SHARED_N>::NSTAGES;
+    constexpr int STAGE_BYTES = Cfg<SHARED_N>::STAGE_BYTES;
+    constexpr int W_OFF = 2 * Cfg<SHARED_N>::TILE_SETS * TILE_BYTES;
     extern __shared__ __align__(128) unsigned char rk_smem[];
     uint64_t *full = reinterpret_cast<uint64_t *>(rk_smem + STAGES * STAGE_BYTES);
     uint64_t *empty = full + STAGES;
@@ -68,11 +81,11 @@ rank_k_kernel(const cd *__restrict__ Nb, int64_t ldn, int Kpad, const double *__
     while ((ti + 1) * (ti + 2) / 2 <= t) ti++;
     while (ti * (ti + 1) / 2 > t) ti--;
     const int tj = t - ti * (ti + 1) / 2;
-    const int row0 = ti * T, col0 = tj * T;
+    const int row0 = g0 + ti * T, col0 = g0 + tj * T;
     const int om0 = blockIdx.y * NW;
     const int n_om = min(NW, n_omega - om0);
     const uint32_t rowbytes = (uint32_t)min(T, ng - row0) * 16u, colbytes = (uint32_t)min(T, ng - col0) * 16u;
-    const uint32_t stage_tx = KC * (rowbytes + colbytes) + (uint32_t)n_om * KC * 8u;
+    const uint32_t stage_tx = KC * (rowbytes + colbytes) * (SHARED_N ? 1u : (uint32_t)n_om) + (uint32_t)n_om * KC * 8u;
 
     // zero the ring once so that the never-copied tail columns of edge tiles hold finite numbers
     for (int i = tid; i < STAGES * STAGE_BYTES / 16; i += THREADS)
@@ -97,11 +110,17 @@ rank_k_kernel(const cd *__restrict__ Nb, int64_t ldn, int Kpad, const double *__
             if (lane == 0) mbar_arrive_expect_tx(&full[s], stage_tx);
             __syncwarp();
             const size_t krow = (size_t)it * KC + (lane & 15);
-            if (lane < 16) bulk_g2s(st + lane * PITCH, Nb + krow * ldn + row0, rowbytes, &full[s]);
-            else bulk_g2s(st + TILE_BYTES + (lane - 16) * PITCH, Nb + krow * ldn + col0, colbytes, &full[s]);
+#pragma unroll
+            for (int ts = 0; ts < Cfg<SHARED_N>::TILE_SETS; ts++) {
+                if (ts < n_om) {
+                    const cd *Nw = Nb + (size_t)(om0 + ts) * strideN + krow * ldn;
+                    unsigned char *dst = st + ts * 2 * TILE_BYTES;
+                    if (lane < 16) bulk_g2s(dst + lane * PITCH, Nw + row0, rowbytes, &full[s]);
+                    else bulk_g2s(dst + TILE_BYTES + (lane - 16) * PITCH, Nw + col0, colbytes, &full[s]);
+                }
+            }
             if (lane < n_om)
-                bulk_g2s(st + 2 * TILE_BYTES + lane * KC * 8, w + (size_t)(om0 + lane) * ldw + (size_t)it * KC, KC * 8,
-                         &full[s]);
+                bulk_g2s(st + W_OFF + lane * KC * 8, w + (size_t)(om0 + lane) * ldw + (size_t)it * KC, KC * 8, &full[s]);
         }
         return;
     }
@@ -119,9 +138,10 @@ rank_k_kernel(const cd *__restrict__ Nb, int64_t ldn, int Kpad, const double *__
 #pragma unroll
         for (int ni = 0; ni < 4; ni++) re[mi][ni][0] = re[mi][ni][1] = im[mi][ni][0] = im[mi][ni][1] = 0.0;
 
-    const uint32_t a_off = pp * PITCH + (rowoff + g) * 16;
-    const uint32_t b_off = TILE_BYTES + pp * PITCH + (coloff + g) * 16 + c * 8;
-    const uint32_t w_off = 2 * TILE_BYTES + (wsel * KC + pp) * 8;
+    const uint32_t set_off = SHARED_N ? 0u : (uint32_t)wsel * 2 * TILE_BYTES;
+    const uint32_t a_off = set_off + pp * PITCH + (rowoff + g) * 16;
+    const uint32_t b_off = set_off + TILE_BYTES + pp * PITCH + (coloff + g) * 16 + c * 8;
+    const uint32_t w_off = W_OFF + (wsel * KC + pp) * 8;
     const uint32_t sign_hi = (uint32_t)c << 31;   // A'[2p+1] = -re: flip the sign bit on odd k lanes (ALU pipe, not FP64)
 
     for (int it = 0; it < nk; it++) {

@@ -43,7 +43,7 @@ constexpr int MAX_SLOTS = 16;          // occupied bands per batch
 constexpr int MAX_BANDS = 1 << 17;     // eps/f scratch
 constexpr int MAX_ATOMS = 4096;
 constexpr int MAX_PROJ = 1 << 16;
-constexpr int EC_GROUP = 4;            // frequencies factorised together in rpa_ec_q
+constexpr int EC_GROUP = 16;           // frequencies factorised together in rpa_ec_q
 constexpr size_t I_BUDGET = 64u << 20; // pruned intermediate kept L2-sized
 constexpr int NSTAGE = 5;
 
@@ -109,7 +109,7 @@ void build_sphere(const int32_t grid[3], const double B[9], const double q[3], d
 }
 
 struct Layout {
-    size_t S, Nbuf, w, I, T, M, tw1, tw2, tw3, box2s, Kc, omega, wt, band, R, aj_atom, aj_j, atom_poff, atom_ni,
+    size_t S, Nbuf, w, I, T, M, Lt, wneg, tw1, tw2, tw3, box2s, Kc, omega, wt, band, R, aj_atom, aj_j, atom_poff, atom_ni,
         atom_qoff, v, e, tr, logdet, flag, ec, total;
     int64_t ldS, ldn, ldw;
     int Kmax, sub_pairs, ec_group;
@@ -149,6 +149,8 @@ void make_layout(const int32_t grid[3], const Sphere &sp, int n_omega, int max_b
     L->I = take((size_t)L->sub_pairs * L->I_pair_bytes);
     L->T = take((size_t)MAX_SLOTS * std::max(max_proj, 0) * L->ldn * sizeof(cd));
     L->M = take((size_t)L->ec_group * ng * ng * sizeof(cd));
+    L->Lt = take((size_t)L->ec_group * CH_NB * L->ldn * sizeof(cd));
+    L->wneg = take((size_t)L->ec_group * CH_NB * sizeof(double));
     L->tw1 = take((size_t)grid[0] * sizeof(cd));
     L->tw2 = take((size_t)grid[1] * sizeof(cd));
     L->tw3 = take((size_t)grid[2] * sizeof(cd));
@@ -388,7 +390,8 @@ int rpa_chi0_create(rpa_chi0_t **out, const int32_t grid[3], const double cell[9
     } while (0)
 
     CREATE_TRY(cudaFuncSetAttribute(h->pd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->pd_smem));
-    CREATE_TRY(cudaFuncSetAttribute(rank_k_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, rk::SMEM_BYTES));
+    CREATE_TRY(cudaFuncSetAttribute(rank_k_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, rk::Cfg<true>::SMEM_BYTES));
+    CREATE_TRY(cudaFuncSetAttribute(rank_k_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, rk::Cfg<false>::SMEM_BYTES));
 
     // tables: twiddles in extended precision, box -> sphere map
     const Sphere &sp = h->sp;
@@ -415,6 +418,12 @@ int rpa_chi0_create(rpa_chi0_t **out, const int32_t grid[3], const double cell[9
     CREATE_TRY(cudaMemcpyAsync(h->ws + L.Kc, sp.Kc.data(), sp.Kc.size() * sizeof(double), cudaMemcpyHostToDevice, h->stream));
     CREATE_TRY(cudaMemcpyAsync(h->ws + L.omega, h->omega.data(), n_omega * sizeof(double), cudaMemcpyHostToDevice, h->stream));
     CREATE_TRY(cudaMemcpyAsync(h->ws + L.wt, h->wt.data(), n_omega * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+    {
+        std::vector<double> wneg((size_t)L.ec_group * CH_NB, -1.0);   // weight of the Cholesky trailing update
+        CREATE_TRY(cudaMemcpyAsync(h->ws + L.wneg, wneg.data(), wneg.size() * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+        CREATE_TRY(cudaStreamSynchronize(h->stream));
+    }
+    CREATE_TRY(cudaMemsetAsync(h->ws + L.Lt, 0, (size_t)L.ec_group * CH_NB * L.ldn * sizeof(cd), h->stream));
     CREATE_TRY(cudaMemsetAsync(h->ws + L.S, 0, (size_t)n_omega * sp.ng * L.ldS * sizeof(cd), h->stream));
     CREATE_TRY(cudaMemsetAsync(h->ws + L.Nbuf, 0, (size_t)L.Kmax * L.ldn * sizeof(cd), h->stream));
     CREATE_TRY(cudaStreamSynchronize(h->stream));
@@ -561,8 +570,9 @@ int rpa_chi0_add_kpoint(rpa_chi0_t *h, double kweight, int32_t n_occ, const void
             // S6: rank-K update of every frequency
             {
                 StageTimer tm(h, 4, 1);
-                rank_k_kernel<<<dim3(ntiles_lower(ng, rk::T), (h->n_omega + rk::NW - 1) / rk::NW), rk::THREADS, rk::SMEM_BYTES, st>>>(
-                    Nbuf, L.ldn, Kpad, w, L.ldw, h->ptr<cd>(L.S), L.ldS, (int64_t)ng * L.ldS, ng, h->n_omega);
+                rank_k_kernel<true><<<dim3(ntiles_lower(ng, rk::T), (h->n_omega + rk::NW - 1) / rk::NW), rk::THREADS,
+                                      rk::Cfg<true>::SMEM_BYTES, st>>>(
+                    Nbuf, L.ldn, 0, Kpad, w, L.ldw, h->ptr<cd>(L.S), L.ldS, (int64_t)ng * L.ldS, ng, 0, h->n_omega);
                 CUDA_TRY(cudaGetLastError());
             }
         }
@@ -609,8 +619,12 @@ int rpa_ec_q(rpa_chi0_t *h, const double *v_G, double *ec_ha, double *e_omega) {
             h->launches += 1;
             const int rest = ng - (k0 + CH_NB);
             if (rest > 0) {
-                chol_panel_kernel<<<dim3((rest + 127) / 128, nm), 128, 0, st>>>(M, ng, k0);
-                chol_update_kernel<<<dim3(ntiles_lower(rest, 64), nm), 256, 0, st>>>(M, ng, k0);
+                chol_panel_kernel<<<dim3((rest + 127) / 128, nm), 128, 0, st>>>(M, ng, k0, h->ptr<cd>(L.Lt), L.ldn);
+                // trailing update M[g][g'] -= sum_t L[g][t] conj(L[g'][t]), g >= g' >= k0 + 32, on the DMMA path
+                rank_k_kernel<false><<<dim3(ntiles_lower(rest, rk::T), (nm + rk::NW - 1) / rk::NW), rk::THREADS,
+                                       rk::Cfg<false>::SMEM_BYTES, st>>>(
+                    h->ptr<cd>(L.Lt), L.ldn, (int64_t)CH_NB * L.ldn, CH_NB, h->ptr<double>(L.wneg), CH_NB, M, ng,
+                    (int64_t)ng * ng, ng, k0 + CH_NB, nm);
                 h->launches += 2;
             }
         }
