@@ -152,6 +152,35 @@ struct Bfly<6> {
     }
 };
 
+template <>
+struct Bfly<12> {
+    // 12 = 4 x 3 Cooley-Tukey in registers: j = 3 j1 + j2 (j1 < 4, j2 < 3), k = k1 + 4 k2:
+    //   X[k1 + 4 k2] = sum_j2 W3^(j2 k2) W12^(j2 k1) sum_j1 v[3 j1 + j2] W4^(j1 k1)
+    HD static void run(cd *v) {
+        const double c = 0.86602540378443864676;  // cos(pi/6) = sin(pi/3)
+        cd e[3][4];
+#pragma unroll
+        for (int j2 = 0; j2 < 3; j2++) {
+            e[j2][0] = v[j2]; e[j2][1] = v[j2 + 3]; e[j2][2] = v[j2 + 6]; e[j2][3] = v[j2 + 9];
+            Bfly<4>::run(e[j2]);
+        }
+        // W12^(j2 k1): W12 = c - i/2, W12^2 = 1/2 - i c, W12^3 = -i, W12^4 = -1/2 - i c, W12^6 = -1
+        cd a;
+        a = e[1][1]; e[1][1] = make_double2(c * a.x + 0.5 * a.y, c * a.y - 0.5 * a.x);
+        a = e[1][2]; e[1][2] = make_double2(0.5 * a.x + c * a.y, 0.5 * a.y - c * a.x);
+        e[1][3] = h_mni(e[1][3]);
+        a = e[2][1]; e[2][1] = make_double2(0.5 * a.x + c * a.y, 0.5 * a.y - c * a.x);
+        a = e[2][2]; e[2][2] = make_double2(-0.5 * a.x + c * a.y, -0.5 * a.y - c * a.x);
+        e[2][3] = make_double2(-e[2][3].x, -e[2][3].y);
+#pragma unroll
+        for (int k1 = 0; k1 < 4; k1++) {
+            cd t[3] = {e[0][k1], e[1][k1], e[2][k1]};
+            Bfly<3>::run(t);
+            v[k1] = t[0]; v[k1 + 4] = t[1]; v[k1 + 8] = t[2];
+        }
+    }
+};
+
 // One Stockham pass of radix R over `nlines` lines of length N, butterflies tid, tid+nthreads, ...
 //   ns = product of the radices of the earlier passes (1 for the first pass).
 //   ld(line, idx) -> cd      reads element idx of the line in the pass's input

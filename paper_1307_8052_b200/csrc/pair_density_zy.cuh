@@ -1,0 +1,332 @@
+// pd_zy_kernel -- pair product + z and y transforms of the pruned 3-D FFT (Table 1 step 5; Eq. 12,
+// P:L104-106) for planes that fit one CTA, written for a low instruction count per grid point: every loop is
+// unrolled at compile time, all shared-memory addresses are a per-thread base plus constants.
+//
+// Both axes use the same two-level split N = NA * NB:
+//   pass A  (full)    A_j[k1] = sum_s x[j + NB s] W_NA^(s k1)            one radix-NA butterfly in registers
+//   pass B  (pruned)  X[f]    = sum_j W_N^(j f) A_j[f mod NA]            direct NB-term sum, only for f in the box
+// so the work after the butterfly is proportional to the number of frequencies kept (ng3 of N3, ng2 of N2).
+//
+// z axis: a warp owns LPW whole lines (NB3 lanes per line): pass A -> padded exchange buffer of the warp -> pass B
+// needs __syncwarp only, no block barrier.  u_m is prefetched into registers TWO iterations ahead (two register
+// buffers used alternately; plain 16-byte loads, 128 contiguous bytes per line and instruction), which covers the
+// HBM latency with 8 warps per SM.  The chunk of u_n is reused for the G pairs (same occupied band) a CTA
+// transforms together, so it costs 1/G global loads per point; it lives in thread-private shared-memory slots
+// (cp.async, conflict-free [element][thread] layout) to leave the registers to the second prefetch buffer.
+// y axis: the ng3 * G surviving columns: pass A in place in shared memory, pass B writes I[pair][j1][g2i][g3i]
+// (coalesced: consecutive threads -> consecutive g3i).
+#pragma once
+#include "fft.cuh"
+
+#define PDZY_MAXK1 4   // k1 values per z pass-B thread: ceil(NA3 / NB3)
+
+// z pass B for a box inside [-NA, NA): k1 keeps at most the two frequencies g = k1 (>= 0) and g = k1 - NA (< 0), and
+// W_N^(j (k1 - NA)) = W_N^(j k1) conj(W_NB^j): with B[j] = W_N^(j k1) A_j[k1],
+//   o0 = sum_j B[j]   (g = k1),      o1 = sum_j conj(W_NB^j) B[j]   (g = k1 - NA).
+template <int NB>
+struct PairSum {
+    __device__ __forceinline__ static void run(const cd *B, cd &o0, cd &o1) {
+        o0 = B[0];
+        o1 = B[0];
+#pragma unroll
+        for (int j = 1; j < NB; j++) {
+            double sn, cs;
+            sincospi(2.0 * j / NB, &sn, &cs);   // folded at compile time (j, NB constant)
+            o0 = cadd(o0, B[j]);
+            o1 = cfma(make_double2(cs, sn), B[j], o1);
+        }
+    }
+};
+template <>
+struct PairSum<2> {
+    __device__ __forceinline__ static void run(const cd *B, cd &o0, cd &o1) {
+        o0 = cadd(B[0], B[1]);
+        o1 = csub(B[0], B[1]);
+    }
+};
+template <>
+struct PairSum<3> {
+    __device__ __forceinline__ static void run(const cd *B, cd &o0, cd &o1) {
+        const double s = 0.86602540378443864676;
+        const cd t = cadd(B[1], B[2]), d = csub(B[1], B[2]);
+        o0 = cadd(B[0], t);
+        // conj(W3) = -1/2 + i s, conj(W3^2) = -1/2 - i s
+        o1 = make_double2(fma(-0.5, t.x, B[0].x) - s * d.y, fma(-0.5, t.y, B[0].y) + s * d.x);
+    }
+};
+template <>
+struct PairSum<8> {
+    __device__ __forceinline__ static void run(const cd *B, cd &o0, cd &o1) {
+        const double h = 0.70710678118654752440;
+        o0 = cadd(cadd(cadd(B[0], B[4]), cadd(B[2], B[6])), cadd(cadd(B[1], B[5]), cadd(B[3], B[7])));
+        const cd d = csub(B[0], B[4]), e = csub(B[2], B[6]), u = csub(B[1], B[5]), w = csub(B[3], B[7]);
+        // (B0 - B4) + i (B2 - B6) + h [(1 + i)(B1 - B5) + (-1 + i)(B3 - B7)]
+        const double re = (u.x - u.y) - (w.x + w.y), im = (u.x + u.y) + (w.x - w.y);
+        o1 = make_double2(fma(h, re, d.x - e.y), fma(h, im, d.y + e.x));
+    }
+};
+
+struct PdZyParams {
+    const cd *psi_occ, *psi_unocc;  // [band][N1][N2][N3]
+    cd *I;                          // [pair - p_begin][N1][ng2][ng3]
+    const cd *tw3, *tw2;            // exp(-2 pi i t/N3), exp(-2 pi i t/N2)
+    int N1;
+    int n0, mlen, m0;               // pair p of the batch -> band n = n0 + p / mlen, m = m0 + p % mlen
+    int p_begin, p_count;           // pairs of the batch handled by this launch
+    int n_units;                    // groups of <= G consecutive pairs with the same occupied band
+    int g2min, ng2, g3min, ng3;
+};
+
+template <int N3, int NA3, int N2, int NA2, int NW, int LPW, int G>
+struct PdZy {
+    static constexpr int NB3 = N3 / NA3, NB2 = N2 / NA2;
+    static constexpr int K1PT = (NA3 + NB3 - 1) / NB3;
+    static constexpr int XP = NB3 + ((NB3 & 1) ? 0 : 1);  // pitch of one k1 row of the exchange line (odd: conflict-free)
+    static constexpr int XLINE = NA3 * XP;
+    static constexpr int ROWS = NW * LPW;                 // z lines per chunk
+    static constexpr int NCH = (N2 + ROWS - 1) / ROWS;
+    static constexpr int NTH = NW * 32;
+    static_assert(N3 % NA3 == 0 && N2 % NA2 == 0, "split");
+    static_assert(LPW * NB3 <= 32, "lanes");
+    static_assert(K1PT <= PDZY_MAXK1, "k1 per thread");
+
+    // shared memory (cd): tw2[N2] | X[NW][LPW][XLINE] | UN[NA3][NTH] | Y[N2][G * ng3] ; then int32 otab[ng2 * ng3]
+    static size_t smem_bytes(int ng2, int ng3) {
+        return ((size_t)N2 + (size_t)NW * LPW * XLINE + (size_t)NA3 * NTH + (size_t)N2 * G * ng3) * sizeof(cd) +
+               (size_t)ng2 * ng3 * sizeof(int32_t);
+    }
+    // the z pass B (PairSum) keeps g = k1 and g = k1 - NA3 only: the box must lie inside [-NA3, NA3)
+    static bool box_ok(int g3min, int ng3) { return g3min >= -NA3 && g3min + ng3 <= NA3 && 2 * NA3 <= N3 + 1; }
+};
+
+// unit u of the launch -> first pair p (relative to the batch) and the number of pairs cnt <= G, all in one row.
+template <int G>
+__device__ __forceinline__ void pdzy_unit(const PdZyParams &P, int u, int &p, int &cnt) {
+    p = P.p_begin;
+    const int p_end = P.p_begin + P.p_count;
+    while (true) {
+        const int row = p / P.mlen;
+        const int rend = min((row + 1) * P.mlen, p_end);
+        const int nu = (rend - p + G - 1) / G;
+        if (u < nu) {
+            p += u * G;
+            cnt = min(G, rend - p);
+            return;
+        }
+        u -= nu;
+        p = rend;
+    }
+}
+
+static inline int pdzy_count_units(int p_begin, int p_count, int mlen, int G) {
+    int p = p_begin, n = 0;
+    const int p_end = p_begin + p_count;
+    while (p < p_end) {
+        const int row = p / mlen;
+        const int rend = std::min((row + 1) * mlen, p_end);
+        n += (rend - p + G - 1) / G;
+        p = rend;
+    }
+    return n;
+}
+
+
+__device__ __forceinline__ void pdzy_cp_async16(void *dst_smem, const void *src_gmem) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst_smem)), "l"(src_gmem) : "memory");
+}
+__device__ __forceinline__ void pdzy_cp_async_wait() {
+    asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;" ::: "memory");
+}
+
+// position of a CTA in its sequence of z iterations: work item w = u N1 + j1 (unit u: pairs p0 .. p0 + cnt - 1 of
+// occupied band n, first unoccupied band m; plane j1), chunk c of the plane, pair g of the unit.  The grid is 1-D
+// and persistent (CTAs = resident slots of the GPU): CTA b takes items b, b + gridDim.x, ...
+struct PdZyCursor {
+    int w, p0, cnt, n, m, c, g, j1;
+};
+
+template <int N3, int NA3, int N2, int NA2, int NW, int LPW, int G, int MINB>
+__global__ void __launch_bounds__(NW * 32, MINB) pd_zy_kernel(const __grid_constant__ PdZyParams P) {
+    using C = PdZy<N3, NA3, N2, NA2, NW, LPW, G>;
+    constexpr int NB3 = C::NB3, NB2 = C::NB2, K1PT = C::K1PT, XP = C::XP, XLINE = C::XLINE, ROWS = C::ROWS, NCH = C::NCH,
+                  NTH = C::NTH;
+    extern __shared__ __align__(16) unsigned char pd_smem[];
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int ng2 = P.ng2, ng3 = P.ng3, nb2 = ng2 * ng3;
+    cd *tw2s = reinterpret_cast<cd *>(pd_smem);
+    cd *X = tw2s + N2;
+    cd *UN = X + NW * LPW * XLINE;
+    cd *Y = UN + NA3 * NTH;
+    int32_t *otab = reinterpret_cast<int32_t *>(Y + (size_t)N2 * G * ng3);
+    for (int i = tid; i < N2; i += NTH) tw2s[i] = P.tw2[i];
+    for (int i = tid; i < nb2; i += NTH) {
+        const int o = i / ng3;
+        otab[i] = (o << 16) | (i - o * ng3);
+    }
+
+    // ---- this thread's z role: line lw of the warp, butterfly / pass-B slot j ------------------------------------
+    const int lw = lane / NB3, j = lane - lw * NB3;
+    const bool zact = lw < LPW;
+    cd *Xl = X + (warp * LPW + (zact ? lw : 0)) * XLINE;
+    cd *uns = UN + tid;   // this thread's u_n elements: uns[t * NTH]
+    // pass B: k1 = j + a NB3 keeps g = k1 (box index oi0) and g = k1 - NA3 (oi1); twiddles W_N3^(jj k1)
+    cd twb[K1PT][NB3];
+    int oi0[K1PT], oi1[K1PT];
+#pragma unroll
+    for (int a = 0; a < K1PT; a++) {
+        const int k1 = j + a * NB3;
+        oi0[a] = oi1[a] = -1;
+        if (k1 < NA3) {
+            const int i0 = k1 - P.g3min, i1 = k1 - NA3 - P.g3min;
+            if (i0 >= 0 && i0 < ng3) oi0[a] = i0;
+            if (i1 >= 0 && i1 < ng3) oi1[a] = i1;
+        }
+#pragma unroll
+        for (int jj = 0; jj < NB3; jj++) twb[a][jj] = P.tw3[(jj * (k1 < NA3 ? k1 : 0)) % N3];
+    }
+
+    constexpr int plane = N2 * N3;
+    const size_t vol = (size_t)plane * P.N1;
+    // element offset of this thread's first input inside a plane, chunk 0: row (warp LPW + lw), column j
+    const int row_in_chunk = warp * LPW + lw;
+    const int off0 = row_in_chunk * N3 + j;
+    const int n_items = P.n_units * P.N1;
+
+    auto decode = [&](PdZyCursor &k) {   // k.w set; fills the other fields (cnt = 0 past the end)
+        k.c = 0;
+        k.g = 0;
+        k.cnt = 0;
+        if (k.w < n_items) {
+            const int u = k.w / P.N1;
+            k.j1 = k.w - u * P.N1;
+            pdzy_unit<G>(P, u, k.p0, k.cnt);
+            k.n = P.n0 + k.p0 / P.mlen;
+            k.m = P.m0 + k.p0 % P.mlen;
+        }
+    };
+    auto advance = [&](PdZyCursor &k) {
+        if (++k.g >= k.cnt) {
+            k.g = 0;
+            if (++k.c == NCH) {
+                k.w += gridDim.x;
+                decode(k);
+            }
+        }
+    };
+    auto load_m = [&](cd (&nx)[NA3], const PdZyCursor &k) {
+        if (k.cnt > 0 && zact && k.c * ROWS + row_in_chunk < N2) {
+            const cd *s = P.psi_unocc + (size_t)(k.m + k.g) * vol + (k.j1 * plane + k.c * ROWS * N3 + off0);
+#pragma unroll
+            for (int t = 0; t < NA3; t++) nx[t] = __ldcs(s + t * NB3);  // streamed once
+        }
+    };
+    auto load_n = [&](const PdZyCursor &k) {   // u_n chunk of the cursor -> this thread's shared-memory slots
+        if (k.cnt > 0 && zact && k.c * ROWS + row_in_chunk < N2) {
+            const cd *s = P.psi_occ + (size_t)k.n * vol + (k.j1 * plane + k.c * ROWS * N3 + off0);
+#pragma unroll
+            for (int t = 0; t < NA3; t++) pdzy_cp_async16(uns + t * NTH, s + t * NB3);
+        }
+    };
+
+    PdZyCursor cur, pf;
+    cur.w = blockIdx.x;
+    cur.p0 = cur.n = cur.m = cur.j1 = 0;
+    decode(cur);
+    pf = cur;
+    cd nxA[NA3], nxB[NA3];
+    load_n(cur);
+    load_m(nxA, pf);
+    if (pf.cnt > 0) advance(pf);
+    load_m(nxB, pf);
+    if (pf.cnt > 0) advance(pf);
+    // y pass-B start position of this thread: task t = tid -> (pair g, r = o ng3 + col)
+    const int yb_g0 = tid / nb2, yb_r0 = tid - yb_g0 * nb2;
+    __syncthreads();
+
+    // one z iteration (chunk c of pair g of the unit) on the inputs in nx; refills nx for two iterations later
+    auto step = [&](cd (&nx)[NA3]) {
+        const int c = cur.c, g = cur.g, cnt = cur.cnt, p0 = cur.p0, j1 = cur.j1;
+        const int row = c * ROWS + row_in_chunk;
+        const bool act = zact && row < N2;
+        const int pitch = cnt * ng3;   // Y row pitch of this unit: [row][g][g3i]
+        if (g == 0) pdzy_cp_async_wait();   // u_n of this chunk has landed in this thread's slots
+        cd v[NA3];
+#pragma unroll
+        for (int t = 0; t < NA3; t++) v[t] = cmulc(uns[t * NTH], nx[t]);
+        load_m(nx, pf);
+        if (pf.cnt > 0) advance(pf);
+        advance(cur);
+        if (g + 1 == cnt) load_n(cur);   // next chunk's u_n: the slots have just been read (in-order LSU)
+        if (act) {
+            Bfly<NA3>::run(v);
+#pragma unroll
+            for (int t = 0; t < NA3; t++) Xl[t * XP + j] = v[t];
+        }
+        __syncwarp();
+        if (act) {
+            cd *yrow = Y + (size_t)row * pitch + g * ng3;
+#pragma unroll
+            for (int a = 0; a < K1PT; a++) {
+                if (j + a * NB3 < NA3) {
+                    cd B[NB3];
+                    B[0] = Xl[(j + a * NB3) * XP];
+#pragma unroll
+                    for (int jj = 1; jj < NB3; jj++) B[jj] = h_mul(twb[a][jj], Xl[(j + a * NB3) * XP + jj]);
+                    cd o0, o1;
+                    PairSum<NB3>::run(B, o0, o1);
+                    if (oi0[a] >= 0) yrow[oi0[a]] = o0;
+                    if (oi1[a] >= 0) yrow[oi1[a]] = o1;
+                }
+            }
+        }
+        __syncwarp();
+        if (c != NCH - 1 || g + 1 != cnt) return;
+
+        // ---- last z iteration of the unit: y axis on its cnt * ng3 columns ------------------------------------------
+        __syncthreads();
+        {   // pass A in place: x = j2 pitch + (g, g3i); inputs at rows j2 + NB2 s, outputs k1 at the same rows
+            const int ntask = NB2 * pitch;
+            for (int x = tid; x < ntask; x += NTH) {
+                cd w[NA2];
+#pragma unroll
+                for (int s = 0; s < NA2; s++) w[s] = Y[x + s * ntask];
+                Bfly<NA2>::run(w);
+#pragma unroll
+                for (int s = 0; s < NA2; s++) Y[x + s * ntask] = w[s];
+            }
+        }
+        __syncthreads();
+        {   // pass B: out[g][o][g3i] = sum_j2 W_N2^(j2 f) A[j2 + NB2 (f mod NA2)][g][g3i]
+            int gg = yb_g0, r = yb_r0;
+            cd *Io = P.I + ((size_t)(p0 - P.p_begin) * P.N1 + j1) * nb2;
+            while (gg < cnt) {
+                const int oc = otab[r];
+                const int o = oc >> 16, col = oc & 0xffff;
+                int f = P.g2min + o;
+                if (f < 0) f += N2;
+                const int k1 = f % NA2;
+                const cd *src = Y + (size_t)(NB2 * k1) * pitch + gg * ng3 + col;
+                cd acc = src[0];
+                int ti = 0;
+#pragma unroll
+                for (int j2 = 1; j2 < NB2; j2++) {
+                    ti += f;
+                    if (ti >= N2) ti -= N2;
+                    acc = cfma(tw2s[ti], src[j2 * pitch], acc);
+                }
+                Io[(size_t)gg * P.N1 * nb2 + r] = acc;
+                r += NTH;
+                while (r >= nb2) { r -= nb2; gg++; }
+            }
+        }
+        __syncthreads();   // Y is rewritten by the next unit's z stage
+    };
+
+    while (cur.cnt > 0) {
+        step(nxA);
+        if (cur.cnt == 0) break;
+        step(nxB);
+    }
+}
+
+typedef void (*PdZyKernel)(const PdZyParams);

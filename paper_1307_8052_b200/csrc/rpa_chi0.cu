@@ -17,6 +17,7 @@
 #include "energy.cuh"
 #include "fft.cuh"
 #include "pair_density.cuh"
+#include "pair_density_zy.cuh"
 #include "paw.cuh"
 #include "rank_k.cuh"
 
@@ -195,6 +196,9 @@ struct rpa_chi0 {
     int RC, pd_threads, pd_nbuf;
     PdPlaneKernel pd_kernel = nullptr;
     size_t pd_smem;
+    PdZyKernel zy_kernel = nullptr;   // low-instruction-count z+y kernel (planes that fit one CTA), else pd_kernel
+    int zy_G = 1, zy_threads = 0, zy_ctas_per_sm = 1, n_sm = 148;
+    size_t zy_smem = 0;
     unsigned char *ws;
     // profiling
     bool prof = false;
@@ -265,9 +269,36 @@ int ntiles_lower(int n, int t) {
 //  several CTAs per SM (shared memory is small: no staging).
 //  run-time path: cp.async staging, two CTAs per SM preferred.
 // Returns false if even one z line per chunk does not fit.
+template <class C, class K>
+void try_zy(rpa_chi0 *h, K kernel, int G, int minb) {
+    const int ng2 = h->sp.gmax[1] - h->sp.gmin[1] + 1, ng3 = h->sp.gmax[2] - h->sp.gmin[2] + 1;
+    if (!C::box_ok(h->sp.gmin[2], ng3)) return;
+    const size_t smem = C::smem_bytes(ng2, ng3);
+    if (smem > 200 * 1024) return;
+    h->zy_kernel = kernel;
+    h->zy_G = G;
+    h->zy_threads = C::NTH;
+    h->zy_smem = smem;
+    h->zy_ctas_per_sm = (int)std::max<size_t>(1, std::min<size_t>((size_t)minb, (227 * 1024) / (smem + 1024)));
+}
+
+// Specialisations of the z+y kernel for the plane shapes of BASELINE.json configs[0..2] (G pairs per unit and CTAs
+// per SM tuned on B200: 8 warps per SM without spills beat 12 with); other shapes take the pd_plane kernels.
+void plan_zy_kernel(rpa_chi0 *h) {
+    const int N2 = h->grid[1], N3 = h->grid[2];
+    h->zy_kernel = nullptr;
+#define ZY(N3_, NA3_, N2_, NA2_, NW_, LPW_, G_, MINB_) \
+    try_zy<PdZy<N3_, NA3_, N2_, NA2_, NW_, LPW_, G_>>(h, pd_zy_kernel<N3_, NA3_, N2_, NA2_, NW_, LPW_, G_, MINB_>, G_, MINB_)
+    if (N2 == 60 && N3 == 64) ZY(64, 8, 60, 12, 4, 4, 4, 2);
+    else if (N2 == 24 && N3 == 24) ZY(24, 8, 24, 8, 3, 8, 4, 3);
+    else if (N2 == 16 && N3 == 16) ZY(16, 8, 16, 8, 1, 16, 4, 8);
+#undef ZY
+}
+
 bool plan_plane_kernel(rpa_chi0 *h) {
     const int N2 = h->grid[1], N3 = h->grid[2];
     const int ng3 = h->sp.gmax[2] - h->sp.gmin[2] + 1;
+    plan_zy_kernel(h);
     const int N3p = N3 + (N3 >> 3) + 1;
     const int nbuf = h->pz.npass >= 3 ? 2 : (h->pz.npass == 2 ? 1 : 0);
     h->pd_nbuf = nbuf;
@@ -390,6 +421,15 @@ int rpa_chi0_create(rpa_chi0_t **out, const int32_t grid[3], const double cell[9
     } while (0)
 
     CREATE_TRY(cudaFuncSetAttribute(h->pd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->pd_smem));
+    if (h->zy_kernel) {
+        CREATE_TRY(cudaFuncSetAttribute(h->zy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->zy_smem));
+        int dev = 0, per_sm = 0;
+        CREATE_TRY(cudaGetDevice(&dev));
+        CREATE_TRY(cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, dev));
+        CREATE_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, h->zy_kernel, h->zy_threads, h->zy_smem));
+        if (per_sm < 1) { delete h; return fail(RPA_ERR_CUDA, "rpa_chi0_create: pd_zy kernel does not fit an SM"); }
+        h->zy_ctas_per_sm = per_sm;
+    }
     CREATE_TRY(cudaFuncSetAttribute(rank_k_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, rk::Cfg<true>::SMEM_BYTES));
     CREATE_TRY(cudaFuncSetAttribute(rank_k_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, rk::Cfg<false>::SMEM_BYTES));
 
@@ -525,7 +565,22 @@ int rpa_chi0_add_kpoint(rpa_chi0_t *h, double kweight, int32_t n_occ, const void
             // S2 + S3: pair product, pruned 3-D FFT, sphere gather
             for (int p0 = 0; p0 < K; p0 += L.sub_pairs) {
                 const int pc = std::min(L.sub_pairs, K - p0);
-                {
+                if (h->zy_kernel) {
+                    StageTimer tm(h, 0, 1);
+                    PdZyParams P;
+                    P.psi_occ = (const cd *)psi_occ; P.psi_unocc = (const cd *)psi_unocc;
+                    P.I = h->ptr<cd>(L.I);
+                    P.tw3 = h->ptr<cd>(L.tw3); P.tw2 = h->ptr<cd>(L.tw2);
+                    P.N1 = N1;
+                    P.n0 = n0; P.mlen = mlen; P.m0 = m0;
+                    P.p_begin = p0; P.p_count = pc;
+                    P.n_units = pdzy_count_units(p0, pc, mlen, h->zy_G);
+                    P.g2min = sp.gmin[1]; P.ng2 = ng2; P.g3min = sp.gmin[2]; P.ng3 = ng3;
+                    // persistent 1-D grid: one CTA per resident slot, work items (unit, plane) dealt round-robin
+                    const int nctas = std::max(1, std::min(P.n_units * N1, h->n_sm * h->zy_ctas_per_sm));
+                    h->zy_kernel<<<nctas, h->zy_threads, h->zy_smem, st>>>(P);
+                    CUDA_TRY(cudaGetLastError());
+                } else {
                     StageTimer tm(h, 0, 1);
                     PdPlaneParams P;
                     P.psi_occ = (const cd *)psi_occ; P.psi_unocc = (const cd *)psi_unocc;

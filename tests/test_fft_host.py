@@ -1,0 +1,27 @@
+"""Host logic of the CUDA path: the register butterflies (radix 2-8, 12) and the mixed-radix Stockham passes of
+csrc/fft.cuh are __host__ __device__; tests/host/fft_host_check.cu runs them on the CPU against a direct DFT in
+long double (Eq. 12, P:L104-106 needs a forward transform with exp(-2 pi i jk/N))."""
+import os
+import shutil
+import subprocess
+
+import pytest
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+
+
+@pytest.mark.skipif(not (os.path.exists(NVCC) or shutil.which("nvcc")), reason="nvcc not available")
+def test_butterflies_and_lines_match_direct_dft(tmp_path):
+    exe = str(tmp_path / "fft_host_check")
+    src = os.path.join(HERE, "host", "fft_host_check.cu")
+    r = subprocess.run([NVCC, "-O1", "-std=c++17", "--extended-lambda", "-o", exe, src], capture_output=True, text=True)
+    assert r.returncode == 0, r.stderr
+    out = subprocess.run([exe], capture_output=True, text=True, check=True).stdout
+    rows = [ln.split() for ln in out.strip().splitlines()]
+    assert len(rows) == 8 + 13
+    for kind, n, err in rows:
+        err = float(err)
+        assert err >= 0.0, (kind, n)
+        tol = 1e-14 * max(4.0, float(n))
+        assert err < tol, (kind, n, err)
