@@ -185,7 +185,7 @@ def run_ours(args, cfg):
     out = torch.empty((ng, ng), dtype=torch.complex128, device=dev)
     S = B.rpa_chi0_accumulators(h) if world > 1 else None
 
-    def step(from_host):
+    def step(from_host, tail_ms=None):
         B.rpa_chi0_reset(h)
         nb = 0
         for _ in my_k:
@@ -196,9 +196,19 @@ def run_ours(args, cfg):
                                       kd.f_unocc, npj, devt["P_occ"], devt["P_unocc"], Qd, R)
         if world > 1:
             sharding.allreduce_accumulators(S)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)] if tail_ms is not None else None
+        if ev:
+            ev[0].record()
         for i in range(cfg.n_omega):
             B.rpa_chi0_get(h, i, out)
+        if ev:
+            ev[1].record()
         ec, e = B.rpa_ec_q(h, v)  # blocks; reads E_c(q), e(omega) back to the host
+        if ev:
+            ev[2].record()
+            ev[2].synchronize()
+            tail_ms[0] += ev[0].elapsed_time(ev[1])
+            tail_ms[1] += ev[1].elapsed_time(ev[2])
         return nb, ec, e
 
     def barrier():
@@ -206,7 +216,7 @@ def run_ours(args, cfg):
             dist.barrier()
         torch.cuda.synchronize()
 
-    def timed(from_host, steps, warmup):
+    def timed(from_host, steps, warmup, tail_ms=None):
         for _ in range(warmup):
             step(from_host)
         barrier()
@@ -214,7 +224,7 @@ def run_ours(args, cfg):
         e0.record()
         nb = 0
         for _ in range(steps):
-            nb, ec, e = step(from_host)
+            nb, ec, e = step(from_host, tail_ms)
         e1.record()
         barrier()
         ms = e0.elapsed_time(e1)
@@ -239,7 +249,8 @@ def run_ours(args, cfg):
     launches0 = B.rpa_chi0_launch_count(h)
     if rank == 0:
         sampler.start()
-    ms_step, _, ec_dev = timed(False, args.steps, 0)
+    tail_ms = [0.0, 0.0]   # rpa_chi0_get x n_omega, rpa_ec_q (CUDA events on the handle's stream, inside the timed steps)
+    ms_step, _, ec_dev = timed(False, args.steps, 0, tail_ms)
     clocks = sampler.stop() if rank == 0 else None
     launches = B.rpa_chi0_launch_count(h) - launches0
     stage_ms, stage_n = B.rpa_chi0_stage_times(h)
@@ -283,6 +294,7 @@ def run_ours(args, cfg):
                          "flops_per_launch": rk_flops, "ms_per_launch": rk_ms, "launches": rk_launches,
                          "share_of_step": float(stage_ms[4]) / args.steps / ms_step},
             "stages": {"ms_per_step": {n: float(t) / args.steps for n, t in zip(B.STAGE_NAMES, stage_ms)},
+                       "get_all_omega_ms": tail_ms[0] / args.steps, "ec_q_ms": tail_ms[1] / args.steps,
                        "sum_ms": total_stage,
                        "pair_density": {"bound": "hbm", "achieved": pd_gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                                         "frac": pd_gbs / peaks["hbm_gbs"], "peak_kind": peak_kind,

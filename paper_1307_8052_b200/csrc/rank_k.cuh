@@ -23,20 +23,23 @@ namespace rk {
 constexpr int T = 64;        // tile edge (complex elements)
 constexpr int KC = 16;       // pairs per stage
 constexpr int STAGES = 5;
-constexpr int NW = 2;        // frequencies per CTA
-constexpr int CONSUMER_WARPS = 8;
-constexpr int THREADS = (CONSUMER_WARPS + 1) * 32;   // warp 8 is the TMA producer
 constexpr int PITCH = T * 16 + 64;               // bytes per pair row in shared memory (= 64 mod 128, see below)
 constexpr int TILE_BYTES = KC * PITCH;           // 17408
-constexpr int W_BYTES = NW * KC * 8;             // 256
-// SHARED_N = true : both frequencies of a CTA read the same N tiles (the chi0 accumulation), 5 stages.
-// SHARED_N = false: every frequency has its own N (the Cholesky trailing update of rpa_ec_q, where N is the
-//                   transposed panel of that frequency's matrix): two tile sets per stage, 3 stages.
+// SHARED_N = true : the chi0 accumulation: 2 frequencies per CTA read the same N tiles; 8 consumer warps + the TMA
+//                   producer warp, 5 stages, one CTA per SM (K is thousands of pairs: the ring never drains).
+// SHARED_N = false: the Cholesky trailing update of rpa_ec_q: every frequency has its own N (the transposed panel of
+//                   that frequency's matrix) and K is one panel (32 pairs), so a CTA is mostly prologue (TMA round
+//                   trip) and epilogue (read-modify-write of its tile): 1 frequency per CTA, 4 consumer warps,
+//                   2 stages (= the whole panel), two CTAs per SM so that one computes while the other loads / stores.
 template <bool SHARED_N>
 struct Cfg {
-    static constexpr int NSTAGES = SHARED_N ? STAGES : 3;
-    static constexpr int TILE_SETS = SHARED_N ? 1 : NW;
-    static constexpr int STAGE_BYTES = 2 * TILE_SETS * TILE_BYTES + W_BYTES;
+    static constexpr int NW = SHARED_N ? 2 : 1;               // frequencies per CTA
+    static constexpr int CONSUMER_WARPS = 4 * NW;
+    static constexpr int THREADS = (CONSUMER_WARPS + 1) * 32; // the last warp is the TMA producer
+    static constexpr int MIN_CTAS = SHARED_N ? 1 : 2;
+    static constexpr int NSTAGES = SHARED_N ? STAGES : 2;
+    static constexpr int W_BYTES = NW * KC * 8;
+    static constexpr int STAGE_BYTES = 2 * TILE_BYTES + W_BYTES;
     static constexpr int SMEM_BYTES = NSTAGES * STAGE_BYTES + 2 * NSTAGES * 8;
 };
 }  // namespace rk
@@ -61,15 +64,16 @@ __global__ void weights_kernel(double *__restrict__ w, int64_t ldw, int K, int K
 
 // Nb[Kpad][ldn] (rows >= K are zero; frequency iw reads Nb + iw*strideN, strideN = 0 when SHARED_N), w[n_omega][ldw],
 // S[n_omega][ng][ldS] (lower triangle accumulated).  Only rows / columns g >= g0 are touched (g0 % 1 == 0; tiles
-// start at g0).  Kpad % KC == 0.  grid = (ntiles_lower(ng - g0), ceil(n_omega / 2)).
+// start at g0).  Kpad % KC == 0.  grid = (ntiles_lower(ng - g0), ceil(n_omega / Cfg::NW)).
 template <bool SHARED_N>
-__global__ void __launch_bounds__(rk::THREADS, 1)
+__global__ void __launch_bounds__(rk::Cfg<SHARED_N>::THREADS, rk::Cfg<SHARED_N>::MIN_CTAS)
 rank_k_kernel(const cd *__restrict__ Nb, int64_t ldn, int64_t strideN, int Kpad, const double *__restrict__ w,
               int64_t ldw, cd *__restrict__ S, int64_t ldS, int64_t strideS, int ng, int g0, int n_omega) {
     using namespace rk;
     constexpr int STAGES = Cfg<SHARED_N>::NSTAGES;
     constexpr int STAGE_BYTES = Cfg<SHARED_N>::STAGE_BYTES;
-    constexpr int W_OFF = 2 * Cfg<SHARED_N>::TILE_SETS * TILE_BYTES;
+    constexpr int NW = Cfg<SHARED_N>::NW, CONSUMER_WARPS = Cfg<SHARED_N>::CONSUMER_WARPS, THREADS = Cfg<SHARED_N>::THREADS;
+    constexpr int W_OFF = 2 * TILE_BYTES;
     extern __shared__ __align__(128) unsigned char rk_smem[];
     uint64_t *full = reinterpret_cast<uint64_t *>(rk_smem + STAGES * STAGE_BYTES);
     uint64_t *empty = full + STAGES;
@@ -85,7 +89,7 @@ rank_k_kernel(const cd *__restrict__ Nb, int64_t ldn, int64_t strideN, int Kpad,
     const int om0 = blockIdx.y * NW;
     const int n_om = min(NW, n_omega - om0);
     const uint32_t rowbytes = (uint32_t)min(T, ng - row0) * 16u, colbytes = (uint32_t)min(T, ng - col0) * 16u;
-    const uint32_t stage_tx = KC * (rowbytes + colbytes) * (SHARED_N ? 1u : (uint32_t)n_om) + (uint32_t)n_om * KC * 8u;
+    const uint32_t stage_tx = KC * (rowbytes + colbytes) + (uint32_t)n_om * KC * 8u;
 
     // zero the ring once so that the never-copied tail columns of edge tiles hold finite numbers
     for (int i = tid; i < STAGES * STAGE_BYTES / 16; i += THREADS)
@@ -110,15 +114,9 @@ rank_k_kernel(const cd *__restrict__ Nb, int64_t ldn, int64_t strideN, int Kpad,
             if (lane == 0) mbar_arrive_expect_tx(&full[s], stage_tx);
             __syncwarp();
             const size_t krow = (size_t)it * KC + (lane & 15);
-#pragma unroll
-            for (int ts = 0; ts < Cfg<SHARED_N>::TILE_SETS; ts++) {
-                if (ts < n_om) {
-                    const cd *Nw = Nb + (size_t)(om0 + ts) * strideN + krow * ldn;
-                    unsigned char *dst = st + ts * 2 * TILE_BYTES;
-                    if (lane < 16) bulk_g2s(dst + lane * PITCH, Nw + row0, rowbytes, &full[s]);
-                    else bulk_g2s(dst + TILE_BYTES + (lane - 16) * PITCH, Nw + col0, colbytes, &full[s]);
-                }
-            }
+            const cd *Nw = Nb + (size_t)om0 * strideN + krow * ldn;   // strideN = 0 when SHARED_N
+            if (lane < 16) bulk_g2s(st + lane * PITCH, Nw + row0, rowbytes, &full[s]);
+            else bulk_g2s(st + TILE_BYTES + (lane - 16) * PITCH, Nw + col0, colbytes, &full[s]);
             if (lane < n_om)
                 bulk_g2s(st + W_OFF + lane * KC * 8, w + (size_t)(om0 + lane) * ldw + (size_t)it * KC, KC * 8, &full[s]);
         }
@@ -132,15 +130,23 @@ rank_k_kernel(const cd *__restrict__ Nb, int64_t ldn, int64_t strideN, int Kpad,
     // barriers moving
     const bool active = (wsel < n_om) && !(ti == tj && coloff > rowoff);
 
+    if (!SHARED_N && active) {   // short K: pull this warp's part of the accumulator tile towards L2 while the K loop runs
+        const cd *Sp = S + (size_t)(om0 + wsel) * strideS;
+#pragma unroll
+        for (int i = 0; i < 4; i++) {
+            const int r = row0 + rowoff + i * 8 + g, cc = col0 + coloff + kq * 8;
+            if (r < ng && cc < ng && cc <= r) asm volatile("prefetch.global.L2 [%0];" ::"l"(Sp + (size_t)r * ldS + cc));
+        }
+    }
+
     double re[4][4][2], im[4][4][2];
 #pragma unroll
     for (int mi = 0; mi < 4; mi++)
 #pragma unroll
         for (int ni = 0; ni < 4; ni++) re[mi][ni][0] = re[mi][ni][1] = im[mi][ni][0] = im[mi][ni][1] = 0.0;
 
-    const uint32_t set_off = SHARED_N ? 0u : (uint32_t)wsel * 2 * TILE_BYTES;
-    const uint32_t a_off = set_off + pp * PITCH + (rowoff + g) * 16;
-    const uint32_t b_off = set_off + TILE_BYTES + pp * PITCH + (coloff + g) * 16 + c * 8;
+    const uint32_t a_off = pp * PITCH + (rowoff + g) * 16;
+    const uint32_t b_off = TILE_BYTES + pp * PITCH + (coloff + g) * 16 + c * 8;
     const uint32_t w_off = W_OFF + (wsel * KC + pp) * 8;
     const uint32_t sign_hi = (uint32_t)c << 31;   // A'[2p+1] = -re: flip the sign bit on odd k lanes (ALU pipe, not FP64)
 
@@ -179,23 +185,54 @@ rank_k_kernel(const cd *__restrict__ Nb, int64_t ldn, int64_t strideN, int Kpad,
 
     if (!active) return;
     cd *Sw = S + (size_t)(om0 + wsel) * strideS;
+    if constexpr (SHARED_N) {
+        // long K: the epilogue is < 1 % of the CTA; plain read-modify-write keeps the register count of the K loop
 #pragma unroll
-    for (int mi = 0; mi < 4; mi++) {
-        const int r = row0 + rowoff + mi * 8 + g;
-        if (r >= ng) continue;
+        for (int mi = 0; mi < 4; mi++) {
+            const int r = row0 + rowoff + mi * 8 + g;
+            if (r >= ng) continue;
 #pragma unroll
-        for (int ni = 0; ni < 4; ni++) {
-            const int cc = col0 + coloff + ni * 8 + 2 * kq;
+            for (int ni = 0; ni < 4; ni++) {
+                const int cc = col0 + coloff + ni * 8 + 2 * kq;
 #pragma unroll
-            for (int e = 0; e < 2; e++) {
-                const int col = cc + e;
-                if (col < ng && col <= r) {
-                    cd *ptr = Sw + (size_t)r * ldS + col;
-                    cd v = *ptr;
-                    v.x += re[mi][ni][e];
-                    v.y += im[mi][ni][e];
-                    *ptr = v;
+                for (int e = 0; e < 2; e++) {
+                    const int col = cc + e;
+                    if (col < ng && col <= r) {
+                        cd *ptr = Sw + (size_t)r * ldS + col;
+                        cd v = *ptr;
+                        v.x += re[mi][ni][e];
+                        v.y += im[mi][ni][e];
+                        *ptr = v;
+                    }
                 }
+            }
+        }
+    } else {
+        // short K: the read-modify-write is a large part of the CTA: all loads of an 8-row group are issued before
+        // its stores (a CTA owns its tile, but the compiler cannot know that the pointers do not alias)
+#pragma unroll
+        for (int mi = 0; mi < 4; mi++) {
+            const int r = row0 + rowoff + mi * 8 + g;
+            if (r >= ng) continue;
+            cd *rowp = Sw + (size_t)r * ldS;
+            cd v[4][2];
+#pragma unroll
+            for (int ni = 0; ni < 4; ni++) {
+                const int cc = col0 + coloff + ni * 8 + 2 * kq;
+#pragma unroll
+                for (int e = 0; e < 2; e++)
+                    if (cc + e < ng && cc + e <= r) v[ni][e] = rowp[cc + e];
+            }
+#pragma unroll
+            for (int ni = 0; ni < 4; ni++) {
+                const int cc = col0 + coloff + ni * 8 + 2 * kq;
+#pragma unroll
+                for (int e = 0; e < 2; e++)
+                    if (cc + e < ng && cc + e <= r) {
+                        v[ni][e].x += re[mi][ni][e];
+                        v[ni][e].y += im[mi][ni][e];
+                        rowp[cc + e] = v[ni][e];
+                    }
             }
         }
     }

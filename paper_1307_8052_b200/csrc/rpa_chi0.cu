@@ -625,8 +625,8 @@ int rpa_chi0_add_kpoint(rpa_chi0_t *h, double kweight, int32_t n_occ, const void
             // S6: rank-K update of every frequency
             {
                 StageTimer tm(h, 4, 1);
-                rank_k_kernel<true><<<dim3(ntiles_lower(ng, rk::T), (h->n_omega + rk::NW - 1) / rk::NW), rk::THREADS,
-                                      rk::Cfg<true>::SMEM_BYTES, st>>>(
+                rank_k_kernel<true><<<dim3(ntiles_lower(ng, rk::T), (h->n_omega + rk::Cfg<true>::NW - 1) / rk::Cfg<true>::NW),
+                                      rk::Cfg<true>::THREADS, rk::Cfg<true>::SMEM_BYTES, st>>>(
                     Nbuf, L.ldn, 0, Kpad, w, L.ldw, h->ptr<cd>(L.S), L.ldS, (int64_t)ng * L.ldS, ng, 0, h->n_omega);
                 CUDA_TRY(cudaGetLastError());
             }
@@ -676,7 +676,7 @@ int rpa_ec_q(rpa_chi0_t *h, const double *v_G, double *ec_ha, double *e_omega) {
             if (rest > 0) {
                 chol_panel_kernel<<<dim3((rest + 127) / 128, nm), 128, 0, st>>>(M, ng, k0, h->ptr<cd>(L.Lt), L.ldn);
                 // trailing update M[g][g'] -= sum_t L[g][t] conj(L[g'][t]), g >= g' >= k0 + 32, on the DMMA path
-                rank_k_kernel<false><<<dim3(ntiles_lower(rest, rk::T), (nm + rk::NW - 1) / rk::NW), rk::THREADS,
+                rank_k_kernel<false><<<dim3(ntiles_lower(rest, rk::T), nm), rk::Cfg<false>::THREADS,
                                        rk::Cfg<false>::SMEM_BYTES, st>>>(
                     h->ptr<cd>(L.Lt), L.ldn, (int64_t)CH_NB * L.ldn, CH_NB, h->ptr<double>(L.wneg), CH_NB, M, ng,
                     (int64_t)ng * ng, ng, k0 + CH_NB, nm);
