@@ -307,22 +307,58 @@ def rpa_probe_fp64_tensor_peak(device="cuda:0") -> float:
 
 # ---- host-buffer convenience on top of the calls above (the end-to-end path bench.py times) ------------------
 
-def add_kpoint_host(h: Handle, kd, n_proj=None, Q_dev=None, R_cart=None, pinned=None, kweight=None):
-    """Copy one k-point's host arrays (workload.KPointData) to the device and add it.  `pinned` may hold
-    pre-pinned host tensors keyed like the KPointData fields; returns the bytes copied host->device."""
+def add_kpoint_host(h: Handle, kd, n_proj=None, Q_dev=None, R_cart=None, pinned=None, kweight=None, chunk_bands=128):
+    """Copy one k-point's host arrays (workload.KPointData) to the device and add it; returns the bytes copied
+    host->device.  `pinned` may hold pre-pinned host tensors keyed like the KPointData fields.
+
+    The unoccupied orbitals (the bulk of the bytes) are uploaded in slices of `chunk_bands` bands on a side stream
+    into two alternating device buffers, and every slice is added with its own rpa_chi0_add_kpoint call (the
+    accumulation is additive over any split of the bands), so the copy of slice i+1 overlaps the
+    kernels of slice i.  Only marshalling happens here: all arithmetic is in the library."""
     torch = _torch()
+    dev = h.device
 
-    def up(name):
-        src = pinned[name] if pinned is not None else torch.from_numpy(getattr(kd, name))
-        return src.to(h.device, non_blocking=True)
+    def host(name):
+        return pinned[name] if pinned is not None else torch.from_numpy(getattr(kd, name))
 
-    psi_o, psi_u = up("psi_occ"), up("psi_unocc")
-    nbytes = psi_o.numel() * 16 + psi_u.numel() * 16
-    if n_proj is not None and len(n_proj):
-        P_o, P_u = up("P_occ"), up("P_unocc")
-        nbytes += P_o.numel() * 16 + P_u.numel() * 16
-    else:
+    kw = kd.kweight if kweight is None else kweight
+    have_paw = n_proj is not None and len(n_proj) > 0
+    main = h.stream
+    with torch.cuda.device(dev), torch.cuda.stream(main):
+        psi_o = host("psi_occ").to(dev, non_blocking=True)
+        nbytes = psi_o.numel() * 16
         P_o = P_u = None
-    rpa_chi0_add_kpoint(h, kd.kweight if kweight is None else kweight, psi_o, psi_u, kd.eps_occ, kd.eps_unocc, kd.f_occ, kd.f_unocc, n_proj, P_o, P_u,
-                        Q_dev, R_cart)
+        if have_paw:
+            P_o, P_u = host("P_occ").to(dev, non_blocking=True), host("P_unocc").to(dev, non_blocking=True)
+            nbytes += P_o.numel() * 16 + P_u.numel() * 16
+        src = host("psi_unocc")
+        n_un = int(src.shape[0])
+        nbytes += src.numel() * 16
+        if n_un <= chunk_bands or not src.is_pinned():
+            psi_u = src.to(dev, non_blocking=True)
+            rpa_chi0_add_kpoint(h, kw, psi_o, psi_u, kd.eps_occ, kd.eps_unocc, kd.f_occ, kd.f_unocc, n_proj, P_o, P_u,
+                                Q_dev, R_cart)
+            return nbytes
+        side = getattr(h, "_copy_stream", None)
+        if side is None:
+            side = h._copy_stream = torch.cuda.Stream(device=dev)
+        bufs = [torch.empty((chunk_bands,) + tuple(src.shape[1:]), dtype=src.dtype, device=dev) for _ in range(2)]
+        free = [None, None]   # event: the kernels that read this buffer have been enqueued and finished
+        side.wait_stream(main)   # the buffers were allocated on the main stream
+        for i, m0 in enumerate(range(0, n_un, chunk_bands)):
+            m1 = min(m0 + chunk_bands, n_un)
+            b = i & 1
+            with torch.cuda.stream(side):
+                if free[b] is not None:
+                    side.wait_event(free[b])
+                bufs[b][:m1 - m0].copy_(src[m0:m1], non_blocking=True)
+                ready = torch.cuda.Event()
+                ready.record(side)
+            main.wait_event(ready)
+            rpa_chi0_add_kpoint(h, kw, psi_o, bufs[b][:m1 - m0], kd.eps_occ, kd.eps_unocc[m0:m1], kd.f_occ,
+                                kd.f_unocc[m0:m1], n_proj, P_o, None if P_u is None else P_u[m0:m1].contiguous(),
+                                Q_dev, R_cart)
+            free[b] = torch.cuda.Event()
+            free[b].record(main)
+        side.wait_stream(main)   # the buffers may be released once the main stream has passed this point
     return nbytes

@@ -171,3 +171,28 @@ def test_config1_full_size_bench_configuration():
     frequencies (every element of Eq. 17 is an independent sum); E_c(q) is checked by the eigenvalue route."""
     cfg = W.CONFIGS[1]
     _big_config_slice(cfg, occ=None, unocc=None, n_sample=72, k_list=(0,), device_resident=True)
+
+
+def test_pipelined_host_upload_matches_single_call():
+    """binding.add_kpoint_host with pinned inputs uploads the unoccupied bands in slices on a side stream and adds
+    every slice with its own call; the result must equal the one-call result (additivity) to rounding."""
+    import torch
+    from paper_1307_8052_b200 import binding as B
+    cfg = W.CONFIGS[0]
+    kd = W.kpoint(cfg, 0)
+    a, _, _, _ = gpu_run(cfg, [kd], True, 0, want_ec=False)
+    om, wt = W.omega_grid(cfg.n_omega)
+    h = B.rpa_chi0_create(cfg.grid, cfg.cell, cfg.q_red, W.tuned_ecut(cfg), om, wt, 0, int(cfg.n_proj.sum()), "cuda:0")
+    try:
+        g, K2 = B.rpa_chi0_gvectors(h)
+        Qd = torch.from_numpy(W.paw_Q(cfg, K2)).to("cuda:0")
+        pinned = {k: torch.from_numpy(getattr(kd, k)).pin_memory() for k in ("psi_occ", "psi_unocc", "P_occ", "P_unocc")}
+        for _ in range(2):   # twice: the alternating buffers and their events are reused
+            B.rpa_chi0_reset(h)
+            nb = B.add_kpoint_host(h, kd, cfg.n_proj, Qd, W.atom_positions(cfg), pinned=pinned, chunk_bands=5)
+            assert nb == sum(t.numel() * 16 for t in pinned.values())
+            for i in range(cfg.n_omega):
+                b = B.rpa_chi0_get(h, i).cpu().numpy()
+                assert rel_fro(b, a[i]) <= 1e-12
+    finally:
+        h.close()
