@@ -404,45 +404,55 @@ static inline PdPlaneChoice pd_plane_pick(int N2, int N3) {
 
 // x axis + gather.  Thread (pair, b) with b = g2i*ng3 + g3i a column of the pruned box; tw1[t] = exp(-2 pi i t/N1).
 // box2s[g1i*nb2 + b] = index of (g1min+g1i, ., .) in the sphere list, or -1 outside the sphere.
-#define PD_G1_BLOCK 8
+// The (ng1 x N1) DFT matrix of the kept frequencies is tabulated in shared memory ([j1][g1i], read as a warp-wide
+// broadcast); a thread keeps PD_G1_BLOCK accumulators, so a sphere with ng1 <= PD_G1_BLOCK reads I once, and the
+// loads of four x planes are issued together to cover the L2 latency.
+// Dynamic shared memory: N1 * PD_G1_BLOCK * sizeof(cd).
+#define PD_G1_BLOCK 16
 __global__ void __launch_bounds__(128) pd_xaxis_kernel(const cd *__restrict__ I, cd *__restrict__ Nbuf, int64_t ldn,
                                                       const cd *__restrict__ tw1, const int32_t *__restrict__ box2s,
                                                       int N1, int nb2, int g1min, int ng1, int p_begin, double inv_n) {
     extern __shared__ __align__(16) unsigned char pd_smem[];
-    cd *tws = reinterpret_cast<cd *>(pd_smem);
-    for (int i = threadIdx.x; i < N1; i += blockDim.x) tws[i] = tw1[i];
-    __syncthreads();
+    cd *twt = reinterpret_cast<cd *>(pd_smem);   // [j1][t]
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= nb2) return;
+    const bool act = b < nb2;
     const int pl = blockIdx.y;
-    const cd *Ip = I + (size_t)pl * N1 * nb2 + b;
+    const cd *Ip = I + (size_t)pl * N1 * nb2 + (act ? b : 0);
     cd *out = Nbuf + (size_t)(p_begin + pl) * ldn;
     for (int gc = 0; gc < ng1; gc += PD_G1_BLOCK) {
-        cd acc[PD_G1_BLOCK];
-        int step[PD_G1_BLOCK], idx[PD_G1_BLOCK];
-#pragma unroll
-        for (int t = 0; t < PD_G1_BLOCK; t++) {
-            acc[t] = cmake(0.0, 0.0);
-            int g1 = g1min + gc + t;
-            g1 %= N1;
+        __syncthreads();
+        for (int i = threadIdx.x; i < N1 * PD_G1_BLOCK; i += blockDim.x) {
+            const int j1 = i / PD_G1_BLOCK, t = i - j1 * PD_G1_BLOCK;
+            int g1 = (g1min + gc + t) % N1;
             if (g1 < 0) g1 += N1;
-            step[t] = g1;
-            idx[t] = 0;
+            twt[i] = (gc + t < ng1) ? tw1[(int)(((int64_t)g1 * j1) % N1)] : cmake(0.0, 0.0);
         }
-        for (int j1 = 0; j1 < N1; j1++) {
-            const cd x = Ip[(size_t)j1 * nb2];
+        __syncthreads();
+        cd acc[PD_G1_BLOCK];
+#pragma unroll
+        for (int t = 0; t < PD_G1_BLOCK; t++) acc[t] = cmake(0.0, 0.0);
+        if (act) {
+            int j1 = 0;
+            for (; j1 + 4 <= N1; j1 += 4) {
+                cd x[4];
+#pragma unroll
+                for (int u = 0; u < 4; u++) x[u] = Ip[(size_t)(j1 + u) * nb2];
+#pragma unroll
+                for (int u = 0; u < 4; u++)
+#pragma unroll
+                    for (int t = 0; t < PD_G1_BLOCK; t++) acc[t] = cfma(twt[(j1 + u) * PD_G1_BLOCK + t], x[u], acc[t]);
+            }
+            for (; j1 < N1; j1++) {
+                const cd x = Ip[(size_t)j1 * nb2];
+#pragma unroll
+                for (int t = 0; t < PD_G1_BLOCK; t++) acc[t] = cfma(twt[j1 * PD_G1_BLOCK + t], x, acc[t]);
+            }
 #pragma unroll
             for (int t = 0; t < PD_G1_BLOCK; t++) {
-                acc[t] = cfma(tws[idx[t]], x, acc[t]);
-                idx[t] += step[t];
-                if (idx[t] >= N1) idx[t] -= N1;
-            }
-        }
-#pragma unroll
-        for (int t = 0; t < PD_G1_BLOCK; t++) {
-            if (gc + t < ng1) {
-                const int s = box2s[(size_t)(gc + t) * nb2 + b];
-                if (s >= 0) out[s] = cscale(inv_n, acc[t]);
+                if (gc + t < ng1) {
+                    const int s = box2s[(size_t)(gc + t) * nb2 + b];
+                    if (s >= 0) out[s] = cscale(inv_n, acc[t]);
+                }
             }
         }
     }

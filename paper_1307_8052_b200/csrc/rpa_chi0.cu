@@ -421,6 +421,11 @@ int rpa_chi0_create(rpa_chi0_t **out, const int32_t grid[3], const double cell[9
     } while (0)
 
     CREATE_TRY(cudaFuncSetAttribute(h->pd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->pd_smem));
+    {
+        const size_t xs = (size_t)grid[0] * PD_G1_BLOCK * sizeof(cd);   // DFT table of pd_xaxis_kernel
+        if (xs > 220 * 1024) { delete h; return fail(RPA_ERR_UNSUPPORTED, "rpa_chi0_create: N1 = %d too large for the x-axis table", grid[0]); }
+        if (xs > 48 * 1024) CREATE_TRY(cudaFuncSetAttribute(pd_xaxis_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)xs));
+    }
     if (h->zy_kernel) {
         CREATE_TRY(cudaFuncSetAttribute(h->zy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->zy_smem));
         int dev = 0, per_sm = 0;
@@ -597,7 +602,7 @@ int rpa_chi0_add_kpoint(rpa_chi0_t *h, double kweight, int32_t n_occ, const void
                 }
                 {
                     StageTimer tm(h, 1, 1);
-                    pd_xaxis_kernel<<<dim3((nb2 + 127) / 128, pc), 128, N1 * sizeof(cd), st>>>(
+                    pd_xaxis_kernel<<<dim3((nb2 + 127) / 128, pc), 128, (size_t)N1 * PD_G1_BLOCK * sizeof(cd), st>>>(
                         h->ptr<cd>(L.I), Nbuf, L.ldn, h->ptr<cd>(L.tw1), h->ptr<int32_t>(L.box2s), N1, nb2, sp.gmin[0], ng1, p0, inv_n);
                     CUDA_TRY(cudaGetLastError());
                 }
