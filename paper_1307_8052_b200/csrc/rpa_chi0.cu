@@ -675,17 +675,18 @@ int rpa_ec_q(rpa_chi0_t *h, const double *v_G, double *ec_ha, double *e_omega) {
         ec_trace_kernel<<<nm, 256, 0, st>>>(S + (size_t)iw0 * strideS, L.ldS, strideS, ng, scale, d_v, d_tr);
         h->launches += 2;
         for (int k0 = 0; k0 < ng; k0 += CH_NB) {
-            chol_diag_kernel<<<nm, dim3(CH_NB, CH_NB), 0, st>>>(M, ng, k0, d_flag, d_ld);
-            h->launches += 1;
             const int rest = ng - (k0 + CH_NB);
+            // diagonal block (factored redundantly by every CTA) + panel solve in one launch
+            chol_panel_kernel<<<dim3(std::max(1, (rest + 127) / 128), nm), 128, 0, st>>>(M, ng, k0, h->ptr<cd>(L.Lt), L.ldn,
+                                                                                     d_flag, d_ld);
+            h->launches += 1;
             if (rest > 0) {
-                chol_panel_kernel<<<dim3((rest + 127) / 128, nm), 128, 0, st>>>(M, ng, k0, h->ptr<cd>(L.Lt), L.ldn);
                 // trailing update M[g][g'] -= sum_t L[g][t] conj(L[g'][t]), g >= g' >= k0 + 32, on the DMMA path
                 rank_k_kernel<false><<<dim3(ntiles_lower(rest, rk::T), nm), rk::Cfg<false>::THREADS,
                                        rk::Cfg<false>::SMEM_BYTES, st>>>(
                     h->ptr<cd>(L.Lt), L.ldn, (int64_t)CH_NB * L.ldn, CH_NB, h->ptr<double>(L.wneg), CH_NB, M, ng,
                     (int64_t)ng * ng, ng, k0 + CH_NB, nm);
-                h->launches += 2;
+                h->launches += 1;
             }
         }
         CUDA_TRY(cudaGetLastError());
