@@ -20,49 +20,88 @@
 
 #define PDZY_MAXK1 4   // k1 values per z pass-B thread: ceil(NA3 / NB3)
 
-// z pass B for a box inside [-NA, NA): k1 keeps at most the two frequencies g = k1 (>= 0) and g = k1 - NA (< 0), and
-// W_N^(j (k1 - NA)) = W_N^(j k1) conj(W_NB^j): with B[j] = W_N^(j k1) A_j[k1],
-//   o0 = sum_j B[j]   (g = k1),      o1 = sum_j conj(W_NB^j) B[j]   (g = k1 - NA).
-template <int NB>
-struct PairSum {
-    __device__ __forceinline__ static void run(const cd *B, cd &o0, cd &o1) {
-        o0 = B[0];
-        o1 = B[0];
-#pragma unroll
-        for (int j = 1; j < NB; j++) {
-            double sn, cs;
-            sincospi(2.0 * j / NB, &sn, &cs);   // folded at compile time (j, NB constant)
-            o0 = cadd(o0, B[j]);
-            o1 = cfma(make_double2(cs, sn), B[j], o1);
+// cos / sin of 2 pi num / den as compile-time constants (Taylor series in long double after reduction to
+// [-pi, pi]; error < 1e-18): the pruned pass-B sums below then multiply by immediates / constant-bank operands.
+__host__ __device__ constexpr long double pdzy_angle(int num, int den) {
+    int r = num % den;
+    if (r < 0) r += den;
+    if (2 * r > den) r -= den;
+    return 2.0L * 3.14159265358979323846264338327950288L * (long double)r / (long double)den;
+}
+__host__ __device__ constexpr double pdzy_cos(int num, int den) {
+    const long double x = pdzy_angle(num, den);
+    long double term = 1.0L, sum = 1.0L;
+    for (int k = 1; k <= 24; k++) {
+        term *= -x * x / (long double)((2 * k - 1) * (2 * k));
+        sum += term;
+    }
+    return (double)sum;
+}
+__host__ __device__ constexpr double pdzy_sin(int num, int den) {
+    const long double x = pdzy_angle(num, den);
+    long double term = x, sum = x;
+    for (int k = 1; k <= 24; k++) {
+        term *= -x * x / (long double)((2 * k) * (2 * k + 1));
+        sum += term;
+    }
+    return (double)sum;
+}
+
+// z pass B: with N = NA NB and x[j] = W_N^(j k1) A_j[k1], the frequencies f = k1 + NA d kept by the box are
+//   out[d - DLO] = sum_{j < NB} W_NB^(j d) x[j],   d = DLO .. DHI   (a pruned NB-point DFT).
+// For even NB halves first (W_NB^((j + NB/2) d) = (-1)^d W_NB^(j d)): e = x_lo + x_hi feeds even d, f = x_lo - x_hi odd d; then
+// +d and -d share the cosine and sine sums P = sum cos(2 pi j d / NB) s_j, Q = sum sin(2 pi j d / NB) s_j:
+//   out[+d] = P - i Q,  out[-d] = P + i Q.
+template <int NB, int DLO, int DHI>
+struct PrunedDft {
+    static_assert(DLO <= 0 && DHI >= 0, "pruned DFT");
+    static constexpr bool EVEN = (NB % 2 == 0);
+    static constexpr int H = EVEN ? NB / 2 : NB;   // terms per sum
+    static constexpr int ADMAX = (-DLO > DHI) ? -DLO : DHI;
+    template <int AD, int J>
+    __device__ __forceinline__ static void acc(const cd *s, cd &Pv, cd &Qv) {
+        if constexpr (J < H) {
+            constexpr double c = pdzy_cos(J * AD, NB), sn = pdzy_sin(J * AD, NB);
+            if constexpr (J == 0) {
+                Pv = s[0];
+                Qv = make_double2(0.0, 0.0);
+            } else {
+                Pv = make_double2(fma(c, s[J].x, Pv.x), fma(c, s[J].y, Pv.y));
+                Qv = make_double2(fma(sn, s[J].x, Qv.x), fma(sn, s[J].y, Qv.y));
+            }
+            acc<AD, J + 1>(s, Pv, Qv);
         }
     }
-};
-template <>
-struct PairSum<2> {
-    __device__ __forceinline__ static void run(const cd *B, cd &o0, cd &o1) {
-        o0 = cadd(B[0], B[1]);
-        o1 = csub(B[0], B[1]);
+    template <int AD>
+    __device__ __forceinline__ static void level(const cd *e, const cd *f, cd *out) {
+        if constexpr (AD <= ADMAX) {
+            const cd *s = (AD % 2 == 0) ? e : f;
+            if constexpr (AD == 0) {
+                cd t = s[0];
+#pragma unroll
+                for (int j = 1; j < H; j++) t = h_add(t, s[j]);
+                out[-DLO] = t;
+            } else {
+                cd Pv, Qv;
+                acc<AD, 0>(s, Pv, Qv);
+                if constexpr (AD <= DHI) out[AD - DLO] = make_double2(Pv.x + Qv.y, Pv.y - Qv.x);
+                if constexpr (-AD >= DLO) out[-AD - DLO] = make_double2(Pv.x - Qv.y, Pv.y + Qv.x);
+            }
+            level<AD + 1>(e, f, out);
+        }
     }
-};
-template <>
-struct PairSum<3> {
-    __device__ __forceinline__ static void run(const cd *B, cd &o0, cd &o1) {
-        const double s = 0.86602540378443864676;
-        const cd t = cadd(B[1], B[2]), d = csub(B[1], B[2]);
-        o0 = cadd(B[0], t);
-        // conj(W3) = -1/2 + i s, conj(W3^2) = -1/2 - i s
-        o1 = make_double2(fma(-0.5, t.x, B[0].x) - s * d.y, fma(-0.5, t.y, B[0].y) + s * d.x);
-    }
-};
-template <>
-struct PairSum<8> {
-    __device__ __forceinline__ static void run(const cd *B, cd &o0, cd &o1) {
-        const double h = 0.70710678118654752440;
-        o0 = cadd(cadd(cadd(B[0], B[4]), cadd(B[2], B[6])), cadd(cadd(B[1], B[5]), cadd(B[3], B[7])));
-        const cd d = csub(B[0], B[4]), e = csub(B[2], B[6]), u = csub(B[1], B[5]), w = csub(B[3], B[7]);
-        // (B0 - B4) + i (B2 - B6) + h [(1 + i)(B1 - B5) + (-1 + i)(B3 - B7)]
-        const double re = (u.x - u.y) - (w.x + w.y), im = (u.x + u.y) + (w.x - w.y);
-        o1 = make_double2(fma(h, re, d.x - e.y), fma(h, im, d.y + e.x));
+    __device__ __forceinline__ static void run(const cd *x, cd *out) {
+        if constexpr (EVEN) {
+            cd e[H], f[H];
+#pragma unroll
+            for (int j = 0; j < H; j++) {
+                e[j] = h_add(x[j], x[j + H]);
+                f[j] = h_sub(x[j], x[j + H]);
+            }
+            level<0>(e, f, out);
+        } else {
+            level<0>(x, x, out);
+        }
     }
 };
 
@@ -77,7 +116,7 @@ struct PdZyParams {
     int g2min, ng2, g3min, ng3;
 };
 
-template <int N3, int NA3, int N2, int NA2, int NW, int LPW, int G>
+template <int N3, int NA3, int DLO, int DHI, int N2, int NA2, int NW, int LPW, int G>
 struct PdZy {
     static constexpr int NB3 = N3 / NA3, NB2 = N2 / NA2;
     static constexpr int K1PT = (NA3 + NB3 - 1) / NB3;
@@ -95,8 +134,10 @@ struct PdZy {
         return ((size_t)N2 + (size_t)NW * LPW * XLINE + (size_t)NA3 * NTH + (size_t)N2 * G * ng3) * sizeof(cd) +
                (size_t)ng2 * ng3 * sizeof(int32_t);
     }
-    // the z pass B (PairSum) keeps g = k1 and g = k1 - NA3 only: the box must lie inside [-NA3, NA3)
-    static bool box_ok(int g3min, int ng3) { return g3min >= -NA3 && g3min + ng3 <= NA3 && 2 * NA3 <= N3 + 1; }
+    static constexpr int ND = DHI - DLO + 1;
+    static_assert(NA3 * ND <= N3, "kept frequencies must be distinct modulo N3");
+    // the z pass B keeps g = k1 + NA3 d, d = DLO .. DHI: the box must lie inside [NA3 DLO, NA3 (DHI + 1))
+    static bool box_ok(int g3min, int ng3) { return g3min >= NA3 * DLO && g3min + ng3 <= NA3 * (DHI + 1); }
 };
 
 // unit u of the launch -> first pair p (relative to the batch) and the number of pairs cnt <= G, all in one row.
@@ -145,9 +186,10 @@ struct PdZyCursor {
     int w, p0, cnt, n, m, c, g, j1;
 };
 
-template <int N3, int NA3, int N2, int NA2, int NW, int LPW, int G, int MINB>
+template <int N3, int NA3, int DLO, int DHI, int N2, int NA2, int NW, int LPW, int G, int MINB>
 __global__ void __launch_bounds__(NW * 32, MINB) pd_zy_kernel(const __grid_constant__ PdZyParams P) {
-    using C = PdZy<N3, NA3, N2, NA2, NW, LPW, G>;
+    using C = PdZy<N3, NA3, DLO, DHI, N2, NA2, NW, LPW, G>;
+    constexpr int ND = C::ND;
     constexpr int NB3 = C::NB3, NB2 = C::NB2, K1PT = C::K1PT, XP = C::XP, XLINE = C::XLINE, ROWS = C::ROWS, NCH = C::NCH,
                   NTH = C::NTH;
     extern __shared__ __align__(16) unsigned char pd_smem[];
@@ -169,17 +211,16 @@ __global__ void __launch_bounds__(NW * 32, MINB) pd_zy_kernel(const __grid_const
     const bool zact = lw < LPW;
     cd *Xl = X + (warp * LPW + (zact ? lw : 0)) * XLINE;
     cd *uns = UN + tid;   // this thread's u_n elements: uns[t * NTH]
-    // pass B: k1 = j + a NB3 keeps g = k1 (box index oi0) and g = k1 - NA3 (oi1); twiddles W_N3^(jj k1)
+    // pass B: k1 = j + a NB3 keeps g = k1 + NA3 d, d = DLO .. DHI (box index oi, -1 outside); twiddles W_N3^(jj k1)
     cd twb[K1PT][NB3];
-    int oi0[K1PT], oi1[K1PT];
+    int oi[K1PT][ND];
 #pragma unroll
     for (int a = 0; a < K1PT; a++) {
         const int k1 = j + a * NB3;
-        oi0[a] = oi1[a] = -1;
-        if (k1 < NA3) {
-            const int i0 = k1 - P.g3min, i1 = k1 - NA3 - P.g3min;
-            if (i0 >= 0 && i0 < ng3) oi0[a] = i0;
-            if (i1 >= 0 && i1 < ng3) oi1[a] = i1;
+#pragma unroll
+        for (int d = 0; d < ND; d++) {
+            const int i = k1 + NA3 * (d + DLO) - P.g3min;
+            oi[a][d] = (k1 < NA3 && i >= 0 && i < ng3) ? i : -1;
         }
 #pragma unroll
         for (int jj = 0; jj < NB3; jj++) twb[a][jj] = P.tw3[(jj * (k1 < NA3 ? k1 : 0)) % N3];
@@ -272,10 +313,11 @@ __global__ void __launch_bounds__(NW * 32, MINB) pd_zy_kernel(const __grid_const
                     B[0] = Xl[(j + a * NB3) * XP];
 #pragma unroll
                     for (int jj = 1; jj < NB3; jj++) B[jj] = h_mul(twb[a][jj], Xl[(j + a * NB3) * XP + jj]);
-                    cd o0, o1;
-                    PairSum<NB3>::run(B, o0, o1);
-                    if (oi0[a] >= 0) yrow[oi0[a]] = o0;
-                    if (oi1[a] >= 0) yrow[oi1[a]] = o1;
+                    cd o[ND];
+                    PrunedDft<NB3, DLO, DHI>::run(B, o);
+#pragma unroll
+                    for (int d = 0; d < ND; d++)
+                        if (oi[a][d] >= 0) yrow[oi[a][d]] = o[d];
                 }
             }
         }
