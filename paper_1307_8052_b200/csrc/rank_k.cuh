@@ -64,7 +64,10 @@ __global__ void weights_kernel(double *__restrict__ w, int64_t ldw, int K, int K
 
 // Nb[Kpad][ldn] (rows >= K are zero; frequency iw reads Nb + iw*strideN, strideN = 0 when SHARED_N), w[n_omega][ldw],
 // S[n_omega][ng][ldS] (lower triangle accumulated).  Only rows / columns g >= g0 are touched (g0 % 1 == 0; tiles
-// start at g0).  Kpad % KC == 0.  grid = (ntiles_lower(ng - g0), ceil(n_omega / Cfg::NW)).
+// start at g0).  Kpad % KC == 0.  grid = (ntiles_lower(ng - g0), ceil(n_omega / Cfg::NW), ksplit).
+// ksplit > 1 (chi0 accumulation only): CTA z takes the z-th slice of the K chunks and adds its tile with
+// red.global.add.f64, so that tiles x frequency pairs x slices fill the last wave of the grid (the host picks
+// ksplit); the order of those additions is not fixed, i.e. S is then reproducible to rounding, not bitwise.
 template <bool SHARED_N>
 __global__ void __launch_bounds__(rk::Cfg<SHARED_N>::THREADS, rk::Cfg<SHARED_N>::MIN_CTAS)
 rank_k_kernel(const cd *__restrict__ Nb, int64_t ldn, int64_t strideN, int Kpad, const double *__restrict__ w,
@@ -104,7 +107,10 @@ rank_k_kernel(const cd *__restrict__ Nb, int64_t ldn, int64_t strideN, int Kpad,
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     __syncthreads();
 
-    const int nk = Kpad / KC;
+    // this CTA's slice of the K chunks
+    const int nk_all = Kpad / KC, ksplit = (int)gridDim.z;
+    const int it0 = (int)(((int64_t)nk_all * blockIdx.z) / ksplit), it1 = (int)(((int64_t)nk_all * (blockIdx.z + 1)) / ksplit);
+    const int nk = it1 - it0;
     if (warp == CONSUMER_WARPS) {
         // ---- producer warp: keeps the ring full, never touches the tensor pipe -------------------------------
         for (int it = 0; it < nk; it++) {
@@ -113,12 +119,12 @@ rank_k_kernel(const cd *__restrict__ Nb, int64_t ldn, int64_t strideN, int Kpad,
             unsigned char *st = rk_smem + s * STAGE_BYTES;
             if (lane == 0) mbar_arrive_expect_tx(&full[s], stage_tx);
             __syncwarp();
-            const size_t krow = (size_t)it * KC + (lane & 15);
+            const size_t krow = (size_t)(it0 + it) * KC + (lane & 15);
             const cd *Nw = Nb + (size_t)om0 * strideN + krow * ldn;   // strideN = 0 when SHARED_N
             if (lane < 16) bulk_g2s(st + lane * PITCH, Nw + row0, rowbytes, &full[s]);
             else bulk_g2s(st + TILE_BYTES + (lane - 16) * PITCH, Nw + col0, colbytes, &full[s]);
             if (lane < n_om)
-                bulk_g2s(st + W_OFF + lane * KC * 8, w + (size_t)(om0 + lane) * ldw + (size_t)it * KC, KC * 8, &full[s]);
+                bulk_g2s(st + W_OFF + lane * KC * 8, w + (size_t)(om0 + lane) * ldw + (size_t)(it0 + it) * KC, KC * 8, &full[s]);
         }
         return;
     }
@@ -199,10 +205,15 @@ rank_k_kernel(const cd *__restrict__ Nb, int64_t ldn, int64_t strideN, int Kpad,
                     const int col = cc + e;
                     if (col < ng && col <= r) {
                         cd *ptr = Sw + (size_t)r * ldS + col;
-                        cd v = *ptr;
-                        v.x += re[mi][ni][e];
-                        v.y += im[mi][ni][e];
-                        *ptr = v;
+                        if (ksplit > 1) {   // several CTAs add into this tile
+                            atomicAdd(&ptr->x, re[mi][ni][e]);
+                            atomicAdd(&ptr->y, im[mi][ni][e]);
+                        } else {
+                            cd v = *ptr;
+                            v.x += re[mi][ni][e];
+                            v.y += im[mi][ni][e];
+                            *ptr = v;
+                        }
                     }
                 }
             }

@@ -264,6 +264,20 @@ int ntiles_lower(int n, int t) {
     return nt * (nt + 1) / 2;
 }
 
+// K slices of the rank-K launch: one CTA per SM, `units` equal work items (tile x frequency pair).  With s slices
+// the grid needs ceil(units s / n_sm) rounds of 1/s of an item each; take the s that minimises that time, charging
+// 0.4 % per extra slice for its prologue / atomic epilogue, and keep at least 16 chunks (256 pairs) per slice.
+int pick_ksplit(int units, int nchunks, int n_sm) {
+    int best = 1;
+    double best_cost = 1e300;
+    for (int s = 1; s <= 8 && nchunks / s >= 16; s++) {
+        const double rounds = (double)(((int64_t)units * s + n_sm - 1) / n_sm) / s;
+        const double cost = rounds * (1.0 + 0.004 * (s - 1));
+        if (cost < best_cost * (1.0 - 1e-9)) { best_cost = cost; best = s; }
+    }
+    return best;
+}
+
 // Launch plan of the plane kernel: rows per chunk, threads, dynamic shared memory.
 //  fast path (grid lengths known at build time): one butterfly per thread per pass, so threads = RC * max_nb <= 256;
 //  several CTAs per SM (shared memory is small: no staging).
@@ -294,7 +308,7 @@ void plan_zy_kernel(rpa_chi0 *h) {
     else if (N2 == 24 && N3 == 24) ZY(24, 8, -1, 0, 24, 8, 3, 8, 4, 3);
     else if (N2 == 16 && N3 == 16) ZY(16, 8, -1, 0, 16, 8, 1, 16, 4, 8);
     else if (N2 == 40 && N3 == 168) ZY(168, 12, -2, 1, 40, 8, 4, 2, 2, 2);
-    else if (N2 == 48 && N3 == 192) ZY(192, 12, -3, 2, 48, 8, 8, 2, 2, 1);
+    else if (N2 == 48 && N3 == 192) ZY(192, 12, -3, 2, 48, 12, 8, 2, 2, 1);
 #undef ZY
 }
 
@@ -429,11 +443,14 @@ int rpa_chi0_create(rpa_chi0_t **out, const int32_t grid[3], const double cell[9
         if (xs > 220 * 1024) { delete h; return fail(RPA_ERR_UNSUPPORTED, "rpa_chi0_create: N1 = %d too large for the x-axis table", grid[0]); }
         if (xs > 48 * 1024) CREATE_TRY(cudaFuncSetAttribute(pd_xaxis_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)xs));
     }
-    if (h->zy_kernel) {
-        CREATE_TRY(cudaFuncSetAttribute(h->zy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->zy_smem));
-        int dev = 0, per_sm = 0;
+    {
+        int dev = 0;
         CREATE_TRY(cudaGetDevice(&dev));
         CREATE_TRY(cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, dev));
+    }
+    if (h->zy_kernel) {
+        CREATE_TRY(cudaFuncSetAttribute(h->zy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->zy_smem));
+        int per_sm = 0;
         CREATE_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, h->zy_kernel, h->zy_threads, h->zy_smem));
         if (per_sm < 1) { delete h; return fail(RPA_ERR_CUDA, "rpa_chi0_create: pd_zy kernel does not fit an SM"); }
         h->zy_ctas_per_sm = per_sm;
@@ -633,7 +650,9 @@ int rpa_chi0_add_kpoint(rpa_chi0_t *h, double kweight, int32_t n_occ, const void
             // S6: rank-K update of every frequency
             {
                 StageTimer tm(h, 4, 1);
-                rank_k_kernel<true><<<dim3(ntiles_lower(ng, rk::T), (h->n_omega + rk::Cfg<true>::NW - 1) / rk::Cfg<true>::NW),
+                const int units = ntiles_lower(ng, rk::T) * ((h->n_omega + rk::Cfg<true>::NW - 1) / rk::Cfg<true>::NW);
+                const int ksplit = pick_ksplit(units, Kpad / rk::KC, h->n_sm);
+                rank_k_kernel<true><<<dim3(ntiles_lower(ng, rk::T), (h->n_omega + rk::Cfg<true>::NW - 1) / rk::Cfg<true>::NW, ksplit),
                                       rk::Cfg<true>::THREADS, rk::Cfg<true>::SMEM_BYTES, st>>>(
                     Nbuf, L.ldn, 0, Kpad, w, L.ldw, h->ptr<cd>(L.S), L.ldS, (int64_t)ng * L.ldS, ng, 0, h->n_omega);
                 CUDA_TRY(cudaGetLastError());
