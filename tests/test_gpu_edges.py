@@ -1,0 +1,126 @@
+"""Edge cases and error behaviour of the C ABI on a real device (include/rpa_chi0.h: "errors" paragraph)."""
+import numpy as np
+import pytest
+
+from paper_1307_8052_b200 import workload as W
+from tests.parity_util import oracle_run, rel_fro
+
+pytestmark = pytest.mark.gpu
+
+
+def _handle(cfg, ptot=None, batch=0):
+    from paper_1307_8052_b200 import binding as B
+    om, wt = W.omega_grid(cfg.n_omega)
+    ptot = int(cfg.n_proj.sum()) if ptot is None else ptot
+    return B.rpa_chi0_create(cfg.grid, cfg.cell, cfg.q_red, W.tuned_ecut(cfg), om, wt, batch, ptot, "cuda:0")
+
+
+def _dev(kd):
+    import torch
+    return {k: torch.from_numpy(getattr(kd, k)).to("cuda:0") for k in ("psi_occ", "psi_unocc", "P_occ", "P_unocc")}
+
+
+def test_empty_band_sets_are_a_no_op_and_reset_zeroes():
+    import torch
+    from paper_1307_8052_b200 import binding as B
+    cfg = W.CONFIGS[0]
+    h = _handle(cfg)
+    try:
+        kd = W.kpoint(cfg, 0)
+        d = _dev(kd)
+        empty = torch.empty((0,) + tuple(cfg.grid), dtype=torch.complex128, device="cuda:0")
+        B.rpa_chi0_add_kpoint(h, 1.0, empty, d["psi_unocc"], [], kd.eps_unocc, [], kd.f_unocc)
+        B.rpa_chi0_add_kpoint(h, 1.0, d["psi_occ"], empty, kd.eps_occ, [], kd.f_occ, [])
+        assert float(B.rpa_chi0_get(h, 0).abs().max()) == 0.0
+        B.rpa_chi0_add_kpoint(h, 1.0, d["psi_occ"], d["psi_unocc"], kd.eps_occ, kd.eps_unocc, kd.f_occ, kd.f_unocc)
+        assert float(B.rpa_chi0_get(h, 0).abs().max()) > 0.0
+        B.rpa_chi0_reset(h)
+        for i in range(cfg.n_omega):
+            assert float(B.rpa_chi0_get(h, i).abs().max()) == 0.0
+    finally:
+        h.close()
+
+
+def test_single_pair_and_single_band_tails():
+    """K = 1 (one chunk of 16 pairs, 15 of them padding) and 1 x n / n x 1 band sets against the oracle."""
+    from paper_1307_8052_b200 import binding as B
+    import torch
+    cfg = W.CONFIGS[0]
+    for occ, unocc in (([1], [5]), ([0, 2, 3], [7]), ([2], list(range(0, 28, 3)))):
+        kd = W.kpoint(cfg, 0, occ=occ, unocc=unocc)
+        h = _handle(cfg)
+        try:
+            g, K2 = B.rpa_chi0_gvectors(h)
+            Qd = torch.from_numpy(W.paw_Q(cfg, K2)).to("cuda:0")
+            B.add_kpoint_host(h, kd, cfg.n_proj, Qd, W.atom_positions(cfg))
+            chi_g = [B.rpa_chi0_get(h, i).cpu().numpy() for i in range(cfg.n_omega)]
+        finally:
+            h.close()
+        chi_o, _, _, _ = oracle_run(cfg, [kd], True, want_ec=False)
+        for i in range(cfg.n_omega):
+            assert rel_fro(chi_g[i], chi_o[i]) <= 1e-10
+
+
+def test_argument_errors_are_reported_not_thrown():
+    import torch
+    from paper_1307_8052_b200 import binding as B
+    cfg = W.CONFIGS[0]
+    h = _handle(cfg, ptot=4)   # room for 4 projectors only
+    try:
+        kd = W.kpoint(cfg, 0)
+        d = _dev(kd)
+        g, K2 = B.rpa_chi0_gvectors(h)
+        for bad in (-1, cfg.n_omega):
+            with pytest.raises(B.RpaError) as ei:
+                B.rpa_chi0_get(h, bad)
+            assert ei.value.code == B.RPA_ERR_INVALID_ARG
+        Qd = torch.from_numpy(W.paw_Q(cfg, K2)).to("cuda:0")
+        with pytest.raises(B.RpaError) as ei:   # 8 projectors > max_proj_total = 4 given at create
+            B.rpa_chi0_add_kpoint(h, 1.0, d["psi_occ"], d["psi_unocc"], kd.eps_occ, kd.eps_unocc, kd.f_occ, kd.f_unocc,
+                                  cfg.n_proj, d["P_occ"], d["P_unocc"], Qd, W.atom_positions(cfg))
+        assert ei.value.code == B.RPA_ERR_WORKSPACE
+        v = W.coulomb(K2)
+        for bad_v in (np.where(np.arange(len(v)) == 3, 0.0, v), np.where(np.arange(len(v)) == 5, np.nan, v), -v):
+            with pytest.raises(B.RpaError) as ei:
+                B.rpa_ec_q(h, bad_v)
+            assert ei.value.code == B.RPA_ERR_INVALID_ARG
+        assert "v_G" in B.rpa_last_error()
+        # the handle is still usable after the errors
+        B.rpa_chi0_add_kpoint(h, 1.0, d["psi_occ"], d["psi_unocc"], kd.eps_occ, kd.eps_unocc, kd.f_occ, kd.f_unocc)
+        ec, e = B.rpa_ec_q(h, v)
+        assert np.isfinite(ec) and ec < 0.0
+    finally:
+        h.close()
+
+
+def test_not_positive_definite_is_detected():
+    """Swapped occupations give positive weights, chi0 >= 0, and I - v^1/2 chi0 v^1/2 loses positive definiteness
+    once scaled up: rpa_ec_q must return RPA_ERR_NOT_PD, and chi0 must be left untouched."""
+    from paper_1307_8052_b200 import binding as B
+    cfg = W.CONFIGS[0]
+    h = _handle(cfg, ptot=0)
+    try:
+        kd = W.kpoint(cfg, 0)
+        d = _dev(kd)
+        g, K2 = B.rpa_chi0_gvectors(h)
+        B.rpa_chi0_add_kpoint(h, 1.0e3, d["psi_occ"], d["psi_unocc"], kd.eps_occ, kd.eps_unocc, kd.f_unocc[:cfg.n_occ] * 0.0,
+                              np.ones(cfg.n_unocc))
+        before = B.rpa_chi0_get(h, 0).cpu().numpy()
+        assert np.linalg.eigvalsh(before).min() >= -1e-10 * np.abs(before).max()
+        with pytest.raises(B.RpaError) as ei:
+            B.rpa_ec_q(h, W.coulomb(K2))
+        assert ei.value.code == B.RPA_ERR_NOT_PD
+        assert np.array_equal(B.rpa_chi0_get(h, 0).cpu().numpy(), before)
+    finally:
+        h.close()
+
+
+def test_unsupported_grid_length_is_rejected():
+    from paper_1307_8052_b200 import binding as B
+    cell = np.diag([6.0, 6.5, 7.0])
+    om, wt = W.omega_grid(4)
+    with pytest.raises(B.RpaError) as ei:   # N3 = 11: prime factor other than 2, 3, 5, 7
+        B.rpa_chi0_create((6, 6, 11), cell, (0.25, 0.0, 0.0), 1.0, om, wt, 0, 0, "cuda:0")
+    assert ei.value.code == B.RPA_ERR_UNSUPPORTED
+    h = B.rpa_chi0_create((11, 6, 8), cell, (0.25, 0.0, 0.0), 1.0, om, wt, 0, 0, "cuda:0")   # N1 is unrestricted
+    h.close()
