@@ -44,6 +44,10 @@ def lib():
         L.orc_chi0_from_S.argtypes = [C.c_int64, f64, vp, vp]
         L.orc_ec_q.restype = i32
         L.orc_ec_q.argtypes = [i32, i32, vp, vp, vp, vp, vp]
+        L.orc_pw_to_grid.restype = None
+        L.orc_pw_to_grid.argtypes = [vp, i32, i32, vp, vp, C.c_int64, vp, vp]
+        L.orc_symmetry_remap.restype = i32
+        L.orc_symmetry_remap.argtypes = [vp, vp, i32, i32, vp, vp]
         _lib = L
     return _lib
 
@@ -145,6 +149,28 @@ def ec_q(chi0, v, omega_wt):
     if st != 0:
         raise FloatingPointError(f"I - v^1/2 chi0 v^1/2 not positive definite at omega index {-st - 1}")
     return float(ec.value), e
+
+
+def pw_to_grid(grid, g_pw, C_pw, pts=None):
+    """Eq. 10: u[band][pt] = sum_Q C[band][Q] exp(+2 pi i Q.j/N) at the flat grid indices `pts` (default: all)."""
+    grid, g_pw, C_pw = _i32(grid), _i32(g_pw).reshape(-1, 3), _c128(C_pw)
+    C_pw = C_pw.reshape(-1, g_pw.shape[0])
+    N = int(np.prod(grid))
+    pts = np.arange(N, dtype=np.int64) if pts is None else np.ascontiguousarray(pts, dtype=np.int64)
+    out = np.zeros((C_pw.shape[0], pts.size), dtype=np.complex128)
+    lib().orc_pw_to_grid(_p(grid), C_pw.shape[0], g_pw.shape[0], _p(g_pw), _p(C_pw), pts.size, _p(pts), _p(out))
+    return out
+
+
+def symmetry_remap(grid, M, time_reversal, u):
+    """Eq. 11: u_out(r) = u_in(M r) in reduced coordinates (M = T^-1, integer 3x3), conj if time_reversal."""
+    grid, M, u = _i32(grid), _i32(M).reshape(9), _c128(u)
+    N = int(np.prod(grid))
+    out = np.empty_like(u)
+    st = lib().orc_symmetry_remap(_p(grid), _p(M), int(bool(time_reversal)), u.size // N, _p(u), _p(out))
+    if st != 0:
+        raise ValueError("the symmetry operation does not map the grid onto itself")
+    return out
 
 
 class Chi0Oracle:

@@ -352,3 +352,62 @@ int32_t orc_ec_q(int32_t ng, int32_t n_omega, const zd *chi0, const double *v, c
     free(e);
     return status;
 }
+
+/*
+ * ---- NEXT-1: Table 1 steps 3-4 -----------------------------------------------------------------
+ * Eq. 10: the periodic part of the pseudo wave function on the grid from its plane-wave coefficients,
+ *   u(r_j) = sum_Q C(Q) exp(+2 pi i (Q1 j1/N1 + Q2 j2/N2 + Q3 j3/N3)),
+ * by direct summation (the Bloch phase exp(i k.r) of Eq. 10 is not applied: reading A5, the library works with
+ * periodic parts).  Evaluated at the n_pts grid points listed in pts (flat C-order indices); out[band][pt].
+ * No normalisation: (1/N) sum_j |u_j|^2 = sum_Q |C(Q)|^2 (Parseval) is the caller's.
+ */
+void orc_pw_to_grid(const int32_t grid[3], int32_t n_bands, int32_t n_pw, const int32_t *g_pw, const zd *C,
+                    int64_t n_pts, const int64_t *pts, zd *out) {
+    const int32_t N1 = grid[0], N2 = grid[1], N3 = grid[2];
+    zd *t1 = phase_table(N1), *t2 = phase_table(N2), *t3 = phase_table(N3);
+#pragma omp parallel for collapse(2) schedule(dynamic, 64)
+    for (int32_t b = 0; b < n_bands; b++)
+        for (int64_t ip = 0; ip < n_pts; ip++) {
+            const int64_t j = pts[ip];
+            const int32_t j3 = (int32_t)(j % N3), j2 = (int32_t)((j / N3) % N2), j1 = (int32_t)(j / ((int64_t)N2 * N3));
+            zd acc = 0.0;
+            for (int32_t q = 0; q < n_pw; q++) {
+                /* exp(+2 pi i t/n) = conj(exp(-2 pi i t/n)) */
+                const zd ph = conj(t1[pmod((int64_t)g_pw[3 * q] * j1, N1)] * t2[pmod((int64_t)g_pw[3 * q + 1] * j2, N2)] *
+                                   t3[pmod((int64_t)g_pw[3 * q + 2] * j3, N3)]);
+                acc += C[(int64_t)b * n_pw + q] * ph;
+            }
+            out[(int64_t)b * n_pts + ip] = acc;
+        }
+    free(t1); free(t2); free(t3);
+}
+
+/*
+ * Eq. 11: IBZ -> BZ transformation of the periodic part on the grid,
+ *   u_out(r) = u_in(T^-1 r)            (crystal symmetry),     then conj if time reversal is used,
+ * with T^-1 given in reduced (fractional) coordinates as the integer matrix M: a point with fractional
+ * coordinates x_i = j_i/N_i is taken from x'_i = sum_k M[i][k] x_k, i.e. grid index j'_i = sum_k M[i][k] j_k N_i/N_k
+ * (mod N_i), which must be an integer for every grid point (returns -1 otherwise, 0 on success).
+ */
+int32_t orc_symmetry_remap(const int32_t grid[3], const int32_t M[9], int32_t time_reversal, int32_t n_bands,
+                           const zd *in, zd *out) {
+    const int64_t N = (int64_t)grid[0] * grid[1] * grid[2];
+    for (int i = 0; i < 3; i++)
+        for (int k = 0; k < 3; k++)
+            if (((int64_t)M[3 * i + k] * grid[i]) % grid[k] != 0) return -1;
+    for (int32_t b = 0; b < n_bands; b++)
+        for (int32_t j1 = 0; j1 < grid[0]; j1++)
+            for (int32_t j2 = 0; j2 < grid[1]; j2++)
+                for (int32_t j3 = 0; j3 < grid[2]; j3++) {
+                    const int64_t j[3] = {j1, j2, j3};
+                    int64_t jp[3];
+                    for (int i = 0; i < 3; i++) {
+                        int64_t s = 0;
+                        for (int k = 0; k < 3; k++) s += (int64_t)M[3 * i + k] * grid[i] / grid[k] * j[k];
+                        jp[i] = pmod(s, grid[i]);
+                    }
+                    const zd v = in[b * N + (jp[0] * grid[1] + jp[1]) * grid[2] + jp[2]];
+                    out[b * N + ((int64_t)j1 * grid[1] + j2) * grid[2] + j3] = time_reversal ? conj(v) : v;
+                }
+    return 0;
+}

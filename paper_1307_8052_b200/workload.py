@@ -171,6 +171,19 @@ def orbital(cfg: Config, k: int, band: int, _cache={}) -> np.ndarray:
     return np.ascontiguousarray(u)
 
 
+def orbital_coefficients(cfg: Config, k: int, band: int):
+    """(g_pw[n_pw][3] int32, C[n_pw]): the plane-wave coefficients behind `orbital`, scaled so that sum |C|^2 = 1
+    (Parseval: the grid orbital sum_Q C(Q) exp(2 pi i Q.j/N) is then grid-normalised).  Same random stream as
+    `orbital`, so pw -> grid of these coefficients reproduces it to rounding."""
+    ok, decay = _coef_mask(cfg)
+    rng_ax = [np.fft.fftfreq(n, 1.0 / n).astype(np.int64) for n in cfg.grid]
+    g = np.stack(np.meshgrid(*rng_ax, indexing="ij"), axis=-1)
+    xi = _rng(cfg, _KIND_COEF, k, band).standard_normal((int(ok.sum()), 2))
+    C = (xi[:, 0] + 1j * xi[:, 1]) * decay[ok]
+    C *= 1.0 / np.sqrt(np.sum(np.abs(C) ** 2))
+    return np.ascontiguousarray(g[ok].astype(np.int32)), np.ascontiguousarray(C)
+
+
 def eigenvalues(cfg: Config, k: int):
     """eps (Ha) sorted, occupations per spin channel in [0,1]."""
     nb = cfg.n_occ + cfg.n_unocc
