@@ -136,6 +136,29 @@ int rpa_chi0_launch_count(const rpa_chi0_t *h, int64_t *count);
  */
 int rpa_chi0_accumulators(const rpa_chi0_t *h, void **S, size_t *bytes);
 
+/*
+ * Table 1 steps 3-4, upstream of rpa_chi0_add_kpoint.
+ *
+ * rpa_pw_to_grid -- Eq. 10: the cell-periodic part of n_bands pseudo wave functions on the handle's grid
+ * from their plane-wave coefficients,
+ *     psi_out[b][j1][j2][j3] = sum_Q C[b][Q] exp(+2 pi i (Q1 j1/N1 + Q2 j2/N2 + Q3 j3/N3)),
+ * g_pw: host int32 [n_pw][3], the integer reciprocal vectors Q (distinct; any range that fits the scratch);
+ * C: dev cdouble [n_bands][n_pw]; psi_out: dev cdouble [n_bands][N1][N2][N3].  No Bloch phase exp(i k.r) is applied
+ * (the library works with periodic parts) and no normalisation: (1/N) sum |psi|^2 = sum_Q |C(Q)|^2.
+ * Uses the handle's pair-density scratch: stream-ordered with the other calls of the handle.
+ * Errors: RPA_ERR_INVALID_ARG (NULL, duplicate Q), RPA_ERR_WORKSPACE / RPA_ERR_UNSUPPORTED (box of the Q too large).
+ *
+ * rpa_symmetry_remap -- Eq. 11: IBZ -> BZ transformation psi_out(r) = psi_in(T^-1 r), complex conjugated
+ * if time_reversal != 0.  M (host int32 [3][3]) is T^-1 in reduced coordinates: the value at fractional coordinates x
+ * is taken from M x, i.e. grid index j'_i = sum_k M[i][k] j_k N_i/N_k mod N_i.  psi_in, psi_out: dev cdouble
+ * [n_bands][N1][N2][N3], must not alias.  RPA_ERR_UNSUPPORTED if M N_i/N_k is not integer (the operation does not
+ * map the grid onto itself).  Fractional translations and the reciprocal-vector shift of a folded-back k are the
+ * caller's (reading A5).
+ */
+int rpa_pw_to_grid(rpa_chi0_t *h, int32_t n_bands, int32_t n_pw, const int32_t *g_pw, const void *C, void *psi_out);
+int rpa_symmetry_remap(rpa_chi0_t *h, int32_t n_bands, const int32_t M[9], int32_t time_reversal, const void *psi_in,
+                       void *psi_out);
+
 void rpa_chi0_destroy(rpa_chi0_t *h);
 
 /* Register-only DMMA issue-rate probe: runs `iters` dependent-free mma.sync.m8n8k4.f64 per warp on every SM and

@@ -25,6 +25,7 @@ EXPORTS = (
     "rpa_chi0_workspace_bytes", "rpa_chi0_create", "rpa_chi0_ng", "rpa_chi0_gvectors", "rpa_chi0_add_kpoint",
     "rpa_chi0_get", "rpa_ec_q", "rpa_chi0_reset", "rpa_chi0_sync", "rpa_chi0_set_profiling", "rpa_chi0_stage_times",
     "rpa_chi0_launch_count", "rpa_chi0_accumulators", "rpa_chi0_destroy", "rpa_probe_fp64_tensor_peak", "rpa_last_error",
+    "rpa_pw_to_grid", "rpa_symmetry_remap",
 )
 
 STAGE_NAMES = ("pair_product_fft_yz", "fft_x_gather", "paw", "weights", "rank_k")
@@ -85,6 +86,10 @@ def lib():
     L.rpa_chi0_destroy.argtypes = [vp]
     L.rpa_probe_fp64_tensor_peak.restype = C.c_int
     L.rpa_probe_fp64_tensor_peak.argtypes = [vp, C.POINTER(f64)]
+    L.rpa_pw_to_grid.restype = C.c_int
+    L.rpa_pw_to_grid.argtypes = [vp, i32, i32, vp, vp, vp]
+    L.rpa_symmetry_remap.restype = C.c_int
+    L.rpa_symmetry_remap.argtypes = [vp, i32, vp, i32, vp, vp]
     L.rpa_last_error.restype = C.c_char_p
     L.rpa_last_error.argtypes = []
     _lib = L
@@ -291,6 +296,36 @@ def rpa_chi0_accumulators(h: Handle):
     _check(lib().rpa_chi0_accumulators(h.ptr, C.byref(p), C.byref(n)))
     off = int(p.value) - h.workspace.data_ptr()
     return h.workspace[off:off + int(n.value)].view(torch.complex128)
+
+
+def rpa_pw_to_grid(h: Handle, g_pw, C_pw, out=None):
+    """Eq. 10: C_pw CUDA complex128 [n_bands][n_pw], g_pw host int [n_pw][3] -> psi [n_bands][N1][N2][N3] (CUDA)."""
+    torch = _torch()
+    g = _np(g_pw, np.int32).reshape(-1, 3)
+    n_pw = g.shape[0]
+    if C_pw.dim() != 2 or int(C_pw.shape[1]) != n_pw:
+        raise ValueError("C_pw must be [n_bands][n_pw]")
+    n_bands = int(C_pw.shape[0])
+    if out is None:
+        out = torch.empty((n_bands,) + h.grid, dtype=torch.complex128, device=h.device)
+    elif out.numel() != n_bands * int(np.prod(h.grid)):
+        raise ValueError("out must be [n_bands][N1][N2][N3]")
+    _check(lib().rpa_pw_to_grid(h.ptr, n_bands, n_pw, _hp(g), _dev_ptr(C_pw, "C_pw", torch.complex128, h.device) if n_bands else None,
+                                _dev_ptr(out, "out", torch.complex128, h.device) if n_bands else None))
+    return out
+
+
+def rpa_symmetry_remap(h: Handle, psi, M, time_reversal=False, out=None):
+    """Eq. 11: psi_out(r) = psi(M r) in reduced coordinates (M = T^-1, integer 3x3), conjugated under time reversal."""
+    torch = _torch()
+    Mi = _np(M, np.int32).reshape(9)
+    N = int(np.prod(h.grid))
+    n_bands = psi.numel() // N
+    if out is None:
+        out = torch.empty_like(psi)
+    _check(lib().rpa_symmetry_remap(h.ptr, n_bands, _hp(Mi), 1 if time_reversal else 0,
+                                    _dev_ptr(psi, "psi", torch.complex128, h.device), _dev_ptr(out, "out", torch.complex128, h.device)))
+    return out
 
 
 def rpa_chi0_destroy(h: Handle):

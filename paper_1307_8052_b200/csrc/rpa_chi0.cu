@@ -18,6 +18,7 @@
 #include "fft.cuh"
 #include "pair_density.cuh"
 #include "pair_density_zy.cuh"
+#include "orbitals.cuh"
 #include "paw.cuh"
 #include "rank_k.cuh"
 
@@ -777,6 +778,90 @@ void rpa_chi0_destroy(rpa_chi0_t *h) {
     for (auto &ev : h->events) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
     for (auto &e : h->pool) cudaEventDestroy(e);
     delete h;
+}
+
+// ---- Table 1 steps 3-4: plane-wave coefficients -> grid orbitals (Eq. 10), IBZ -> BZ remap (Eq. 11) -----------------
+int rpa_pw_to_grid(rpa_chi0_t *h, int32_t n_bands, int32_t n_pw, const int32_t *g_pw, const void *C, void *psi_out) {
+    if (!h) return fail(RPA_ERR_INVALID_ARG, "rpa_pw_to_grid: handle is NULL");
+    if (n_bands < 0 || n_pw < 0) return fail(RPA_ERR_INVALID_ARG, "rpa_pw_to_grid: negative count");
+    if (n_bands == 0) return RPA_OK;
+    if (!psi_out || (n_pw > 0 && (!g_pw || !C))) return fail(RPA_ERR_INVALID_ARG, "rpa_pw_to_grid: NULL array");
+    const Layout &L = h->L;
+    cudaStream_t st = h->stream;
+    const int N1 = h->grid[0], N2 = h->grid[1], N3 = h->grid[2];
+    const size_t N = (size_t)N1 * N2 * N3;
+    if (n_pw == 0) {
+        CUDA_TRY(cudaMemsetAsync(psi_out, 0, (size_t)n_bands * N * sizeof(cd), st));
+        return RPA_OK;
+    }
+    int qmin[3], qmax[3];
+    for (int d = 0; d < 3; d++) qmin[d] = qmax[d] = g_pw[d];
+    for (int i = 0; i < n_pw; i++)
+        for (int d = 0; d < 3; d++) {
+            qmin[d] = std::min(qmin[d], (int)g_pw[3 * i + d]);
+            qmax[d] = std::max(qmax[d], (int)g_pw[3 * i + d]);
+        }
+    const int64_t nq1 = (int64_t)qmax[0] - qmin[0] + 1, nq2 = (int64_t)qmax[1] - qmin[1] + 1, nq3 = (int64_t)qmax[2] - qmin[2] + 1;
+    const int64_t ncol = nq2 * nq3;
+    const size_t scratch = (size_t)L.sub_pairs * L.I_pair_bytes;
+    const size_t table_bytes = align_up((size_t)(nq1 * ncol) * sizeof(int32_t), 256);
+    const size_t t1_band = (size_t)N1 * ncol * sizeof(cd);
+    const size_t smem = ((size_t)N2 + N3 + ncol + (size_t)N2 * nq3) * sizeof(cd);
+    if (nq1 * ncol > ((int64_t)1 << 28) || table_bytes + t1_band > scratch)
+        return fail(RPA_ERR_WORKSPACE, "rpa_pw_to_grid: plane-wave box %lld x %lld x %lld does not fit the handle's scratch (%zu B)",
+                    (long long)nq1, (long long)nq2, (long long)nq3, scratch);
+    if (smem > 200 * 1024)
+        return fail(RPA_ERR_UNSUPPORTED, "rpa_pw_to_grid: plane of the plane-wave box too large for shared memory (%zu B)", smem);
+    std::vector<int32_t> table((size_t)(nq1 * ncol), -1);
+    for (int i = 0; i < n_pw; i++) {
+        const size_t at = ((size_t)(g_pw[3 * i] - qmin[0]) * nq2 + (g_pw[3 * i + 1] - qmin[1])) * nq3 + (g_pw[3 * i + 2] - qmin[2]);
+        if (table[at] >= 0) return fail(RPA_ERR_INVALID_ARG, "rpa_pw_to_grid: plane wave %d duplicates plane wave %d", i, table[at]);
+        table[at] = i;
+    }
+    unsigned char *base = h->ws + L.I;
+    int32_t *d_table = reinterpret_cast<int32_t *>(base);
+    cd *T1 = reinterpret_cast<cd *>(base + table_bytes);
+    CUDA_TRY(cudaMemcpyAsync(d_table, table.data(), table.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaStreamSynchronize(st));   // `table` is pageable host memory about to go out of scope
+    if (smem > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(pw_zy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const int chunk = (int)std::min<size_t>((size_t)n_bands, std::min<size_t>(65535, (scratch - table_bytes) / t1_band));
+    for (int b0 = 0; b0 < n_bands; b0 += chunk) {
+        const int nb = std::min(chunk, n_bands - b0);
+        pw_xaxis_kernel<<<dim3((unsigned)((ncol + 127) / 128), N1, nb), 128, 0, st>>>(
+            (const cd *)C + (size_t)b0 * n_pw, n_pw, d_table, h->ptr<cd>(L.tw1), N1, qmin[0], (int)nq1, (int)ncol, T1);
+        pw_zy_kernel<<<dim3(N1, nb), 256, smem, st>>>(T1, h->ptr<cd>(L.tw2), h->ptr<cd>(L.tw3), N1, N2, N3, qmin[1], (int)nq2,
+                                                     qmin[2], (int)nq3, (cd *)psi_out + (size_t)b0 * N);
+        h->launches += 2;
+        CUDA_TRY(cudaGetLastError());
+    }
+    return RPA_OK;
+}
+
+int rpa_symmetry_remap(rpa_chi0_t *h, int32_t n_bands, const int32_t M[9], int32_t time_reversal, const void *psi_in,
+                       void *psi_out) {
+    if (!h || !M) return fail(RPA_ERR_INVALID_ARG, "rpa_symmetry_remap: NULL argument");
+    if (n_bands < 0) return fail(RPA_ERR_INVALID_ARG, "rpa_symmetry_remap: negative count");
+    if (n_bands == 0) return RPA_OK;
+    if (!psi_in || !psi_out || psi_in == psi_out) return fail(RPA_ERR_INVALID_ARG, "rpa_symmetry_remap: NULL or aliased arrays");
+    RemapParams R;
+    R.N1 = h->grid[0]; R.N2 = h->grid[1]; R.N3 = h->grid[2];
+    R.conj = time_reversal != 0;
+    for (int i = 0; i < 3; i++)
+        for (int k = 0; k < 3; k++) {
+            const int64_t num = (int64_t)M[3 * i + k] * h->grid[i];
+            if (num % h->grid[k] != 0)
+                return fail(RPA_ERR_UNSUPPORTED, "rpa_symmetry_remap: the operation does not map the grid onto itself (M[%d][%d])", i, k);
+            R.S[3 * i + k] = (int)(num / h->grid[k]);
+        }
+    const int64_t N = (int64_t)R.N1 * R.N2 * R.N3;
+    for (int b0 = 0; b0 < n_bands; b0 += 65535) {
+        const int nb = std::min(65535, n_bands - b0);
+        symmetry_remap_kernel<<<dim3((unsigned)((N + 255) / 256), nb), 256, 0, h->stream>>>(
+            (const cd *)psi_in + (size_t)b0 * N, (cd *)psi_out + (size_t)b0 * N, R);
+        h->launches += 1;
+    }
+    CUDA_TRY(cudaGetLastError());
+    return RPA_OK;
 }
 
 // ---- FP64 tensor issue-rate probe -----------------------------------------------------------------------------

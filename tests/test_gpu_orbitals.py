@@ -1,0 +1,125 @@
+"""Parity of rpa_pw_to_grid (Eq. 10) and rpa_symmetry_remap (Eq. 11) against the CPU oracle,
+through the C ABI.  Tolerance: 1e-12 relative to max |u| for the transform (sums of up to ~1e4
+terms of unit-modulus phases in fp64: DESIGN.md section 5), bit-exact for the remap (pure data movement)."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_1307_8052_b200 import workload as W
+from tests.parity_util import gpu_run, rel_fro
+
+pytestmark = pytest.mark.gpu
+
+
+def _handle(cfg):
+    from paper_1307_8052_b200 import binding as B
+    om, wt = W.omega_grid(cfg.n_omega)
+    return B.rpa_chi0_create(cfg.grid, cfg.cell, cfg.q_red, W.tuned_ecut(cfg), om, wt, 0, int(cfg.n_proj.sum()), "cuda:0")
+
+
+def _coeffs(cfg, k, bands):
+    g = None
+    C = []
+    for b in bands:
+        g, c = W.orbital_coefficients(cfg, k, b)
+        C.append(c)
+    return g, np.stack(C)
+
+
+def test_pw_to_grid_toy_full_and_ragged_lists():
+    import torch
+    from paper_1307_8052_b200 import binding as B
+    cfg = W.CONFIGS[0]
+    g, C = _coeffs(cfg, 0, range(5))
+    h = _handle(cfg)
+    try:
+        u = B.rpa_pw_to_grid(h, g, torch.from_numpy(C).cuda()).cpu().numpy()
+        want = oracle.pw_to_grid(cfg.grid, g, C).reshape(u.shape)
+        assert np.abs(u - want).max() <= 1e-12 * np.abs(want).max()
+        # an odd sub-list of plane waves in shuffled order, one band; a single plane wave; no plane wave at all
+        sel = np.random.default_rng(1).permutation(len(g))[:37]
+        u1 = B.rpa_pw_to_grid(h, g[sel], torch.from_numpy(C[:1, sel].copy()).cuda()).cpu().numpy()
+        assert np.abs(u1 - oracle.pw_to_grid(cfg.grid, g[sel], C[:1, sel]).reshape(u1.shape)).max() <= 1e-12
+        u2 = B.rpa_pw_to_grid(h, [[1, -2, 3]], torch.ones((1, 1), dtype=torch.complex128, device="cuda")).cpu().numpy()
+        assert np.abs(u2 - oracle.pw_to_grid(cfg.grid, [[1, -2, 3]], [1.0]).reshape(u2.shape)).max() <= 1e-14
+        u3 = B.rpa_pw_to_grid(h, np.zeros((0, 3), dtype=np.int32), torch.zeros((2, 0), dtype=torch.complex128, device="cuda"))
+        assert float(u3.abs().max()) == 0.0
+        with pytest.raises(B.RpaError) as ei:   # duplicate plane wave
+            B.rpa_pw_to_grid(h, [[0, 0, 1], [0, 0, 1]], torch.ones((1, 2), dtype=torch.complex128, device="cuda"))
+        assert ei.value.code == B.RPA_ERR_INVALID_ARG
+    finally:
+        h.close()
+
+
+def test_pw_to_grid_config1_full_size_sampled_points():
+    """56x60x64 grid, ~9.4e3 plane waves (|G|^2/2 <= 6 Ha), 3 bands: the oracle sums at 400 sampled grid points
+    (first / last point, plane and row boundaries, random rest); the generator's own orbital must also come out."""
+    import torch
+    from paper_1307_8052_b200 import binding as B
+    cfg = W.CONFIGS[1]
+    bands = [0, 11, 300]
+    g, C = _coeffs(cfg, 0, bands)
+    h = _handle(cfg)
+    try:
+        u = B.rpa_pw_to_grid(h, g, torch.from_numpy(C).cuda()).cpu().numpy().reshape(len(bands), -1)
+    finally:
+        h.close()
+    N = cfg.n_grid
+    rng = np.random.default_rng(2)
+    pts = np.unique(np.concatenate([[0, 1, 63, 64, 3839, 3840, N - 1, N - 64], rng.choice(N, 392, replace=False)]))
+    want = oracle.pw_to_grid(cfg.grid, g, C, pts)
+    assert np.abs(u[:, pts] - want).max() <= 1e-12 * np.abs(want).max()
+    assert abs(np.mean(np.abs(u[0]) ** 2) - 1.0) < 1e-12                      # Parseval with sum |C|^2 = 1
+    assert np.abs(u[1] - W.orbital(cfg, 0, 11).reshape(-1)).max() <= 1e-11   # numpy's inverse FFT route
+
+
+def test_chi0_from_plane_wave_coefficients_matches_grid_route():
+    """Config 0 end to end: orbitals made on the device from their coefficients give the same chi0 as the orbitals
+    the generator makes on the host (both routes agree to rounding, so chi0 agrees to ~1e-13)."""
+    import torch
+    from paper_1307_8052_b200 import binding as B
+    cfg = W.CONFIGS[0]
+    kd = W.kpoint(cfg, 0)
+    chi_ref, _, _, _ = gpu_run(cfg, [kd], False, 0, want_ec=False)
+    g, Co = _coeffs(cfg, 0, range(cfg.n_occ))
+    _, Cu = _coeffs(cfg, 0, range(cfg.n_occ, cfg.n_occ + cfg.n_unocc))
+    h = _handle(cfg)
+    try:
+        po = B.rpa_pw_to_grid(h, g, torch.from_numpy(Co).cuda())
+        pu = B.rpa_pw_to_grid(h, g, torch.from_numpy(Cu).cuda())
+        B.rpa_chi0_add_kpoint(h, kd.kweight, po, pu, kd.eps_occ, kd.eps_unocc, kd.f_occ, kd.f_unocc)
+        for i in range(cfg.n_omega):
+            assert rel_fro(B.rpa_chi0_get(h, i).cpu().numpy(), chi_ref[i]) <= 1e-11
+    finally:
+        h.close()
+
+
+@pytest.mark.parametrize("M,tr", [(np.eye(3, dtype=int), True), (-np.eye(3, dtype=int), False),
+                                  ([[0, -1, 0], [1, 0, 0], [0, 0, 1]], False), ([[0, 1, 0], [1, 0, 0], [0, 0, -1]], True)])
+def test_symmetry_remap_bit_exact(M, tr):
+    import torch
+    from paper_1307_8052_b200 import binding as B
+    cfg = W.CONFIGS[0]   # cubic 16^3 grid: every point-group operation maps it onto itself
+    kd = W.kpoint(cfg, 0, occ=[0, 1], unocc=[0])
+    h = _handle(cfg)
+    try:
+        out = B.rpa_symmetry_remap(h, torch.from_numpy(kd.psi_occ).cuda(), M, tr).cpu().numpy()
+    finally:
+        h.close()
+    assert np.array_equal(out, oracle.symmetry_remap(cfg.grid, M, tr, kd.psi_occ))
+
+
+def test_symmetry_remap_rejects_incompatible_operation():
+    import torch
+    from paper_1307_8052_b200 import binding as B
+    cfg = W.CONFIGS[1]   # 56 x 60 x 64: swapping x and z does not map the grid onto itself
+    h = _handle(cfg)
+    try:
+        psi = torch.zeros((1,) + tuple(cfg.grid), dtype=torch.complex128, device="cuda")
+        with pytest.raises(B.RpaError) as ei:
+            B.rpa_symmetry_remap(h, psi, [[0, 0, 1], [0, 1, 0], [1, 0, 0]])
+        assert ei.value.code == B.RPA_ERR_UNSUPPORTED
+        out = B.rpa_symmetry_remap(h, psi, [[-1, 0, 0], [0, 1, 0], [0, 0, -1]])   # a mirror pair is fine
+        assert out.shape == psi.shape
+    finally:
+        h.close()
