@@ -7,7 +7,7 @@
 // rows (nq3 terms) in shared memory and streams the plane out with coalesced 16-byte stores.  The work is per band,
 // not per pair: for BASELINE.json configs[1] it is 1/12 of the pair-density traffic.
 #pragma once
-#include "common.cuh"
+#include "fft.cuh"
 
 // T1[b][j1][c] = sum_q1i Cbox[q1i][c] exp(+2 pi i q1 j1 / N1); c = q2i nq3 + q3i a box column,
 // table[q1i ncol + c] = index of that plane wave in C (or -1).  grid (ceil(ncol/128), N1, bands), block 128.
@@ -33,13 +33,61 @@ __global__ void __launch_bounds__(128) pw_xaxis_kernel(const cd *__restrict__ C,
     T1[((size_t)b * N1 + j1) * ncol + c] = acc;
 }
 
+// Input-pruned inverse transform of one line by the two-level split N = NA NB (the transpose of the forward
+// pair-density split): for the outputs j + NB s (s < NA) of one j < NB,
+//   Z[k1] = sum_{q in box, q = k1 mod NA} x[q] exp(+2 pi i q j / N),      u[j + NB s] = sum_k1 exp(+2 pi i k1 s / NA) Z[k1],
+// i.e. nq twiddled terms per j (not per output) followed by one inverse radix-NA butterfly in registers
+// (inverse = conj o forward o conj).  NA = 1 degenerates to the direct sum.
+//   ld(qi) reads x at box position qi (q = qmin + qi), st(n, v) writes output n.
+template <int NA, class LD, class ST>
+__device__ __forceinline__ void pw_expand_line(int N, int j, int qmin, int nq, const cd *__restrict__ tw, LD ld, ST st) {
+    const int NB = N / NA;
+    int r0 = qmin % NA;
+    if (r0 < 0) r0 += NA;                              // the box is read from q0 = qmin - r0 = 0 (mod NA): k1 = position mod NA
+    const int q0 = qmin - r0;
+    const int step = (int)(((int64_t)NA * j) % N);     // twiddle index step between q and q + NA
+    cd z[NA];
+    int t[NA];
+#pragma unroll
+    for (int k1 = 0; k1 < NA; k1++) {
+        z[k1] = cmake(0.0, 0.0);
+        int tt = (int)(((int64_t)(q0 + k1) * j) % N);
+        t[k1] = tt < 0 ? tt + N : tt;
+    }
+    for (int base = -r0; base < nq; base += NA) {      // NA independent accumulations per trip
+#pragma unroll
+        for (int k1 = 0; k1 < NA; k1++) {
+            const int qi = base + k1;
+            if (qi >= 0 && qi < nq) {
+                const cd w = tw[t[k1]];                // exp(-2 pi i t/N): the inverse needs the conjugate
+                z[k1] = cfma(cmake(w.x, -w.y), ld(qi), z[k1]);
+            }
+            t[k1] += step;
+            if (t[k1] >= N) t[k1] -= N;
+        }
+    }
+    if constexpr (NA > 1) {                            // inverse butterfly = conj o forward o conj
+#pragma unroll
+        for (int k1 = 0; k1 < NA; k1++) z[k1].y = -z[k1].y;
+        Bfly<NA>::run(z);
+#pragma unroll
+        for (int s = 0; s < NA; s++) z[s].y = -z[s].y;
+    }
+#pragma unroll
+    for (int s = 0; s < NA; s++) st(j + NB * s, z[s]);
+}
+
+// radix of the register butterfly for an axis of length n (1: direct sum)
+static inline int pw_pick_na(int n) { return n % 12 == 0 ? 12 : n % 8 == 0 ? 8 : 1; }
+
 // One CTA per (x-plane j1, band).  Shared memory (cd): tw2[N2] | tw3[N3] | P[nq2][nq3] | Y[N2][nq3].
-//   Y[j2][q3i] = sum_q2i P[q2i][q3i] exp(+2 pi i q2 j2 / N2)
-//   u[j2][j3]  = sum_q3i Y[j2][q3i] exp(+2 pi i q3 j3 / N3)      4 rows per thread share the twiddle
-#define PW_ROWS 4
-__global__ void __launch_bounds__(256) pw_zy_kernel(const cd *__restrict__ T1, const cd *__restrict__ tw2,
-                                                   const cd *__restrict__ tw3, int N1, int N2, int N3, int q2min, int nq2,
-                                                   int q3min, int nq3, cd *__restrict__ out) {
+//   y: Y[.][q3i] from the box column P[.][q3i]   (task = (j < N2/NA2, q3i))
+//   z: u[j2][.]  from the row Y[j2][.]           (task = (j2, j < N3/NA3); the NA3 stores of a task are 16 bytes at a
+//      stride of N3/NA3 elements, consecutive j -> consecutive addresses)
+template <int NA2, int NA3>
+__global__ void __launch_bounds__(128, 3) pw_zy_kernel(const cd *__restrict__ T1, const cd *__restrict__ tw2,
+                                                      const cd *__restrict__ tw3, int N1, int N2, int N3, int q2min, int nq2,
+                                                      int q3min, int nq3, cd *__restrict__ out) {
     extern __shared__ __align__(16) unsigned char pw_smem[];
     cd *tw2s = reinterpret_cast<cd *>(pw_smem);
     cd *tw3s = tw2s + N2;
@@ -53,43 +101,34 @@ __global__ void __launch_bounds__(256) pw_zy_kernel(const cd *__restrict__ T1, c
     const cd *Tp = T1 + ((size_t)b * N1 + j1) * ncol;
     for (int i = tid; i < ncol; i += nth) P[i] = Tp[i];
     __syncthreads();
-    for (int i = tid; i < N2 * nq3; i += nth) {
-        const int j2 = i / nq3, c3 = i - j2 * nq3;
-        int t = (int)(((int64_t)q2min * j2) % N2);
-        if (t < 0) t += N2;
-        cd acc = cmake(0.0, 0.0);
-        for (int q = 0; q < nq2; q++) {
-            const cd w = tw2s[t];
-            acc = cfma(cmake(w.x, -w.y), P[q * nq3 + c3], acc);
-            t += j2;
-            if (t >= N2) t -= N2;
-        }
-        Y[i] = acc;
+    const int NB2 = N2 / NA2, NB3 = N3 / NA3;
+    for (int i = tid; i < NB2 * nq3; i += nth) {
+        const int j = i / nq3, c3 = i - j * nq3;
+        pw_expand_line<NA2>(N2, j, q2min, nq2, tw2s, [&](int qi) { return P[qi * nq3 + c3]; },
+                            [&](int n, cd v) { Y[n * nq3 + c3] = v; });
     }
     __syncthreads();
     cd *op = out + ((size_t)b * N1 + j1) * N2 * N3;
-    const int nrb = (N2 + PW_ROWS - 1) / PW_ROWS;
-    for (int i = tid; i < nrb * N3; i += nth) {
-        const int rb = i / N3, j3 = i - rb * N3;
-        const int r0 = rb * PW_ROWS;
-        int t = (int)(((int64_t)q3min * j3) % N3);
-        if (t < 0) t += N3;
-        cd acc[PW_ROWS];
-#pragma unroll
-        for (int r = 0; r < PW_ROWS; r++) acc[r] = cmake(0.0, 0.0);
-        for (int q = 0; q < nq3; q++) {
-            const cd w0 = tw3s[t];
-            const cd w = cmake(w0.x, -w0.y);
-#pragma unroll
-            for (int r = 0; r < PW_ROWS; r++)
-                if (r0 + r < N2) acc[r] = cfma(w, Y[(r0 + r) * nq3 + q], acc[r]);
-            t += j3;
-            if (t >= N3) t -= N3;
-        }
-#pragma unroll
-        for (int r = 0; r < PW_ROWS; r++)
-            if (r0 + r < N2) op[(size_t)(r0 + r) * N3 + j3] = acc[r];
+    for (int i = tid; i < N2 * NB3; i += nth) {
+        const int j2 = i / NB3, j = i - j2 * NB3;
+        const cd *yr = Y + (size_t)j2 * nq3;
+        cd *orow = op + (size_t)j2 * N3;
+        pw_expand_line<NA3>(N3, j, q3min, nq3, tw3s, [&](int qi) { return yr[qi]; }, [&](int n, cd v) { orow[n] = v; });
     }
+}
+
+typedef void (*PwZyKernel)(const cd *, const cd *, const cd *, int, int, int, int, int, int, int, cd *);
+static inline PwZyKernel pw_zy_pick(int N2, int N3) {
+    const int a2 = pw_pick_na(N2), a3 = pw_pick_na(N3);
+    if (a2 == 12 && a3 == 12) return pw_zy_kernel<12, 12>;
+    if (a2 == 12 && a3 == 8) return pw_zy_kernel<12, 8>;
+    if (a2 == 8 && a3 == 12) return pw_zy_kernel<8, 12>;
+    if (a2 == 8 && a3 == 8) return pw_zy_kernel<8, 8>;
+    if (a2 == 12) return pw_zy_kernel<12, 1>;
+    if (a2 == 8) return pw_zy_kernel<8, 1>;
+    if (a3 == 12) return pw_zy_kernel<1, 12>;
+    if (a3 == 8) return pw_zy_kernel<1, 8>;
+    return pw_zy_kernel<1, 1>;
 }
 
 // out[b][j] = in[b][j'] (conjugated under time reversal), j'_i = sum_k S[i][k] j_k mod N_i with the integer matrix

@@ -823,14 +823,15 @@ int rpa_pw_to_grid(rpa_chi0_t *h, int32_t n_bands, int32_t n_pw, const int32_t *
     cd *T1 = reinterpret_cast<cd *>(base + table_bytes);
     CUDA_TRY(cudaMemcpyAsync(d_table, table.data(), table.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
     CUDA_TRY(cudaStreamSynchronize(st));   // `table` is pageable host memory about to go out of scope
-    if (smem > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(pw_zy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const PwZyKernel zy = pw_zy_pick(N2, N3);
+    if (smem > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(zy, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const int chunk = (int)std::min<size_t>((size_t)n_bands, std::min<size_t>(65535, (scratch - table_bytes) / t1_band));
     for (int b0 = 0; b0 < n_bands; b0 += chunk) {
         const int nb = std::min(chunk, n_bands - b0);
         pw_xaxis_kernel<<<dim3((unsigned)((ncol + 127) / 128), N1, nb), 128, 0, st>>>(
             (const cd *)C + (size_t)b0 * n_pw, n_pw, d_table, h->ptr<cd>(L.tw1), N1, qmin[0], (int)nq1, (int)ncol, T1);
-        pw_zy_kernel<<<dim3(N1, nb), 256, smem, st>>>(T1, h->ptr<cd>(L.tw2), h->ptr<cd>(L.tw3), N1, N2, N3, qmin[1], (int)nq2,
-                                                     qmin[2], (int)nq3, (cd *)psi_out + (size_t)b0 * N);
+        zy<<<dim3(N1, nb), 128, smem, st>>>(T1, h->ptr<cd>(L.tw2), h->ptr<cd>(L.tw3), N1, N2, N3, qmin[1], (int)nq2, qmin[2],
+                                           (int)nq3, (cd *)psi_out + (size_t)b0 * N);
         h->launches += 2;
         CUDA_TRY(cudaGetLastError());
     }
