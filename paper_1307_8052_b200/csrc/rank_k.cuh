@@ -64,14 +64,15 @@ __global__ void weights_kernel(double *__restrict__ w, int64_t ldw, int K, int K
 
 // Nb[Kpad][ldn] (rows >= K are zero; frequency iw reads Nb + iw*strideN, strideN = 0 when SHARED_N), w[n_omega][ldw],
 // S[n_omega][ng][ldS] (lower triangle accumulated).  Only rows / columns g >= g0 are touched (g0 % 1 == 0; tiles
-// start at g0).  Kpad % KC == 0.  grid = (ntiles_lower(ng - g0), ceil(n_omega / Cfg::NW), ksplit).
+// start at g0).  Kpad % KC == 0.  grid = (tiles selected by tile_mode, ceil(n_omega / Cfg::NW), ksplit).
 // ksplit > 1 (chi0 accumulation only): CTA z takes the z-th slice of the K chunks and adds its tile with
 // red.global.add.f64, so that tiles x frequency pairs x slices fill the last wave of the grid (the host picks
 // ksplit); the order of those additions is not fixed, i.e. S is then reproducible to rounding, not bitwise.
 template <bool SHARED_N>
 __global__ void __launch_bounds__(rk::Cfg<SHARED_N>::THREADS, rk::Cfg<SHARED_N>::MIN_CTAS)
 rank_k_kernel(const cd *__restrict__ Nb, int64_t ldn, int64_t strideN, int Kpad, const double *__restrict__ w,
-              int64_t ldw, cd *__restrict__ S, int64_t ldS, int64_t strideS, int ng, int g0, int n_omega) {
+              int64_t ldw, cd *__restrict__ S, int64_t ldS, int64_t strideS, int ng, int g0, int n_omega,
+              int tile_mode) {
     using namespace rk;
     constexpr int STAGES = Cfg<SHARED_N>::NSTAGES;
     constexpr int STAGE_BYTES = Cfg<SHARED_N>::STAGE_BYTES;
@@ -83,11 +84,20 @@ rank_k_kernel(const cd *__restrict__ Nb, int64_t ldn, int64_t strideN, int Kpad,
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     // lower-triangle tile (ti >= tj) from the linear index
+    // tile_mode 0: all lower tiles; 1: only the first tile column (tj = 0, blockIdx.x = ti); 2: all the others
+    // (the lower tiles of the triangle shifted by one tile) -- the Cholesky look-ahead of rpa_ec_q uses 1 and 2
     const int t = blockIdx.x;
-    int ti = (int)((sqrt(8.0 * (double)t + 1.0) - 1.0) * 0.5);
-    while ((ti + 1) * (ti + 2) / 2 <= t) ti++;
-    while (ti * (ti + 1) / 2 > t) ti--;
-    const int tj = t - ti * (ti + 1) / 2;
+    int ti, tj;
+    if (tile_mode == 1) {
+        ti = t;
+        tj = 0;
+    } else {
+        ti = (int)((sqrt(8.0 * (double)t + 1.0) - 1.0) * 0.5);
+        while ((ti + 1) * (ti + 2) / 2 <= t) ti++;
+        while (ti * (ti + 1) / 2 > t) ti--;
+        tj = t - ti * (ti + 1) / 2;
+        if (tile_mode == 2) { ti++; tj++; }
+    }
     const int row0 = g0 + ti * T, col0 = g0 + tj * T;
     const int om0 = blockIdx.y * NW;
     const int n_om = min(NW, n_omega - om0);

@@ -151,7 +151,7 @@ void make_layout(const int32_t grid[3], const Sphere &sp, int n_omega, int max_b
     L->I = take((size_t)L->sub_pairs * L->I_pair_bytes);
     L->T = take((size_t)MAX_SLOTS * std::max(max_proj, 0) * L->ldn * sizeof(cd));
     L->M = take((size_t)L->ec_group * ng * ng * sizeof(cd));
-    L->Lt = take((size_t)L->ec_group * CH_NB * L->ldn * sizeof(cd));
+    L->Lt = take(2 * (size_t)L->ec_group * CH_NB * L->ldn * sizeof(cd));   // two panels: Cholesky look-ahead
     L->wneg = take((size_t)L->ec_group * CH_NB * sizeof(double));
     L->tw1 = take((size_t)grid[0] * sizeof(cd));
     L->tw2 = take((size_t)grid[1] * sizeof(cd));
@@ -199,6 +199,8 @@ struct rpa_chi0 {
     size_t pd_smem;
     PdZyKernel zy_kernel = nullptr;   // low-instruction-count z+y kernel (planes that fit one CTA), else pd_kernel
     int zy_G = 1, zy_threads = 0, zy_ctas_per_sm = 1, n_sm = 148;
+    cudaStream_t side = nullptr;       // panel factorisations of rpa_ec_q run here, ahead of the trailing updates
+    cudaEvent_t ev_panel[2] = {nullptr, nullptr}, ev_col = nullptr, ev_fork = nullptr;
     size_t zy_smem = 0;
     unsigned char *ws;
     // profiling
@@ -448,6 +450,13 @@ int rpa_chi0_create(rpa_chi0_t **out, const int32_t grid[3], const double cell[9
         int dev = 0;
         CREATE_TRY(cudaGetDevice(&dev));
         CREATE_TRY(cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, dev));
+        // highest priority: the block scheduler then places the (small) panel grids as soon as slots free up, instead
+        // of after the last CTA of the trailing update in flight has been dispatched
+        int prio_lo = 0, prio_hi = 0;
+        CREATE_TRY(cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi));
+        CREATE_TRY(cudaStreamCreateWithPriority(&h->side, cudaStreamNonBlocking, prio_hi));
+        for (cudaEvent_t *e : {&h->ev_panel[0], &h->ev_panel[1], &h->ev_col, &h->ev_fork})
+            CREATE_TRY(cudaEventCreateWithFlags(e, cudaEventDisableTiming));
     }
     if (h->zy_kernel) {
         CREATE_TRY(cudaFuncSetAttribute(h->zy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->zy_smem));
@@ -489,7 +498,7 @@ int rpa_chi0_create(rpa_chi0_t **out, const int32_t grid[3], const double cell[9
         CREATE_TRY(cudaMemcpyAsync(h->ws + L.wneg, wneg.data(), wneg.size() * sizeof(double), cudaMemcpyHostToDevice, h->stream));
         CREATE_TRY(cudaStreamSynchronize(h->stream));
     }
-    CREATE_TRY(cudaMemsetAsync(h->ws + L.Lt, 0, (size_t)L.ec_group * CH_NB * L.ldn * sizeof(cd), h->stream));
+    CREATE_TRY(cudaMemsetAsync(h->ws + L.Lt, 0, 2 * (size_t)L.ec_group * CH_NB * L.ldn * sizeof(cd), h->stream));
     CREATE_TRY(cudaMemsetAsync(h->ws + L.S, 0, (size_t)n_omega * sp.ng * L.ldS * sizeof(cd), h->stream));
     CREATE_TRY(cudaMemsetAsync(h->ws + L.Nbuf, 0, (size_t)L.Kmax * L.ldn * sizeof(cd), h->stream));
     CREATE_TRY(cudaStreamSynchronize(h->stream));
@@ -655,7 +664,7 @@ int rpa_chi0_add_kpoint(rpa_chi0_t *h, double kweight, int32_t n_occ, const void
                 const int ksplit = pick_ksplit(units, Kpad / rk::KC, h->n_sm);
                 rank_k_kernel<true><<<dim3(ntiles_lower(ng, rk::T), (h->n_omega + rk::Cfg<true>::NW - 1) / rk::Cfg<true>::NW, ksplit),
                                       rk::Cfg<true>::THREADS, rk::Cfg<true>::SMEM_BYTES, st>>>(
-                    Nbuf, L.ldn, 0, Kpad, w, L.ldw, h->ptr<cd>(L.S), L.ldS, (int64_t)ng * L.ldS, ng, 0, h->n_omega);
+                    Nbuf, L.ldn, 0, Kpad, w, L.ldw, h->ptr<cd>(L.S), L.ldS, (int64_t)ng * L.ldS, ng, 0, h->n_omega, 0);
                 CUDA_TRY(cudaGetLastError());
             }
         }
@@ -697,19 +706,37 @@ int rpa_ec_q(rpa_chi0_t *h, const double *v_G, double *ec_ha, double *e_omega) {
         ec_build_kernel<<<dim3((ng + 127) / 128, ng, nm), 128, 0, st>>>(S + (size_t)iw0 * strideS, L.ldS, strideS, ng, scale, d_v, M);
         ec_trace_kernel<<<nm, 256, 0, st>>>(S + (size_t)iw0 * strideS, L.ldS, strideS, ng, scale, d_v, d_tr);
         h->launches += 2;
-        for (int k0 = 0; k0 < ng; k0 += CH_NB) {
+        // Look-ahead: the panel of step k+1 only needs the first tile column of the trailing update of step k.  Panels run
+        // on the side stream, updates on the caller's stream; per step the update is split into that first tile column
+        // (then the next panel may start) and the rest (which the next panel overlaps).  Two panel buffers alternate.
+        const size_t lt_elems = (size_t)L.ec_group * CH_NB * L.ldn;
+        CUDA_TRY(cudaEventRecord(h->ev_fork, st));
+        CUDA_TRY(cudaStreamWaitEvent(h->side, h->ev_fork, 0));
+        int step = 0;
+        for (int k0 = 0; k0 < ng; k0 += CH_NB, step++) {
             const int rest = ng - (k0 + CH_NB);
+            cd *Lt = h->ptr<cd>(L.Lt) + (size_t)(step & 1) * lt_elems;
             // diagonal block (factored redundantly by every CTA) + panel solve in one launch
-            chol_panel_kernel<<<dim3(std::max(1, (rest + 127) / 128), nm), 128, 0, st>>>(M, ng, k0, h->ptr<cd>(L.Lt), L.ldn,
-                                                                                     d_flag, d_ld);
+            chol_panel_kernel<<<dim3(std::max(1, (rest + 127) / 128), nm), 128, 0, h->side>>>(M, ng, k0, Lt, L.ldn, d_flag, d_ld);
+            CUDA_TRY(cudaEventRecord(h->ev_panel[step & 1], h->side));
+            CUDA_TRY(cudaStreamWaitEvent(st, h->ev_panel[step & 1], 0));
             h->launches += 1;
             if (rest > 0) {
                 // trailing update M[g][g'] -= sum_t L[g][t] conj(L[g'][t]), g >= g' >= k0 + 32, on the DMMA path
-                rank_k_kernel<false><<<dim3(ntiles_lower(rest, rk::T), nm), rk::Cfg<false>::THREADS,
-                                       rk::Cfg<false>::SMEM_BYTES, st>>>(
-                    h->ptr<cd>(L.Lt), L.ldn, (int64_t)CH_NB * L.ldn, CH_NB, h->ptr<double>(L.wneg), CH_NB, M, ng,
-                    (int64_t)ng * ng, ng, k0 + CH_NB, nm);
-                h->launches += 1;
+                const int nt = (rest + rk::T - 1) / rk::T;
+                for (int mode = 1; mode <= 2; mode++) {
+                    const int tiles = mode == 1 ? nt : ntiles_lower(rest, rk::T) - nt;
+                    if (tiles > 0) {
+                        rank_k_kernel<false><<<dim3(tiles, nm), rk::Cfg<false>::THREADS, rk::Cfg<false>::SMEM_BYTES, st>>>(
+                            Lt, L.ldn, (int64_t)CH_NB * L.ldn, CH_NB, h->ptr<double>(L.wneg), CH_NB, M, ng, (int64_t)ng * ng, ng,
+                            k0 + CH_NB, nm, mode);
+                        h->launches += 1;
+                    }
+                    if (mode == 1) {
+                        CUDA_TRY(cudaEventRecord(h->ev_col, st));
+                        CUDA_TRY(cudaStreamWaitEvent(h->side, h->ev_col, 0));
+                    }
+                }
             }
         }
         CUDA_TRY(cudaGetLastError());
@@ -775,6 +802,9 @@ int rpa_chi0_accumulators(const rpa_chi0_t *h, void **S, size_t *bytes) {
 
 void rpa_chi0_destroy(rpa_chi0_t *h) {
     if (!h) return;
+    if (h->side) cudaStreamDestroy(h->side);
+    for (cudaEvent_t e : {h->ev_panel[0], h->ev_panel[1], h->ev_col, h->ev_fork})
+        if (e) cudaEventDestroy(e);
     for (auto &ev : h->events) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
     for (auto &e : h->pool) cudaEventDestroy(e);
     delete h;
