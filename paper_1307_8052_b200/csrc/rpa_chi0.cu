@@ -21,6 +21,7 @@
 #include "orbitals.cuh"
 #include "paw.cuh"
 #include "rank_k.cuh"
+#include "rank_k3m.cuh"
 
 namespace {
 
@@ -199,6 +200,7 @@ struct rpa_chi0 {
     size_t pd_smem;
     PdZyKernel zy_kernel = nullptr;   // low-instruction-count z+y kernel (planes that fit one CTA), else pd_kernel
     int zy_G = 1, zy_threads = 0, zy_ctas_per_sm = 1, n_sm = 148;
+    bool use_3m = true;                // rank_k3m_kernel (3-multiplication complex product) for the chi0 accumulation
     cudaStream_t side = nullptr;       // panel factorisations of rpa_ec_q run here, ahead of the trailing updates
     cudaEvent_t ev_panel[2] = {nullptr, nullptr}, ev_col = nullptr, ev_fork = nullptr;
     size_t zy_smem = 0;
@@ -466,6 +468,8 @@ int rpa_chi0_create(rpa_chi0_t **out, const int32_t grid[3], const double cell[9
         h->zy_ctas_per_sm = per_sm;
     }
     CREATE_TRY(cudaFuncSetAttribute(rank_k_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, rk::Cfg<true>::SMEM_BYTES));
+    CREATE_TRY(cudaFuncSetAttribute(rank_k3m_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, rk3::SMEM_BYTES));
+    h->use_3m = getenv("RPA_RANK_K_4M") == nullptr;
     CREATE_TRY(cudaFuncSetAttribute(rank_k_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, rk::Cfg<false>::SMEM_BYTES));
 
     // tables: twiddles in extended precision, box -> sphere map
@@ -660,11 +664,18 @@ int rpa_chi0_add_kpoint(rpa_chi0_t *h, double kweight, int32_t n_occ, const void
             // S6: rank-K update of every frequency
             {
                 StageTimer tm(h, 4, 1);
-                const int units = ntiles_lower(ng, rk::T) * ((h->n_omega + rk::Cfg<true>::NW - 1) / rk::Cfg<true>::NW);
-                const int ksplit = pick_ksplit(units, Kpad / rk::KC, h->n_sm);
-                rank_k_kernel<true><<<dim3(ntiles_lower(ng, rk::T), (h->n_omega + rk::Cfg<true>::NW - 1) / rk::Cfg<true>::NW, ksplit),
-                                      rk::Cfg<true>::THREADS, rk::Cfg<true>::SMEM_BYTES, st>>>(
-                    Nbuf, L.ldn, 0, Kpad, w, L.ldw, h->ptr<cd>(L.S), L.ldS, (int64_t)ng * L.ldS, ng, 0, h->n_omega, 0);
+                if (h->use_3m) {
+                    const int units = ntiles_lower(ng, rk3::T) * h->n_omega;
+                    const int ksplit = pick_ksplit(units, Kpad / rk3::KC, h->n_sm);
+                    rank_k3m_kernel<<<dim3(ntiles_lower(ng, rk3::T), h->n_omega, ksplit), rk3::THREADS, rk3::SMEM_BYTES, st>>>(
+                        Nbuf, L.ldn, Kpad, w, L.ldw, h->ptr<cd>(L.S), L.ldS, (int64_t)ng * L.ldS, ng);
+                } else {
+                    const int units = ntiles_lower(ng, rk::T) * ((h->n_omega + rk::Cfg<true>::NW - 1) / rk::Cfg<true>::NW);
+                    const int ksplit = pick_ksplit(units, Kpad / rk::KC, h->n_sm);
+                    rank_k_kernel<true><<<dim3(ntiles_lower(ng, rk::T), (h->n_omega + rk::Cfg<true>::NW - 1) / rk::Cfg<true>::NW, ksplit),
+                                          rk::Cfg<true>::THREADS, rk::Cfg<true>::SMEM_BYTES, st>>>(
+                        Nbuf, L.ldn, 0, Kpad, w, L.ldw, h->ptr<cd>(L.S), L.ldS, (int64_t)ng * L.ldS, ng, 0, h->n_omega, 0);
+                }
                 CUDA_TRY(cudaGetLastError());
             }
         }
