@@ -32,10 +32,9 @@ from paper_1307_8052_b200 import workload as W  # noqa: E402
 
 METRIC = "chi0 pair transitions/s (rank-K FP64 TFLOP/s in roofline), 1 q-point, all omega"
 UNIT = "transitions/s"
-# ncu --set full capture of rank_k_kernel<1> on configs[1] (profiles/r1c_bench_cfg1.md): dram__bytes_read.sum +
-# dram__bytes_write.sum per launch (781.6 + 175.6 MB); other configs have no capture
-RANK_K_DRAM_TRAFFIC_BYTES = {1: 957.2e6}
-
+# ncu --set full capture of rank_k3m_kernel on configs[1] (profiles/r1d_bench_cfg1.md): dram__bytes_read.sum +
+# dram__bytes_write.sum per launch (622.0 + 499.6 MB); other configs have no capture
+RANK_K_DRAM_TRAFFIC_BYTES = {1: 1121.6e6}
 
 def rank_k_useful_flops(ng, n_omega, n_pairs):
     """8 flop per complex MAC on one triangle: 4 nG (nG+1) n_omega per pair."""
@@ -287,11 +286,15 @@ def run_ours(args, cfg):
             "e2e": {"value": pairs_total / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e,
                     "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": 8 * (1 + cfg.n_omega) + 16},
             "gpu_launches": int(launches),
-            "roofline": {"kernel": "rank_k_kernel", "bound": "tensor", "achieved": rk_tf, "peak": peak_tf, "unit": "TFLOP/s",
+            "roofline": {"kernel": "rank_k3m_kernel", "bound": "tensor", "achieved": rk_tf, "peak": peak_tf, "unit": "TFLOP/s",
                          "frac": rk_tf / peak_tf if peak_tf else None, "traffic": RANK_K_DRAM_TRAFFIC_BYTES.get(cfg.index),
                          "peak_source": "FP64 DMMA issue rate measured live by rpa_probe_fp64_tensor_peak (register-only "
                                         "mma.sync.m8n8k4.f64, all SMs); MEASURED_PEAKS.json has no FP64 entry",
                          "peak_alt_tflops_from_bf16": peaks.get("bf16_tflops", 0) * 40.0 / 2250.0,
+                         "note": "achieved = ALGORITHMIC flops (8 per complex multiply-add on one triangle) / time; the "
+                                 "kernel forms the complex product with 3 real multiplications (3M), so it EXECUTES 3/4 of "
+                                 "them: executed_frac = tensor-pipe flops actually issued / peak",
+                         "executed_frac": 0.75 * rk_tf / peak_tf if peak_tf else None,
                          "flops_per_launch": rk_flops, "ms_per_launch": rk_ms, "launches": rk_launches,
                          "share_of_step": float(stage_ms[4]) / args.steps / ms_step},
             "stages": {"ms_per_step": {n: float(t) / args.steps for n, t in zip(B.STAGE_NAMES, stage_ms)},

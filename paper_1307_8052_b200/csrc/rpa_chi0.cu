@@ -271,13 +271,13 @@ int ntiles_lower(int n, int t) {
 
 // K slices of the rank-K launch: one CTA per SM, `units` equal work items (tile x frequency pair).  With s slices
 // the grid needs ceil(units s / n_sm) rounds of 1/s of an item each; take the s that minimises that time, charging
-// 0.4 % per extra slice for its prologue / atomic epilogue, and keep at least 16 chunks (256 pairs) per slice.
+// 1 % per extra slice for its prologue / atomic epilogue, and keep at least 16 chunks (256 pairs) per slice.
 int pick_ksplit(int units, int nchunks, int n_sm) {
     int best = 1;
     double best_cost = 1e300;
     for (int s = 1; s <= 8 && nchunks / s >= 16; s++) {
         const double rounds = (double)(((int64_t)units * s + n_sm - 1) / n_sm) / s;
-        const double cost = rounds * (1.0 + 0.004 * (s - 1));
+        const double cost = rounds * (1.0 + 0.01 * (s - 1));
         if (cost < best_cost * (1.0 - 1e-9)) { best_cost = cost; best = s; }
     }
     return best;

@@ -196,3 +196,17 @@ def test_pipelined_host_upload_matches_single_call():
                 assert rel_fro(b, a[i]) <= 1e-12
     finally:
         h.close()
+
+
+def test_four_multiplication_rank_k_path_still_agrees():
+    """RPA_RANK_K_4M=1 (read at rpa_chi0_create) selects rank_k_kernel<true>, the 4-multiplication real-view
+    kernel that rank_k3m_kernel replaced for the chi0 accumulation; it stays the reference implementation of the
+    update (and its <false> variant serves the Cholesky), so its parity is kept under test."""
+    import os
+    import subprocess
+    import sys
+    env = dict(os.environ, RPA_RANK_K_4M="1")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, "-m", "pytest", "-x", "-q", "-m", "gpu", "tests/test_gpu_parity.py", "-k",
+                        "config0_toy_full or tiny_skewed or config2_bulk"], cwd=root, env=env, capture_output=True, text=True)
+    assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
