@@ -10,7 +10,7 @@
 // ulp of |S|, far inside the 1e-10 relative Frobenius tolerance of the path).
 //
 // One CTA = one 64 x 64 complex tile of the lower triangle, ONE frequency; 8 consumer warps, each 32 rows x 16 columns
-// (3 x 4 x 2 DMMA accumulators = 96 registers) + the TMA producer warp with the 5-stage ring of rank_k.cuh.  A DMMA
+// (3 x 4 x 2 DMMA accumulators = 96 registers) + a TMA producer warp with a 3-stage ring of 32-pair chunks.  A DMMA
 // k-step covers 4 pairs; a lane loads its (row, pair) / (column, pair) element with one LDS.128 (row pitch = 32 mod
 // 128 bytes: the 8 lanes of a quarter-warp hit 8 distinct 16-byte bank groups) and forms a + b, w c, w d, w (c - d)
 // on the FP64 ALU (10 operations per 24 DMMA).
@@ -19,8 +19,8 @@
 
 namespace rk3 {
 constexpr int T = 64;
-constexpr int KC = 16;                      // pairs per stage
-constexpr int STAGES = 5;
+constexpr int KC = 32;                      // pairs per stage
+constexpr int STAGES = 3;
 constexpr int CONSUMER_WARPS = 8;
 constexpr int THREADS = (CONSUMER_WARPS + 1) * 32;
 constexpr int PITCH = T * 16 + 32;          // bytes per pair row (= 32 mod 128)
@@ -30,7 +30,7 @@ constexpr int STAGE_BYTES = 2 * TILE_BYTES + W_BYTES;
 constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 2 * STAGES * 8;
 }  // namespace rk3
 
-// Nb[Kpad][ldn] (rows >= K zero), w[n_omega][ldw], S[n_omega][ng][ldS] (lower triangle accumulated), Kpad % 16 == 0.
+// Nb[Kpad][ldn] (rows >= K zero), w[n_omega][ldw], S[n_omega][ng][ldS] (lower triangle accumulated), Kpad % 32 == 0.
 // grid = (ntiles_lower(ng), n_omega, ksplit); ksplit as in rank_k_kernel (atomic tile adds when > 1).
 __global__ void __launch_bounds__(rk3::THREADS, 1)
 rank_k3m_kernel(const cd *__restrict__ Nb, int64_t ldn, int Kpad, const double *__restrict__ w, int64_t ldw,
@@ -74,9 +74,9 @@ rank_k3m_kernel(const cd *__restrict__ Nb, int64_t ldn, int Kpad, const double *
             unsigned char *st = rk_smem + s * STAGE_BYTES;
             if (lane == 0) mbar_arrive_expect_tx(&full[s], stage_tx);
             __syncwarp();
-            const cd *Nw = Nb + ((size_t)(it0 + it) * KC + (lane & 15)) * ldn;
-            if (lane < 16) bulk_g2s(st + lane * PITCH, Nw + row0, rowbytes, &full[s]);
-            else bulk_g2s(st + TILE_BYTES + (lane - 16) * PITCH, Nw + col0, colbytes, &full[s]);
+            const cd *Nw = Nb + ((size_t)(it0 + it) * KC + lane) * ldn;   // KC = 32: one pair row per lane
+            bulk_g2s(st + lane * PITCH, Nw + row0, rowbytes, &full[s]);
+            bulk_g2s(st + TILE_BYTES + lane * PITCH, Nw + col0, colbytes, &full[s]);
             if (lane == 0) bulk_g2s(st + 2 * TILE_BYTES, w + (size_t)iw * ldw + (size_t)(it0 + it) * KC, KC * 8, &full[s]);
         }
         return;

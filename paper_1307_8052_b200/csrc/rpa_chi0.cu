@@ -49,6 +49,8 @@ constexpr int MAX_PROJ = 1 << 16;
 constexpr int EC_GROUP = 16;           // frequencies factorised together in rpa_ec_q
 constexpr size_t I_BUDGET = 64u << 20; // pruned intermediate kept L2-sized
 constexpr int NSTAGE = 5;
+constexpr int K_ALIGN = 32;            // pairs per batch are padded to the chunk size of both rank-K kernels (16, 32)
+static_assert(K_ALIGN % rk::KC == 0 && K_ALIGN % rk3::KC == 0, "batch padding");
 
 size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
@@ -130,7 +132,7 @@ bool valid_dims(const int32_t grid[3], const double cell[9], const double q[3], 
 void make_layout(const int32_t grid[3], const Sphere &sp, int n_omega, int max_batch, int max_proj, Layout *L) {
     const int ng = sp.ng;
     int Kmax = max_batch <= 0 ? DEFAULT_BATCH : max_batch;
-    Kmax = (int)align_up((size_t)std::max(Kmax, rk::KC), rk::KC);
+    Kmax = (int)align_up((size_t)std::max(Kmax, K_ALIGN), K_ALIGN);
     L->Kmax = Kmax;
     L->ldS = ng;
     L->ldn = (int64_t)align_up((size_t)ng, 8);
@@ -580,7 +582,7 @@ int rpa_chi0_add_kpoint(rpa_chi0_t *h, double kweight, int32_t n_occ, const void
     int rows_per_batch = 1, mchunk = n_unocc;
     if (n_unocc >= Kmax) {
         const int nch = (n_unocc + Kmax - 1) / Kmax;
-        mchunk = (int)align_up((size_t)(n_unocc + nch - 1) / nch, rk::KC);
+        mchunk = (int)align_up((size_t)(n_unocc + nch - 1) / nch, K_ALIGN);
         mchunk = std::min(mchunk, Kmax);
     } else {
         rows_per_batch = std::max(1, std::min(MAX_SLOTS, Kmax / n_unocc));
@@ -597,7 +599,7 @@ int rpa_chi0_add_kpoint(rpa_chi0_t *h, double kweight, int32_t n_occ, const void
         for (int m0 = 0; m0 < n_unocc; m0 += mchunk) {
             const int mlen = std::min(mchunk, n_unocc - m0);
             const int K = nslots * mlen;
-            const int Kpad = (int)align_up((size_t)K, rk::KC);
+            const int Kpad = (int)align_up((size_t)K, K_ALIGN);
             // rows K..Kpad of the N buffer must be zero (they meet zero weights, but 0 * NaN is NaN)
             if (Kpad > K) CUDA_TRY(cudaMemsetAsync(Nbuf + (size_t)K * L.ldn, 0, (size_t)(Kpad - K) * L.ldn * sizeof(cd), st));
 
