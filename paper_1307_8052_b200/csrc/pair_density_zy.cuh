@@ -120,8 +120,12 @@ template <int N3, int NA3, int DLO, int DHI, int N2, int NA2, int NW, int LPW, i
 struct PdZy {
     static constexpr int NB3 = N3 / NA3, NB2 = N2 / NA2;
     static constexpr int K1PT = (NA3 + NB3 - 1) / NB3;
-    static constexpr int XP = NB3 + ((NB3 & 1) ? 0 : 1);  // pitch of one k1 row of the exchange line (odd: conflict-free)
-    static constexpr int XLINE = NA3 * XP;
+    // exchange line of the z stage: element (k1, j) at k1 XP + j, lines XLINE apart (units of 16 bytes).  Pitches found by
+    // enumerating the quarter-warp bank groups of the pass-A stores (k1 fixed) and pass-B loads (j fixed) of this lane
+    // layout: conflict-free for NB3 = 2, 3, 8, 16, 10 % over the minimum for NB3 = 14
+    static constexpr int XP = NB3 == 2 ? 3 : NB3 == 3 ? 9 : NB3 == 14 ? 17 : NB3 + ((NB3 & 1) ? 0 : 1);
+    static constexpr int XLINE = NB3 == 2 ? 26 : NB3 == 3 ? 75 : NB3 == 14 ? 206 : NA3 * XP;
+    static_assert(XLINE >= (NA3 - 1) * XP + NB3, "exchange line too short");
     static constexpr int ROWS = NW * LPW;                 // z lines per chunk
     static constexpr int NCH = (N2 + ROWS - 1) / ROWS;
     static constexpr int NTH = NW * 32;
