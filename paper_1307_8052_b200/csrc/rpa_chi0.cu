@@ -47,7 +47,7 @@ constexpr int MAX_BANDS = 1 << 17;     // eps/f scratch
 constexpr int MAX_ATOMS = 4096;
 constexpr int MAX_PROJ = 1 << 16;
 constexpr int EC_GROUP = 16;           // frequencies factorised together in rpa_ec_q
-constexpr size_t I_BUDGET = 64u << 20; // pruned intermediate kept L2-sized
+constexpr size_t I_BUDGET = (size_t)4 << 30; // pruned intermediate of a whole batch when it fits (fewer, larger launches beat L2 residency)
 constexpr int NSTAGE = 5;
 constexpr int K_ALIGN = 32;            // pairs per batch are padded to the chunk size of both rank-K kernels (16, 32)
 static_assert(K_ALIGN % rk::KC == 0 && K_ALIGN % rk3::KC == 0, "batch padding");
