@@ -277,7 +277,7 @@ def run_ours(args, cfg):
             "dtype": "f64 (complex128)", "data": "synthetic",
             "config": {"workload": f"configs[{cfg.index}] {cfg.name}", "grid": list(cfg.grid), "n_k_per_gpu": len(my_k),
                        "n_occ": cfg.n_occ, "n_unocc": cfg.n_unocc, "n_pairs": pairs_total, "nG": ng, "n_omega": cfg.n_omega,
-                       "atoms_x_proj": [cfg.n_atoms, cfg.n_proj_per_atom], "max_batch_pairs": args.batch or 4096,
+                       "atoms_x_proj": [cfg.n_atoms, cfg.n_proj_per_atom], "max_batch_pairs": args.batch or 8192,
                        "l2": "inputs (%.2f GB of orbitals per k-point) exceed the 126 MB L2; no explicit flush" %
                              ((cfg.n_occ + cfg.n_unocc) * cfg.n_grid * 16 / 1e9),
                        "step": "reset + add_kpoint (S2-S6) + get x n_omega (S7) + ec_q (S8)",

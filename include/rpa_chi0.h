@@ -53,7 +53,7 @@ typedef struct rpa_chi0 rpa_chi0_t; /* opaque, owned by the library, freed by rp
 /*
  * Bytes of device workspace rpa_chi0_create needs for this sphere (Table 1 step 6) and omega count.
  * max_batch_pairs bounds how many (n,m) transitions are grouped into one batched pass (the paper's "Nu",
- * Eq. 20); <= 0 picks the default (4096).  Results never depend on it beyond rounding order.
+ * Eq. 20); <= 0 picks the default (8192).  Results never depend on it beyond rounding order.
  * max_proj_total bounds sum_a n_proj[a] of later rpa_chi0_add_kpoint calls (0: no PAW term will be used); it
  * sizes the scratch of the PAW contraction (Table 1 steps 8-9).
  * All pointers host.  Returns 0 on invalid arguments.

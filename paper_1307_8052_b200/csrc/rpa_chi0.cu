@@ -41,7 +41,7 @@ int fail(int code, const char *fmt, ...) {
         if (e_ != cudaSuccess) return fail(RPA_ERR_CUDA, "%s: %s (%s:%d)", #expr, cudaGetErrorString(e_), __FILE__, __LINE__); \
     } while (0)
 
-constexpr int DEFAULT_BATCH = 4096;
+constexpr int DEFAULT_BATCH = 8192;
 constexpr int MAX_SLOTS = 16;          // occupied bands per batch
 constexpr int MAX_BANDS = 1 << 17;     // eps/f scratch
 constexpr int MAX_ATOMS = 4096;

@@ -53,7 +53,7 @@ def test_workspace_bytes_host_only():
     assert n >= cfg.n_omega * ng * ng * 16
     # more omega, more batch, more projectors: never smaller
     assert B.rpa_chi0_workspace_bytes(cfg.grid, cfg.cell, cfg.q_red, W.tuned_ecut(cfg), 16, 0, 8) > n
-    assert B.rpa_chi0_workspace_bytes(cfg.grid, cfg.cell, cfg.q_red, W.tuned_ecut(cfg), cfg.n_omega, 8192, 8) > n
+    assert B.rpa_chi0_workspace_bytes(cfg.grid, cfg.cell, cfg.q_red, W.tuned_ecut(cfg), cfg.n_omega, 16384, 8) > n
     assert B.rpa_chi0_workspace_bytes(cfg.grid, cfg.cell, cfg.q_red, W.tuned_ecut(cfg), cfg.n_omega, 0, 64) > n
 
 
