@@ -32,9 +32,9 @@ from paper_1307_8052_b200 import workload as W  # noqa: E402
 
 METRIC = "chi0 pair transitions/s (rank-K FP64 TFLOP/s in roofline), 1 q-point, all omega"
 UNIT = "transitions/s"
-# ncu --set full capture of rank_k3m_kernel on configs[1] (profiles/r1d_bench_cfg1.md): dram__bytes_read.sum +
-# dram__bytes_write.sum per launch (622.0 + 499.6 MB); other configs have no capture
-RANK_K_DRAM_TRAFFIC_BYTES = {1: 1121.6e6}
+# ncu --set full capture of rank_k3m_kernel on configs[1] (profiles/r1e_bench_cfg1.md): dram__bytes_read.sum +
+# dram__bytes_write.sum per launch (3.025 GB + 184.5 MB, one launch of 7200 pairs); other configs have no capture
+RANK_K_DRAM_TRAFFIC_BYTES = {1: 3209.1e6}
 
 def rank_k_useful_flops(ng, n_omega, n_pairs):
     """8 flop per complex MAC on one triangle: 4 nG (nG+1) n_omega per pair."""
