@@ -84,8 +84,9 @@ rank_k3m_kernel(const cd *__restrict__ Nb, int64_t ldn, int Kpad, const double *
 
     const int g = lane >> 2, kq = lane & 3;
     const int rowoff = (warp >> 2) * 32, coloff = (warp & 3) * 16;
-    // a warp whose sub-tile lies strictly above the diagonal only keeps the barriers moving
-    const bool active = !(ti == tj && coloff > rowoff + 31);
+    // a warp whose sub-tile lies strictly above the diagonal, or wholly beyond the matrix edge (ragged last tile row /
+    // column), only keeps the barriers moving: the warp sharing its scheduler then has the tensor pipe to itself
+    const bool active = !(ti == tj && coloff > rowoff + 31) && row0 + rowoff < ng && col0 + coloff < ng;
 
     double p1[4][2][2], p2[4][2][2], p3[4][2][2];
 #pragma unroll
