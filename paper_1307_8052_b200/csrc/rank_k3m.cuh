@@ -96,6 +96,8 @@ rank_k3m_kernel(const cd *__restrict__ Nb, int64_t ldn, int Kpad, const double *
 #pragma unroll
             for (int e = 0; e < 2; e++) p1[mi][ni][e] = p2[mi][ni][e] = p3[mi][ni][e] = 0.0;
 
+    // 8-row blocks of this warp's sub-tile that hold matrix rows (ragged last tile row): the others are skipped
+    const int mi_valid = min(4, (ng - (row0 + rowoff) + 7) / 8);
     const uint32_t a_off = kq * PITCH + (rowoff + g) * 16;
     const uint32_t b_off = TILE_BYTES + kq * PITCH + (coloff + g) * 16;
     const uint32_t w_off = 2 * TILE_BYTES + kq * 8;
@@ -125,13 +127,16 @@ rank_k3m_kernel(const cd *__restrict__ Nb, int64_t ldn, int Kpad, const double *
                     bdif[ni] = bre[ni] - bim[ni];
                 }
 #pragma unroll
-                for (int mi = 0; mi < 4; mi++)
+                for (int mi = 0; mi < 4; mi++) {
+                    if (mi < mi_valid) {   // warp-uniform
 #pragma unroll
-                    for (int ni = 0; ni < 2; ni++) {
-                        dmma(p1[mi][ni][0], p1[mi][ni][1], are[mi], bre[ni]);
-                        dmma(p2[mi][ni][0], p2[mi][ni][1], aim[mi], bim[ni]);
-                        dmma(p3[mi][ni][0], p3[mi][ni][1], asum[mi], bdif[ni]);
+                        for (int ni = 0; ni < 2; ni++) {
+                            dmma(p1[mi][ni][0], p1[mi][ni][1], are[mi], bre[ni]);
+                            dmma(p2[mi][ni][0], p2[mi][ni][1], aim[mi], bim[ni]);
+                            dmma(p3[mi][ni][0], p3[mi][ni][1], asum[mi], bdif[ni]);
+                        }
                     }
+                }
             }
         }
         __syncwarp();
