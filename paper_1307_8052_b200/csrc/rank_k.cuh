@@ -72,7 +72,7 @@ template <bool SHARED_N>
 __global__ void __launch_bounds__(rk::Cfg<SHARED_N>::THREADS, rk::Cfg<SHARED_N>::MIN_CTAS)
 rank_k_kernel(const cd *__restrict__ Nb, int64_t ldn, int64_t strideN, int Kpad, const double *__restrict__ w,
               int64_t ldw, cd *__restrict__ S, int64_t ldS, int64_t strideS, int ng, int g0, int n_omega,
-              int tile_mode) {
+              int tile_mode, int col_limit) {
     using namespace rk;
     constexpr int STAGES = Cfg<SHARED_N>::NSTAGES;
     constexpr int STAGE_BYTES = Cfg<SHARED_N>::STAGE_BYTES;
@@ -85,7 +85,8 @@ rank_k_kernel(const cd *__restrict__ Nb, int64_t ldn, int64_t strideN, int Kpad,
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     // lower-triangle tile (ti >= tj) from the linear index
     // tile_mode 0: all lower tiles; 1: only the first tile column (tj = 0, blockIdx.x = ti); 2: all the others
-    // (the lower tiles of the triangle shifted by one tile) -- the Cholesky look-ahead of rpa_ec_q uses 1 and 2
+    // (the lower tiles of the triangle shifted by one tile) -- the blocked Cholesky of rpa_ec_q uses 1 and 2.
+    // Columns >= col_limit (<= ng) are not written (a strip update inside a Cholesky block touches one 32-column panel).
     const int t = blockIdx.x;
     int ti, tj;
     if (tile_mode == 1) {
@@ -213,7 +214,7 @@ rank_k_kernel(const cd *__restrict__ Nb, int64_t ldn, int64_t strideN, int Kpad,
 #pragma unroll
                 for (int e = 0; e < 2; e++) {
                     const int col = cc + e;
-                    if (col < ng && col <= r) {
+                    if (col < col_limit && col <= r) {
                         cd *ptr = Sw + (size_t)r * ldS + col;
                         if (ksplit > 1) {   // several CTAs add into this tile
                             atomicAdd(&ptr->x, re[mi][ni][e]);
@@ -242,14 +243,14 @@ rank_k_kernel(const cd *__restrict__ Nb, int64_t ldn, int64_t strideN, int Kpad,
                 const int cc = col0 + coloff + ni * 8 + 2 * kq;
 #pragma unroll
                 for (int e = 0; e < 2; e++)
-                    if (cc + e < ng && cc + e <= r) v[ni][e] = rowp[cc + e];
+                    if (cc + e < col_limit && cc + e <= r) v[ni][e] = rowp[cc + e];
             }
 #pragma unroll
             for (int ni = 0; ni < 4; ni++) {
                 const int cc = col0 + coloff + ni * 8 + 2 * kq;
 #pragma unroll
                 for (int e = 0; e < 2; e++)
-                    if (cc + e < ng && cc + e <= r) {
+                    if (cc + e < col_limit && cc + e <= r) {
                         v[ni][e].x += re[mi][ni][e];
                         v[ni][e].y += im[mi][ni][e];
                         rowp[cc + e] = v[ni][e];
