@@ -27,6 +27,13 @@
  * may return before the device work finishes; device inputs must stay alive until the stream reaches that
  * point.  Host input arrays are consumed before the call returns.  rpa_ec_q and rpa_chi0_sync block.
  *
+ * Internal resources: besides the workspace the handle owns one CUDA stream (high priority, used by rpa_ec_q to factor
+ * panels ahead of the trailing updates; ordered with the caller's stream by events) and a few events, all released by
+ * rpa_chi0_destroy.  Reproducibility: when the accumulation splits K over several CTAs per tile (small problems, chosen
+ * by the library) the tile sums use floating-point atomics, so chi0 is reproducible to rounding (~1e-16 relative), not
+ * bitwise, from run to run.  Environment: RPA_RANK_K_4M=1 at rpa_chi0_create selects the 4-multiplication rank-K kernel
+ * instead of the default 3-multiplication one (same results to rounding; kept for comparison).
+ *
  * Errors: every int-returning call gives 0 on success or a negative RPA_ERR_* code; rpa_last_error() holds
  * a thread-local message.  Nothing is thrown across the ABI.  A handle is not thread-safe; distinct handles
  * are independent.
