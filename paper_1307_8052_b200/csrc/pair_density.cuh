@@ -1,7 +1,8 @@
 // Pair densities on the |q+G| sphere (Table 1 steps 5-6; Eq. 7 / Eq. 12):
 //   ntilde_nm(g) = (1/N) sum_j conj(u_n[j]) u_m[j] exp(-2 pi i (g1 j1/N1 + g2 j2/N2 + g3 j3/N3)),   g in the sphere.
 //
-// Two kernels, both pruned to the bounding box [g1min..g1max] x [g2min..g2max] x [g3min..g3max] of the sphere:
+// The general path (any plane whose lengths factor into 2, 3, 5, 7; pd_zy_kernel of pair_density_zy.cuh replaces the
+// first kernel for the plane shapes it is specialised for).  Two kernels, both pruned to the bounding box [g1min..g1max] x [g2min..g2max] x [g3min..g3max] of the sphere:
 //   pd_plane_kernel  one CTA per (x-plane j1, pair): the plane u[j1][:][:] is contiguous in HBM (N2*N3*16 B), so it
 //                    is streamed once with fully coalesced 16-byte loads; the product conj(u_n) u_m is formed in
 //                    registers on the way into the first radix pass of the z FFT; z lines are transformed in
@@ -215,192 +216,7 @@ __global__ void __launch_bounds__(256) pd_plane_kernel(const __grid_constant__ P
     }
 }
 
-// ---- fast path: grid lengths fixed at compile time, one butterfly per thread per pass, no staging -----------------
-// Each thread owns the same butterfly (line l, index j) of every z chunk: its R0 inputs of u_m and u_n for the NEXT
-// chunk are prefetched into registers with plain 16-byte loads (consecutive threads -> consecutive addresses) while
-// the current chunk is transformed, so HBM latency is covered by a full chunk of work and the input never passes
-// through shared memory.  The twiddles of the later z passes depend only on the thread and live in registers.
-// Shared memory (cd): tw2[N2] | zbuf[nbuf][RC*N3p] | Y0[N2*ng3] (| Y1[N2*ng3] unless it fits inside zbuf).
-template <int NC, int PS, int NS>
-struct ZFast {
-    static constexpr FftPlanResult pr = fft_plan_c(NC);
-    static constexpr int NP = pr.plan.npass;
-    static constexpr int R = pr.plan.radix[PS < NP ? PS : 0];
-    static constexpr int NB = NC / R;
-    static constexpr int N3p = NC + (NC >> 3) + 1;
-
-    // largest butterfly count per line over the passes PS.. (threads needed per line)
-    static constexpr int max_nb() {
-        if constexpr (PS + 1 < NP) {
-            constexpr int rest = ZFast<NC, PS + 1, NS * R>::max_nb();
-            return NB > rest ? NB : rest;
-        } else {
-            return NB;
-        }
-    }
-
-    __device__ __forceinline__ static void load_tw(int tid, const cd *__restrict__ tw3, cd (&twr)[FFT_MAX_PASSES][7]) {
-        if constexpr (PS < NP) {
-            if constexpr (PS > 0) {
-                const int j = tid % NB, k = j % NS;
-                constexpr int TSTEP = NB / NS;
-#pragma unroll
-                for (int s = 1; s < R; s++) twr[PS][s - 1] = tw3[(s * k * TSTEP) % NC];
-            }
-            ZFast<NC, PS + 1, NS * R>::load_tw(tid, tw3, twr);
-        }
-    }
-
-    // v: the R inputs of pass 0 (already conj(u_n) u_m); later passes read their inputs from zbuf.
-    __device__ __forceinline__ static void run(int tid, int rc, int row0, int RC, cd *v0, cd *zbuf, cd *Y0, int g3min,
-                                               int ng3, const cd (&twr)[FFT_MAX_PASSES][7]) {
-        if constexpr (PS < NP) {
-            constexpr bool last = (PS == NP - 1);
-            const int line = tid / NB, j = tid - line * NB;
-            const bool act = line < rc;
-            cd v[R];
-            if constexpr (PS == 0) {
-#pragma unroll
-                for (int s = 0; s < R; s++) v[s] = v0[s];
-            } else {
-                const cd *src = zbuf + (size_t)((PS + 1) & 1) * RC * N3p + line * N3p;
-                if (act) {
-#pragma unroll
-                    for (int s = 0; s < R; s++) v[s] = src[zpad(j + s * NB)];
-#pragma unroll
-                    for (int s = 1; s < R; s++) v[s] = h_mul(v[s], twr[PS][s - 1]);
-                }
-            }
-            if (act) {
-                Bfly<R>::run(v);
-                const int k = j % NS;
-                const int jj0 = (j - k) * R + k;
-                if constexpr (last) {
-                    cd *yrow = Y0 + (size_t)(row0 + line) * ng3;
-#pragma unroll
-                    for (int s = 0; s < R; s++) {
-                        const int gi = freq_to_box(jj0 + s * NS, NC, g3min, ng3);
-                        if (gi >= 0) yrow[gi] = v[s];
-                    }
-                } else {
-                    cd *dst = zbuf + (size_t)(PS & 1) * RC * N3p + line * N3p;
-#pragma unroll
-                    for (int s = 0; s < R; s++) dst[zpad(jj0 + s * NS)] = v[s];
-                }
-            }
-            if constexpr (!last) {
-                __syncthreads();
-                ZFast<NC, PS + 1, NS * R>::run(tid, rc, row0, RC, v0, zbuf, Y0, g3min, ng3, twr);
-            }
-        }
-    }
-};
-
-template <int N3C, int N2C, int NTH, int MINB>
-__global__ void __launch_bounds__(NTH, MINB) pd_plane_fast_kernel(const __grid_constant__ PdPlaneParams P) {
-    extern __shared__ __align__(16) unsigned char pd_smem[];
-    using Z0 = ZFast<N3C, 0, 1>;
-    constexpr int R0 = Z0::R, NB0 = Z0::NB, N3p = Z0::N3p;
-    const int tid = threadIdx.x, nth = blockDim.x;
-    const int ng2 = P.ng2, ng3 = P.ng3, RC = P.RC;
-    cd *tw2s = reinterpret_cast<cd *>(pd_smem);
-    cd *zbuf = tw2s + N2C;                          // [nbuf][RC*N3p]
-    cd *Y0 = zbuf + (size_t)P.nbuf * RC * N3p;
-    const int ysz = ng3 * N2C;
-    cd *Y1 = (ysz <= P.nbuf * RC * N3p) ? zbuf : Y0 + ysz;
-    for (int i = tid; i < N2C; i += nth) tw2s[i] = P.tw2[i];
-    cd twr[FFT_MAX_PASSES][7];
-    Z0::load_tw(tid, P.tw3, twr);
-
-    const int j1 = blockIdx.x;
-    constexpr size_t plane = (size_t)N2C * N3C;
-    const size_t vol = plane * P.N1;
-    const int nb2 = ng2 * ng3;
-    const int nchunks = (N2C + RC - 1) / RC;
-    const int npairs = (P.p_count - (int)blockIdx.y + (int)gridDim.y - 1) / (int)gridDim.y;  // pairs of this CTA
-    const int total = npairs * nchunks;
-    const int l0 = tid / NB0, jz0 = tid - l0 * NB0;   // this thread's pass-0 butterfly
-
-    cd nxm[R0], nxn[R0];
-    auto prefetch = [&](int pi, int c) {
-        const int p = P.p_begin + blockIdx.y + pi * gridDim.y;
-        const int row = c * RC + l0;
-        if (l0 < RC && row < N2C) {
-            const int n = P.n0 + p / P.mlen, m = P.m0 + p % P.mlen;
-            const size_t off = (size_t)j1 * plane + (size_t)row * N3C + jz0;
-            const cd *um = P.psi_unocc + (size_t)m * vol + off;
-            const cd *un = P.psi_occ + (size_t)n * vol + off;
-#pragma unroll
-            for (int s = 0; s < R0; s++) {
-                nxm[s] = __ldcs(um + s * NB0);   // streamed once
-                nxn[s] = __ldg(un + s * NB0);    // shared by every pair of this occupied band: keep cached
-            }
-        }
-    };
-    if (total > 0) prefetch(0, 0);
-
-    int c = 0, pi = 0;
-    for (int q = 0; q < total; q++) {
-        const int row0 = c * RC;
-        const int rc = min(RC, N2C - row0);
-        cd v0[R0];
-#pragma unroll
-        for (int s = 0; s < R0; s++) v0[s] = cmulc(nxn[s], nxm[s]);
-        {   // next chunk's inputs: in flight while this chunk is transformed
-            int c2 = c + 1, pi2 = pi;
-            if (c2 == nchunks) { c2 = 0; pi2++; }
-            if (q + 1 < total) prefetch(pi2, c2);
-        }
-        __syncthreads();  // everybody is done with zbuf / Y of the previous chunk or pair
-        Z0::run(tid, rc, row0, RC, v0, zbuf, Y0, P.g3min, ng3, twr);
-        if (++c < nchunks) continue;
-        c = 0;
-        __syncthreads();
-
-        // ---- last chunk of the pair: y axis on the ng3 surviving columns, then write out ---------------------------
-        const int p = P.p_begin + blockIdx.y + pi * gridDim.y;
-        pi++;
-        // pass ps reads (ps even ? Y0 : Y1) and writes the other; the last pass writes [g2i][g3i]
-        auto my_ld = [=](int ps) {
-            const cd *s_ = (ps & 1) ? Y1 : Y0;
-            return [=](int line, int i) { return s_[i * ng3 + line]; };
-        };
-        auto my_st = [=](int ps) {
-            cd *d_ = (ps & 1) ? Y0 : Y1;
-            return [=](int line, int i, cd v) { d_[i * ng3 + line] = v; };
-        };
-        auto my_sto = [=](int ps) {
-            cd *d_ = (ps & 1) ? Y0 : Y1;
-            return [=](int line, int f, cd v) {
-                const int gi = freq_to_box(f, N2C, P.g2min, ng2);
-                if (gi >= 0) d_[gi * ng3 + line] = v;
-            };
-        };
-        constexpr FftPlanResult pry = fft_plan_c(N2C);
-        y_passes_ct<N2C, 0, 1>(tid, nth, ng3, tw2s, my_ld, my_st, my_sto);
-        const cd *out = (pry.plan.npass & 1) ? Y1 : Y0;
-        cd *Io = P.I + ((size_t)(p - P.p_begin) * P.N1 + j1) * nb2;
-        for (int i = tid; i < nb2; i += nth) Io[i] = out[i];
-        // the next z pass writes zbuf / Y0 only after the __syncthreads at the top of the loop
-    }
-}
-
 typedef void (*PdPlaneKernel)(const PdPlaneParams);
-struct PdPlaneChoice {
-    PdPlaneKernel kernel;
-    bool fast;
-    int max_nb;       // fast path: threads per z line
-    int max_threads;  // fast path: the kernel's __launch_bounds__
-};
-// Fast specialisations for the grid shapes of BASELINE.json configs[0..4]; anything else takes the run-time kernel.
-static inline PdPlaneChoice pd_plane_pick(int N2, int N3) {
-    if (N2 == 16 && N3 == 16) return {pd_plane_fast_kernel<16, 16, 256, 1>, true, ZFast<16, 0, 1>::max_nb(), 256};
-    if (N2 == 60 && N3 == 64) return {pd_plane_fast_kernel<64, 60, 128, 3>, true, ZFast<64, 0, 1>::max_nb(), 128};
-    if (N2 == 24 && N3 == 24) return {pd_plane_fast_kernel<24, 24, 256, 1>, true, ZFast<24, 0, 1>::max_nb(), 256};
-    if (N2 == 40 && N3 == 168) return {pd_plane_fast_kernel<168, 40, 256, 1>, true, ZFast<168, 0, 1>::max_nb(), 256};
-    if (N2 == 48 && N3 == 192) return {pd_plane_fast_kernel<192, 48, 256, 1>, true, ZFast<192, 0, 1>::max_nb(), 256};
-    return {pd_plane_kernel<0, 0>, false, 0, 256};
-}
 
 // x axis + gather.  Thread (pair, b) with b = g2i*ng3 + g3i a column of the pruned box; tw1[t] = exp(-2 pi i t/N1).
 // box2s[g1i*nb2 + b] = index of (g1min+g1i, ., .) in the sphere list, or -1 outside the sphere.

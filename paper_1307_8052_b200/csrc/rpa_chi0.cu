@@ -286,9 +286,8 @@ int pick_ksplit(int units, int nchunks, int n_sm) {
 }
 
 // Launch plan of the plane kernel: rows per chunk, threads, dynamic shared memory.
-//  fast path (grid lengths known at build time): one butterfly per thread per pass, so threads = RC * max_nb <= 256;
-//  several CTAs per SM (shared memory is small: no staging).
-//  run-time path: cp.async staging, two CTAs per SM preferred.
+//  run-time radix passes with cp.async staging, two CTAs per SM preferred (the specialised pd_zy_kernel, when one
+//  exists for the plane shape, is planned by plan_zy_kernel).
 // Returns false if even one z line per chunk does not fit.
 template <class C, class K>
 void try_zy(rpa_chi0 *h, K kernel, int G, int minb) {
@@ -326,20 +325,8 @@ bool plan_plane_kernel(rpa_chi0 *h) {
     const int N3p = N3 + (N3 >> 3) + 1;
     const int nbuf = h->pz.npass >= 3 ? 2 : (h->pz.npass == 2 ? 1 : 0);
     h->pd_nbuf = nbuf;
-    const PdPlaneChoice ch = pd_plane_pick(N2, N3);
-    h->pd_kernel = ch.kernel;
+    h->pd_kernel = pd_plane_kernel<0, 0>;   // run-time radix passes: any 2-3-5-7 plane shape
     const size_t ysz = (size_t)ng3 * N2;
-    if (ch.fast) {
-        int rc = std::max(1, std::min(N2, ch.max_threads / ch.max_nb));
-        const int chunks = (N2 + rc - 1) / rc;
-        rc = (N2 + chunks - 1) / chunks;
-        const size_t zsz = (size_t)nbuf * rc * N3p;
-        const size_t elems = (size_t)N2 + zsz + ysz + (ysz <= zsz ? 0 : ysz);
-        h->RC = rc;
-        h->pd_smem = elems * sizeof(cd);
-        h->pd_threads = (int)align_up((size_t)std::max(32, rc * ch.max_nb), 32);
-        return h->pd_smem <= 220 * 1024 && h->pd_threads <= ch.max_threads;
-    }
     const size_t fixed = ((size_t)N3 + N2 + 2 * ysz) * sizeof(cd);
     const size_t per_row = (4 * (size_t)N3 + (size_t)nbuf * N3p) * sizeof(cd);
     const size_t caps[3] = {72 * 1024, 110 * 1024, 224 * 1024};   // 3, 2, 1 CTAs per SM
@@ -433,7 +420,11 @@ int rpa_chi0_create(rpa_chi0_t **out, const int32_t grid[3], const double cell[9
         return fail(RPA_ERR_WORKSPACE, "rpa_chi0_create: workspace %zu B < required %zu B", workspace_bytes, need);
     }
     h->ws = (unsigned char *)workspace;
-    if (!plan_plane_kernel(h)) { delete h; return fail(RPA_ERR_UNSUPPORTED, "rpa_chi0_create: grid plane too large for shared memory"); }
+    const bool pd_ok = plan_plane_kernel(h);
+    if (!pd_ok && !h->zy_kernel) {
+        delete h;
+        return fail(RPA_ERR_UNSUPPORTED, "rpa_chi0_create: grid plane too large for shared memory");
+    }
 
 #define CREATE_TRY(expr)                                                                        \
     do {                                                                                        \
@@ -444,7 +435,7 @@ int rpa_chi0_create(rpa_chi0_t **out, const int32_t grid[3], const double cell[9
         }                                                                                       \
     } while (0)
 
-    CREATE_TRY(cudaFuncSetAttribute(h->pd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->pd_smem));
+    if (pd_ok) CREATE_TRY(cudaFuncSetAttribute(h->pd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->pd_smem));
     {
         const size_t xs = (size_t)grid[0] * PD_G1_BLOCK * sizeof(cd);   // DFT table of pd_xaxis_kernel
         if (xs > 220 * 1024) { delete h; return fail(RPA_ERR_UNSUPPORTED, "rpa_chi0_create: N1 = %d too large for the x-axis table", grid[0]); }
