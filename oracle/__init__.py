@@ -48,6 +48,10 @@ def lib():
         L.orc_pw_to_grid.argtypes = [vp, i32, i32, vp, vp, C.c_int64, vp, vp]
         L.orc_symmetry_remap.restype = i32
         L.orc_symmetry_remap.argtypes = [vp, vp, i32, i32, vp, vp]
+        L.orc_momentum_pw.restype = None
+        L.orc_momentum_pw.argtypes = [vp, vp, i32, vp, i32, vp, i32, vp, i32, vp, vp, vp, vp, vp]
+        L.orc_optical_head.restype = None
+        L.orc_optical_head.argtypes = [i32, i32, vp, vp, vp, vp, vp]
         _lib = L
     return _lib
 
@@ -173,6 +177,29 @@ def symmetry_remap(grid, M, time_reversal, u):
     return out
 
 
+def momentum_pw(cell, k_cart, g_pw, C_occ, C_unocc, n_proj=None, P_occ=None, P_unocc=None, Qgrad=None):
+    """Eq. 15 / 19: grad[3][n_occ][n_unocc] = <psi_n| nabla |psi_m> from plane-wave coefficients (+ PAW term)."""
+    g_pw = _i32(g_pw).reshape(-1, 3)
+    C_occ, C_unocc = _c128(C_occ).reshape(-1, g_pw.shape[0]), _c128(C_unocc).reshape(-1, g_pw.shape[0])
+    out = np.zeros((3, C_occ.shape[0], C_unocc.shape[0]), dtype=np.complex128)
+    if n_proj is not None and len(n_proj):
+        n_proj, P_occ, P_unocc, Qgrad = _i32(n_proj), _c128(P_occ), _c128(P_unocc), _c128(Qgrad)
+        args = (n_proj.size, _p(n_proj), _p(P_occ), _p(P_unocc), _p(Qgrad))
+    else:
+        args = (0, None, None, None, None)
+    lib().orc_momentum_pw(_p(_f64(cell).reshape(9)), _p(_f64(k_cart)), g_pw.shape[0], _p(g_pw), C_occ.shape[0], _p(C_occ),
+                          C_unocc.shape[0], _p(C_unocc), *args, _p(out))
+    return out
+
+
+def optical_head(eps_occ, eps_unocc, qdir, grad):
+    """Eq. 13: head[n][m] = -i qdir . grad[:, n, m] / (eps_m - eps_n)."""
+    eo, eu, qd, grad = _f64(eps_occ), _f64(eps_unocc), _f64(qdir), _c128(grad)
+    out = np.zeros((eo.size, eu.size), dtype=np.complex128)
+    lib().orc_optical_head(eo.size, eu.size, _p(eo), _p(eu), _p(qd), _p(grad), _p(out))
+    return out
+
+
 class Chi0Oracle:
     """Same call shape as the library boundary (include/rpa_chi0.h), every step by the C oracle.
 
@@ -200,9 +227,15 @@ class Chi0Oracle:
             paw_add(self.cell, self.q, self.g, n_proj, kd.P_occ[n], kd.P_unocc, Q, R_cart, nt)
         return nt
 
-    def add_kpoint(self, kd, n_proj=None, Q=None, R_cart=None):
+    def add_kpoint(self, kd, n_proj=None, Q=None, R_cart=None, head=None):
+        """head[n][m] (optical limit, Eq. 13) replaces the G = 0 element of every pair density when given."""
+        i0 = None
+        if head is not None:
+            i0 = int(np.flatnonzero((self.g == 0).all(axis=1))[0])
         for n in range(kd.psi_occ.shape[0]):
             nt = self.pair_densities(n, kd, n_proj, Q, R_cart)
+            if head is not None:
+                nt[:, i0] = head[n]
             w = weights(kd.eps_occ[n], kd.f_occ[n], kd.eps_unocc, kd.f_unocc, self.omega)
             accumulate(self.S, nt, w, kd.kweight)
             self.n_pairs += nt.shape[0]

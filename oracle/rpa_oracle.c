@@ -411,3 +411,59 @@ int32_t orc_symmetry_remap(const int32_t grid[3], const int32_t M[9], int32_t ti
                 }
     return 0;
 }
+
+/*
+ * ---- NEXT-2: Table 1 step 10, the optical limit q -> 0 of the G = 0 element --------------------------
+ * Eq. 15 with Eq. 19: matrix elements of the gradient between pseudo wave functions expanded
+ * in plane waves on a common set {Q} (same k for n and m), plus the PAW term,
+ *   grad[al][n][m] = sum_Q conj(C_n(Q)) i (k + Q B)_al C_m(Q)
+ *                    + sum_a sum_ij conj(P^a_{i,n}) Qgrad^a_al[i][j] P^a_{j,m},          al = x, y, z,
+ * with sum_Q |C(Q)|^2 = 1 <=> the wave functions normalised in the cell.  Qgrad (Eq. 16; printed as Q_ii, read as
+ * Q_ij like reading A8) is an input: per atom [3][n_i][n_i], atoms concatenated.  Plain loops.
+ */
+void orc_momentum_pw(const double cell[9], const double k_cart[3], int32_t n_pw, const int32_t *g_pw, int32_t n_occ,
+                     const zd *C_occ, int32_t n_unocc, const zd *C_unocc, int32_t n_atoms, const int32_t *n_proj,
+                     const zd *P_occ, const zd *P_unocc, const zd *Qgrad, zd *grad) {
+    double B[9];
+    recip_cell(cell, B);
+    int32_t ptot = 0;
+    for (int32_t a = 0; a < n_atoms; a++) ptot += n_proj[a];
+    for (int al = 0; al < 3; al++)
+        for (int32_t n = 0; n < n_occ; n++)
+            for (int32_t m = 0; m < n_unocc; m++) {
+                zd acc = 0.0;
+                for (int32_t q = 0; q < n_pw; q++) {
+                    const double G = g_pw[3 * q] * B[al] + g_pw[3 * q + 1] * B[3 + al] + g_pw[3 * q + 2] * B[6 + al];
+                    acc += conj(C_occ[(int64_t)n * n_pw + q]) * (I * (k_cart[al] + G)) * C_unocc[(int64_t)m * n_pw + q];
+                }
+                int32_t poff = 0;
+                int64_t qoff = 0;
+                for (int32_t a = 0; a < n_atoms; a++) {
+                    const int32_t ni = n_proj[a];
+                    for (int32_t i = 0; i < ni; i++)
+                        for (int32_t j = 0; j < ni; j++)
+                            acc += conj(P_occ[(int64_t)n * ptot + poff + i]) * Qgrad[qoff + ((int64_t)al * ni + i) * ni + j] *
+                                   P_unocc[(int64_t)m * ptot + poff + j];
+                    poff += ni;
+                    qoff += (int64_t)3 * ni * ni;
+                }
+                grad[((int64_t)al * n_occ + n) * n_unocc + m] = acc;
+            }
+}
+
+/*
+ * Eq. 13 (printed twice, the second line is the result): the G = 0 pair density in the limit q -> 0 along
+ * the unit vector qdir, per unit |q|,
+ *   n_nm(G = 0) = -i qdir . grad[.][n][m] / (eps_m - eps_n),        0 when eps_m = eps_n (its weight is 0 anyway).
+ * head[n][m].
+ */
+void orc_optical_head(int32_t n_occ, int32_t n_unocc, const double *eps_occ, const double *eps_unocc, const double qdir[3],
+                      const zd *grad, zd *head) {
+    for (int32_t n = 0; n < n_occ; n++)
+        for (int32_t m = 0; m < n_unocc; m++) {
+            const double de = eps_unocc[m] - eps_occ[n];
+            zd s = 0.0;
+            for (int al = 0; al < 3; al++) s += qdir[al] * grad[((int64_t)al * n_occ + n) * n_unocc + m];
+            head[(int64_t)n * n_unocc + m] = de != 0.0 ? -I * s / de : 0.0;
+        }
+}
