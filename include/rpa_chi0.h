@@ -50,7 +50,7 @@ extern "C" {
 
 #define RPA_OK 0
 #define RPA_ERR_INVALID_ARG (-1)  /* null pointer, non-positive size, omega <= 0, i_omega out of range, |K_g| = 0 */
-#define RPA_ERR_UNSUPPORTED (-2)  /* q = 0 optical limit (out of scope, reading A13); unsupported grid */
+#define RPA_ERR_UNSUPPORTED (-2)  /* unsupported grid length; plain add_kpoint on a q = 0 handle; grid-incompatible symmetry */
 #define RPA_ERR_WORKSPACE (-3)    /* workspace too small or misaligned */
 #define RPA_ERR_CUDA (-4)         /* a CUDA runtime call or kernel launch failed */
 #define RPA_ERR_NOT_PD (-5)       /* 1 - v^1/2 chi0 v^1/2 not positive definite in rpa_ec_q */
@@ -165,6 +165,35 @@ int rpa_chi0_accumulators(const rpa_chi0_t *h, void **S, size_t *bytes);
 int rpa_pw_to_grid(rpa_chi0_t *h, int32_t n_bands, int32_t n_pw, const int32_t *g_pw, const void *C, void *psi_out);
 int rpa_symmetry_remap(rpa_chi0_t *h, int32_t n_bands, const int32_t M[9], int32_t time_reversal, const void *psi_in,
                        void *psi_out);
+
+/*
+ * Table 1 step 10: the optical limit q -> 0.  A handle created with q_red = (0,0,0)
+ * has G = 0 inside its sphere, where Eq. 4 degenerates to delta_nn' and v diverges; the G = 0 element of every pair
+ * density is then the perturbative limit of Eq. 13, per unit |q| along a direction qdir,
+ *     n_nm(G = 0) = -i qdir . <psi_n| nabla |psi_m> / (eps_m - eps_n)          (0 when eps_m = eps_n),
+ * so that with v_G=0 = 4 pi passed to rpa_ec_q the products v^1/2 chi0 v^1/2 are the finite q -> 0 values.
+ *
+ * rpa_momentum_pw -- Eq. 15 with the plane-wave form of the gradient, Eq. 19 (the paper's GPU
+ * reformulation of the CPU code's 13-point stencil):
+ *     grad_out[al][n][m] = sum_Q conj(C_occ[n][Q]) i (k_cart + Q B)_al C_unocc[m][Q]
+ *                          + sum_a sum_ij conj(P_occ[n][a,i]) Qgrad[a][al][i][j] P_unocc[m][a,j],      al = x, y, z
+ * k_cart: host [3] (bohr^-1); g_pw: host int32 [n_pw][3]; C_*: dev cdouble [bands][n_pw], both on the same plane-wave
+ * set, sum_Q |C|^2 = 1; Qgrad: dev cdouble, per atom [3][n_i][n_i], atoms concatenated (Eq. 16, computed by the caller
+ * from the PAW data sets); n_atoms == 0: no PAW term.  grad_out: dev cdouble [3][n_occ][n_unocc].
+ *
+ * rpa_chi0_add_kpoint_optical -- rpa_chi0_add_kpoint for a q = 0 handle: same arguments, plus the direction qdir_cart
+ * (host [3], normalised by the library) and grad (dev [3][n_occ][n_unocc], e.g. from rpa_momentum_pw).  On a q = 0
+ * handle the plain rpa_chi0_add_kpoint returns RPA_ERR_UNSUPPORTED, on a q != 0 handle this call returns
+ * RPA_ERR_INVALID_ARG.
+ */
+int rpa_momentum_pw(rpa_chi0_t *h, const double k_cart[3], int32_t n_pw, const int32_t *g_pw, int32_t n_occ, const void *C_occ,
+                    int32_t n_unocc, const void *C_unocc, int32_t n_atoms, const int32_t *n_proj, const void *P_occ,
+                    const void *P_unocc, const void *Qgrad, void *grad_out);
+int rpa_chi0_add_kpoint_optical(rpa_chi0_t *h, double kweight, int32_t n_occ, const void *psi_occ, int32_t n_unocc,
+                                const void *psi_unocc, const double *eps_occ, const double *eps_unocc, const double *f_occ,
+                                const double *f_unocc, int32_t n_atoms, const int32_t *n_proj, const void *P_occ,
+                                const void *P_unocc, const void *Q, const double *R_cart, const double qdir_cart[3],
+                                const void *grad);
 
 void rpa_chi0_destroy(rpa_chi0_t *h);
 

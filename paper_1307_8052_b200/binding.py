@@ -25,7 +25,7 @@ EXPORTS = (
     "rpa_chi0_workspace_bytes", "rpa_chi0_create", "rpa_chi0_ng", "rpa_chi0_gvectors", "rpa_chi0_add_kpoint",
     "rpa_chi0_get", "rpa_ec_q", "rpa_chi0_reset", "rpa_chi0_sync", "rpa_chi0_set_profiling", "rpa_chi0_stage_times",
     "rpa_chi0_launch_count", "rpa_chi0_accumulators", "rpa_chi0_destroy", "rpa_probe_fp64_tensor_peak", "rpa_last_error",
-    "rpa_pw_to_grid", "rpa_symmetry_remap",
+    "rpa_pw_to_grid", "rpa_symmetry_remap", "rpa_momentum_pw", "rpa_chi0_add_kpoint_optical",
 )
 
 STAGE_NAMES = ("pair_product_fft_yz", "fft_x_gather", "paw", "weights", "rank_k")
@@ -90,6 +90,10 @@ def lib():
     L.rpa_pw_to_grid.argtypes = [vp, i32, i32, vp, vp, vp]
     L.rpa_symmetry_remap.restype = C.c_int
     L.rpa_symmetry_remap.argtypes = [vp, i32, vp, i32, vp, vp]
+    L.rpa_momentum_pw.restype = C.c_int
+    L.rpa_momentum_pw.argtypes = [vp, vp, i32, vp, i32, vp, i32, vp, i32, vp, vp, vp, vp, vp]
+    L.rpa_chi0_add_kpoint_optical.restype = C.c_int
+    L.rpa_chi0_add_kpoint_optical.argtypes = [vp, f64, i32, vp, i32, vp, vp, vp, vp, vp, i32, vp, vp, vp, vp, vp, vp, vp]
     L.rpa_last_error.restype = C.c_char_p
     L.rpa_last_error.argtypes = []
     _lib = L
@@ -207,8 +211,10 @@ def rpa_chi0_gvectors(h: Handle):
 
 
 def rpa_chi0_add_kpoint(h: Handle, kweight, psi_occ, psi_unocc, eps_occ, eps_unocc, f_occ, f_unocc,
-                        n_proj: Optional[Sequence[int]] = None, P_occ=None, P_unocc=None, Q=None, R_cart=None):
-    """psi_*, P_*, Q: CUDA complex128 tensors (layouts of include/rpa_chi0.h); eps_*, f_*, n_proj, R_cart: host."""
+                        n_proj: Optional[Sequence[int]] = None, P_occ=None, P_unocc=None, Q=None, R_cart=None,
+                        qdir_cart=None, grad=None):
+    """psi_*, P_*, Q: CUDA complex128 tensors (layouts of include/rpa_chi0.h); eps_*, f_*, n_proj, R_cart: host.
+    With qdir_cart and grad (CUDA [3][n_occ][n_unocc]) this is rpa_chi0_add_kpoint_optical (q = 0 handles)."""
     torch = _torch()
     c128 = torch.complex128
     N = int(np.prod(h.grid))
@@ -237,9 +243,15 @@ def rpa_chi0_add_kpoint(h: Handle, kweight, psi_occ, psi_unocc, eps_occ, eps_uno
                 _dev_ptr(P_unocc, "P_unocc", c128, h.device) if n_unocc else None, _dev_ptr(Q, "Q", c128, h.device), _hp(R))
     else:
         args = (0, None, None, None, None, None)
-    rc = lib().rpa_chi0_add_kpoint(
-        h.ptr, float(kweight), n_occ, _dev_ptr(psi_occ, "psi_occ", c128, h.device) if n_occ else None, n_unocc,
-        _dev_ptr(psi_unocc, "psi_unocc", c128, h.device) if n_unocc else None, _hp(eo), _hp(eu), _hp(fo), _hp(fu), *args)
+    common = (h.ptr, float(kweight), n_occ, _dev_ptr(psi_occ, "psi_occ", c128, h.device) if n_occ else None, n_unocc,
+              _dev_ptr(psi_unocc, "psi_unocc", c128, h.device) if n_unocc else None, _hp(eo), _hp(eu), _hp(fo), _hp(fu), *args)
+    if grad is None and qdir_cart is None:
+        rc = lib().rpa_chi0_add_kpoint(*common)
+    else:
+        if grad is None or qdir_cart is None or grad.numel() != 3 * n_occ * n_unocc:
+            raise ValueError("optical limit: qdir_cart and grad [3][n_occ][n_unocc] are both required")
+        qd = _np(qdir_cart, np.float64).reshape(3)
+        rc = lib().rpa_chi0_add_kpoint_optical(*common, _hp(qd), _dev_ptr(grad, "grad", c128, h.device))
     _check(rc)
 
 
@@ -325,6 +337,34 @@ def rpa_symmetry_remap(h: Handle, psi, M, time_reversal=False, out=None):
         out = torch.empty_like(psi)
     _check(lib().rpa_symmetry_remap(h.ptr, n_bands, _hp(Mi), 1 if time_reversal else 0,
                                     _dev_ptr(psi, "psi", torch.complex128, h.device), _dev_ptr(out, "out", torch.complex128, h.device)))
+    return out
+
+
+def rpa_chi0_add_kpoint_optical(h: Handle, kweight, psi_occ, psi_unocc, eps_occ, eps_unocc, f_occ, f_unocc, qdir_cart, grad,
+                                n_proj=None, P_occ=None, P_unocc=None, Q=None, R_cart=None):
+    rpa_chi0_add_kpoint(h, kweight, psi_occ, psi_unocc, eps_occ, eps_unocc, f_occ, f_unocc, n_proj, P_occ, P_unocc, Q, R_cart,
+                        qdir_cart, grad)
+
+
+def rpa_momentum_pw(h: Handle, k_cart, g_pw, C_occ, C_unocc, n_proj=None, P_occ=None, P_unocc=None, Qgrad=None):
+    """Eq. 15 / 19: grad[3][n_occ][n_unocc] (CUDA) from plane-wave coefficients C_* (CUDA [bands][n_pw]) + PAW term."""
+    torch = _torch()
+    c128 = torch.complex128
+    g = _np(g_pw, np.int32).reshape(-1, 3)
+    k = _np(k_cart, np.float64).reshape(3)
+    n_pw = g.shape[0]
+    n_occ, n_unocc = int(C_occ.shape[0]), int(C_unocc.shape[0])
+    if int(C_occ.shape[1]) != n_pw or int(C_unocc.shape[1]) != n_pw:
+        raise ValueError("C_occ / C_unocc must be [bands][n_pw]")
+    out = torch.empty((3, n_occ, n_unocc), dtype=c128, device=h.device)
+    if n_proj is not None and len(n_proj):
+        npj = _np(n_proj, np.int32)
+        paw = (len(npj), _hp(npj), _dev_ptr(P_occ, "P_occ", c128, h.device), _dev_ptr(P_unocc, "P_unocc", c128, h.device),
+               _dev_ptr(Qgrad, "Qgrad", c128, h.device))
+    else:
+        paw = (0, None, None, None, None)
+    _check(lib().rpa_momentum_pw(h.ptr, _hp(k), n_pw, _hp(g), n_occ, _dev_ptr(C_occ, "C_occ", c128, h.device), n_unocc,
+                                 _dev_ptr(C_unocc, "C_unocc", c128, h.device), *paw, _dev_ptr(out, "grad", c128, h.device)))
     return out
 
 

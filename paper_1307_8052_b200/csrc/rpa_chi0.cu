@@ -19,6 +19,7 @@
 #include "pair_density.cuh"
 #include "pair_density_zy.cuh"
 #include "orbitals.cuh"
+#include "optical.cuh"
 #include "paw.cuh"
 #include "rank_k.cuh"
 #include "rank_k3m.cuh"
@@ -202,6 +203,8 @@ struct rpa_chi0 {
     size_t pd_smem;
     PdZyKernel zy_kernel = nullptr;   // low-instruction-count z+y kernel (planes that fit one CTA), else pd_kernel
     int zy_G = 1, zy_threads = 0, zy_ctas_per_sm = 1, n_sm = 148;
+    bool q0 = false;                   // q = 0: pair densities need the optical-limit head (rpa_chi0_add_kpoint_optical)
+    int idx0 = -1;                     // sphere index of G = 0 when q0
     bool use_3m = true;                // rank_k3m_kernel (3-multiplication complex product) for the chi0 accumulation
     cudaStream_t side = nullptr;       // panel factorisations of rpa_ec_q run here, ahead of the trailing updates
     cudaEvent_t ev_panel[2] = {nullptr, nullptr}, ev_col = nullptr, ev_fork = nullptr;
@@ -387,8 +390,6 @@ int rpa_chi0_create(rpa_chi0_t **out, const int32_t grid[3], const double cell[9
         return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_create: invalid arguments");
     for (int i = 0; i < n_omega; i++)
         if (!(omega_ha[i] > 0.0)) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_create: omega[%d] must be > 0", i);
-    if (q_red[0] == 0.0 && q_red[1] == 0.0 && q_red[2] == 0.0)
-        return fail(RPA_ERR_UNSUPPORTED, "rpa_chi0_create: q = 0 (optical limit, P:L113-134) is out of scope");
     if (!workspace) return fail(RPA_ERR_WORKSPACE, "rpa_chi0_create: workspace is NULL");
     if (((uintptr_t)workspace & 255) != 0) return fail(RPA_ERR_WORKSPACE, "rpa_chi0_create: workspace not 256-byte aligned");
 
@@ -420,6 +421,12 @@ int rpa_chi0_create(rpa_chi0_t **out, const int32_t grid[3], const double cell[9
         return fail(RPA_ERR_WORKSPACE, "rpa_chi0_create: workspace %zu B < required %zu B", workspace_bytes, need);
     }
     h->ws = (unsigned char *)workspace;
+    h->q0 = q_red[0] == 0.0 && q_red[1] == 0.0 && q_red[2] == 0.0;
+    if (h->q0) {
+        for (int s = 0; s < h->sp.ng; s++)
+            if (h->sp.g[3 * s] == 0 && h->sp.g[3 * s + 1] == 0 && h->sp.g[3 * s + 2] == 0) h->idx0 = s;
+        if (h->idx0 < 0) { delete h; return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_create: q = 0 but G = 0 is outside the sphere"); }
+    }
     const bool pd_ok = plan_plane_kernel(h);
     if (!pd_ok && !h->zy_kernel) {
         delete h;
@@ -517,11 +524,18 @@ int rpa_chi0_gvectors(const rpa_chi0_t *h, int32_t *g, double *K2) {
     return RPA_OK;
 }
 
-int rpa_chi0_add_kpoint(rpa_chi0_t *h, double kweight, int32_t n_occ, const void *psi_occ, int32_t n_unocc,
-                        const void *psi_unocc, const double *eps_occ, const double *eps_unocc, const double *f_occ,
-                        const double *f_unocc, int32_t n_atoms, const int32_t *n_proj, const void *P_occ,
-                        const void *P_unocc, const void *Q, const double *R_cart) {
+}  // extern "C"
+
+namespace {
+// rpa_chi0_add_kpoint, and rpa_chi0_add_kpoint_optical when grad != NULL (q = 0 handle: G = 0 element replaced)
+int add_kpoint_impl(rpa_chi0_t *h, double kweight, int32_t n_occ, const void *psi_occ, int32_t n_unocc,
+                    const void *psi_unocc, const double *eps_occ, const double *eps_unocc, const double *f_occ,
+                    const double *f_unocc, int32_t n_atoms, const int32_t *n_proj, const void *P_occ,
+                    const void *P_unocc, const void *Q, const double *R_cart, const double *qdir, const void *grad) {
     if (!h) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_add_kpoint: handle is NULL");
+    if (h->q0 && !grad)
+        return fail(RPA_ERR_UNSUPPORTED, "rpa_chi0_add_kpoint: the handle has q = 0: use rpa_chi0_add_kpoint_optical (P:L113-134)");
+    if (!h->q0 && grad) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_add_kpoint_optical: the handle has q != 0");
     if (n_occ < 0 || n_unocc < 0 || n_atoms < 0) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_add_kpoint: negative count");
     if (n_occ == 0 || n_unocc == 0) return RPA_OK;  // empty band set: nothing to add
     if (!psi_occ || !psi_unocc || !eps_occ || !eps_unocc || !f_occ || !f_unocc)
@@ -647,6 +661,13 @@ int rpa_chi0_add_kpoint(rpa_chi0_t *h, double kweight, int32_t n_occ, const void
                     Nbuf, L.ldn, ng, ptot, h->ptr<cd>(L.T), (const cd *)P_unocc, mlen, m0);
                 CUDA_TRY(cudaGetLastError());
             }
+            // step 10: optical limit, the G = 0 element of every pair density of the batch
+            if (grad) {
+                optical_head_kernel<<<(K + 127) / 128, 128, 0, st>>>(Nbuf, L.ldn, h->idx0, K, n0, mlen, m0, n_occ, n_unocc, d_eo,
+                                                                    d_eu, qdir[0], qdir[1], qdir[2], (const cd *)grad);
+                h->launches += 1;
+                CUDA_TRY(cudaGetLastError());
+            }
             // S5: weights
             {
                 StageTimer tm(h, 3, 1);
@@ -671,6 +692,83 @@ int rpa_chi0_add_kpoint(rpa_chi0_t *h, double kweight, int32_t n_occ, const void
                 }
                 CUDA_TRY(cudaGetLastError());
             }
+        }
+    }
+    return RPA_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int rpa_chi0_add_kpoint(rpa_chi0_t *h, double kweight, int32_t n_occ, const void *psi_occ, int32_t n_unocc,
+                        const void *psi_unocc, const double *eps_occ, const double *eps_unocc, const double *f_occ,
+                        const double *f_unocc, int32_t n_atoms, const int32_t *n_proj, const void *P_occ,
+                        const void *P_unocc, const void *Q, const double *R_cart) {
+    return add_kpoint_impl(h, kweight, n_occ, psi_occ, n_unocc, psi_unocc, eps_occ, eps_unocc, f_occ, f_unocc, n_atoms, n_proj,
+                           P_occ, P_unocc, Q, R_cart, nullptr, nullptr);
+}
+
+int rpa_chi0_add_kpoint_optical(rpa_chi0_t *h, double kweight, int32_t n_occ, const void *psi_occ, int32_t n_unocc,
+                                const void *psi_unocc, const double *eps_occ, const double *eps_unocc, const double *f_occ,
+                                const double *f_unocc, int32_t n_atoms, const int32_t *n_proj, const void *P_occ,
+                                const void *P_unocc, const void *Q, const double *R_cart, const double qdir_cart[3],
+                                const void *grad) {
+    if (!qdir_cart || !grad) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_add_kpoint_optical: NULL direction or gradient");
+    const double nrm = sqrt(qdir_cart[0] * qdir_cart[0] + qdir_cart[1] * qdir_cart[1] + qdir_cart[2] * qdir_cart[2]);
+    if (!(nrm > 0.0) || !std::isfinite(nrm)) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_add_kpoint_optical: zero direction");
+    const double qd[3] = {qdir_cart[0] / nrm, qdir_cart[1] / nrm, qdir_cart[2] / nrm};
+    return add_kpoint_impl(h, kweight, n_occ, psi_occ, n_unocc, psi_unocc, eps_occ, eps_unocc, f_occ, f_unocc, n_atoms, n_proj,
+                           P_occ, P_unocc, Q, R_cart, qd, grad);
+}
+
+// Eq. 15 / Eq. 19: gradient matrix elements between occupied and unoccupied bands given on a common plane-wave set.
+int rpa_momentum_pw(rpa_chi0_t *h, const double k_cart[3], int32_t n_pw, const int32_t *g_pw, int32_t n_occ, const void *C_occ,
+                    int32_t n_unocc, const void *C_unocc, int32_t n_atoms, const int32_t *n_proj, const void *P_occ,
+                    const void *P_unocc, const void *Qgrad, void *grad_out) {
+    if (!h || !k_cart) return fail(RPA_ERR_INVALID_ARG, "rpa_momentum_pw: NULL argument");
+    if (n_pw < 0 || n_occ < 0 || n_unocc < 0 || n_atoms < 0) return fail(RPA_ERR_INVALID_ARG, "rpa_momentum_pw: negative count");
+    if (n_occ == 0 || n_unocc == 0) return RPA_OK;
+    if (!grad_out || (n_pw > 0 && (!g_pw || !C_occ || !C_unocc))) return fail(RPA_ERR_INVALID_ARG, "rpa_momentum_pw: NULL array");
+    const Layout &L = h->L;
+    cudaStream_t st = h->stream;
+    const size_t out_bytes = (size_t)3 * n_occ * n_unocc * sizeof(cd);
+    if ((size_t)3 * n_pw * sizeof(double) > (size_t)L.sub_pairs * L.I_pair_bytes)
+        return fail(RPA_ERR_WORKSPACE, "rpa_momentum_pw: %d plane waves do not fit the handle's scratch", n_pw);
+    if (n_pw == 0) {
+        CUDA_TRY(cudaMemsetAsync(grad_out, 0, out_bytes, st));
+    } else {
+        std::vector<double> Kc((size_t)3 * n_pw);
+        for (int q = 0; q < n_pw; q++)
+            for (int al = 0; al < 3; al++)
+                Kc[(size_t)al * n_pw + q] = k_cart[al] + g_pw[3 * q] * h->B[al] + g_pw[3 * q + 1] * h->B[3 + al] + g_pw[3 * q + 2] * h->B[6 + al];
+        double *d_Kc = h->ptr<double>(L.I);
+        CUDA_TRY(cudaMemcpyAsync(d_Kc, Kc.data(), Kc.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+        CUDA_TRY(cudaStreamSynchronize(st));   // Kc is pageable host memory about to go out of scope
+        momentum_pw_kernel<<<dim3(n_unocc, (n_occ + OPT_NB - 1) / OPT_NB), 128, 0, st>>>((const cd *)C_occ, (const cd *)C_unocc, d_Kc,
+                                                                                      n_pw, n_occ, n_unocc, (cd *)grad_out);
+        h->launches += 1;
+        CUDA_TRY(cudaGetLastError());
+    }
+    if (n_atoms > 0) {
+        if (!n_proj || !P_occ || !P_unocc || !Qgrad) return fail(RPA_ERR_INVALID_ARG, "rpa_momentum_pw: NULL PAW array");
+        if (n_atoms > MAX_ATOMS) return fail(RPA_ERR_INVALID_ARG, "rpa_momentum_pw: more than %d atoms", MAX_ATOMS);
+        std::vector<int32_t> poff(n_atoms), ni(n_atoms);
+        int ptot = 0;
+        for (int a = 0; a < n_atoms; a++) {
+            if (n_proj[a] < 0) return fail(RPA_ERR_INVALID_ARG, "rpa_momentum_pw: n_proj[%d] < 0", a);
+            poff[a] = ptot;
+            ni[a] = n_proj[a];
+            ptot += n_proj[a];
+        }
+        if (ptot > 0) {
+            CUDA_TRY(cudaMemcpyAsync(h->ws + L.atom_poff, poff.data(), n_atoms * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+            CUDA_TRY(cudaMemcpyAsync(h->ws + L.atom_ni, ni.data(), n_atoms * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+            CUDA_TRY(cudaStreamSynchronize(st));
+            momentum_paw_kernel<<<dim3((n_unocc + 127) / 128, n_occ, 3), 128, 0, st>>>(
+                (cd *)grad_out, n_occ, n_unocc, ptot, n_atoms, h->ptr<int32_t>(L.atom_poff), h->ptr<int32_t>(L.atom_ni),
+                (const cd *)P_occ, (const cd *)P_unocc, (const cd *)Qgrad);
+            h->launches += 1;
+            CUDA_TRY(cudaGetLastError());
         }
     }
     return RPA_OK;

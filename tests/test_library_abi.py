@@ -88,7 +88,7 @@ def test_null_handle_calls_return_invalid_arg():
     assert isinstance(B.rpa_last_error(), str)
 
 
-def test_create_rejects_q_zero_and_null_workspace_without_gpu():
+def test_create_rejects_bad_workspace_and_omega_without_gpu():
     """Validation happens before any CUDA call, so these run on the CPU box."""
     lib = B.lib()
     cfg = W.CONFIGS[0]
@@ -104,7 +104,8 @@ def test_create_rejects_q_zero_and_null_workspace_without_gpu():
                                    omega.ctypes.data_as(ctypes.c_void_p), wt.ctypes.data_as(ctypes.c_void_p), 0, 0, ws,
                                    ctypes.c_size_t(nbytes), None)
 
-    assert create((0.0, 0.0, 0.0), ctypes.c_void_p(256), 1 << 40) == B.RPA_ERR_UNSUPPORTED
+    # q = 0 is accepted since the optical limit (NEXT-2) exists: the same workspace checks apply to it
+    assert create((0.0, 0.0, 0.0), None, 1 << 40) == B.RPA_ERR_WORKSPACE
     assert create(cfg.q_red, None, 1 << 40) == B.RPA_ERR_WORKSPACE
     assert create(cfg.q_red, ctypes.c_void_p(8), 1 << 40) == B.RPA_ERR_WORKSPACE  # misaligned
     assert create(cfg.q_red, ctypes.c_void_p(256), 16) == B.RPA_ERR_WORKSPACE     # too small
