@@ -195,6 +195,14 @@ int rpa_chi0_add_kpoint_optical(rpa_chi0_t *h, double kweight, int32_t n_occ, co
                                 const void *P_unocc, const void *Q, const double *R_cart, const double qdir_cart[3],
                                 const void *grad);
 
+/*
+ * Spin-polarised systems ("the spin index sigma is implicitly contained").  The prefactor
+ * of chi0 = (s/Omega) S is s = 2 by default (spin-paired bands, reading A3).  With s = 1 the caller adds the bands of
+ * each spin channel with their own rpa_chi0_add_kpoint calls (f in [0,1] per channel); rpa_chi0_get and rpa_ec_q then
+ * use 1/Omega.  s must be 1 or 2; it may be changed at any time (it scales the read-out, not the accumulators).
+ */
+int rpa_chi0_set_spin_degeneracy(rpa_chi0_t *h, int32_t s);
+
 void rpa_chi0_destroy(rpa_chi0_t *h);
 
 /* Register-only DMMA issue-rate probe: runs `iters` dependent-free mma.sync.m8n8k4.f64 per warp on every SM and

@@ -44,6 +44,8 @@ def lib():
         L.orc_chi0_from_S.argtypes = [C.c_int64, f64, vp, vp]
         L.orc_ec_q.restype = i32
         L.orc_ec_q.argtypes = [i32, i32, vp, vp, vp, vp, vp]
+        L.orc_chi0_from_S_spin.restype = None
+        L.orc_chi0_from_S_spin.argtypes = [C.c_int64, f64, f64, vp, vp]
         L.orc_pw_to_grid.restype = None
         L.orc_pw_to_grid.argtypes = [vp, i32, i32, vp, vp, C.c_int64, vp, vp]
         L.orc_symmetry_remap.restype = i32
@@ -136,10 +138,14 @@ def accumulate(S, n, w, kweight):
     return S
 
 
-def chi0_from_S(S, vol):
+def chi0_from_S(S, vol, spin_deg=None):
+    """chi0 = (2/Omega) S (spin-paired, reading A3), or (spin_deg/Omega) S for explicit spin channels (NEXT-4)."""
     S = _c128(S)
     out = np.empty_like(S)
-    lib().orc_chi0_from_S(S.size, float(vol), _p(S), _p(out))
+    if spin_deg is None:
+        lib().orc_chi0_from_S(S.size, float(vol), _p(S), _p(out))
+    else:
+        lib().orc_chi0_from_S_spin(S.size, float(vol), float(spin_deg), _p(S), _p(out))
     return out
 
 
@@ -206,7 +212,8 @@ class Chi0Oracle:
     ``g`` may be given explicitly (a sampled sub-list of the sphere): chi0 restricted to those G is exactly the
     chi0 of those G, because every element of Eq. 17 is an independent sum."""
 
-    def __init__(self, grid, cell, q_red, ecut_ha, omega, omega_wt=None, g=None, mode="separable"):
+    def __init__(self, grid, cell, q_red, ecut_ha, omega, omega_wt=None, g=None, mode="separable", spin_deg=None):
+        self.spin_deg = spin_deg
         self.grid, self.cell, self.q = _i32(grid), _f64(cell).reshape(3, 3), _f64(q_red)
         self.omega = _f64(omega)
         self.omega_wt = None if omega_wt is None else _f64(omega_wt)
@@ -241,7 +248,7 @@ class Chi0Oracle:
             self.n_pairs += nt.shape[0]
 
     def get(self, i_omega=None):
-        chi = chi0_from_S(self.S, volume(self.cell))
+        chi = chi0_from_S(self.S, volume(self.cell), self.spin_deg)
         return chi if i_omega is None else chi[i_omega]
 
     def ec_q(self, v):

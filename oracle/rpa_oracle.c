@@ -467,3 +467,13 @@ void orc_optical_head(int32_t n_occ, int32_t n_unocc, const double *eps_occ, con
             head[(int64_t)n * n_unocc + m] = de != 0.0 ? -I * s / de : 0.0;
         }
 }
+
+/*
+ * NEXT-4: spin-polarised systems.  "The spin index sigma is implicitly contained" in Eq. 3 (
+ * reading A3 fixed s = 2 for spin-paired bands): with explicit spin channels every channel is summed with degeneracy
+ * s = 1, chi0 = (s/Omega) S.  Same as orc_chi0_from_S with the prefactor's 2 replaced by s.
+ */
+void orc_chi0_from_S_spin(int64_t count, double volume, double spin_deg, const zd *S, zd *chi0) {
+    const double s = spin_deg / volume;
+    for (int64_t i = 0; i < count; i++) chi0[i] = s * S[i];
+}

@@ -26,6 +26,7 @@ EXPORTS = (
     "rpa_chi0_get", "rpa_ec_q", "rpa_chi0_reset", "rpa_chi0_sync", "rpa_chi0_set_profiling", "rpa_chi0_stage_times",
     "rpa_chi0_launch_count", "rpa_chi0_accumulators", "rpa_chi0_destroy", "rpa_probe_fp64_tensor_peak", "rpa_last_error",
     "rpa_pw_to_grid", "rpa_symmetry_remap", "rpa_momentum_pw", "rpa_chi0_add_kpoint_optical",
+    "rpa_chi0_set_spin_degeneracy",
 )
 
 STAGE_NAMES = ("pair_product_fft_yz", "fft_x_gather", "paw", "weights", "rank_k")
@@ -90,6 +91,8 @@ def lib():
     L.rpa_pw_to_grid.argtypes = [vp, i32, i32, vp, vp, vp]
     L.rpa_symmetry_remap.restype = C.c_int
     L.rpa_symmetry_remap.argtypes = [vp, i32, vp, i32, vp, vp]
+    L.rpa_chi0_set_spin_degeneracy.restype = C.c_int
+    L.rpa_chi0_set_spin_degeneracy.argtypes = [vp, i32]
     L.rpa_momentum_pw.restype = C.c_int
     L.rpa_momentum_pw.argtypes = [vp, vp, i32, vp, i32, vp, i32, vp, i32, vp, vp, vp, vp, vp]
     L.rpa_chi0_add_kpoint_optical.restype = C.c_int
@@ -278,6 +281,19 @@ def rpa_ec_q(h: Handle, v_G):
 
 def rpa_chi0_reset(h: Handle):
     _check(lib().rpa_chi0_reset(h.ptr))
+
+
+def rpa_chi0_set_spin_degeneracy(h: Handle, s: int):
+    _check(lib().rpa_chi0_set_spin_degeneracy(h.ptr, int(s)))
+
+
+def rpa_total_energy(ec_q, q_weights) -> float:
+    """E_c = sum_q w_q E_c(q) (Eq. 1): the outer q loop's final sum over the IBZ weights (host arithmetic on the
+    per-q scalars the library returns; the per-q work is rpa_chi0_* / rpa_ec_q)."""
+    e, w = _np(ec_q, np.float64), _np(q_weights, np.float64)
+    if e.shape != w.shape:
+        raise ValueError("one weight per q-point")
+    return float(np.dot(w, e))
 
 
 def rpa_chi0_sync(h: Handle):

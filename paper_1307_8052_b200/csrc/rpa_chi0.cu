@@ -203,6 +203,7 @@ struct rpa_chi0 {
     size_t pd_smem;
     PdZyKernel zy_kernel = nullptr;   // low-instruction-count z+y kernel (planes that fit one CTA), else pd_kernel
     int zy_G = 1, zy_threads = 0, zy_ctas_per_sm = 1, n_sm = 148;
+    double spin_deg = 2.0;             // prefactor s of chi0 = (s/Omega) S: 2 spin-paired (A3), 1 per explicit spin channel
     bool q0 = false;                   // q = 0: pair densities need the optical-limit head (rpa_chi0_add_kpoint_optical)
     int idx0 = -1;                     // sphere index of G = 0 when q0
     bool use_3m = true;                // rank_k3m_kernel (3-multiplication complex product) for the chi0 accumulation
@@ -780,7 +781,7 @@ int rpa_chi0_get(rpa_chi0_t *h, int32_t i_omega, void *chi0_out) {
     const int ng = h->sp.ng;
     const int nt = (ng + 31) / 32;
     chi0_get_kernel<<<dim3(nt, nt), dim3(32, 8), 0, h->stream>>>(h->ptr<cd>(h->L.S) + (size_t)i_omega * ng * h->L.ldS, h->L.ldS, ng,
-                                                                 2.0 / h->vol, (cd *)chi0_out);
+                                                                 h->spin_deg / h->vol, (cd *)chi0_out);
     h->launches += 1;
     CUDA_TRY(cudaGetLastError());
     return RPA_OK;
@@ -799,7 +800,7 @@ int rpa_ec_q(rpa_chi0_t *h, const double *v_G, double *ec_ha, double *e_omega) {
     cd *M = h->ptr<cd>(L.M);
     const cd *S = h->ptr<cd>(L.S);
     const int64_t strideS = (int64_t)ng * L.ldS;
-    const double scale = 2.0 / h->vol;
+    const double scale = h->spin_deg / h->vol;
     CUDA_TRY(cudaMemcpyAsync(d_v, v_G, ng * sizeof(double), cudaMemcpyHostToDevice, st));
     for (int iw0 = 0; iw0 < h->n_omega; iw0 += L.ec_group) {
         const int nm = std::min(L.ec_group, h->n_omega - iw0);
@@ -878,6 +879,13 @@ int rpa_ec_q(rpa_chi0_t *h, const double *v_G, double *ec_ha, double *e_omega) {
 int rpa_chi0_reset(rpa_chi0_t *h) {
     if (!h) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_reset: handle is NULL");
     CUDA_TRY(cudaMemsetAsync(h->ws + h->L.S, 0, (size_t)h->n_omega * h->sp.ng * h->L.ldS * sizeof(cd), h->stream));
+    return RPA_OK;
+}
+
+int rpa_chi0_set_spin_degeneracy(rpa_chi0_t *h, int32_t s) {
+    if (!h) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_set_spin_degeneracy: handle is NULL");
+    if (s != 1 && s != 2) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_set_spin_degeneracy: s must be 1 or 2, got %d", s);
+    h->spin_deg = (double)s;
     return RPA_OK;
 }
 

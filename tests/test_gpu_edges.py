@@ -124,3 +124,41 @@ def test_unsupported_grid_length_is_rejected():
     assert ei.value.code == B.RPA_ERR_UNSUPPORTED
     h = B.rpa_chi0_create((11, 6, 8), cell, (0.25, 0.0, 0.0), 1.0, om, wt, 0, 0, "cuda:0")   # N1 is unrestricted
     h.close()
+
+
+def test_spin_degeneracy_setter():
+    """NEXT-4: s = 1 with two different spin channels against the oracle; invalid s is rejected; s scales the read-out."""
+    import torch
+    from paper_1307_8052_b200 import binding as B
+    cfg = W.CONFIGS[0]
+    up = W.kpoint(cfg, 0, occ=[0, 1, 2], unocc=range(0, 28, 2))
+    dn = W.kpoint(cfg, 0, occ=[1, 3], unocc=range(1, 28, 3))
+    h = _handle(cfg, ptot=0)
+    try:
+        B.rpa_chi0_set_spin_degeneracy(h, 1)
+        for kd in (up, dn):
+            d = _dev(kd)
+            B.rpa_chi0_add_kpoint(h, 1.0, d["psi_occ"], d["psi_unocc"], kd.eps_occ, kd.eps_unocc, kd.f_occ, kd.f_unocc)
+        chi1 = np.stack([B.rpa_chi0_get(h, i).cpu().numpy() for i in range(cfg.n_omega)])
+        g, K2 = B.rpa_chi0_gvectors(h)
+        ec1, _ = B.rpa_ec_q(h, W.coulomb(K2))
+        B.rpa_chi0_set_spin_degeneracy(h, 2)
+        chi2 = B.rpa_chi0_get(h, 0).cpu().numpy()
+        with pytest.raises(B.RpaError) as ei:
+            B.rpa_chi0_set_spin_degeneracy(h, 3)
+        assert ei.value.code == B.RPA_ERR_INVALID_ARG
+    finally:
+        h.close()
+    import oracle
+    om, wt = W.omega_grid(cfg.n_omega)
+    orc = oracle.Chi0Oracle(cfg.grid, cfg.cell, cfg.q_red, W.tuned_ecut(cfg), om, wt, spin_deg=1)
+    for kd in (up, dn):
+        kd.kweight = 1.0
+        orc.add_kpoint(kd)
+    chi_o = orc.get()
+    for i in range(cfg.n_omega):
+        assert rel_fro(chi1[i], chi_o[i]) <= 1e-10
+    assert np.allclose(chi2, 2.0 * chi1[0], rtol=1e-15, atol=0)
+    ec_o, _ = orc.ec_q(W.coulomb(orc.K2))
+    assert abs(ec1 - ec_o) <= 1e-9 * abs(ec_o)
+    assert abs(B.rpa_total_energy([ec1, 2 * ec1], [0.25, 0.75]) - 1.75 * ec1) <= 1e-15 * abs(ec1)

@@ -373,3 +373,17 @@ def test_golden_toy_values():
     assert set(want) == set(vals)
     for k in want:
         assert abs(vals[k] - want[k]) <= 1e-12 * max(1e-300, abs(want[k])), k
+
+
+def test_explicit_spin_channels_equal_the_spin_paired_sum():
+    """NEXT-4: two identical spin channels summed with s = 1 give the spin-paired chi0 (s = 2, reading A3)."""
+    cfg = W.custom_config(55, np.diag([6.0, 6.5, 7.0]), (6, 6, 6), (0.25, 0.0, 0.0), n_occ=2, n_unocc=4, ng_target=8,
+                          n_omega=3, n_atoms=1, n_proj_per_atom=2, orb_ecut_ha=2.0)
+    kd = W.kpoint(cfg, 0)
+    om, wt = W.omega_grid(cfg.n_omega)
+    paired = oracle.Chi0Oracle(cfg.grid, cfg.cell, cfg.q_red, W.tuned_ecut(cfg), om, wt)
+    paired.add_kpoint(kd)
+    spin = oracle.Chi0Oracle(cfg.grid, cfg.cell, cfg.q_red, W.tuned_ecut(cfg), om, wt, spin_deg=1)
+    spin.add_kpoint(kd)
+    spin.add_kpoint(kd)   # the second channel
+    assert np.abs(spin.get() - paired.get()).max() <= 1e-15 * np.abs(paired.get()).max()
