@@ -273,3 +273,73 @@ __global__ void __launch_bounds__(128) pd_xaxis_kernel(const cd *__restrict__ I,
         }
     }
 }
+
+// x axis + gather with the two-level split N1 = 8 NB (N1 % 8 == 0, at most PD_X8_ND kept frequencies per residue mod 8):
+//   A_j[k1] = sum_s x[j + NB s] W_8^(s k1)   (radix-8 butterfly over 8 planes loaded together),
+//   X[f]    = sum_j W_N1^(j f) A_j[f mod 8]  for the ng1 kept f = k1 + 8 d only:
+// 8 independent loads in flight per thread and NB (8 log 8 + ng1) instead of N1 ng1 multiply-adds per column.
+// Dynamic shared memory: N1 * PD_X8_ND * sizeof(cd) (twiddle products per (j, kept-frequency slot)).  Same arguments
+// as pd_xaxis_kernel.
+#define PD_X8_ND 3
+__global__ void __launch_bounds__(128) pd_xaxis8_kernel(const cd *__restrict__ I, cd *__restrict__ Nbuf, int64_t ldn,
+                                                       const cd *__restrict__ tw1, const int32_t *__restrict__ box2s,
+                                                       int N1, int nb2, int g1min, int ng1, int p_begin, double inv_n) {
+    extern __shared__ __align__(16) unsigned char pd_smem[];
+    cd *twt = reinterpret_cast<cd *>(pd_smem);   // [j][slot], slot = k1 PD_X8_ND + d: W_N1^(j f_slot)
+    const int NB = N1 >> 3;
+    // kept frequencies of residue k1: f = k1 + 8 (dlo + d), box index f - g1min (the same for every thread)
+    const int dlo = (g1min >= 0 ? g1min : g1min - 7) / 8;
+    for (int i = threadIdx.x; i < NB * 8 * PD_X8_ND; i += blockDim.x) {
+        const int j = i / (8 * PD_X8_ND), slot = i - j * 8 * PD_X8_ND;
+        const int f = slot / PD_X8_ND + 8 * (dlo + slot % PD_X8_ND);
+        int fp = f % N1;
+        if (fp < 0) fp += N1;
+        twt[i] = tw1[(int)(((int64_t)fp * j) % N1)];
+    }
+    uint32_t mask = 0;
+#pragma unroll
+    for (int slot = 0; slot < 8 * PD_X8_ND; slot++) {
+        const int gi = slot / PD_X8_ND + 8 * (dlo + slot % PD_X8_ND) - g1min;
+        if (gi >= 0 && gi < ng1) mask |= 1u << slot;
+    }
+    __syncthreads();
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= nb2) return;
+    const int pl = blockIdx.y;
+    const cd *Ip = I + (size_t)pl * N1 * nb2 + b;
+    cd acc[8][PD_X8_ND];
+#pragma unroll
+    for (int k1 = 0; k1 < 8; k1++)
+#pragma unroll
+        for (int d = 0; d < PD_X8_ND; d++) acc[k1][d] = cmake(0.0, 0.0);
+    for (int j = 0; j < NB; j++) {
+        cd v[8];
+#pragma unroll
+        for (int s = 0; s < 8; s++) v[s] = Ip[(size_t)(j + NB * s) * nb2];
+        Bfly<8>::run(v);
+        const cd *tj = twt + j * 8 * PD_X8_ND;
+#pragma unroll
+        for (int k1 = 0; k1 < 8; k1++)
+#pragma unroll
+            for (int d = 0; d < PD_X8_ND; d++)
+                if (mask & (1u << (k1 * PD_X8_ND + d))) acc[k1][d] = cfma(tj[k1 * PD_X8_ND + d], v[k1], acc[k1][d]);
+    }
+    cd *out = Nbuf + (size_t)(p_begin + pl) * ldn;
+#pragma unroll
+    for (int k1 = 0; k1 < 8; k1++)
+#pragma unroll
+        for (int d = 0; d < PD_X8_ND; d++)
+            if (mask & (1u << (k1 * PD_X8_ND + d))) {
+                const int gi = k1 + 8 * (dlo + d) - g1min;
+                const int s = box2s[(size_t)gi * nb2 + b];
+                if (s >= 0) out[s] = cscale(inv_n, acc[k1][d]);
+            }
+}
+// can pd_xaxis8_kernel serve this x axis?  (every kept frequency must fall in one of its PD_X8_ND slots per residue)
+static inline bool pd_xaxis8_ok(int N1, int g1min, int ng1) {
+    if (N1 % 8 != 0 || N1 < 16 || ng1 > N1) return false;
+    const int dlo = (g1min >= 0 ? g1min : g1min - 7) / 8;
+    const int gmax = g1min + ng1 - 1;
+    const int dhi = (gmax >= 0 ? gmax : gmax - 7) / 8;
+    return dhi - dlo + 1 <= PD_X8_ND && 8 * (dhi - dlo + 1) <= N1;
+}
