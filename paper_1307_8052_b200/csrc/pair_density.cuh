@@ -274,13 +274,14 @@ __global__ void __launch_bounds__(128) pd_xaxis_kernel(const cd *__restrict__ I,
     }
 }
 
-// x axis + gather with the two-level split N1 = 8 NB (N1 % 8 == 0, at most PD_X8_ND kept frequencies per residue mod 8):
+// x axis + gather with the two-level split N1 = 8 NB (N1 % 8 == 0, at most PD_X8_ND_MAX kept frequencies per residue mod 8):
 //   A_j[k1] = sum_s x[j + NB s] W_8^(s k1)   (radix-8 butterfly over 8 planes loaded together),
 //   X[f]    = sum_j W_N1^(j f) A_j[f mod 8]  for the ng1 kept f = k1 + 8 d only:
 // 8 independent loads in flight per thread and NB (8 log 8 + ng1) instead of N1 ng1 multiply-adds per column.
 // Dynamic shared memory: N1 * PD_X8_ND * sizeof(cd) (twiddle products per (j, kept-frequency slot)).  Same arguments
 // as pd_xaxis_kernel.
-#define PD_X8_ND 3
+#define PD_X8_ND_MAX 3
+template <int PD_X8_ND>   // kept-frequency slots per residue mod 8 (2 when the box needs no more: fewer registers)
 __global__ void __launch_bounds__(128) pd_xaxis8_kernel(const cd *__restrict__ I, cd *__restrict__ Nbuf, int64_t ldn,
                                                        const cd *__restrict__ tw1, const int32_t *__restrict__ box2s,
                                                        int N1, int nb2, int g1min, int ng1, int p_begin, double inv_n) {
@@ -336,10 +337,13 @@ __global__ void __launch_bounds__(128) pd_xaxis8_kernel(const cd *__restrict__ I
             }
 }
 // can pd_xaxis8_kernel serve this x axis?  (every kept frequency must fall in one of its PD_X8_ND slots per residue)
-static inline bool pd_xaxis8_ok(int N1, int g1min, int ng1) {
-    if (N1 % 8 != 0 || N1 < 16 || ng1 > N1) return false;
+// returns the number of slots needed (2 or 3), or 0 if the kernel cannot serve this x axis
+static inline int pd_xaxis8_slots(int N1, int g1min, int ng1) {
+    if (N1 % 8 != 0 || N1 < 16 || ng1 > N1) return 0;
     const int dlo = (g1min >= 0 ? g1min : g1min - 7) / 8;
     const int gmax = g1min + ng1 - 1;
     const int dhi = (gmax >= 0 ? gmax : gmax - 7) / 8;
-    return dhi - dlo + 1 <= PD_X8_ND && 8 * (dhi - dlo + 1) <= N1;
+    const int nd = dhi - dlo + 1;
+    if (nd > PD_X8_ND_MAX || 8 * nd > N1) return 0;
+    return nd <= 2 ? 2 : 3;
 }

@@ -644,8 +644,12 @@ int add_kpoint_impl(rpa_chi0_t *h, double kweight, int32_t n_occ, const void *ps
                 }
                 {
                     StageTimer tm(h, 1, 1);
-                    if (pd_xaxis8_ok(N1, sp.gmin[0], ng1))
-                        pd_xaxis8_kernel<<<dim3((nb2 + 127) / 128, pc), 128, (size_t)N1 * PD_X8_ND * sizeof(cd), st>>>(
+                    const int xslots = pd_xaxis8_slots(N1, sp.gmin[0], ng1);
+                    if (xslots == 2)
+                        pd_xaxis8_kernel<2><<<dim3((nb2 + 127) / 128, pc), 128, (size_t)N1 * 2 * sizeof(cd), st>>>(
+                            h->ptr<cd>(L.I), Nbuf, L.ldn, h->ptr<cd>(L.tw1), h->ptr<int32_t>(L.box2s), N1, nb2, sp.gmin[0], ng1, p0, inv_n);
+                    else if (xslots == 3)
+                        pd_xaxis8_kernel<3><<<dim3((nb2 + 127) / 128, pc), 128, (size_t)N1 * 3 * sizeof(cd), st>>>(
                             h->ptr<cd>(L.I), Nbuf, L.ldn, h->ptr<cd>(L.tw1), h->ptr<int32_t>(L.box2s), N1, nb2, sp.gmin[0], ng1, p0, inv_n);
                     else
                         pd_xaxis_kernel<<<dim3((nb2 + 127) / 128, pc), 128, (size_t)N1 * PD_G1_BLOCK * sizeof(cd), st>>>(
