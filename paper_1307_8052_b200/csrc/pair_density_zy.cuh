@@ -190,7 +190,9 @@ struct PdZyCursor {
     int w, p0, cnt, n, m, c, g, j1;
 };
 
-template <int N3, int NA3, int DLO, int DHI, int N2, int NA2, int NW, int LPW, int G, int MINB>
+// YROW: y pass B with one output row per thread and its twiddles in registers (else tasks dealt round-robin with the
+// twiddles read from shared memory); measured better for the 60- and 48-row planes, worse for 24 and 40
+template <int N3, int NA3, int DLO, int DHI, int N2, int NA2, int NW, int LPW, int G, int MINB, bool YROW = false>
 __global__ void __launch_bounds__(NW * 32, MINB) pd_zy_kernel(const __grid_constant__ PdZyParams P) {
     using C = PdZy<N3, NA3, DLO, DHI, N2, NA2, NW, LPW, G>;
     constexpr int ND = C::ND;
@@ -286,6 +288,20 @@ __global__ void __launch_bounds__(NW * 32, MINB) pd_zy_kernel(const __grid_const
     if (pf.cnt > 0) advance(pf);
     // y pass-B start position of this thread: task t = tid -> (pair g, r = o ng3 + col)
     const int yb_g0 = tid / nb2, yb_r0 = tid - yb_g0 * nb2;
+    // YROW: output row o = tid / tpo (tpo threads per row), first column tid % tpo; the row's frequency f, its source
+    // rows NB2 (f mod NA2) + j2 and its twiddles W_N2^(j2 f) never change
+    const int yb_tpo = max(1, NTH / ng2);
+    const int yb_o = (tid / yb_tpo < ng2) ? tid / yb_tpo : -1, yb_c0 = tid % yb_tpo;
+    int yb_row = 0;
+    cd ytw[(YROW && NB2 > 1) ? NB2 - 1 : 1];
+    if constexpr (YROW) {
+        int f = P.g2min + (yb_o >= 0 ? yb_o : 0);
+        f %= N2;
+        if (f < 0) f += N2;
+        yb_row = NB2 * (f % NA2);
+#pragma unroll
+        for (int j2 = 1; j2 < NB2; j2++) ytw[j2 - 1] = P.tw2[(j2 * f) % N2];
+    }
     __syncthreads();
 
     // one z iteration (chunk c of pair g of the unit) on the inputs in nx; refills nx for two iterations later
@@ -342,7 +358,23 @@ __global__ void __launch_bounds__(NW * 32, MINB) pd_zy_kernel(const __grid_const
             }
         }
         __syncthreads();
-        {   // pass B: out[g][o][g3i] = sum_j2 W_N2^(j2 f) A[j2 + NB2 (f mod NA2)][g][g3i]
+        if constexpr (YROW) {   // pass B, this thread's output row: columns gc = gg ng3 + col with stride yb_tpo
+            if (yb_o >= 0) {
+                cd *Io = P.I + ((size_t)(p0 - P.p_begin) * P.N1 + j1) * nb2 + yb_o * ng3;
+                const cd *src = Y + (size_t)yb_row * pitch;
+                int gg = 0, col = yb_c0;
+                while (col >= ng3) { col -= ng3; gg++; }
+                while (gg < cnt) {
+                    const cd *sp = src + gg * ng3 + col;
+                    cd acc = sp[0];
+#pragma unroll
+                    for (int j2 = 1; j2 < NB2; j2++) acc = cfma(ytw[j2 - 1], sp[j2 * pitch], acc);
+                    Io[(size_t)gg * P.N1 * nb2 + col] = acc;
+                    col += yb_tpo;
+                    while (col >= ng3) { col -= ng3; gg++; }
+                }
+            }
+        } else {   // pass B: out[g][o][g3i] = sum_j2 W_N2^(j2 f) A[j2 + NB2 (f mod NA2)][g][g3i]
             int gg = yb_g0, r = yb_r0;
             cd *Io = P.I + ((size_t)(p0 - P.p_begin) * P.N1 + j1) * nb2;
             while (gg < cnt) {

@@ -311,14 +311,14 @@ void try_zy(rpa_chi0 *h, K kernel, int G, int minb) {
 void plan_zy_kernel(rpa_chi0 *h) {
     const int N2 = h->grid[1], N3 = h->grid[2];
     h->zy_kernel = nullptr;
-#define ZY(N3_, NA3_, DLO_, DHI_, N2_, NA2_, NW_, LPW_, G_, MINB_)                     \
+#define ZY(N3_, NA3_, DLO_, DHI_, N2_, NA2_, NW_, LPW_, G_, MINB_, ...)                \
     try_zy<PdZy<N3_, NA3_, DLO_, DHI_, N2_, NA2_, NW_, LPW_, G_>>(                     \
-        h, pd_zy_kernel<N3_, NA3_, DLO_, DHI_, N2_, NA2_, NW_, LPW_, G_, MINB_>, G_, MINB_)
-    if (N2 == 60 && N3 == 64) ZY(64, 8, -1, 0, 60, 12, 4, 4, 4, 2);
+        h, pd_zy_kernel<N3_, NA3_, DLO_, DHI_, N2_, NA2_, NW_, LPW_, G_, MINB_, ##__VA_ARGS__>, G_, MINB_)
+    if (N2 == 60 && N3 == 64) ZY(64, 8, -1, 0, 60, 12, 4, 4, 4, 2, true);
     else if (N2 == 24 && N3 == 24) ZY(24, 8, -1, 0, 24, 8, 3, 8, 4, 3);
     else if (N2 == 16 && N3 == 16) ZY(16, 8, -1, 0, 16, 8, 1, 16, 4, 8);
     else if (N2 == 40 && N3 == 168) ZY(168, 12, -2, 1, 40, 8, 4, 2, 2, 2);
-    else if (N2 == 48 && N3 == 192) ZY(192, 12, -3, 2, 48, 12, 8, 2, 2, 1);
+    else if (N2 == 48 && N3 == 192) ZY(192, 12, -3, 2, 48, 12, 8, 2, 2, 1, true);
 #undef ZY
 }
 
