@@ -317,7 +317,7 @@ void plan_zy_kernel(rpa_chi0 *h) {
     if (N2 == 60 && N3 == 64) ZY(64, 8, -1, 0, 60, 12, 4, 4, 4, 2, true);
     else if (N2 == 24 && N3 == 24) ZY(24, 8, -1, 0, 24, 8, 3, 8, 4, 3);
     else if (N2 == 16 && N3 == 16) ZY(16, 8, -1, 0, 16, 8, 1, 16, 4, 8);
-    else if (N2 == 40 && N3 == 168) ZY(168, 12, -2, 1, 40, 8, 4, 2, 2, 2);
+    else if (N2 == 40 && N3 == 168) ZY(168, 12, -2, 1, 40, 8, 4, 2, 1, 2);
     else if (N2 == 48 && N3 == 192) ZY(192, 12, -3, 2, 48, 12, 8, 2, 2, 1, true);
 #undef ZY
 }
