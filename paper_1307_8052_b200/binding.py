@@ -398,7 +398,7 @@ def rpa_probe_fp64_tensor_peak(device="cuda:0") -> float:
 
 # ---- host-buffer convenience on top of the calls above (the end-to-end path bench.py times) ------------------
 
-def add_kpoint_host(h: Handle, kd, n_proj=None, Q_dev=None, R_cart=None, pinned=None, kweight=None, chunk_bands=128):
+def add_kpoint_host(h: Handle, kd, n_proj=None, Q_dev=None, R_cart=None, pinned=None, kweight=None, chunk_bands=64):
     """Copy one k-point's host arrays (workload.KPointData) to the device and add it; returns the bytes copied
     host->device.  `pinned` may hold pre-pinned host tensors keyed like the KPointData fields.
 
