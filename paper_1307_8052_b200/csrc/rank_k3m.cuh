@@ -31,22 +31,24 @@ constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 2 * STAGES * 8;
 }  // namespace rk3
 
 // Nb[Kpad][ldn] (rows >= K zero), w[n_omega][ldw], S[n_omega][ng][ldS] (lower triangle accumulated), Kpad % 32 == 0.
-// grid = (ntiles_lower(ng), n_omega, ksplit); ksplit as in rank_k_kernel (atomic tile adds when > 1).
+// Work items (tile, frequency) are numbered item = iw * ntiles + tile; grid = (n_items_of_this_launch, 1, ksplit), the
+// launch covers items item_off .. item_off + gridDim.x - 1; ksplit as in rank_k_kernel (atomic tile adds when > 1).
+// The host issues the whole waves with ksplit = 1 and the last partial wave K-sliced so that it also fills the GPU.
 __global__ void __launch_bounds__(rk3::THREADS, 1)
 rank_k3m_kernel(const cd *__restrict__ Nb, int64_t ldn, int Kpad, const double *__restrict__ w, int64_t ldw,
-                cd *__restrict__ S, int64_t ldS, int64_t strideS, int ng) {
+                cd *__restrict__ S, int64_t ldS, int64_t strideS, int ng, int ntiles, int item_off) {
     using namespace rk3;
     extern __shared__ __align__(128) unsigned char rk_smem[];
     uint64_t *full = reinterpret_cast<uint64_t *>(rk_smem + STAGES * STAGE_BYTES);
     uint64_t *empty = full + STAGES;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int t = blockIdx.x;
+    const int item = item_off + (int)blockIdx.x;
+    const int iw = item / ntiles, t = item - iw * ntiles;
     int ti = (int)((sqrt(8.0 * (double)t + 1.0) - 1.0) * 0.5);
     while ((ti + 1) * (ti + 2) / 2 <= t) ti++;
     while (ti * (ti + 1) / 2 > t) ti--;
     const int tj = t - ti * (ti + 1) / 2;
     const int row0 = ti * T, col0 = tj * T;
-    const int iw = blockIdx.y;
     const uint32_t rowbytes = (uint32_t)min(T, ng - row0) * 16u, colbytes = (uint32_t)min(T, ng - col0) * 16u;
     const uint32_t stage_tx = KC * (rowbytes + colbytes) + KC * 8u;
 

@@ -278,7 +278,7 @@ int ntiles_lower(int n, int t) {
 // K slices of the rank-K launch: one CTA per SM, `units` equal work items (tile x frequency pair).  With s slices
 // the grid needs ceil(units s / n_sm) rounds of 1/s of an item each; take the s that minimises that time, charging
 // 1 % per extra slice for its prologue / atomic epilogue, and keep at least 16 chunks (256 pairs) per slice.
-int pick_ksplit(int units, int nchunks, int n_sm) {
+int pick_ksplit(int units, int nchunks, int n_sm, double *cost_out = nullptr) {
     int best = 1;
     double best_cost = 1e300;
     for (int s = 1; s <= 8 && nchunks / s >= 16; s++) {
@@ -286,6 +286,7 @@ int pick_ksplit(int units, int nchunks, int n_sm) {
         const double cost = rounds * (1.0 + 0.01 * (s - 1));
         if (cost < best_cost * (1.0 - 1e-9)) { best_cost = cost; best = s; }
     }
+    if (cost_out) *cost_out = best_cost;   // in units of one full-K item
     return best;
 }
 
@@ -688,10 +689,25 @@ int add_kpoint_impl(rpa_chi0_t *h, double kweight, int32_t n_occ, const void *ps
             {
                 StageTimer tm(h, 4, 1);
                 if (h->use_3m) {
-                    const int units = ntiles_lower(ng, rk3::T) * h->n_omega;
-                    const int ksplit = pick_ksplit(units, Kpad / rk3::KC, h->n_sm);
-                    rank_k3m_kernel<<<dim3(ntiles_lower(ng, rk3::T), h->n_omega, ksplit), rk3::THREADS, rk3::SMEM_BYTES, st>>>(
-                        Nbuf, L.ldn, Kpad, w, L.ldw, h->ptr<cd>(L.S), L.ldS, (int64_t)ng * L.ldS, ng);
+                    // whole waves (one CTA per SM) with full K, then the last partial wave K-sliced so that it fills the GPU too
+                    const int ntiles = ntiles_lower(ng, rk3::T), units = ntiles * h->n_omega, nchunks = Kpad / rk3::KC;
+                    const int whole = units / h->n_sm * h->n_sm;
+                    const int tail = units - whole;
+                    auto launch = [&](int off, int count, int ksplit) {
+                        rank_k3m_kernel<<<dim3(count, 1, ksplit), rk3::THREADS, rk3::SMEM_BYTES, st>>>(
+                            Nbuf, L.ldn, Kpad, w, L.ldw, h->ptr<cd>(L.S), L.ldS, (int64_t)ng * L.ldS, ng, ntiles, off);
+                    };
+                    double c_single = 0.0, c_tail = 0.0;
+                    const int s_single = pick_ksplit(units, nchunks, h->n_sm, &c_single);
+                    const int s_tail = tail > 0 ? pick_ksplit(tail, nchunks, h->n_sm, &c_tail) : 1;
+                    // two launches only if the model says they save at least a tenth of an item
+                    if (whole > 0 && tail > 0 && whole / h->n_sm + c_tail + 0.1 < c_single) {
+                        launch(0, whole, 1);
+                        launch(whole, tail, s_tail);
+                        h->launches += 1;
+                    } else {
+                        launch(0, units, s_single);
+                    }
                 } else {
                     const int units = ntiles_lower(ng, rk::T) * ((h->n_omega + rk::Cfg<true>::NW - 1) / rk::Cfg<true>::NW);
                     const int ksplit = pick_ksplit(units, Kpad / rk::KC, h->n_sm);
