@@ -40,6 +40,10 @@ def lib():
         L.orc_weights.argtypes = [f64, f64, i32, vp, vp, i32, vp, vp]
         L.orc_accumulate.restype = None
         L.orc_accumulate.argtypes = [i32, i32, vp, i32, vp, f64, vp]
+        L.orc_weights_z.restype = None
+        L.orc_weights_z.argtypes = [f64, f64, i32, vp, vp, i32, vp, vp]
+        L.orc_accumulate_z.restype = None
+        L.orc_accumulate_z.argtypes = [i32, i32, vp, i32, vp, f64, vp]
         L.orc_chi0_from_S.restype = None
         L.orc_chi0_from_S.argtypes = [C.c_int64, f64, vp, vp]
         L.orc_ec_q.restype = i32
@@ -138,6 +142,22 @@ def accumulate(S, n, w, kweight):
     return S
 
 
+def weights_z(eps_n, f_n, eps_m, f_m, z):
+    """Complex weights of Eq. 3 at the complex frequencies z (NEXT-4 real axis: z = omega + i eta): [iz][m]."""
+    eps_m, f_m, z = _f64(eps_m), _f64(f_m), _c128(z)
+    w = np.zeros((z.size, eps_m.size), dtype=np.complex128)
+    lib().orc_weights_z(float(eps_n), float(f_n), eps_m.size, _p(eps_m), _p(f_m), z.size, _p(z), _p(w))
+    return w
+
+
+def accumulate_z(S, n, w, kweight):
+    """S[nz][ng][ng] += kweight * sum_p w[iz][p] n[p][g] conj(n[p][g']) with complex w."""
+    n, w = _c128(n), _c128(w)
+    assert S.dtype == np.complex128 and S.flags.c_contiguous
+    lib().orc_accumulate_z(n.shape[1], n.shape[0], _p(n), w.shape[0], _p(w), float(kweight), _p(S))
+    return S
+
+
 def chi0_from_S(S, vol, spin_deg=None):
     """chi0 = (2/Omega) S (spin-paired, reading A3), or (spin_deg/Omega) S for explicit spin channels (NEXT-4)."""
     S = _c128(S)
@@ -212,8 +232,12 @@ class Chi0Oracle:
     ``g`` may be given explicitly (a sampled sub-list of the sphere): chi0 restricted to those G is exactly the
     chi0 of those G, because every element of Eq. 17 is an independent sum."""
 
-    def __init__(self, grid, cell, q_red, ecut_ha, omega, omega_wt=None, g=None, mode="separable", spin_deg=None):
+    def __init__(self, grid, cell, q_red, ecut_ha, omega, omega_wt=None, g=None, mode="separable", spin_deg=None,
+                 eta=None):
+        """eta = None: omega are points i omega of the imaginary axis (the path).  eta > 0 (NEXT-4): omega are real
+        frequencies and chi0 is evaluated at z = omega + i eta with the complex weights of ``weights_z``."""
         self.spin_deg = spin_deg
+        self.eta = eta
         self.grid, self.cell, self.q = _i32(grid), _f64(cell).reshape(3, 3), _f64(q_red)
         self.omega = _f64(omega)
         self.omega_wt = None if omega_wt is None else _f64(omega_wt)
@@ -243,8 +267,12 @@ class Chi0Oracle:
             nt = self.pair_densities(n, kd, n_proj, Q, R_cart)
             if head is not None:
                 nt[:, i0] = head[n]
-            w = weights(kd.eps_occ[n], kd.f_occ[n], kd.eps_unocc, kd.f_unocc, self.omega)
-            accumulate(self.S, nt, w, kd.kweight)
+            if self.eta is None:
+                w = weights(kd.eps_occ[n], kd.f_occ[n], kd.eps_unocc, kd.f_unocc, self.omega)
+                accumulate(self.S, nt, w, kd.kweight)
+            else:
+                w = weights_z(kd.eps_occ[n], kd.f_occ[n], kd.eps_unocc, kd.f_unocc, self.omega + 1j * self.eta)
+                accumulate_z(self.S, nt, w, kd.kweight)
             self.n_pairs += nt.shape[0]
 
     def get(self, i_omega=None):

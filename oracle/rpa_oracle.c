@@ -290,6 +290,39 @@ void orc_accumulate(int32_t ng, int32_t n_p, const zd *n, int32_t n_omega, const
         }
 }
 
+/*
+ * SURVEY 8(f) NEXT-4, second workload ("the non-interacting response function is one key ingredient" of
+ * TDDFT / GW / BSE): Eq. 3 at a general complex frequency z in place of i omega (z = omega + i eta on the
+ * real axis), reading A19.  Eq. 3 sums over BOTH orderings of every band pair; under time reversal the
+ * reversed ordering (m -> n) has the same n n^H as (n -> m) (reading A1), so for one occupied n and n_m unoccupied m
+ *   w_nm(z) = (f_n - f_m) / (z + eps_n - eps_m)  +  (f_m - f_n) / (z + eps_m - eps_n)        (complex),
+ * each term written as printed.  w[iz][m].
+ */
+void orc_weights_z(double eps_n, double f_n, int32_t n_m, const double *eps_m, const double *f_m, int32_t n_z,
+                   const zd *z, zd *w) {
+    for (int32_t iz = 0; iz < n_z; iz++)
+        for (int32_t m = 0; m < n_m; m++) {
+            const zd forward = (f_n - f_m[m]) / (z[iz] + eps_n - eps_m[m]);
+            const zd reversed = (f_m[m] - f_n) / (z[iz] + eps_m[m] - eps_n);
+            w[(int64_t)iz * n_m + m] = forward + reversed;
+        }
+}
+
+/* Eq. 17 with those complex weights: S_z[g][g'] += kweight * sum_p w[iz][p] n_p(g) conj(n_p(g')). */
+void orc_accumulate_z(int32_t ng, int32_t n_p, const zd *n, int32_t n_z, const zd *w, double kweight, zd *S) {
+#pragma omp parallel for collapse(2) schedule(static)
+    for (int32_t iz = 0; iz < n_z; iz++)
+        for (int32_t a = 0; a < ng; a++) {
+            zd *row = S + ((int64_t)iz * ng + a) * ng;
+            for (int32_t b = 0; b < ng; b++) {
+                zd acc = 0.0;
+                for (int32_t p = 0; p < n_p; p++)
+                    acc += w[(int64_t)iz * n_p + p] * (n[(int64_t)p * ng + a] * conj(n[(int64_t)p * ng + b]));
+                row[b] += kweight * acc;
+            }
+        }
+}
+
 /* Step 6, prefactor of Eq. 3 (readings A1-A3): chi0 = (2/Omega) S, spin-paired. */
 void orc_chi0_from_S(int64_t count, double volume, const zd *S, zd *chi0) {
     const double s = 2.0 / volume;
