@@ -74,13 +74,34 @@ size_t rpa_chi0_workspace_bytes(const int32_t grid[3], const double cell[9], con
  *   grid, cell, q_red, omega_ha[n_omega] (> 0), omega_wt[n_omega] (may be NULL if rpa_ec_q is not used): host.
  *   workspace: dev, 256-byte aligned, at least rpa_chi0_workspace_bytes(...) bytes, must outlive the handle.
  *   cuda_stream: a cudaStream_t (NULL = legacy default stream).
- * q_red = 0 gives RPA_ERR_UNSUPPORTED; so does a grid length N2 or N3 with a prime factor other than 2, 3, 5, 7
- * (N1 is unrestricted) or a grid so large that one z line per chunk does not fit shared memory.
+ * q_red = 0 creates an optical-limit handle (pair densities then come from rpa_chi0_add_kpoint_optical).  A grid
+ * length N2 or N3 with a prime factor other than 2, 3, 5, 7 (N1 is unrestricted), or a grid so large that one z line
+ * per chunk does not fit shared memory, gives RPA_ERR_UNSUPPORTED.
  */
 int rpa_chi0_create(rpa_chi0_t **out, const int32_t grid[3], const double cell[9], const double q_red[3],
                     double ecut_ha, int32_t n_omega, const double *omega_ha, const double *omega_wt,
                     int32_t max_batch_pairs, int32_t max_proj_total, void *workspace, size_t workspace_bytes,
                     void *cuda_stream);
+
+/*
+ * SURVEY 8(f) NEXT-4, second workload (chi0 as the ingredient of TDDFT / GW / BSE): the same chi0 on the REAL
+ * frequency axis.  Eq. 3 is evaluated at z = omega + i eta instead of i omega, both orderings of each band
+ * pair as printed, the reversed one folded onto the occ -> unocc pair by time reversal (readings A1, A19):
+ *   chi0_GG'(omega) = (s/Omega) sum_k wk sum_{n occ, m unocc} w_nm(z) n_nm(G) conj(n_nm(G')),
+ *   w_nm(z) = (f_n - f_m) [ 1/(z + e_n - e_m) - 1/(z + e_m - e_n) ]                 (complex; chi0 is not Hermitian).
+ * The weight splits into real and imaginary parts, so the handle keeps TWO Hermitian accumulators per frequency and
+ * every add_kpoint call runs the same kernels as on the imaginary axis over 2 n_omega slots:
+ *   workspace: at least rpa_chi0_workspace_bytes(grid, cell, q_red, ecut_ha, 2 * n_omega, ...) bytes.
+ *   omega_ha[n_omega]: host, finite, any sign; eta_ha > 0 (the broadening; omega = 0, eta = u is the point i u of the
+ *   imaginary axis).  Everything else as rpa_chi0_create.
+ * On such a handle rpa_chi0_get(i) returns the full complex matrix chi0(omega_i + i eta); rpa_ec_q returns
+ * RPA_ERR_UNSUPPORTED (Eq. 2 is an imaginary-axis integral); all add_kpoint variants, reset, the spin setter and the
+ * orbital utilities work unchanged.
+ */
+int rpa_chi0_create_real_axis(rpa_chi0_t **out, const int32_t grid[3], const double cell[9], const double q_red[3],
+                              double ecut_ha, int32_t n_omega, const double *omega_ha, double eta_ha,
+                              int32_t max_batch_pairs, int32_t max_proj_total, void *workspace, size_t workspace_bytes,
+                              void *cuda_stream);
 
 /* Number of G vectors in the sphere. */
 int rpa_chi0_ng(const rpa_chi0_t *h, int32_t *ng);

@@ -26,7 +26,7 @@ EXPORTS = (
     "rpa_chi0_get", "rpa_ec_q", "rpa_chi0_reset", "rpa_chi0_sync", "rpa_chi0_set_profiling", "rpa_chi0_stage_times",
     "rpa_chi0_launch_count", "rpa_chi0_accumulators", "rpa_chi0_destroy", "rpa_probe_fp64_tensor_peak", "rpa_last_error",
     "rpa_pw_to_grid", "rpa_symmetry_remap", "rpa_momentum_pw", "rpa_chi0_add_kpoint_optical",
-    "rpa_chi0_set_spin_degeneracy",
+    "rpa_chi0_set_spin_degeneracy", "rpa_chi0_create_real_axis",
 )
 
 STAGE_NAMES = ("pair_product_fft_yz", "fft_x_gather", "paw", "weights", "rank_k")
@@ -62,6 +62,8 @@ def lib():
     L.rpa_chi0_workspace_bytes.argtypes = [vp, vp, vp, f64, i32, i32, i32]
     L.rpa_chi0_create.restype = C.c_int
     L.rpa_chi0_create.argtypes = [C.POINTER(vp), vp, vp, vp, f64, i32, vp, vp, i32, i32, vp, sz, vp]
+    L.rpa_chi0_create_real_axis.restype = C.c_int
+    L.rpa_chi0_create_real_axis.argtypes = [C.POINTER(vp), vp, vp, vp, f64, i32, vp, f64, i32, i32, vp, sz, vp]
     L.rpa_chi0_ng.restype = C.c_int
     L.rpa_chi0_ng.argtypes = [vp, C.POINTER(i32)]
     L.rpa_chi0_gvectors.restype = C.c_int
@@ -177,7 +179,8 @@ def rpa_chi0_workspace_bytes(grid, cell, q_red, ecut_ha, n_omega, max_batch_pair
 
 
 def rpa_chi0_create(grid, cell, q_red, ecut_ha, omega_ha, omega_wt=None, max_batch_pairs=0, max_proj_total=0,
-                    device="cuda:0", stream=None) -> Handle:
+                    device="cuda:0", stream=None, eta_ha=None) -> Handle:
+    """eta_ha given: rpa_chi0_create_real_axis (omega_ha real frequencies, chi0 at omega + i eta, no omega_wt)."""
     torch = _torch()
     device = torch.device(device)
     if device.index is None:
@@ -185,18 +188,32 @@ def rpa_chi0_create(grid, cell, q_red, ecut_ha, omega_ha, omega_wt=None, max_bat
     g, c, q = _np(grid, np.int32), _np(cell, np.float64).reshape(9), _np(q_red, np.float64)
     om = _np(omega_ha, np.float64)
     wt = None if omega_wt is None else _np(omega_wt, np.float64)
-    nbytes = rpa_chi0_workspace_bytes(g, c, q, ecut_ha, om.size, max_batch_pairs, max_proj_total)
+    n_slots = om.size if eta_ha is None else 2 * om.size
+    nbytes = rpa_chi0_workspace_bytes(g, c, q, ecut_ha, n_slots, max_batch_pairs, max_proj_total)
     with torch.cuda.device(device):
         ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=device)
         off = (-ws.data_ptr()) % 256
         if stream is None:
             stream = torch.cuda.current_stream(device)
         out = C.c_void_p()
-        rc = lib().rpa_chi0_create(C.byref(out), _hp(g), _hp(c), _hp(q), float(ecut_ha), int(om.size), _hp(om),
-                                   None if wt is None else _hp(wt), int(max_batch_pairs), int(max_proj_total),
-                                   C.c_void_p(ws.data_ptr() + off), C.c_size_t(nbytes), C.c_void_p(stream.cuda_stream))
+        if eta_ha is None:
+            rc = lib().rpa_chi0_create(C.byref(out), _hp(g), _hp(c), _hp(q), float(ecut_ha), int(om.size), _hp(om),
+                                       None if wt is None else _hp(wt), int(max_batch_pairs), int(max_proj_total),
+                                       C.c_void_p(ws.data_ptr() + off), C.c_size_t(nbytes), C.c_void_p(stream.cuda_stream))
+        else:
+            rc = lib().rpa_chi0_create_real_axis(C.byref(out), _hp(g), _hp(c), _hp(q), float(ecut_ha), int(om.size),
+                                                 _hp(om), float(eta_ha), int(max_batch_pairs), int(max_proj_total),
+                                                 C.c_void_p(ws.data_ptr() + off), C.c_size_t(nbytes),
+                                                 C.c_void_p(stream.cuda_stream))
     _check(rc)
     return Handle(out, ws, device, stream, g, om.size)
+
+
+def rpa_chi0_create_real_axis(grid, cell, q_red, ecut_ha, omega_ha, eta_ha, max_batch_pairs=0, max_proj_total=0,
+                              device="cuda:0", stream=None) -> Handle:
+    """chi0 at the real frequencies omega_ha + i eta_ha (NEXT-4); rpa_chi0_get then returns a non-Hermitian matrix."""
+    return rpa_chi0_create(grid, cell, q_red, ecut_ha, omega_ha, None, max_batch_pairs, max_proj_total, device, stream,
+                           eta_ha=float(eta_ha))
 
 
 def rpa_chi0_ng(h: Handle) -> int:

@@ -44,11 +44,15 @@ struct Cfg {
 };
 }  // namespace rk
 
-// w[iw*ldw + p] = kweight * 2 (f_n - f_m)(e_n - e_m) / (omega_iw^2 + (e_n - e_m)^2) for p < K, 0 for K <= p < Kpad.
+// eta < 0 (imaginary axis, Eq. 18 in its real form, reading A1):
+//   w[iw*ldw + p] = kweight * 2 (f_n - f_m)(e_n - e_m) / (omega_iw^2 + (e_n - e_m)^2) for p < K, 0 for K <= p < Kpad.
+// eta > 0 (real axis, NEXT-4, reading A19): slot iw = 2 i + part holds the real (part 0) or imaginary (part 1) part of
+//   w = kweight (f_n - f_m) [1/(z - D) - 1/(z + D)],  z = omega_i + i eta,  D = e_m - e_n,   1/(x + i eta) = (x - i eta)/(x^2 + eta^2)
+// (omega[] holds omega_i twice), so that chi0 = S(Re w) + i S(Im w) with two Hermitian accumulators.
 __global__ void weights_kernel(double *__restrict__ w, int64_t ldw, int K, int Kpad, const double *__restrict__ omega,
                                int n_omega, const double *__restrict__ eps_occ, const double *__restrict__ f_occ,
                                const double *__restrict__ eps_unocc, const double *__restrict__ f_unocc, int n0,
-                               int mlen, int m0, double kweight) {
+                               int mlen, int m0, double kweight, double eta) {
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     const int iw = blockIdx.y;
     if (p >= Kpad || iw >= n_omega) return;
@@ -57,7 +61,14 @@ __global__ void weights_kernel(double *__restrict__ w, int64_t ldw, int K, int K
         const int n = n0 + p / mlen, m = m0 + p % mlen;
         const double de = eps_occ[n] - eps_unocc[m];
         const double om = omega[iw];
-        val = kweight * (2.0 * (f_occ[n] - f_unocc[m]) * de / (om * om + de * de));
+        const double df = f_occ[n] - f_unocc[m];
+        if (eta < 0.0) {
+            val = kweight * (2.0 * df * de / (om * om + de * de));
+        } else {
+            const double xm = om + de, xp = om - de;   // z - D and z + D without the i eta
+            const double dm = xm * xm + eta * eta, dp = xp * xp + eta * eta;
+            val = (iw & 1) ? kweight * df * (eta / dp - eta / dm) : kweight * df * (xm / dm - xp / dp);
+        }
     }
     w[(size_t)iw * ldw + p] = val;
 }

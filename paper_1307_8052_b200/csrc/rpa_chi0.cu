@@ -191,7 +191,9 @@ struct rpa_chi0 {
     cudaStream_t stream = nullptr;
     int32_t grid[3];
     double cell[9], B[9], q[3], vol, ecut;
-    int n_omega;
+    int n_omega;                       // accumulator slots: the frequencies, or 2 per frequency on the real axis
+    int n_freq;                        // frequencies the caller sees
+    double eta = -1.0;                 // > 0: real-axis handle, chi0 at omega + i eta (slot 2i: Re w, slot 2i+1: Im w)
     bool has_wt;
     std::vector<double> omega, wt;
     Sphere sp;
@@ -382,16 +384,25 @@ size_t rpa_chi0_workspace_bytes(const int32_t grid[3], const double cell[9], con
     return L.total;
 }
 
-int rpa_chi0_create(rpa_chi0_t **out, const int32_t grid[3], const double cell[9], const double q_red[3],
-                    double ecut_ha, int32_t n_omega, const double *omega_ha, const double *omega_wt,
-                    int32_t max_batch_pairs, int32_t max_proj_total, void *workspace, size_t workspace_bytes,
-                    void *cuda_stream) {
+}  // extern "C"
+
+namespace {
+// eta < 0: imaginary axis (n_freq slots); eta > 0: real axis (2 n_freq slots, omega of any sign)
+int create_impl(rpa_chi0_t **out, const int32_t grid[3], const double cell[9], const double q_red[3], double ecut_ha,
+                int32_t n_freq, const double *omega_ha, const double *omega_wt, double eta, int32_t max_batch_pairs,
+                int32_t max_proj_total, void *workspace, size_t workspace_bytes, void *cuda_stream) {
     if (!out) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_create: out is NULL");
     *out = nullptr;
-    if (!valid_dims(grid, cell, q_red, ecut_ha, n_omega) || !omega_ha || max_proj_total < 0 || max_proj_total > MAX_PROJ)
+    if (!valid_dims(grid, cell, q_red, ecut_ha, n_freq) || !omega_ha || max_proj_total < 0 || max_proj_total > MAX_PROJ ||
+        n_freq > (1 << 20))
         return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_create: invalid arguments");
-    for (int i = 0; i < n_omega; i++)
-        if (!(omega_ha[i] > 0.0)) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_create: omega[%d] must be > 0", i);
+    const bool real_axis = eta > 0.0;
+    for (int i = 0; i < n_freq; i++) {
+        if (real_axis ? !std::isfinite(omega_ha[i]) : !(omega_ha[i] > 0.0))
+            return fail(RPA_ERR_INVALID_ARG, real_axis ? "rpa_chi0_create_real_axis: omega[%d] must be finite"
+                                                       : "rpa_chi0_create: omega[%d] must be > 0", i);
+    }
+    const int n_omega = real_axis ? 2 * n_freq : n_freq;
     if (!workspace) return fail(RPA_ERR_WORKSPACE, "rpa_chi0_create: workspace is NULL");
     if (((uintptr_t)workspace & 255) != 0) return fail(RPA_ERR_WORKSPACE, "rpa_chi0_create: workspace not 256-byte aligned");
 
@@ -405,8 +416,11 @@ int rpa_chi0_create(rpa_chi0_t **out, const int32_t grid[3], const double cell[9
     recip_lattice(cell, h->B, &h->vol);
     if (!(h->vol > 0.0)) { delete h; return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_create: singular cell"); }
     h->n_omega = n_omega;
-    h->omega.assign(omega_ha, omega_ha + n_omega);
-    h->has_wt = omega_wt != nullptr;
+    h->n_freq = n_freq;
+    h->eta = real_axis ? eta : -1.0;
+    h->omega.resize(n_omega);
+    for (int i = 0; i < n_omega; i++) h->omega[i] = omega_ha[real_axis ? i / 2 : i];
+    h->has_wt = omega_wt != nullptr && !real_axis;
     if (h->has_wt) h->wt.assign(omega_wt, omega_wt + n_omega);
     else h->wt.assign(n_omega, 0.0);
     build_sphere(grid, h->B, q_red, ecut_ha, &h->sp);
@@ -511,6 +525,28 @@ int rpa_chi0_create(rpa_chi0_t **out, const int32_t grid[3], const double cell[9
 #undef CREATE_TRY
     *out = h;
     return RPA_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int rpa_chi0_create(rpa_chi0_t **out, const int32_t grid[3], const double cell[9], const double q_red[3],
+                    double ecut_ha, int32_t n_omega, const double *omega_ha, const double *omega_wt,
+                    int32_t max_batch_pairs, int32_t max_proj_total, void *workspace, size_t workspace_bytes,
+                    void *cuda_stream) {
+    return create_impl(out, grid, cell, q_red, ecut_ha, n_omega, omega_ha, omega_wt, -1.0, max_batch_pairs, max_proj_total,
+                       workspace, workspace_bytes, cuda_stream);
+}
+
+int rpa_chi0_create_real_axis(rpa_chi0_t **out, const int32_t grid[3], const double cell[9], const double q_red[3],
+                              double ecut_ha, int32_t n_omega, const double *omega_ha, double eta_ha,
+                              int32_t max_batch_pairs, int32_t max_proj_total, void *workspace, size_t workspace_bytes,
+                              void *cuda_stream) {
+    if (out) *out = nullptr;
+    if (!(eta_ha > 0.0) || !std::isfinite(eta_ha))
+        return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_create_real_axis: eta must be finite and > 0");
+    return create_impl(out, grid, cell, q_red, ecut_ha, n_omega, omega_ha, nullptr, eta_ha, max_batch_pairs, max_proj_total,
+                       workspace, workspace_bytes, cuda_stream);
 }
 
 int rpa_chi0_ng(const rpa_chi0_t *h, int32_t *ng) {
@@ -682,7 +718,7 @@ int add_kpoint_impl(rpa_chi0_t *h, double kweight, int32_t n_occ, const void *ps
             {
                 StageTimer tm(h, 3, 1);
                 weights_kernel<<<dim3((Kpad + 127) / 128, h->n_omega), 128, 0, st>>>(
-                    w, L.ldw, K, Kpad, h->ptr<double>(L.omega), h->n_omega, d_eo, d_fo, d_eu, d_fu, n0, mlen, m0, kweight);
+                    w, L.ldw, K, Kpad, h->ptr<double>(L.omega), h->n_omega, d_eo, d_fo, d_eu, d_fu, n0, mlen, m0, kweight, h->eta);
                 CUDA_TRY(cudaGetLastError());
             }
             // S6: rank-K update of every frequency
@@ -801,11 +837,17 @@ int rpa_momentum_pw(rpa_chi0_t *h, const double k_cart[3], int32_t n_pw, const i
 
 int rpa_chi0_get(rpa_chi0_t *h, int32_t i_omega, void *chi0_out) {
     if (!h || !chi0_out) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_get: NULL argument");
-    if (i_omega < 0 || i_omega >= h->n_omega) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_get: i_omega %d out of range", i_omega);
+    if (i_omega < 0 || i_omega >= h->n_freq) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_get: i_omega %d out of range", i_omega);
     const int ng = h->sp.ng;
     const int nt = (ng + 31) / 32;
-    chi0_get_kernel<<<dim3(nt, nt), dim3(32, 8), 0, h->stream>>>(h->ptr<cd>(h->L.S) + (size_t)i_omega * ng * h->L.ldS, h->L.ldS, ng,
-                                                                 h->spin_deg / h->vol, (cd *)chi0_out);
+    const size_t strideS = (size_t)ng * h->L.ldS;
+    if (h->eta > 0.0)
+        chi0_get_real_axis_kernel<<<dim3(nt, nt), dim3(32, 8), 0, h->stream>>>(
+            h->ptr<cd>(h->L.S) + (size_t)(2 * i_omega) * strideS, h->ptr<cd>(h->L.S) + (size_t)(2 * i_omega + 1) * strideS,
+            h->L.ldS, ng, h->spin_deg / h->vol, (cd *)chi0_out);
+    else
+        chi0_get_kernel<<<dim3(nt, nt), dim3(32, 8), 0, h->stream>>>(h->ptr<cd>(h->L.S) + (size_t)i_omega * strideS, h->L.ldS, ng,
+                                                                     h->spin_deg / h->vol, (cd *)chi0_out);
     h->launches += 1;
     CUDA_TRY(cudaGetLastError());
     return RPA_OK;
@@ -813,6 +855,7 @@ int rpa_chi0_get(rpa_chi0_t *h, int32_t i_omega, void *chi0_out) {
 
 int rpa_ec_q(rpa_chi0_t *h, const double *v_G, double *ec_ha, double *e_omega) {
     if (!h || !v_G || !ec_ha) return fail(RPA_ERR_INVALID_ARG, "rpa_ec_q: NULL argument");
+    if (h->eta > 0.0) return fail(RPA_ERR_UNSUPPORTED, "rpa_ec_q: Eq. 2 is an imaginary-axis integral; this is a real-axis handle");
     if (!h->has_wt) return fail(RPA_ERR_INVALID_ARG, "rpa_ec_q: omega_wt was NULL at create");
     const Layout &L = h->L;
     const int ng = h->sp.ng;

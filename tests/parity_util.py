@@ -35,11 +35,14 @@ def gpu_run(cfg, kds, use_paw=True, max_batch_pairs=0, want_ec=True, device="cud
     return chi, ec, g, K2
 
 
-def oracle_run(cfg, kds, use_paw=True, want_ec=True, g=None):
+def oracle_run(cfg, kds, use_paw=True, want_ec=True, g=None, omega=None, eta=None):
+    """omega / eta given: the real-axis route of the oracle (chi0 at omega + i eta, NEXT-4), no E_c."""
     import oracle
     from paper_1307_8052_b200 import workload as W
     om, wt = W.omega_grid(cfg.n_omega)
-    orc = oracle.Chi0Oracle(cfg.grid, cfg.cell, cfg.q_red, W.tuned_ecut(cfg), om, wt, g=g)
+    if eta is not None:
+        om, wt, want_ec = np.asarray(omega, dtype=np.float64), None, False
+    orc = oracle.Chi0Oracle(cfg.grid, cfg.cell, cfg.q_red, W.tuned_ecut(cfg), om, wt, g=g, eta=eta)
     Q = R = npj = None
     if use_paw and int(cfg.n_proj.sum()):
         if g is None:
