@@ -470,3 +470,31 @@ def add_kpoint_host(h: Handle, kd, n_proj=None, Q_dev=None, R_cart=None, pinned=
             free[b].record(main)
         side.wait_stream(main)   # the buffers may be released once the main stream has passed this point
     return nbytes
+
+
+def add_kpoint_host_pw(h: Handle, kweight, g_pw, C_occ, C_unocc, eps_occ, eps_unocc, f_occ, f_unocc, n_proj=None,
+                       P_occ=None, P_unocc=None, Q_dev=None, R_cart=None):
+    """The paper's own pipeline (Table 1 steps 3 and 5-11): the host holds the orbitals as plane-wave coefficients
+    C_*[bands][n_pw] (host tensors, ideally pinned; g_pw[n_pw][3] their integer wave vectors) -- about 1/20 of the
+    bytes of the grid orbitals -- the device expands them with rpa_pw_to_grid (Eq. 10) into buffers kept on the
+    handle and adds the k-point.  Returns the bytes copied host->device.  Marshalling only."""
+    torch = _torch()
+    dev = h.device
+    have_paw = n_proj is not None and len(n_proj) > 0
+    with torch.cuda.device(dev), torch.cuda.stream(h.stream):
+        t = lambda a: a if isinstance(a, torch.Tensor) else torch.from_numpy(np.ascontiguousarray(a))
+        C_o, C_u = t(C_occ).to(dev, non_blocking=True), t(C_unocc).to(dev, non_blocking=True)
+        nbytes = (C_o.numel() + C_u.numel()) * 16
+        P_o = P_u = None
+        if have_paw:
+            P_o, P_u = t(P_occ).to(dev, non_blocking=True), t(P_unocc).to(dev, non_blocking=True)
+            nbytes += (P_o.numel() + P_u.numel()) * 16
+        bufs = getattr(h, "_pw_bufs", None)
+        shape = (int(C_o.shape[0]), int(C_u.shape[0]))
+        if bufs is None or bufs[0] != shape:
+            bufs = h._pw_bufs = (shape, torch.empty((shape[0],) + h.grid, dtype=torch.complex128, device=dev),
+                                 torch.empty((shape[1],) + h.grid, dtype=torch.complex128, device=dev))
+        psi_o = rpa_pw_to_grid(h, g_pw, C_o, bufs[1])
+        psi_u = rpa_pw_to_grid(h, g_pw, C_u, bufs[2])
+        rpa_chi0_add_kpoint(h, kweight, psi_o, psi_u, eps_occ, eps_unocc, f_occ, f_unocc, n_proj, P_o, P_u, Q_dev, R_cart)
+    return nbytes

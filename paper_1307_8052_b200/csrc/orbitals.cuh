@@ -9,30 +9,6 @@
 #pragma once
 #include "fft.cuh"
 
-// T1[b][j1][c] = sum_q1i Cbox[q1i][c] exp(+2 pi i q1 j1 / N1); c = q2i nq3 + q3i a box column,
-// table[q1i ncol + c] = index of that plane wave in C (or -1).  grid (ceil(ncol/128), N1, bands), block 128.
-__global__ void __launch_bounds__(128) pw_xaxis_kernel(const cd *__restrict__ C, int n_pw, const int32_t *__restrict__ table,
-                                                      const cd *__restrict__ tw1, int N1, int q1min, int nq1, int ncol,
-                                                      cd *__restrict__ T1) {
-    const int c = blockIdx.x * blockDim.x + threadIdx.x;
-    if (c >= ncol) return;
-    const int j1 = blockIdx.y, b = blockIdx.z;
-    const cd *Cb = C + (size_t)b * n_pw;
-    cd acc = cmake(0.0, 0.0);
-    int t = (int)(((int64_t)q1min * j1) % N1);
-    if (t < 0) t += N1;
-    for (int q = 0; q < nq1; q++) {
-        const int idx = table[(size_t)q * ncol + c];
-        if (idx >= 0) {
-            const cd w = tw1[t];   // exp(-2 pi i t/N1); the inverse transform needs its conjugate
-            acc = cfma(cmake(w.x, -w.y), Cb[idx], acc);
-        }
-        t += j1;
-        if (t >= N1) t -= N1;
-    }
-    T1[((size_t)b * N1 + j1) * ncol + c] = acc;
-}
-
 // Input-pruned inverse transform of one line by the two-level split N = NA NB (the transpose of the forward
 // pair-density split): for the outputs j + NB s (s < NA) of one j < NB,
 //   Z[k1] = sum_{q in box, q = k1 mod NA} x[q] exp(+2 pi i q j / N),      u[j + NB s] = sum_k1 exp(+2 pi i k1 s / NA) Z[k1],
@@ -79,6 +55,31 @@ __device__ __forceinline__ void pw_expand_line(int N, int j, int qmin, int nq, c
 
 // radix of the register butterfly for an axis of length n (1: direct sum)
 static inline int pw_pick_na(int n) { return n % 12 == 0 ? 12 : n % 8 == 0 ? 8 : 1; }
+
+// x axis: T1[b][j1][c] = sum_q1i Cbox[q1i][c] exp(+2 pi i q1 j1 / N1); c = q2i nq3 + q3i a box column,
+// table[q1i ncol + c] = index of that plane wave in C (or -1: outside the coefficient sphere).  One thread = one
+// (column, j < N1/NA): nq1 twiddled terms and one radix-NA butterfly give its NA planes j + (N1/NA) s.
+// grid (ceil(ncol/128), N1/NA, bands), block 128; consecutive threads = consecutive columns (coalesced table reads
+// and T1 writes).
+template <int NA>
+__global__ void __launch_bounds__(128) pw_xaxis_kernel(const cd *__restrict__ C, int n_pw, const int32_t *__restrict__ table,
+                                                      const cd *__restrict__ tw1, int N1, int q1min, int nq1, int ncol,
+                                                      cd *__restrict__ T1) {
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= ncol) return;
+    const int j = blockIdx.y, b = blockIdx.z;
+    const cd *Cb = C + (size_t)b * n_pw;
+    cd *Tb = T1 + (size_t)b * N1 * ncol + c;
+    pw_expand_line<NA>(N1, j, q1min, nq1, tw1,
+                       [&](int qi) {
+                           const int idx = table[(size_t)qi * ncol + c];
+                           return idx >= 0 ? Cb[idx] : cmake(0.0, 0.0);
+                       },
+                       [&](int n, cd v) { Tb[(size_t)n * ncol] = v; });
+}
+
+typedef void (*PwXKernel)(const cd *, int, const int32_t *, const cd *, int, int, int, int, cd *);
+static inline PwXKernel pw_xaxis_pick(int na) { return na == 12 ? pw_xaxis_kernel<12> : na == 8 ? pw_xaxis_kernel<8> : pw_xaxis_kernel<1>; }
 
 // One CTA per (x-plane j1, band).  Shared memory (cd): tw2[N2] | tw3[N3] | P[nq2][nq3] | Y[N2][nq3].
 //   y: Y[.][q3i] from the box column P[.][q3i]   (task = (j < N2/NA2, q3i))

@@ -1051,7 +1051,8 @@ int rpa_pw_to_grid(rpa_chi0_t *h, int32_t n_bands, int32_t n_pw, const int32_t *
     const int chunk = (int)std::min<size_t>((size_t)n_bands, std::min<size_t>(65535, (scratch - table_bytes) / t1_band));
     for (int b0 = 0; b0 < n_bands; b0 += chunk) {
         const int nb = std::min(chunk, n_bands - b0);
-        pw_xaxis_kernel<<<dim3((unsigned)((ncol + 127) / 128), N1, nb), 128, 0, st>>>(
+        const int na1 = pw_pick_na(N1);
+        pw_xaxis_pick(na1)<<<dim3((unsigned)((ncol + 127) / 128), N1 / na1, nb), 128, 0, st>>>(
             (const cd *)C + (size_t)b0 * n_pw, n_pw, d_table, h->ptr<cd>(L.tw1), N1, qmin[0], (int)nq1, (int)ncol, T1);
         zy<<<dim3(N1, nb), 128, smem, st>>>(T1, h->ptr<cd>(L.tw2), h->ptr<cd>(L.tw3), N1, N2, N3, qmin[1], (int)nq2, qmin[2],
                                            (int)nq3, (cd *)psi_out + (size_t)b0 * N);

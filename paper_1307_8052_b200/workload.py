@@ -171,17 +171,37 @@ def orbital(cfg: Config, k: int, band: int, _cache={}) -> np.ndarray:
     return np.ascontiguousarray(u)
 
 
-def orbital_coefficients(cfg: Config, k: int, band: int):
+def orbital_coefficients(cfg: Config, k: int, band: int, _mask=None):
     """(g_pw[n_pw][3] int32, C[n_pw]): the plane-wave coefficients behind `orbital`, scaled so that sum |C|^2 = 1
     (Parseval: the grid orbital sum_Q C(Q) exp(2 pi i Q.j/N) is then grid-normalised).  Same random stream as
     `orbital`, so pw -> grid of these coefficients reproduces it to rounding."""
+    if _mask is None:   # (ok, decay[ok], g[ok]): the same for every band of a config
+        ok, decay = _coef_mask(cfg)
+        rng_ax = [np.fft.fftfreq(n, 1.0 / n).astype(np.int64) for n in cfg.grid]
+        g = np.stack(np.meshgrid(*rng_ax, indexing="ij"), axis=-1)
+        _mask = (ok, decay[ok], np.ascontiguousarray(g[ok].astype(np.int32)))
+    ok, dec, gsel = _mask
+    xi = _rng(cfg, _KIND_COEF, k, band).standard_normal((dec.size, 2))
+    C = (xi[:, 0] + 1j * xi[:, 1]) * dec
+    C *= 1.0 / np.sqrt(np.sum(np.abs(C) ** 2))
+    return gsel, np.ascontiguousarray(C)
+
+
+def kpoint_coefficients(cfg: Config, k: int, occ: Optional[Sequence[int]] = None,
+                        unocc: Optional[Sequence[int]] = None):
+    """(g_pw, C_occ[n_occ][n_pw], C_unocc[n_unocc][n_pw]): the plane-wave form of `kpoint`'s orbitals (same bands,
+    same random streams; all bands share one coefficient sphere)."""
+    occ = range(cfg.n_occ) if occ is None else occ
+    unocc = range(cfg.n_unocc) if unocc is None else unocc
     ok, decay = _coef_mask(cfg)
     rng_ax = [np.fft.fftfreq(n, 1.0 / n).astype(np.int64) for n in cfg.grid]
     g = np.stack(np.meshgrid(*rng_ax, indexing="ij"), axis=-1)
-    xi = _rng(cfg, _KIND_COEF, k, band).standard_normal((int(ok.sum()), 2))
-    C = (xi[:, 0] + 1j * xi[:, 1]) * decay[ok]
-    C *= 1.0 / np.sqrt(np.sum(np.abs(C) ** 2))
-    return np.ascontiguousarray(g[ok].astype(np.int32)), np.ascontiguousarray(C)
+    mask = (ok, decay[ok], np.ascontiguousarray(g[ok].astype(np.int32)))
+    out = []
+    for bands in ([int(b) for b in occ], [cfg.n_occ + int(b) for b in unocc]):
+        rows = [orbital_coefficients(cfg, k, b, mask)[1] for b in bands]
+        out.append(np.ascontiguousarray(np.stack(rows)) if rows else np.zeros((0, mask[1].size), dtype=np.complex128))
+    return mask[2], out[0], out[1]
 
 
 def eigenvalues(cfg: Config, k: int):

@@ -94,6 +94,37 @@ def test_chi0_from_plane_wave_coefficients_matches_grid_route():
         h.close()
 
 
+def test_add_kpoint_host_pw_pipeline_against_the_oracle():
+    """binding.add_kpoint_host_pw (upload coefficients, expand on the device, add) with PAW on, twice on one handle
+    (buffers reused), against the oracle run on the generator's grid orbitals, and E_c(q)."""
+    import torch
+    from paper_1307_8052_b200 import binding as B
+    from tests.parity_util import oracle_run
+    cfg = W.CONFIGS[0]
+    kd = W.kpoint(cfg, 0)
+    g_pw, Co, Cu = W.kpoint_coefficients(cfg, 0)
+    om, wt = W.omega_grid(cfg.n_omega)
+    h = B.rpa_chi0_create(cfg.grid, cfg.cell, cfg.q_red, W.tuned_ecut(cfg), om, wt, 0, int(cfg.n_proj.sum()), "cuda:0")
+    try:
+        g, K2 = B.rpa_chi0_gvectors(h)
+        Qd = torch.from_numpy(W.paw_Q(cfg, K2)).to("cuda:0")
+        pin = lambda a: torch.from_numpy(a).pin_memory()
+        Cop, Cup, Pop, Pup = pin(Co), pin(Cu), pin(kd.P_occ), pin(kd.P_unocc)
+        for _ in range(2):
+            B.rpa_chi0_reset(h)
+            nb = B.add_kpoint_host_pw(h, kd.kweight, g_pw, Cop, Cup, kd.eps_occ, kd.eps_unocc, kd.f_occ, kd.f_unocc,
+                                      cfg.n_proj, Pop, Pup, Qd, W.atom_positions(cfg))
+            assert nb == 16 * (Co.size + Cu.size + kd.P_occ.size + kd.P_unocc.size)
+            chi = np.stack([B.rpa_chi0_get(h, i).cpu().numpy() for i in range(cfg.n_omega)])
+            ec, _ = B.rpa_ec_q(h, W.coulomb(K2))
+    finally:
+        h.close()
+    chi_o, ec_o, _, _ = oracle_run(cfg, [kd], True)
+    for i in range(cfg.n_omega):
+        assert rel_fro(chi[i], chi_o[i]) <= 1e-10
+    assert abs(ec - ec_o[0]) <= 1e-9 * abs(ec_o[0])
+
+
 @pytest.mark.parametrize("M,tr", [(np.eye(3, dtype=int), True), (-np.eye(3, dtype=int), False),
                                   ([[0, -1, 0], [1, 0, 0], [0, 0, 1]], False), ([[0, 1, 0], [1, 0, 0], [0, 0, -1]], True)])
 def test_symmetry_remap_bit_exact(M, tr):
