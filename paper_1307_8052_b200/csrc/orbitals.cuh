@@ -118,6 +118,107 @@ __global__ void __launch_bounds__(128, 3) pw_zy_kernel(const cd *__restrict__ T1
     }
 }
 
+// Table-driven variant for NA2, NA3 in {8, 12} (all BASELINE.json grids): persistent CTAs loop over (band, x-plane)
+// items.  The twiddle of a term depends on (box position, j) only, so each CTA builds TWy[qi2][j < N2/NA2] and
+// TWz[qi3][j < N3/NA3] once; the box is embedded in zero-padded arrays aligned to the radix (position = q - q0,
+// q0 = qmin - (qmin mod NA)), so the inner loops have no bounds tests, no index updates and no conjugations: per term
+// two LDS.128 with immediate offsets and one complex FMA.  The inverse butterfly is the forward one read at -s.
+// Shared memory (cd): TWy[nq2p][NB2] | TWz[nq3p][NB3] | Pp[nq2p][nq3p] | Y[N2][nq3p].
+struct PwTabDims {
+    int r2, nq2p, r3, nq3p;
+    size_t smem;
+};
+static inline PwTabDims pw_tab_dims(int N2, int N3, int na2, int na3, int q2min, int nq2, int q3min, int nq3) {
+    PwTabDims d;
+    d.r2 = ((q2min % na2) + na2) % na2;
+    d.r3 = ((q3min % na3) + na3) % na3;
+    d.nq2p = (nq2 + d.r2 + na2 - 1) / na2 * na2;
+    d.nq3p = (nq3 + d.r3 + na3 - 1) / na3 * na3;
+    d.smem = ((size_t)d.nq2p * (N2 / na2) + (size_t)d.nq3p * (N3 / na3) + (size_t)d.nq2p * d.nq3p + (size_t)N2 * d.nq3p) * sizeof(cd);
+    return d;
+}
+
+template <int NA2, int NA3>
+__global__ void __launch_bounds__(128) pw_zy_tab_kernel(const cd *__restrict__ T1, const cd *__restrict__ tw2,
+                                                       const cd *__restrict__ tw3, int N1, int N2, int N3, int q2min, int nq2,
+                                                       int q3min, int nq3, int n_items, cd *__restrict__ out) {
+    extern __shared__ __align__(16) unsigned char pw_smem[];
+    const int NB2 = N2 / NA2, NB3 = N3 / NA3;
+    const int r2 = ((q2min % NA2) + NA2) % NA2, r3 = ((q3min % NA3) + NA3) % NA3;
+    const int nq2p = (nq2 + r2 + NA2 - 1) / NA2 * NA2, nq3p = (nq3 + r3 + NA3 - 1) / NA3 * NA3;
+    cd *TWy = reinterpret_cast<cd *>(pw_smem);
+    cd *TWz = TWy + nq2p * NB2;
+    cd *Pp = TWz + nq3p * NB3;
+    cd *Y = Pp + nq2p * nq3p;
+    const int tid = threadIdx.x, nth = blockDim.x;
+    for (int i = tid; i < nq2p * NB2; i += nth) {
+        const int qi = i / NB2, j = i - qi * NB2;
+        int t = (int)(((int64_t)(q2min - r2 + qi) * j) % N2);
+        if (t < 0) t += N2;
+        const cd w = tw2[t];                       // exp(-2 pi i t/N2): the inverse transform takes the conjugate
+        TWy[i] = cmake(w.x, -w.y);
+    }
+    for (int i = tid; i < nq3p * NB3; i += nth) {
+        const int qi = i / NB3, j = i - qi * NB3;
+        int t = (int)(((int64_t)(q3min - r3 + qi) * j) % N3);
+        if (t < 0) t += N3;
+        const cd w = tw3[t];
+        TWz[i] = cmake(w.x, -w.y);
+    }
+    for (int i = tid; i < nq2p * nq3p + N2 * nq3p; i += nth) Pp[i] = cmake(0.0, 0.0);   // Pp and Y: the padding stays zero
+    __syncthreads();
+    const int ncol = nq2 * nq3;
+    for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
+        const cd *Tp = T1 + (size_t)item * ncol;   // item = band * N1 + j1
+        for (int i = tid; i < ncol; i += nth) {
+            const int a = i / nq3, c = i - a * nq3;
+            Pp[(r2 + a) * nq3p + r3 + c] = Tp[i];
+        }
+        __syncthreads();   // Pp complete; every thread has left the z stage of the previous item
+        for (int i = tid; i < NB2 * nq3; i += nth) {
+            const int j = i / nq3, col = r3 + (i - j * nq3);
+            cd z[NA2];
+#pragma unroll
+            for (int k1 = 0; k1 < NA2; k1++) z[k1] = cmake(0.0, 0.0);
+            const cd *twp = TWy + j, *pp = Pp + col;
+            for (int base = 0; base < nq2p; base += NA2) {
+#pragma unroll
+                for (int k1 = 0; k1 < NA2; k1++) z[k1] = cfma(twp[(base + k1) * NB2], pp[(base + k1) * nq3p], z[k1]);
+            }
+            Bfly<NA2>::run(z);
+#pragma unroll
+            for (int s = 0; s < NA2; s++) Y[(j + NB2 * ((NA2 - s) % NA2)) * nq3p + col] = z[s];
+        }
+        __syncthreads();
+        cd *op = out + (size_t)item * N2 * N3;
+        for (int i = tid; i < N2 * NB3; i += nth) {
+            const int j2 = i / NB3, j = i - j2 * NB3;
+            cd z[NA3];
+#pragma unroll
+            for (int k1 = 0; k1 < NA3; k1++) z[k1] = cmake(0.0, 0.0);
+            const cd *twp = TWz + j, *yr = Y + (size_t)j2 * nq3p;
+            for (int base = 0; base < nq3p; base += NA3) {
+#pragma unroll
+                for (int k1 = 0; k1 < NA3; k1++) z[k1] = cfma(twp[(base + k1) * NB3], yr[base + k1], z[k1]);
+            }
+            Bfly<NA3>::run(z);
+            cd *orow = op + (size_t)j2 * N3 + j;
+#pragma unroll
+            for (int s = 0; s < NA3; s++) orow[NB3 * ((NA3 - s) % NA3)] = z[s];
+        }
+    }
+}
+
+typedef void (*PwZyTabKernel)(const cd *, const cd *, const cd *, int, int, int, int, int, int, int, int, cd *);
+static inline PwZyTabKernel pw_zy_tab_pick(int N2, int N3) {
+    const int a2 = pw_pick_na(N2), a3 = pw_pick_na(N3);
+    if (a2 == 12 && a3 == 12) return pw_zy_tab_kernel<12, 12>;
+    if (a2 == 12 && a3 == 8) return pw_zy_tab_kernel<12, 8>;
+    if (a2 == 8 && a3 == 12) return pw_zy_tab_kernel<8, 12>;
+    if (a2 == 8 && a3 == 8) return pw_zy_tab_kernel<8, 8>;
+    return nullptr;   // an axis without radix 8 or 12: pw_zy_kernel
+}
+
 typedef void (*PwZyKernel)(const cd *, const cd *, const cd *, int, int, int, int, int, int, int, cd *);
 static inline PwZyKernel pw_zy_pick(int N2, int N3) {
     const int a2 = pw_pick_na(N2), a3 = pw_pick_na(N3);

@@ -1048,14 +1048,36 @@ int rpa_pw_to_grid(rpa_chi0_t *h, int32_t n_bands, int32_t n_pw, const int32_t *
     CUDA_TRY(cudaStreamSynchronize(st));   // `table` is pageable host memory about to go out of scope
     const PwZyKernel zy = pw_zy_pick(N2, N3);
     if (smem > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(zy, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    // table-driven persistent kernel when both in-plane axes have a radix-8 / radix-12 split and its arrays fit
+    PwZyTabKernel zy_tab = pw_zy_tab_pick(N2, N3);
+    PwTabDims td{};
+    int tab_ctas = 0;
+    if (zy_tab) {
+        td = pw_tab_dims(N2, N3, pw_pick_na(N2), pw_pick_na(N3), qmin[1], (int)nq2, qmin[2], (int)nq3);
+        if (td.smem > 200 * 1024) {
+            zy_tab = nullptr;
+        } else {
+            if (td.smem > 48 * 1024)
+                CUDA_TRY(cudaFuncSetAttribute(zy_tab, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)td.smem));
+            CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&tab_ctas, zy_tab, 128, td.smem));
+            if (tab_ctas < 1) zy_tab = nullptr;
+        }
+    }
     const int chunk = (int)std::min<size_t>((size_t)n_bands, std::min<size_t>(65535, (scratch - table_bytes) / t1_band));
     for (int b0 = 0; b0 < n_bands; b0 += chunk) {
         const int nb = std::min(chunk, n_bands - b0);
         const int na1 = pw_pick_na(N1);
         pw_xaxis_pick(na1)<<<dim3((unsigned)((ncol + 127) / 128), N1 / na1, nb), 128, 0, st>>>(
             (const cd *)C + (size_t)b0 * n_pw, n_pw, d_table, h->ptr<cd>(L.tw1), N1, qmin[0], (int)nq1, (int)ncol, T1);
-        zy<<<dim3(N1, nb), 128, smem, st>>>(T1, h->ptr<cd>(L.tw2), h->ptr<cd>(L.tw3), N1, N2, N3, qmin[1], (int)nq2, qmin[2],
-                                           (int)nq3, (cd *)psi_out + (size_t)b0 * N);
+        if (zy_tab) {
+            const int n_items = nb * N1;
+            zy_tab<<<std::min(n_items, h->n_sm * tab_ctas), 128, td.smem, st>>>(
+                T1, h->ptr<cd>(L.tw2), h->ptr<cd>(L.tw3), N1, N2, N3, qmin[1], (int)nq2, qmin[2], (int)nq3, n_items,
+                (cd *)psi_out + (size_t)b0 * N);
+        } else {
+            zy<<<dim3(N1, nb), 128, smem, st>>>(T1, h->ptr<cd>(L.tw2), h->ptr<cd>(L.tw3), N1, N2, N3, qmin[1], (int)nq2, qmin[2],
+                                               (int)nq3, (cd *)psi_out + (size_t)b0 * N);
+        }
         h->launches += 2;
         CUDA_TRY(cudaGetLastError());
     }

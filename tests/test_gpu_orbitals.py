@@ -51,6 +51,32 @@ def test_pw_to_grid_toy_full_and_ragged_lists():
         h.close()
 
 
+@pytest.mark.parametrize("grid", [(12, 10, 14), (9, 15, 7), (8, 24, 40), (24, 36, 16), (5, 6, 1), (16, 48, 96)])
+def test_pw_to_grid_mixed_grids_all_points(grid):
+    """Every kernel variant: axes with a radix-12 / radix-8 split (table-driven persistent kernel, several items per
+    CTA) and axes without one (direct sums), boxes that start at every residue of the radix, 7 bands."""
+    import torch
+    from paper_1307_8052_b200 import binding as B
+    cell = np.array([[6.0, 0.2, 0.0], [0.1, 5.0, 0.3], [0.0, -0.2, 7.0]])
+    cfg = W.custom_config(300 + sum(grid), cell, grid, (0.25, 0.0, 0.0), n_occ=2, n_unocc=3, ng_target=4, n_omega=2,
+                          n_atoms=1, n_proj_per_atom=1, orb_ecut_ha=2.0)
+    rng = np.random.default_rng(sum(grid))
+    half = [max((n - 1) // 2, 0) for n in grid]
+    lo = [-rng.integers(0, hf + 1) for hf in half]           # asymmetric box: lower corner at a random residue
+    hi = [rng.integers(0, hf + 1) for hf in half]
+    allg = np.array([(a, b, c) for a in range(lo[0], hi[0] + 1) for b in range(lo[1], hi[1] + 1)
+                     for c in range(lo[2], hi[2] + 1)], dtype=np.int32)
+    g = allg[rng.permutation(len(allg))[:max(1, (2 * len(allg)) // 3)]]
+    C = rng.standard_normal((7, len(g))) + 1j * rng.standard_normal((7, len(g)))
+    h = _handle(cfg)
+    try:
+        u = B.rpa_pw_to_grid(h, g, torch.from_numpy(C).cuda()).cpu().numpy()
+    finally:
+        h.close()
+    want = oracle.pw_to_grid(cfg.grid, g, C).reshape(u.shape)
+    assert np.abs(u - want).max() <= 1e-12 * np.abs(want).max()
+
+
 def test_pw_to_grid_config1_full_size_sampled_points():
     """56x60x64 grid, ~9.4e3 plane waves (|G|^2/2 <= 6 Ha), 3 bands: the oracle sums at 400 sampled grid points
     (first / last point, plane and row boundaries, random rest); the generator's own orbital must also come out."""
