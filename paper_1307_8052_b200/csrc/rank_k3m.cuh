@@ -21,7 +21,11 @@ namespace rk3 {
 constexpr int T = 64;
 constexpr int KC = 32;                      // pairs per stage
 constexpr int STAGES = 3;
-constexpr int CONSUMER_WARPS = 8;
+#ifndef RK3_MI
+#define RK3_MI 4
+#endif
+constexpr int MI = RK3_MI;                  // 8-row blocks per warp: warp tile (8 MI) x 16
+constexpr int CONSUMER_WARPS = 4 * (T / (8 * MI));
 constexpr int THREADS = (CONSUMER_WARPS + 1) * 32;
 constexpr int PITCH = T * 16 + 32;          // bytes per pair row (= 32 mod 128)
 constexpr int TILE_BYTES = KC * PITCH;      // 16896
@@ -85,21 +89,21 @@ rank_k3m_kernel(const cd *__restrict__ Nb, int64_t ldn, int Kpad, const double *
     }
 
     const int g = lane >> 2, kq = lane & 3;
-    const int rowoff = (warp >> 2) * 32, coloff = (warp & 3) * 16;
+    const int rowoff = (warp >> 2) * (8 * MI), coloff = (warp & 3) * 16;
     // a warp whose sub-tile lies strictly above the diagonal, or wholly beyond the matrix edge (ragged last tile row /
     // column), only keeps the barriers moving: the warp sharing its scheduler then has the tensor pipe to itself
-    const bool active = !(ti == tj && coloff > rowoff + 31) && row0 + rowoff < ng && col0 + coloff < ng;
+    const bool active = !(ti == tj && coloff > rowoff + 8 * MI - 1) && row0 + rowoff < ng && col0 + coloff < ng;
 
-    double p1[4][2][2], p2[4][2][2], p3[4][2][2];
+    double p1[MI][2][2], p2[MI][2][2], p3[MI][2][2];
 #pragma unroll
-    for (int mi = 0; mi < 4; mi++)
+    for (int mi = 0; mi < MI; mi++)
 #pragma unroll
         for (int ni = 0; ni < 2; ni++)
 #pragma unroll
             for (int e = 0; e < 2; e++) p1[mi][ni][e] = p2[mi][ni][e] = p3[mi][ni][e] = 0.0;
 
     // 8-row blocks of this warp's sub-tile that hold matrix rows (ragged last tile row): the others are skipped
-    const int mi_valid = min(4, (ng - (row0 + rowoff) + 7) / 8);
+    const int mi_valid = min(MI, (ng - (row0 + rowoff) + 7) / 8);
     const uint32_t a_off = kq * PITCH + (rowoff + g) * 16;
     const uint32_t b_off = TILE_BYTES + kq * PITCH + (coloff + g) * 16;
     const uint32_t w_off = 2 * TILE_BYTES + kq * 8;
@@ -113,9 +117,9 @@ rank_k3m_kernel(const cd *__restrict__ Nb, int64_t ldn, int Kpad, const double *
             for (int ks = 0; ks < KC / 4; ks++) {
                 const uint32_t ko = ks * 4 * PITCH;
                 const double wv = *reinterpret_cast<const double *>(st + w_off + ks * 32);
-                double are[4], aim[4], asum[4], bre[2], bim[2], bdif[2];
+                double are[MI], aim[MI], asum[MI], bre[2], bim[2], bdif[2];
 #pragma unroll
-                for (int mi = 0; mi < 4; mi++) {
+                for (int mi = 0; mi < MI; mi++) {
                     const cd a = *reinterpret_cast<const cd *>(st + a_off + ko + mi * 128);
                     are[mi] = a.x;
                     aim[mi] = a.y;
@@ -129,7 +133,7 @@ rank_k3m_kernel(const cd *__restrict__ Nb, int64_t ldn, int Kpad, const double *
                     bdif[ni] = bre[ni] - bim[ni];
                 }
 #pragma unroll
-                for (int mi = 0; mi < 4; mi++) {
+                for (int mi = 0; mi < MI; mi++) {
                     if (mi < mi_valid) {   // warp-uniform
 #pragma unroll
                         for (int ni = 0; ni < 2; ni++) {
@@ -148,7 +152,7 @@ rank_k3m_kernel(const cd *__restrict__ Nb, int64_t ldn, int Kpad, const double *
     if (!active) return;
     cd *Sw = S + (size_t)iw * strideS;
 #pragma unroll
-    for (int mi = 0; mi < 4; mi++) {
+    for (int mi = 0; mi < MI; mi++) {
         const int r = row0 + rowoff + mi * 8 + g;
         if (r >= ng) continue;
 #pragma unroll
