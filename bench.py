@@ -32,9 +32,10 @@ from paper_1307_8052_b200 import workload as W  # noqa: E402
 
 METRIC = "chi0 pair transitions/s (rank-K FP64 TFLOP/s in roofline), 1 q-point, all omega"
 UNIT = "transitions/s"
-# ncu --set full capture of rank_k3m_kernel on configs[1] (profiles/r1e_bench_cfg1.md): dram__bytes_read.sum +
-# dram__bytes_write.sum per launch (3.025 GB + 184.5 MB, one launch of 7200 pairs); other configs have no capture
-RANK_K_DRAM_TRAFFIC_BYTES = {1: 3209.1e6}
+# ncu --set full capture of rank_k3m_kernel on configs[1] (profiles/r1g_bench_cfg1.md): dram__bytes_read.sum +
+# dram__bytes_write.sum of one batch of 7200 pairs = its two launches (whole waves 2.884 GB + 175.7 MB, K-sliced tail
+# 143.8 MB + 4.5 MB); other configs have no capture
+RANK_K_DRAM_TRAFFIC_BYTES = {1: 3208.2e6}
 
 def rank_k_useful_flops(ng, n_omega, n_pairs):
     """8 flop per complex MAC on one triangle: 4 nG (nG+1) n_omega per pair."""
@@ -307,7 +308,8 @@ def run_ours(args, cfg):
                          "peak_alt_tflops_from_bf16": peaks.get("bf16_tflops", 0) * 40.0 / 2250.0,
                          "note": "achieved = ALGORITHMIC flops (8 per complex multiply-add on one triangle) / time; the "
                                  "kernel forms the complex product with 3 real multiplications (3M), so it EXECUTES 3/4 of "
-                                 "them: executed_frac = tensor-pipe flops actually issued / peak",
+                                 "them: executed_frac = tensor-pipe flops actually issued / peak; one 'launch' here is the rank-K of one "
+                                 "batch of transitions = its whole-wave launch + the K-sliced launch of the last partial wave",
                          "executed_frac": 0.75 * rk_tf / peak_tf if peak_tf else None,
                          "flops_per_launch": rk_flops, "ms_per_launch": rk_ms, "launches": rk_launches,
                          "share_of_step": float(stage_ms[4]) / args.steps / ms_step},

@@ -157,7 +157,8 @@ int rpa_chi0_stage_times(rpa_chi0_t *h, double ms[5], int64_t launches[5]);
 int rpa_chi0_launch_count(const rpa_chi0_t *h, int64_t *count);
 
 /*
- * The raw accumulators S[n_omega][ng][ng] (dev cdouble, inside the caller's workspace; only the lower triangle
+ * The raw accumulators S[slots][ng][ldS] (dev cdouble, inside the caller's workspace; row pitch ldS >= ng; slots =
+ * n_omega, or 2 n_omega on a real-axis handle: Re-weight and Im-weight sums interleaved; only the lower triangle
  * g >= g' is meaningful, the rest is zero) and their size in bytes.  For the multi-GPU sum of per-rank partial
  * chi0 (ranks share nothing until the end of a q): all-reduce this buffer in place on the handle's
  * stream, then call rpa_chi0_get / rpa_ec_q.  The pointer stays valid for the life of the handle.
