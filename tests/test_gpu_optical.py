@@ -115,3 +115,39 @@ def test_optical_call_on_finite_q_handle_is_rejected():
         assert ei.value.code == B.RPA_ERR_INVALID_ARG
     finally:
         h.close()
+
+
+def test_real_axis_optical_limit():
+    """The two NEXT rows together (the macroscopic dielectric function's ingredient): a q = 0 real-axis handle, head from
+    the momentum matrix elements, chi0(omega + i eta) against the oracle's complex-weight route with the same head."""
+    import torch
+    from paper_1307_8052_b200 import binding as B
+    cfg = _q0_config(seed=91)
+    kd = W.kpoint(cfg, 0)
+    g, Co = _coeffs(cfg, range(cfg.n_occ))
+    _, Cu = _coeffs(cfg, range(cfg.n_occ, cfg.n_occ + cfg.n_unocc))
+    kc = np.array([0.0, 0.0, 0.0])
+    qdir = np.array([0.0, 0.0, 1.0])
+    Qg = _qgrad(cfg, seed=9)
+    om, eta = np.array([0.0, 0.4, 1.3]), 0.03
+    h = B.rpa_chi0_create_real_axis(cfg.grid, cfg.cell, cfg.q_red, W.tuned_ecut(cfg), om, eta, 0, int(cfg.n_proj.sum()), "cuda:0")
+    try:
+        gv, K2 = B.rpa_chi0_gvectors(h)
+        Qd = torch.from_numpy(W.paw_Q(cfg, K2)).cuda()
+        d = {k: torch.from_numpy(getattr(kd, k)).cuda() for k in ("psi_occ", "psi_unocc", "P_occ", "P_unocc")}
+        grad = B.rpa_momentum_pw(h, kc, g, torch.from_numpy(Co).cuda(), torch.from_numpy(Cu).cuda(), cfg.n_proj, d["P_occ"],
+                                 d["P_unocc"], torch.from_numpy(Qg).cuda())
+        B.rpa_chi0_add_kpoint_optical(h, kd.kweight, d["psi_occ"], d["psi_unocc"], kd.eps_occ, kd.eps_unocc, kd.f_occ,
+                                      kd.f_unocc, qdir, grad, cfg.n_proj, d["P_occ"], d["P_unocc"], Qd, W.atom_positions(cfg))
+        chi = np.stack([B.rpa_chi0_get(h, i).cpu().numpy() for i in range(len(om))])
+    finally:
+        h.close()
+    orc = oracle.Chi0Oracle(cfg.grid, cfg.cell, cfg.q_red, W.tuned_ecut(cfg), om, None, eta=eta)
+    gr = oracle.momentum_pw(cfg.cell, kc, g, Co, Cu, cfg.n_proj, kd.P_occ, kd.P_unocc, Qg)
+    head = oracle.optical_head(kd.eps_occ, kd.eps_unocc, qdir, gr)
+    orc.add_kpoint(kd, cfg.n_proj, W.paw_Q(cfg, orc.K2), W.atom_positions(cfg), head=head)
+    chi_o = orc.get()
+    i0 = int(np.flatnonzero((gv == 0).all(axis=1))[0])
+    for i in range(len(om)):
+        assert rel_fro(chi[i], chi_o[i]) <= 1e-10
+        assert abs(chi[i][i0, i0] - chi_o[i][i0, i0]) <= 1e-12 * abs(chi_o[i][i0, i0])
