@@ -201,16 +201,23 @@ def run_ours(args, cfg):
             else:
                 B.rpa_chi0_add_kpoint(h, kweight, devt["psi_occ"], devt["psi_unocc"], kd.eps_occ, kd.eps_unocc, kd.f_occ,
                                       kd.f_unocc, npj, devt["P_occ"], devt["P_unocc"], Qd, R)
-        if world > 1:
+        lo, hi = 0, cfg.n_omega
+        if world > 1 and args.exchange == "reduce_scatter":
+            lo, hi = sharding.reduce_scatter_accumulators(S, cfg.n_omega)   # this rank now owns frequencies [lo, hi)
+        elif world > 1:
             sharding.allreduce_accumulators(S)
         ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)] if tail_ms is not None else None
         if ev:
             ev[0].record()
-        for i in range(cfg.n_omega):
+        for i in range(lo, hi):
             B.rpa_chi0_get(h, i, out)
         if ev:
             ev[1].record()
-        ec, e = B.rpa_ec_q(h, v)  # blocks; reads E_c(q), e(omega) back to the host
+        if (lo, hi) == (0, cfg.n_omega):
+            ec, e = B.rpa_ec_q(h, v)  # blocks; reads E_c(q), e(omega) back to the host
+        else:
+            ec_part, e = B.rpa_ec_q_range(h, v, lo, hi)
+            ec = sharding.allreduce_scalar(ec_part, dev)
         if ev:
             ev[2].record()
             ev[2].synchronize()
@@ -291,7 +298,7 @@ def run_ours(args, cfg):
                        "l2": "inputs (%.2f GB of orbitals per k-point) exceed the 126 MB L2; no explicit flush" %
                              ((cfg.n_occ + cfg.n_unocc) * cfg.n_grid * 16 / 1e9),
                        "step": "reset + add_kpoint (S2-S6) + get x n_omega (S7) + ec_q (S8)",
-                       "parallelism": "1 GPU" if world == 1 else f"k-points sharded over {world} GPUs + all-reduce of S"},
+                       "parallelism": "1 GPU" if world == 1 else f"k-points sharded over {world} GPUs + {args.exchange} of S"},
             "clocks": clocks,
             "e2e": {"value": pairs_total / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e,
                     "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": 8 * (1 + cfg.n_omega) + 16},
@@ -343,6 +350,9 @@ def main():
     ap.add_argument("--batch", type=int, default=0, help="max_batch_pairs (0: library default)")
     ap.add_argument("--ref-seconds", type=float, default=12.0, help="CPU seconds of oracle work per sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--exchange", default="allreduce", choices=["allreduce", "reduce_scatter"],
+                    help="N > 1: all-reduce of S (every rank reads out and factorises all frequencies) or reduce-scatter "
+                         "by frequency (every rank reads out and factorises its own, scalar all-reduce of E_c)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
     cfg = W.CONFIGS[args.config]

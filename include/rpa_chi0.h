@@ -139,6 +139,17 @@ int rpa_chi0_get(rpa_chi0_t *h, int32_t i_omega, void *chi0_out);
  */
 int rpa_ec_q(rpa_chi0_t *h, const double *v_G, double *ec_ha, double *e_omega);
 
+/*
+ * The same for the frequencies iw_begin <= i < iw_end only (after a reduce-scatter of the accumulators by
+ * frequency every GPU factorises the frequencies it owns; the frequencies are independent terms of Eq. 2):
+ *   ec_partial_ha host double[1] = (1/2pi) sum_{i in range} wt_i e_i  -- the sum of the partial values over disjoint
+ *   ranges covering [0, n_omega) is E_c(q);  e_omega host double [iw_end - iw_begin] or NULL.
+ * Only the accumulators of the range are read, so the others may hold partial sums.  An empty range gives 0.
+ * RPA_ERR_INVALID_ARG if the range is not inside [0, n_omega); otherwise as rpa_ec_q.
+ */
+int rpa_ec_q_range(rpa_chi0_t *h, const double *v_G, int32_t iw_begin, int32_t iw_end, double *ec_partial_ha,
+                   double *e_omega);
+
 /* Zero the accumulators (start another q with the same sphere). */
 int rpa_chi0_reset(rpa_chi0_t *h);
 

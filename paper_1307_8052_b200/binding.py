@@ -26,7 +26,7 @@ EXPORTS = (
     "rpa_chi0_get", "rpa_ec_q", "rpa_chi0_reset", "rpa_chi0_sync", "rpa_chi0_set_profiling", "rpa_chi0_stage_times",
     "rpa_chi0_launch_count", "rpa_chi0_accumulators", "rpa_chi0_destroy", "rpa_probe_fp64_tensor_peak", "rpa_last_error",
     "rpa_pw_to_grid", "rpa_symmetry_remap", "rpa_momentum_pw", "rpa_chi0_add_kpoint_optical",
-    "rpa_chi0_set_spin_degeneracy", "rpa_chi0_create_real_axis",
+    "rpa_chi0_set_spin_degeneracy", "rpa_chi0_create_real_axis", "rpa_ec_q_range",
 )
 
 STAGE_NAMES = ("pair_product_fft_yz", "fft_x_gather", "paw", "weights", "rank_k")
@@ -74,6 +74,8 @@ def lib():
     L.rpa_chi0_get.argtypes = [vp, i32, vp]
     L.rpa_ec_q.restype = C.c_int
     L.rpa_ec_q.argtypes = [vp, vp, C.POINTER(f64), vp]
+    L.rpa_ec_q_range.restype = C.c_int
+    L.rpa_ec_q_range.argtypes = [vp, vp, i32, i32, C.POINTER(f64), vp]
     for name in ("rpa_chi0_reset", "rpa_chi0_sync"):
         getattr(L, name).restype = C.c_int
         getattr(L, name).argtypes = [vp]
@@ -293,6 +295,18 @@ def rpa_ec_q(h: Handle, v_G):
     ec = C.c_double(0.0)
     e = np.zeros(h.n_omega, dtype=np.float64)
     _check(lib().rpa_ec_q(h.ptr, _hp(v), C.byref(ec), _hp(e)))
+    return float(ec.value), e
+
+
+def rpa_ec_q_range(h: Handle, v_G, iw_begin: int, iw_end: int):
+    """(partial E_c(q) of the frequencies [iw_begin, iw_end), their e(omega)); the partial values of disjoint ranges
+    covering all frequencies add up to E_c(q)."""
+    v = _np(v_G, np.float64)
+    if v.size != h.ng:
+        raise ValueError("v_G must have ng entries")
+    ec = C.c_double(0.0)
+    e = np.zeros(max(0, int(iw_end) - int(iw_begin)), dtype=np.float64)
+    _check(lib().rpa_ec_q_range(h.ptr, _hp(v), int(iw_begin), int(iw_end), C.byref(ec), _hp(e) if e.size else None))
     return float(ec.value), e
 
 

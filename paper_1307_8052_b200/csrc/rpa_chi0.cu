@@ -853,10 +853,16 @@ int rpa_chi0_get(rpa_chi0_t *h, int32_t i_omega, void *chi0_out) {
     return RPA_OK;
 }
 
-int rpa_ec_q(rpa_chi0_t *h, const double *v_G, double *ec_ha, double *e_omega) {
+}  // extern "C"
+
+namespace {
+// e(omega_i) for i in [iw_begin, iw_end) and ec = (1/2pi) sum over that range of wt_i e_i
+int ec_q_impl(rpa_chi0_t *h, const double *v_G, int iw_begin, int iw_end, double *ec_ha, double *e_omega) {
     if (!h || !v_G || !ec_ha) return fail(RPA_ERR_INVALID_ARG, "rpa_ec_q: NULL argument");
     if (h->eta > 0.0) return fail(RPA_ERR_UNSUPPORTED, "rpa_ec_q: Eq. 2 is an imaginary-axis integral; this is a real-axis handle");
     if (!h->has_wt) return fail(RPA_ERR_INVALID_ARG, "rpa_ec_q: omega_wt was NULL at create");
+    if (iw_begin < 0 || iw_end > h->n_omega || iw_begin > iw_end)
+        return fail(RPA_ERR_INVALID_ARG, "rpa_ec_q_range: frequency range [%d, %d) outside [0, %d)", iw_begin, iw_end, h->n_omega);
     const Layout &L = h->L;
     const int ng = h->sp.ng;
     for (int i = 0; i < ng; i++)
@@ -869,8 +875,8 @@ int rpa_ec_q(rpa_chi0_t *h, const double *v_G, double *ec_ha, double *e_omega) {
     const int64_t strideS = (int64_t)ng * L.ldS;
     const double scale = h->spin_deg / h->vol;
     CUDA_TRY(cudaMemcpyAsync(d_v, v_G, ng * sizeof(double), cudaMemcpyHostToDevice, st));
-    for (int iw0 = 0; iw0 < h->n_omega; iw0 += L.ec_group) {
-        const int nm = std::min(L.ec_group, h->n_omega - iw0);
+    for (int iw0 = iw_begin; iw0 < iw_end; iw0 += L.ec_group) {
+        const int nm = std::min(L.ec_group, iw_end - iw0);
         CUDA_TRY(cudaMemsetAsync(d_ld, 0, EC_GROUP * sizeof(double), st));
         CUDA_TRY(cudaMemsetAsync(d_flag, 0, EC_GROUP * sizeof(int), st));
         ec_build_kernel<<<dim3((ng + 127) / 128, ng, nm), 128, 0, st>>>(S + (size_t)iw0 * strideS, L.ldS, strideS, ng, scale, d_v, M);
@@ -934,13 +940,25 @@ int rpa_ec_q(rpa_chi0_t *h, const double *v_G, double *ec_ha, double *e_omega) {
         for (int i = 0; i < nm; i++)
             if (flags[i]) return fail(RPA_ERR_NOT_PD, "rpa_ec_q: I - v^1/2 chi0 v^1/2 not positive definite at omega index %d", iw0 + i);
     }
-    ec_sum_kernel<<<1, 32, 0, st>>>(d_e, h->ptr<double>(L.wt), h->n_omega, h->ptr<double>(L.ec));
+    ec_sum_kernel<<<1, 32, 0, st>>>(d_e + iw_begin, h->ptr<double>(L.wt) + iw_begin, iw_end - iw_begin, h->ptr<double>(L.ec));
     h->launches += 1;
     CUDA_TRY(cudaGetLastError());
     CUDA_TRY(cudaMemcpyAsync(ec_ha, h->ptr<double>(L.ec), sizeof(double), cudaMemcpyDeviceToHost, st));
-    if (e_omega) CUDA_TRY(cudaMemcpyAsync(e_omega, d_e, h->n_omega * sizeof(double), cudaMemcpyDeviceToHost, st));
+    if (e_omega && iw_end > iw_begin)
+        CUDA_TRY(cudaMemcpyAsync(e_omega, d_e + iw_begin, (iw_end - iw_begin) * sizeof(double), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaStreamSynchronize(st));
     return RPA_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int rpa_ec_q(rpa_chi0_t *h, const double *v_G, double *ec_ha, double *e_omega) {
+    return ec_q_impl(h, v_G, 0, h ? h->n_omega : 0, ec_ha, e_omega);
+}
+
+int rpa_ec_q_range(rpa_chi0_t *h, const double *v_G, int32_t iw_begin, int32_t iw_end, double *ec_partial_ha, double *e_omega) {
+    return ec_q_impl(h, v_G, iw_begin, iw_end, ec_partial_ha, e_omega);
 }
 
 int rpa_chi0_reset(rpa_chi0_t *h) {

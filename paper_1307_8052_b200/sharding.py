@@ -4,7 +4,8 @@ Transitions are independent ("no MPI communication required during the cal
 one q-point is split into units (k-point, block of occupied bands); every rank accumulates its units into private
 accumulators S and the only exchange is one sum of S over ranks at the end of the q-point (NCCL all-reduce over
 NVLink on GPUs; gloo in the CPU tests).  After the sum every rank holds the full S, so rpa_chi0_get / rpa_ec_q can
-run anywhere (rpa_ec_q's frequencies could also be split, E_c(q) being a plain sum over frequencies).
+run anywhere.  The alternative exchange: reduce-scatter S by frequency, every rank factorises the
+frequencies it owns (rpa_ec_q_range) and one scalar all-reduce completes E_c(q), a plain sum over frequencies.
 """
 from __future__ import annotations
 
@@ -41,3 +42,41 @@ def allreduce_accumulators(S, group=None):
         return S
     dist.all_reduce(torch.view_as_real(S), op=dist.ReduceOp.SUM, group=group)
     return S
+
+
+def omega_range(n_omega: int, rank: int, world: int) -> Tuple[int, int]:
+    """Contiguous, nearly equal frequency ranges [lo, hi) that partition [0, n_omega); empty when world > n_omega."""
+    if world < 1 or not (0 <= rank < world) or n_omega < 0:
+        raise ValueError("bad rank / world / n_omega")
+    base, rem = divmod(n_omega, world)
+    lo = rank * base + min(rank, rem)
+    return lo, lo + base + (1 if rank < rem else 0)
+
+
+def reduce_scatter_accumulators(S, n_omega: int, group=None) -> Tuple[int, int]:
+    """Sum over ranks of the accumulators S (complex128, n_omega equal contiguous slots), each rank receiving only the
+    slots of its own `omega_range`; the other slots are left with partial sums.  One reduce per owner: works for any
+    n_omega / world with both NCCL and gloo.  Returns this rank's (lo, hi)."""
+    import torch
+    import torch.distributed as dist
+    if not dist.is_initialized() or dist.get_world_size(group) == 1:
+        return 0, n_omega
+    world, rank = dist.get_world_size(group), dist.get_rank(group)
+    flat = torch.view_as_real(S).reshape(n_omega, -1)
+    for owner in range(world):
+        lo, hi = omega_range(n_omega, owner, world)
+        if hi > lo:
+            dist.reduce(flat[lo:hi], dst=dist.get_global_rank(group, owner) if group is not None else owner,
+                        op=dist.ReduceOp.SUM, group=group)
+    return omega_range(n_omega, rank, world)
+
+
+def allreduce_scalar(x: float, device=None, group=None) -> float:
+    """Sum of one double over ranks (the partial E_c(q) of every rank's frequencies)."""
+    import torch
+    import torch.distributed as dist
+    if not dist.is_initialized() or dist.get_world_size(group) == 1:
+        return float(x)
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.SUM, group=group)
+    return float(t.item())

@@ -162,3 +162,42 @@ def test_spin_degeneracy_setter():
     ec_o, _ = orc.ec_q(W.coulomb(orc.K2))
     assert abs(ec1 - ec_o) <= 1e-9 * abs(ec_o)
     assert abs(B.rpa_total_energy([ec1, 2 * ec1], [0.25, 0.75]) - 1.75 * ec1) <= 1e-15 * abs(ec1)
+
+
+def test_ec_q_range_partial_sums_and_isolation():
+    """rpa_ec_q_range (reduce-scatter exchange): partial values over disjoint ranges add up to rpa_ec_q,
+    e(omega) agrees value by value, a range reads only its own accumulators (the others are poisoned with NaN, as
+    they would hold partial sums after a reduce-scatter), invalid ranges are rejected, an empty range gives 0."""
+    import torch
+    from paper_1307_8052_b200 import binding as B
+    from paper_1307_8052_b200 import sharding
+    cfg = W.CONFIGS[0]
+    h = _handle(cfg)
+    try:
+        kd = W.kpoint(cfg, 0)
+        g, K2 = B.rpa_chi0_gvectors(h)
+        Qd = torch.from_numpy(W.paw_Q(cfg, K2)).to("cuda:0")
+        B.add_kpoint_host(h, kd, cfg.n_proj, Qd, W.atom_positions(cfg))
+        v = W.coulomb(K2)
+        ec, e = B.rpa_ec_q(h, v)
+        for world in (2, 3, cfg.n_omega + 2):
+            parts = [B.rpa_ec_q_range(h, v, *sharding.omega_range(cfg.n_omega, r, world)) for r in range(world)]
+            assert abs(sum(p[0] for p in parts) - ec) <= 1e-13 * abs(ec)
+            assert np.array_equal(np.concatenate([p[1] for p in parts]), e)
+        assert B.rpa_ec_q_range(h, v, 3, 3) == (0.0, pytest.approx(np.zeros(0)))
+        for lo, hi in ((-1, 2), (0, cfg.n_omega + 1), (5, 4)):
+            with pytest.raises(B.RpaError) as ei:
+                B.rpa_ec_q_range(h, v, lo, hi)
+            assert ei.value.code == B.RPA_ERR_INVALID_ARG
+        S = B.rpa_chi0_accumulators(h).view(cfg.n_omega, -1)
+        lo, hi = 2, 5
+        keep = S[lo:hi].clone()
+        S.fill_(complex(float("nan"), float("nan")))
+        S[lo:hi] = keep
+        torch.cuda.synchronize()
+        ec_p, e_p = B.rpa_ec_q_range(h, v, lo, hi)
+        assert np.array_equal(e_p, e[lo:hi])
+        om, wt = W.omega_grid(cfg.n_omega)
+        assert abs(ec_p - float(np.dot(wt[lo:hi], e[lo:hi])) / (2 * np.pi)) <= 1e-14 * abs(ec)
+    finally:
+        h.close()
