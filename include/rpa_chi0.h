@@ -243,6 +243,13 @@ void rpa_chi0_destroy(rpa_chi0_t *h);
  * call that allocates (and frees) 64 bytes of device memory itself: it has no handle and no workspace. */
 int rpa_probe_fp64_tensor_peak(void *cuda_stream, double *tflops);
 
+/* tcgen05 int8 issue-rate probe (the denominator of the planned int8-sliced rank-K update): on every SM
+ * one thread issues 20000 accumulating tcgen05.mma.kind::i8 of 128 x 256 x 32 (operands in shared memory, s32
+ * accumulator in TMEM); returns the achieved int8 Top/s in *tops.  The first MMA of CTA 0 is read back from TMEM and
+ * compared with the host product of the same seeded operands: *mismatches = number of wrong elements of 32768 (0 on a
+ * working path).  Allocates and frees 140 KB of device memory itself; blocks. */
+int rpa_probe_int8_tensor_peak(void *cuda_stream, double *tops, int32_t *mismatches);
+
 /* Thread-local message of the last error on this thread (static storage, never NULL). */
 const char *rpa_last_error(void);
 

@@ -27,6 +27,7 @@ EXPORTS = (
     "rpa_chi0_launch_count", "rpa_chi0_accumulators", "rpa_chi0_destroy", "rpa_probe_fp64_tensor_peak", "rpa_last_error",
     "rpa_pw_to_grid", "rpa_symmetry_remap", "rpa_momentum_pw", "rpa_chi0_add_kpoint_optical",
     "rpa_chi0_set_spin_degeneracy", "rpa_chi0_create_real_axis", "rpa_ec_q_range",
+    "rpa_probe_int8_tensor_peak",
 )
 
 STAGE_NAMES = ("pair_product_fft_yz", "fft_x_gather", "paw", "weights", "rank_k")
@@ -91,6 +92,8 @@ def lib():
     L.rpa_chi0_destroy.argtypes = [vp]
     L.rpa_probe_fp64_tensor_peak.restype = C.c_int
     L.rpa_probe_fp64_tensor_peak.argtypes = [vp, C.POINTER(f64)]
+    L.rpa_probe_int8_tensor_peak.restype = C.c_int
+    L.rpa_probe_int8_tensor_peak.argtypes = [vp, C.POINTER(f64), C.POINTER(i32)]
     L.rpa_pw_to_grid.restype = C.c_int
     L.rpa_pw_to_grid.argtypes = [vp, i32, i32, vp, vp, vp]
     L.rpa_symmetry_remap.restype = C.c_int
@@ -425,6 +428,15 @@ def rpa_probe_fp64_tensor_peak(device="cuda:0") -> float:
         t = C.c_double(0.0)
         _check(lib().rpa_probe_fp64_tensor_peak(C.c_void_p(torch.cuda.current_stream().cuda_stream), C.byref(t)))
     return float(t.value)
+
+
+def rpa_probe_int8_tensor_peak(device="cuda:0"):
+    """(int8 tcgen05 Top/s, mismatches of the self-checked first MMA)."""
+    torch = _torch()
+    with torch.cuda.device(torch.device(device)):
+        t, bad = C.c_double(0.0), C.c_int32(-1)
+        _check(lib().rpa_probe_int8_tensor_peak(C.c_void_p(torch.cuda.current_stream().cuda_stream), C.byref(t), C.byref(bad)))
+    return float(t.value), int(bad.value)
 
 
 # ---- host-buffer convenience on top of the calls above (the end-to-end path bench.py times) ------------------

@@ -23,6 +23,7 @@
 #include "paw.cuh"
 #include "rank_k.cuh"
 #include "rank_k3m.cuh"
+#include "probe_i8.cuh"
 
 namespace {
 
@@ -1175,6 +1176,62 @@ int rpa_probe_fp64_tensor_peak(void *cuda_stream, double *tflops) {
     cudaEventDestroy(e1);
     cudaFree(buf);
     *tflops = best;
+    return RPA_OK;
+}
+
+int rpa_probe_int8_tensor_peak(void *cuda_stream, double *tops, int32_t *mismatches) {
+    if (!tops || !mismatches) return fail(RPA_ERR_INVALID_ARG, "rpa_probe_int8_tensor_peak: NULL argument");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, nsm = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    CUDA_TRY(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+    std::vector<int8_t> A(I8_M * I8_K), B(I8_N * I8_K);
+    uint32_t x = 12345u;   // small LCG: values in [-64, 63]
+    for (auto *v : {&A, &B})
+        for (auto &e : *v) { x = x * 1664525u + 1013904223u; e = (int8_t)((int)((x >> 24) & 127) - 64); }
+    unsigned char *buf = nullptr;   // like the FP64 probe: no handle, no workspace, allocates and frees its own scratch
+    const size_t nD = (size_t)I8_M * I8_N * sizeof(int32_t);
+    CUDA_TRY(cudaMalloc(&buf, A.size() + B.size() + nD));
+    int8_t *dA = (int8_t *)buf, *dB = dA + A.size();
+    int32_t *dD = (int32_t *)(buf + A.size() + B.size());
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    int rc = RPA_OK;
+    double best = 0.0;
+    std::vector<int32_t> D((size_t)I8_M * I8_N);
+    do {
+#define PROBE_TRY(expr) if ((expr) != cudaSuccess) { rc = fail(RPA_ERR_CUDA, "rpa_probe_int8_tensor_peak: %s", cudaGetErrorString(cudaGetLastError())); break; }
+        PROBE_TRY(cudaMemcpyAsync(dA, A.data(), A.size(), cudaMemcpyHostToDevice, st));
+        PROBE_TRY(cudaMemcpyAsync(dB, B.data(), B.size(), cudaMemcpyHostToDevice, st));
+        PROBE_TRY(cudaMemsetAsync(dD, 0xff, nD, st));
+        PROBE_TRY(cudaEventCreate(&e0));
+        PROBE_TRY(cudaEventCreate(&e1));
+        i8_probe_kernel<<<nsm, 128, 0, st>>>(dA, dB, dD, 100);
+        PROBE_TRY(cudaMemcpyAsync(D.data(), dD, nD, cudaMemcpyDeviceToHost, st));
+        const int iters = 20000;
+        for (int rep = 0; rep < 3 && rc == RPA_OK; rep++) {
+            PROBE_TRY(cudaEventRecord(e0, st));
+            i8_probe_kernel<<<nsm, 128, 0, st>>>(dA, dB, dD, iters);
+            PROBE_TRY(cudaEventRecord(e1, st));
+            PROBE_TRY(cudaEventSynchronize(e1));
+            float ms = 0.f;
+            PROBE_TRY(cudaEventElapsedTime(&ms, e0, e1));
+            best = std::max(best, (double)nsm * (iters + 1.0) * 2.0 * I8_M * I8_N * I8_K / (ms * 1e-3) * 1e-12);
+        }
+#undef PROBE_TRY
+    } while (0);
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    cudaFree(buf);
+    if (rc != RPA_OK) return rc;
+    int bad = 0;
+    for (int i = 0; i < I8_M; i++)
+        for (int j = 0; j < I8_N; j++) {
+            int32_t sum = 0;
+            for (int k = 0; k < I8_K; k++) sum += (int32_t)A[i * I8_K + k] * (int32_t)B[j * I8_K + k];
+            bad += sum != D[(size_t)i * I8_N + j];
+        }
+    *mismatches = bad;
+    *tops = best;
     return RPA_OK;
 }
 

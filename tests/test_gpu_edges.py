@@ -201,3 +201,12 @@ def test_ec_q_range_partial_sums_and_isolation():
         assert abs(ec_p - float(np.dot(wt[lo:hi], e[lo:hi])) / (2 * np.pi)) <= 1e-14 * abs(ec)
     finally:
         h.close()
+
+
+def test_int8_tcgen05_probe_self_check():
+    """rpa_probe_int8_tensor_peak: the TMEM read-back of one tcgen05.mma.kind::i8 equals the host product bit for bit,
+    and the issue rate is in the range of a Blackwell int8 tensor pipe (legacy mma.sync reaches 1.1 Pop/s)."""
+    from paper_1307_8052_b200 import binding as B
+    tops, bad = B.rpa_probe_int8_tensor_peak("cuda:0")
+    assert bad == 0
+    assert 2000.0 < tops < 6000.0
