@@ -8,7 +8,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "librpa_chi0.so")
 SOURCES = ["rpa_chi0.cu"]
-HEADERS = ["common.cuh", "fft.cuh", "pair_density.cuh", "pair_density_zy.cuh", "orbitals.cuh", "optical.cuh", "paw.cuh", "rank_k.cuh", "rank_k3m.cuh", "energy.cuh", "probe_i8.cuh",
+HEADERS = ["common.cuh", "fft.cuh", "pair_density.cuh", "pair_density_zy.cuh", "orbitals.cuh", "optical.cuh", "paw.cuh", "rank_k.cuh", "rank_k3m.cuh", "energy.cuh", "probe_i8.cuh", "rank_k_i8.cuh",
            os.path.join("..", "..", "include", "rpa_chi0.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC",
               "-shared", "-Xptxas", "-v", "-diag-suppress", "20011,20013,20014,20015"]

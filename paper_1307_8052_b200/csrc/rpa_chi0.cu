@@ -24,6 +24,7 @@
 #include "rank_k.cuh"
 #include "rank_k3m.cuh"
 #include "probe_i8.cuh"
+#include "rank_k_i8.cuh"
 
 namespace {
 
@@ -209,6 +210,8 @@ struct rpa_chi0 {
     double spin_deg = 2.0;             // prefactor s of chi0 = (s/Omega) S: 2 spin-paired (A3), 1 per explicit spin channel
     bool q0 = false;                   // q = 0: pair densities need the optical-limit head (rpa_chi0_add_kpoint_optical)
     int idx0 = -1;                     // sphere index of G = 0 when q0
+    bool use_i8 = false;               // RPA_RANK_K_I8: int8-sliced rank-K on tcgen05 (rank_k_i8.cuh)
+    std::vector<int2> i8_tiles;        // (row block, column block) tiles that meet the lower triangle
     bool use_3m = true;                // rank_k3m_kernel (3-multiplication complex product) for the chi0 accumulation
     cudaStream_t side = nullptr;       // panel factorisations of rpa_ec_q run here, ahead of the trailing updates
     cudaEvent_t ev_panel[2] = {nullptr, nullptr}, ev_col = nullptr, ev_fork = nullptr;
@@ -487,6 +490,17 @@ int create_impl(rpa_chi0_t **out, const int32_t grid[3], const double cell[9], c
     CREATE_TRY(cudaFuncSetAttribute(rank_k_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, rk::Cfg<true>::SMEM_BYTES));
     CREATE_TRY(cudaFuncSetAttribute(rank_k3m_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, rk3::SMEM_BYTES));
     h->use_3m = getenv("RPA_RANK_K_4M") == nullptr;
+    h->use_i8 = getenv("RPA_RANK_K_I8") != nullptr;
+    if (h->use_i8) {
+        const int ng_ = h->sp.ng, ngp = (ng_ + rki8::RB - 1) / rki8::RB * rki8::RB;
+        for (int rb = 0; rb < 2 * ngp / rki8::RB; rb++) {
+            const int g_lo = (rb * rki8::RB) % ngp, g_hi = std::min(g_lo + rki8::RB - 1, ng_ - 1);
+            if (g_lo >= ng_) continue;
+            for (int cb = 0; cb * rki8::CB <= g_hi; cb++) h->i8_tiles.push_back(make_int2(rb, cb));
+        }
+        if (cudaFuncSetAttribute(rank_k_i8_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, rki8::SMEM_BYTES) != cudaSuccess)
+            h->use_i8 = false;
+    }
     CREATE_TRY(cudaFuncSetAttribute(rank_k_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, rk::Cfg<false>::SMEM_BYTES));
 
     // tables: twiddles in extended precision, box -> sphere map
@@ -725,7 +739,49 @@ int add_kpoint_impl(rpa_chi0_t *h, double kweight, int32_t n_occ, const void *ps
             // S6: rank-K update of every frequency
             {
                 StageTimer tm(h, 4, 1);
-                if (h->use_3m) {
+                bool done_i8 = false;
+                if (h->use_i8) {
+                    // scratch (the pair-density buffer I is free again): invL | invR | tiles | PL | PR of a frequency group
+                    const int ngp = (ng + rki8::RB - 1) / rki8::RB * rki8::RB, nrb = 2 * ngp / rki8::RB;
+                    const int ncb = (ng + rki8::CB - 1) / rki8::CB, nkb = 2 * Kpad / rki8::KB, nt = (int)h->i8_tiles.size();
+                    const size_t scratch = (size_t)L.sub_pairs * L.I_pair_bytes;
+                    size_t off = 0;
+                    auto carve = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
+                    const size_t o_invL = carve((size_t)(1 + h->n_omega) * ngp * 8), o_invR = o_invL + (size_t)ngp * 8;
+                    const size_t o_tiles = carve((size_t)nt * sizeof(int2));
+                    const size_t o_PL = carve((size_t)nrb * nkb * rki8::S * rki8::A_BYTES);
+                    const size_t per_w = (size_t)ncb * nkb * rki8::S * rki8::B_BYTES;
+                    int wg = off < scratch ? (int)std::min<size_t>((size_t)h->n_omega, (scratch - off) / per_w) : 0;
+                    if (wg >= 1 && h->n_omega <= RKI8_MAXW) {
+                        const int ngroups = (h->n_omega + wg - 1) / wg;
+                        wg = (h->n_omega + ngroups - 1) / ngroups;   // equal groups
+                        unsigned char *base = h->ws + L.I;
+                        double *invL = (double *)(base + o_invL), *invR = (double *)(base + o_invR);
+                        int2 *d_tiles = (int2 *)(base + o_tiles);
+                        int8_t *PL = (int8_t *)(base + o_PL), *PR = (int8_t *)(base + off);
+                        CUDA_TRY(cudaMemcpyAsync(d_tiles, h->i8_tiles.data(), (size_t)nt * sizeof(int2), cudaMemcpyHostToDevice, st));
+                        const int nmx = (1 + h->n_omega) * ngp;
+                        CUDA_TRY(cudaMemsetAsync(invL, 0, (size_t)nmx * 8, st));
+                        rki8_rowmax_kernel<<<dim3((ng + 127) / 128, std::max(1, std::min(64, K / 64))), 128, 0, st>>>(
+                            Nbuf, L.ldn, K, ng, w, L.ldw, h->n_omega, ngp, (unsigned long long *)invL);
+                        rki8_scale_finish_kernel<<<(nmx + 255) / 256, 256, 0, st>>>((unsigned long long *)invL, nmx);
+                        rki8_pack_left_kernel<<<dim3(nkb, nrb), 128, 0, st>>>(Nbuf, L.ldn, Kpad, ng, ngp, invL, PL);
+                        h->launches += 3;
+                        for (int iw0 = 0; iw0 < h->n_omega; iw0 += wg) {
+                            const int nw = std::min(wg, h->n_omega - iw0);
+                            rki8_pack_right_kernel<<<dim3(nkb, ncb, nw), 64, 0, st>>>(Nbuf, L.ldn, Kpad, ng, ngp, w + (size_t)iw0 * L.ldw, L.ldw,
+                                                                                     invR + (size_t)iw0 * ngp, PR);
+                            rank_k_i8_kernel<<<dim3(nt, nw), rki8::THREADS, rki8::SMEM_BYTES, st>>>(
+                                PL, PR, nkb, ncb, d_tiles, invL, invR + (size_t)iw0 * ngp, ng, ngp,
+                                h->ptr<cd>(L.S) + (size_t)iw0 * ng * L.ldS, L.ldS, (int64_t)ng * L.ldS);
+                            h->launches += 2;
+                        }
+                        h->launches -= 1;   // the stage timer counts one
+                        done_i8 = true;
+                    }
+                }
+                if (done_i8) {
+                } else if (h->use_3m) {
                     // whole waves (one CTA per SM) with full K, then the last partial wave K-sliced so that it fills the GPU too
                     const int ntiles = ntiles_lower(ng, rk3::T), units = ntiles * h->n_omega, nchunks = Kpad / rk3::KC;
                     const int whole = units / h->n_sm * h->n_sm;
