@@ -159,10 +159,11 @@ int rpa_chi0_sync(rpa_chi0_t *h);
 /*
  * Per-stage device times (ms, CUDA events on the handle's stream) accumulated by rpa_chi0_add_kpoint while
  * profiling is on: [0] pair product + 2-D FFT, [1] third-axis DFT + sphere gather, [2] PAW, [3] weights,
- * [4] rank-K update; launches[5] = kernel launches per stage.  Turning profiling on adds event records only.
+ * [4] rank-K update (all its kernels), [5] the rank_k_i8_kernel launches alone (part of [4]; 0 when the FP64 tensor
+ * kernel ran); launches[6] = kernel launches per stage.  Turning profiling on adds event records only.
  */
 int rpa_chi0_set_profiling(rpa_chi0_t *h, int32_t on);
-int rpa_chi0_stage_times(rpa_chi0_t *h, double ms[5], int64_t launches[5]);
+int rpa_chi0_stage_times(rpa_chi0_t *h, double ms[6], int64_t launches[6]);
 
 /* Number of kernel launches enqueued through this handle since it was created. */
 int rpa_chi0_launch_count(const rpa_chi0_t *h, int64_t *count);

@@ -30,7 +30,7 @@ EXPORTS = (
     "rpa_probe_int8_tensor_peak",
 )
 
-STAGE_NAMES = ("pair_product_fft_yz", "fft_x_gather", "paw", "weights", "rank_k")
+STAGE_NAMES = ("pair_product_fft_yz", "fft_x_gather", "paw", "weights", "rank_k", "rank_k_i8_mma")
 
 
 class RpaError(RuntimeError):
@@ -339,8 +339,8 @@ def rpa_chi0_set_profiling(h: Handle, on: bool):
 
 
 def rpa_chi0_stage_times(h: Handle):
-    ms = np.zeros(5, dtype=np.float64)
-    n = np.zeros(5, dtype=np.int64)
+    ms = np.zeros(6, dtype=np.float64)
+    n = np.zeros(6, dtype=np.int64)
     _check(lib().rpa_chi0_stage_times(h.ptr, _hp(ms), _hp(n)))
     return ms, n
 

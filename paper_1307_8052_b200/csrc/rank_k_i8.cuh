@@ -19,13 +19,14 @@
 #include "probe_i8.cuh"
 
 namespace rki8 {
-constexpr int S = 6;                 // digits per operand: 6 + 7 (S - 1) = 41 bits
+// S = digits per operand: 6 + 7 (S - 1) bits.  S = 7 (48 bits): the result agrees with the FP64 tensor path to FP64
+// rounding (~1e-14 relative Frobenius); S = 6 (41 bits): ~3e-12, 3/4 of the MMAs.
 constexpr int RB = 128, CB = 64;     // rows / columns of a CTA tile
 constexpr int KB = 32;               // K' entries (bytes) per MMA
 constexpr int A_BYTES = RB * KB, B_BYTES = CB * KB;
-constexpr int STAGE_BYTES = S * (A_BYTES + B_BYTES);   // 36864
 constexpr int STAGES = 4;
-constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 128;
+__host__ __device__ constexpr int stage_bytes(int S) { return S * (A_BYTES + B_BYTES); }   // 36864 (S = 6), 43008 (S = 7)
+__host__ __device__ constexpr int smem_bytes(int S) { return STAGES * stage_bytes(S) + 128; }
 constexpr int THREADS = 192;         // warps 0-3: epilogue (TMEM lanes), warp 4: producer, warp 5: MMA issue
 constexpr uint32_t IDESC = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(CB >> 3) << 17) | ((uint32_t)(RB >> 4) << 24);
 }  // namespace rki8
@@ -69,29 +70,31 @@ __global__ void rki8_scale_finish_kernel(unsigned long long *__restrict__ mx, in
 }
 
 // 16 values x (|x| < 1) -> S x 16 digit bytes, written as one 16-byte store per digit plane
+template <int S>
 __device__ __forceinline__ void rki8_store_digits(const double (&x)[16], int8_t *dst, int plane_stride) {
-    uint32_t pk[rki8::S][4];
+    uint32_t pk[S][4];
 #pragma unroll
-    for (int i = 0; i < rki8::S; i++)
+    for (int i = 0; i < S; i++)
 #pragma unroll
         for (int q = 0; q < 4; q++) pk[i][q] = 0u;
 #pragma unroll
     for (int k = 0; k < 16; k++) {
         double y = x[k] * 64.0;
 #pragma unroll
-        for (int i = 0; i < rki8::S; i++) {
+        for (int i = 0; i < S; i++) {
             const double r = rint(y);
             pk[i][k >> 2] |= ((uint32_t)(int)r & 0xffu) << (8 * (k & 3));
             y = (y - r) * 128.0;
         }
     }
 #pragma unroll
-    for (int i = 0; i < rki8::S; i++)
+    for (int i = 0; i < S; i++)
         *reinterpret_cast<uint4 *>(dst + (size_t)i * plane_stride) = make_uint4(pk[i][0], pk[i][1], pk[i][2], pk[i][3]);
 }
 
 // PL[rb][kb][digit][4096]: left rows R = rb 128 + r: half = R / ngp (0: [a | b], 1: [b | -a]), g = R % ngp (zero rows for
 // g >= ng); K' column k' = kb 32 + kk: part = k' / Kpad, pair p = k' % Kpad.  grid (nkb, nrb), block 128.
+template <int S>
 __global__ void __launch_bounds__(128) rki8_pack_left_kernel(const cd *__restrict__ Nb, int64_t ldn, int Kpad, int ng, int ngp,
                                                             const double *__restrict__ invL, int8_t *__restrict__ PL) {
     const int kb = blockIdx.x, rb = blockIdx.y, r = threadIdx.x, nkb = gridDim.x;
@@ -102,7 +105,7 @@ __global__ void __launch_bounds__(128) rki8_pack_left_kernel(const cd *__restric
     // component: (half, part) = (0,0) a, (0,1) b, (1,0) b, (1,1) -a
     const bool take_im = (half ^ part) != 0;
     const double sgn = (half == 1 && part == 1) ? -sc : sc;
-    int8_t *dst = PL + ((size_t)(rb * nkb + kb) * rki8::S) * rki8::A_BYTES + (r % 8) * 16 + (r / 8) * 256;
+    int8_t *dst = PL + ((size_t)(rb * nkb + kb) * S) * rki8::A_BYTES + (r % 8) * 16 + (r / 8) * 256;
 #pragma unroll
     for (int c = 0; c < 2; c++) {
         double x[16];
@@ -115,11 +118,12 @@ __global__ void __launch_bounds__(128) rki8_pack_left_kernel(const cd *__restric
             }
             x[k] = v * sgn;
         }
-        rki8_store_digits(x, dst + c * 128, rki8::A_BYTES);
+        rki8_store_digits<S>(x, dst + c * 128, rki8::A_BYTES);
     }
 }
 
 // PR[iw][cb][kb][digit][2048]: rows g' = cb 64 + r, value w[iw][p] (a | b) 2^-eR.  grid (nkb, ncb, n_w), block 64.
+template <int S>
 __global__ void __launch_bounds__(64) rki8_pack_right_kernel(const cd *__restrict__ Nb, int64_t ldn, int Kpad, int ng, int ngp,
                                                             const double *__restrict__ w, int64_t ldw,
                                                             const double *__restrict__ invR, int8_t *__restrict__ PR) {
@@ -129,7 +133,7 @@ __global__ void __launch_bounds__(64) rki8_pack_right_kernel(const cd *__restric
     const bool valid = g < ng;
     const double sc = valid ? invR[(size_t)iw * ngp + g] : 0.0;
     const double *wr = w + (size_t)iw * ldw;
-    int8_t *dst = PR + (((size_t)iw * ncb + cb) * nkb + kb) * rki8::S * rki8::B_BYTES + (r % 8) * 16 + (r / 8) * 256;
+    int8_t *dst = PR + (((size_t)iw * ncb + cb) * nkb + kb) * S * rki8::B_BYTES + (r % 8) * 16 + (r / 8) * 256;
 #pragma unroll
     for (int c = 0; c < 2; c++) {
         double x[16];
@@ -143,17 +147,20 @@ __global__ void __launch_bounds__(64) rki8_pack_right_kernel(const cd *__restric
             }
             x[k] = v * sc;
         }
-        rki8_store_digits(x, dst + c * 128, rki8::B_BYTES);
+        rki8_store_digits<S>(x, dst + c * 128, rki8::B_BYTES);
     }
 }
 
 // One CTA = tile (rb, cb) of one frequency: tiles[] lists the tiles that meet the lower triangle.
-// grid (n_tiles, n_w), block 192, dynamic shared memory rki8::SMEM_BYTES.
+// grid (n_tiles, n_w), block 192, dynamic shared memory rki8::smem_bytes(S).
+template <int S>
 __global__ void __launch_bounds__(rki8::THREADS, 1)
 rank_k_i8_kernel(const int8_t *__restrict__ PL, const int8_t *__restrict__ PR, int nkb, int ncb, const int2 *__restrict__ tiles,
                  const double *__restrict__ invL, const double *__restrict__ invR, int ng, int ngp, cd *__restrict__ Sacc,
                  int64_t ldS, int64_t strideS) {
     using namespace rki8;
+    constexpr int STAGE_BYTES = stage_bytes(S);
+    static_assert(S * CB <= 512, "one TMEM accumulator of CB columns per digit level");
     extern __shared__ __align__(128) unsigned char i8_smem[];
     uint64_t *full = reinterpret_cast<uint64_t *>(i8_smem + STAGES * STAGE_BYTES);
     uint64_t *empty = full + STAGES;

@@ -45,13 +45,14 @@ int fail(int code, const char *fmt, ...) {
     } while (0)
 
 constexpr int DEFAULT_BATCH = 8192;
-constexpr int MAX_SLOTS = 16;          // occupied bands per batch
+constexpr int MAX_SLOTS = 16;
+constexpr int I8_MIN_NG = 768, I8_MIN_K = 1024;   // below: the FP64 tensor kernel is faster (measured: nG = 401, K = 2400 loses)          // occupied bands per batch
 constexpr int MAX_BANDS = 1 << 17;     // eps/f scratch
 constexpr int MAX_ATOMS = 4096;
 constexpr int MAX_PROJ = 1 << 16;
 constexpr int EC_GROUP = 16;           // frequencies factorised together in rpa_ec_q
 constexpr size_t I_BUDGET = (size_t)4 << 30; // pruned intermediate of a whole batch when it fits (fewer, larger launches beat L2 residency)
-constexpr int NSTAGE = 5;
+constexpr int NSTAGE = 6;
 constexpr int K_ALIGN = 32;            // pairs per batch are padded to the chunk size of both rank-K kernels (16, 32)
 static_assert(K_ALIGN % rk::KC == 0 && K_ALIGN % rk3::KC == 0, "batch padding");
 
@@ -211,6 +212,8 @@ struct rpa_chi0 {
     bool q0 = false;                   // q = 0: pair densities need the optical-limit head (rpa_chi0_add_kpoint_optical)
     int idx0 = -1;                     // sphere index of G = 0 when q0
     bool use_i8 = false;               // RPA_RANK_K_I8: int8-sliced rank-K on tcgen05 (rank_k_i8.cuh)
+    int i8_digits = 7;
+    bool i8_force = false;             // RPA_RANK_K_I8=1: also for small batches (tests)
     std::vector<int2> i8_tiles;        // (row block, column block) tiles that meet the lower triangle
     bool use_3m = true;                // rank_k3m_kernel (3-multiplication complex product) for the chi0 accumulation
     cudaStream_t side = nullptr;       // panel factorisations of rpa_ec_q run here, ahead of the trailing updates
@@ -221,8 +224,8 @@ struct rpa_chi0 {
     bool prof = false;
     std::vector<StageEvent> events;
     std::vector<cudaEvent_t> pool;
-    double stage_ms[NSTAGE] = {0, 0, 0, 0, 0};
-    int64_t stage_launches[NSTAGE] = {0, 0, 0, 0, 0};
+    double stage_ms[NSTAGE] = {0, 0, 0, 0, 0, 0};
+    int64_t stage_launches[NSTAGE] = {0, 0, 0, 0, 0, 0};
     int64_t launches = 0;  // every kernel launch enqueued through this handle
 
     template <class T>
@@ -490,7 +493,9 @@ int create_impl(rpa_chi0_t **out, const int32_t grid[3], const double cell[9], c
     CREATE_TRY(cudaFuncSetAttribute(rank_k_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, rk::Cfg<true>::SMEM_BYTES));
     CREATE_TRY(cudaFuncSetAttribute(rank_k3m_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, rk3::SMEM_BYTES));
     h->use_3m = getenv("RPA_RANK_K_4M") == nullptr;
-    h->use_i8 = getenv("RPA_RANK_K_I8") != nullptr;
+    // int8-sliced rank-K (rank_k_i8.cuh) unless RPA_RANK_K_FP64 / RPA_RANK_K_4M ask for the FP64 tensor kernels; batches
+    // too small to pay for the slicing passes take the FP64 kernel anyway (I8_MIN_NG, I8_MIN_K below)
+    h->use_i8 = getenv("RPA_RANK_K_FP64") == nullptr && getenv("RPA_RANK_K_4M") == nullptr;
     if (h->use_i8) {
         const int ng_ = h->sp.ng, ngp = (ng_ + rki8::RB - 1) / rki8::RB * rki8::RB;
         for (int rb = 0; rb < 2 * ngp / rki8::RB; rb++) {
@@ -498,7 +503,11 @@ int create_impl(rpa_chi0_t **out, const int32_t grid[3], const double cell[9], c
             if (g_lo >= ng_) continue;
             for (int cb = 0; cb * rki8::CB <= g_hi; cb++) h->i8_tiles.push_back(make_int2(rb, cb));
         }
-        if (cudaFuncSetAttribute(rank_k_i8_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, rki8::SMEM_BYTES) != cudaSuccess)
+        h->i8_force = getenv("RPA_RANK_K_I8") != nullptr;
+        const char *dg = getenv("RPA_RANK_K_I8_DIGITS");
+        h->i8_digits = (dg && atoi(dg) == 6) ? 6 : 7;
+        if (cudaFuncSetAttribute(rank_k_i8_kernel<6>, cudaFuncAttributeMaxDynamicSharedMemorySize, rki8::smem_bytes(6)) != cudaSuccess ||
+            cudaFuncSetAttribute(rank_k_i8_kernel<7>, cudaFuncAttributeMaxDynamicSharedMemorySize, rki8::smem_bytes(7)) != cudaSuccess)
             h->use_i8 = false;
     }
     CREATE_TRY(cudaFuncSetAttribute(rank_k_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, rk::Cfg<false>::SMEM_BYTES));
@@ -740,7 +749,7 @@ int add_kpoint_impl(rpa_chi0_t *h, double kweight, int32_t n_occ, const void *ps
             {
                 StageTimer tm(h, 4, 1);
                 bool done_i8 = false;
-                if (h->use_i8) {
+                if (h->use_i8 && (h->i8_force || (ng >= I8_MIN_NG && K >= I8_MIN_K))) {
                     // scratch (the pair-density buffer I is free again): invL | invR | tiles | PL | PR of a frequency group
                     const int ngp = (ng + rki8::RB - 1) / rki8::RB * rki8::RB, nrb = 2 * ngp / rki8::RB;
                     const int ncb = (ng + rki8::CB - 1) / rki8::CB, nkb = 2 * Kpad / rki8::KB, nt = (int)h->i8_tiles.size();
@@ -749,8 +758,9 @@ int add_kpoint_impl(rpa_chi0_t *h, double kweight, int32_t n_occ, const void *ps
                     auto carve = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
                     const size_t o_invL = carve((size_t)(1 + h->n_omega) * ngp * 8), o_invR = o_invL + (size_t)ngp * 8;
                     const size_t o_tiles = carve((size_t)nt * sizeof(int2));
-                    const size_t o_PL = carve((size_t)nrb * nkb * rki8::S * rki8::A_BYTES);
-                    const size_t per_w = (size_t)ncb * nkb * rki8::S * rki8::B_BYTES;
+                    const int SD = h->i8_digits;
+                    const size_t o_PL = carve((size_t)nrb * nkb * SD * rki8::A_BYTES);
+                    const size_t per_w = (size_t)ncb * nkb * SD * rki8::B_BYTES;
                     int wg = off < scratch ? (int)std::min<size_t>((size_t)h->n_omega, (scratch - off) / per_w) : 0;
                     if (wg >= 1 && h->n_omega <= RKI8_MAXW) {
                         const int ngroups = (h->n_omega + wg - 1) / wg;
@@ -765,16 +775,25 @@ int add_kpoint_impl(rpa_chi0_t *h, double kweight, int32_t n_occ, const void *ps
                         rki8_rowmax_kernel<<<dim3((ng + 127) / 128, std::max(1, std::min(64, K / 64))), 128, 0, st>>>(
                             Nbuf, L.ldn, K, ng, w, L.ldw, h->n_omega, ngp, (unsigned long long *)invL);
                         rki8_scale_finish_kernel<<<(nmx + 255) / 256, 256, 0, st>>>((unsigned long long *)invL, nmx);
-                        rki8_pack_left_kernel<<<dim3(nkb, nrb), 128, 0, st>>>(Nbuf, L.ldn, Kpad, ng, ngp, invL, PL);
+                        if (SD == 6) rki8_pack_left_kernel<6><<<dim3(nkb, nrb), 128, 0, st>>>(Nbuf, L.ldn, Kpad, ng, ngp, invL, PL);
+                        else rki8_pack_left_kernel<7><<<dim3(nkb, nrb), 128, 0, st>>>(Nbuf, L.ldn, Kpad, ng, ngp, invL, PL);
                         h->launches += 3;
                         for (int iw0 = 0; iw0 < h->n_omega; iw0 += wg) {
                             const int nw = std::min(wg, h->n_omega - iw0);
-                            rki8_pack_right_kernel<<<dim3(nkb, ncb, nw), 64, 0, st>>>(Nbuf, L.ldn, Kpad, ng, ngp, w + (size_t)iw0 * L.ldw, L.ldw,
-                                                                                     invR + (size_t)iw0 * ngp, PR);
-                            rank_k_i8_kernel<<<dim3(nt, nw), rki8::THREADS, rki8::SMEM_BYTES, st>>>(
-                                PL, PR, nkb, ncb, d_tiles, invL, invR + (size_t)iw0 * ngp, ng, ngp,
-                                h->ptr<cd>(L.S) + (size_t)iw0 * ng * L.ldS, L.ldS, (int64_t)ng * L.ldS);
-                            h->launches += 2;
+                            const double *w0 = w + (size_t)iw0 * L.ldw, *invR0 = invR + (size_t)iw0 * ngp;
+                            cd *S0 = h->ptr<cd>(L.S) + (size_t)iw0 * ng * L.ldS;
+                            if (SD == 6) {
+                                rki8_pack_right_kernel<6><<<dim3(nkb, ncb, nw), 64, 0, st>>>(Nbuf, L.ldn, Kpad, ng, ngp, w0, L.ldw, invR0, PR);
+                                StageTimer tm5(h, 5, 1);
+                                rank_k_i8_kernel<6><<<dim3(nt, nw), rki8::THREADS, rki8::smem_bytes(6), st>>>(
+                                    PL, PR, nkb, ncb, d_tiles, invL, invR0, ng, ngp, S0, L.ldS, (int64_t)ng * L.ldS);
+                            } else {
+                                rki8_pack_right_kernel<7><<<dim3(nkb, ncb, nw), 64, 0, st>>>(Nbuf, L.ldn, Kpad, ng, ngp, w0, L.ldw, invR0, PR);
+                                StageTimer tm5(h, 5, 1);
+                                rank_k_i8_kernel<7><<<dim3(nt, nw), rki8::THREADS, rki8::smem_bytes(7), st>>>(
+                                    PL, PR, nkb, ncb, d_tiles, invL, invR0, ng, ngp, S0, L.ldS, (int64_t)ng * L.ldS);
+                            }
+                            h->launches += 1;
                         }
                         h->launches -= 1;   // the stage timer counts one
                         done_i8 = true;
