@@ -36,6 +36,8 @@ UNIT = "transitions/s"
 # dram__bytes_write.sum of one batch of 7200 pairs = its two launches (whole waves 2.884 GB + 175.7 MB, K-sliced tail
 # 143.8 MB + 4.5 MB); other configs have no capture
 RANK_K_DRAM_TRAFFIC_BYTES = {1: 3208.2e6}
+# the same for rank_k_i8_kernel (profiles/r1h_bench_cfg1.md): DRAM bytes of one launch (a group of frequencies)
+RANK_K_I8_DRAM_TRAFFIC_BYTES = {}
 
 def rank_k_useful_flops(ng, n_omega, n_pairs):
     """8 flop per complex MAC on one triangle: 4 nG (nG+1) n_omega per pair."""
@@ -283,6 +285,42 @@ def run_ours(args, cfg):
         rk_ms = float(stage_ms[4]) / max(rk_launches, 1)
         rk_flops = rank_k_useful_flops(ng, cfg.n_omega, pairs_per_rank * args.steps) / max(rk_launches, 1)
         rk_tf = rk_flops / (rk_ms * 1e-3) * 1e-12 if rk_ms > 0 else 0.0
+        roofline = {"kernel": "rank_k3m_kernel", "bound": "tensor", "achieved": rk_tf, "peak": peak_tf, "unit": "TFLOP/s",
+                         "frac": rk_tf / peak_tf if peak_tf else None, "traffic": RANK_K_DRAM_TRAFFIC_BYTES.get(cfg.index),
+                         "peak_source": "FP64 DMMA issue rate measured live by rpa_probe_fp64_tensor_peak (register-only "
+                                        "mma.sync.m8n8k4.f64, all SMs); MEASURED_PEAKS.json has no FP64 entry",
+                         "peak_alt_tflops_from_bf16": peaks.get("bf16_tflops", 0) * 40.0 / 2250.0,
+                         "note": "achieved = ALGORITHMIC flops (8 per complex multiply-add on one triangle) / time; the "
+                                 "kernel forms the complex product with 3 real multiplications (3M), so it EXECUTES 3/4 of "
+                                 "them: executed_frac = tensor-pipe flops actually issued / peak; one 'launch' here is the rank-K of one "
+                                 "batch of transitions = its whole-wave launch + the K-sliced launch of the last partial wave",
+                         "executed_frac": 0.75 * rk_tf / peak_tf if peak_tf else None,
+                         "flops_per_launch": rk_flops, "ms_per_launch": rk_ms, "launches": rk_launches,
+                         "share_of_step": float(stage_ms[4]) / args.steps / ms_step}
+        if int(stage_n[5]) > 0:
+            # the int8-sliced kernel ran (rank_k_i8.cuh): its own launches are stage 5, the slicing passes the rest of stage 4
+            digits = 6 if os.environ.get("RPA_RANK_K_I8_DIGITS") == "6" else 7
+            i8_peak, i8_bad = B.rpa_probe_int8_tensor_peak(dev)
+            i8_launches = int(stage_n[5])
+            i8_ms = float(stage_ms[5]) / i8_launches
+            # algorithmic int8 operations: digit pairs i + j < digits, both halves (Re, Im) of the lower triangle, K' = 2K
+            i8_ops = (digits * (digits + 1) // 2) * 2.0 * cfg.n_omega * ng * (ng + 1) * 2.0 * pairs_per_rank * args.steps / i8_launches
+            i8_tops = i8_ops / (i8_ms * 1e-3) * 1e-12
+            roofline = {"kernel": "rank_k_i8_kernel", "bound": "tensor", "achieved": i8_tops, "peak": i8_peak, "unit": "Top/s",
+                        "frac": i8_tops / i8_peak if i8_peak else None, "traffic": RANK_K_I8_DRAM_TRAFFIC_BYTES.get(cfg.index),
+                        "peak_source": "int8 tcgen05 issue rate measured live by rpa_probe_int8_tensor_peak (128x256x32 "
+                                       "tcgen05.mma.kind::i8 from one thread per SM; self-check mismatches: %d); "
+                                       "MEASURED_PEAKS.json has no int8 entry" % i8_bad,
+                        "note": "the rank-K update runs on the int8 tensor pipe: every FP64 operand row is scaled by a power "
+                                "of two and cut into %d signed 7-bit digits, the digit products are exact in s32 (TMEM), the "
+                                "recombination is FP64; achieved = ALGORITHMIC int8 operations (digit pairs x both halves of "
+                                "the lower triangle x K' = 2K) / time of the rank_k_i8_kernel launches" % digits,
+                        "digits": digits, "ops_per_launch": i8_ops, "ms_per_launch": i8_ms, "launches": i8_launches,
+                        "share_of_step": float(stage_ms[5]) / args.steps / ms_step,
+                        "rank_k_stage_ms_per_step": float(stage_ms[4]) / args.steps,
+                        "fp64_equivalent_tflops": rk_tf, "fp64_dmma_peak_tflops": peak_tf,
+                        "fp64_equivalent_note": "8 flop per complex multiply-add on one triangle / time of the WHOLE rank-K "
+                                                "stage (slicing passes + MMA kernels), against the measured FP64 DMMA issue rate"}
         # pair-density stage (HBM-bound): algorithmic bytes = 16 N per pair (stream psi_m) + 16 nG (write n)
         pd_ms = float(stage_ms[0] + stage_ms[1]) / args.steps
         pd_bytes = pairs_per_rank * 16.0 * (cfg.n_grid + ng)
@@ -291,7 +329,8 @@ def run_ours(args, cfg):
         line = {
             "metric": METRIC, "value": pairs_total / (ms_step * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64 (complex128)", "data": "synthetic",
+            "dtype": "f64 (complex128)" + ("; rank-K on int8 digit slices of the f64 operands, exact products, f64 recombination"
+                                            if int(stage_n[5]) > 0 else ""), "data": "synthetic",
             "config": {"workload": f"configs[{cfg.index}] {cfg.name}", "grid": list(cfg.grid), "n_k_per_gpu": len(my_k),
                        "n_occ": cfg.n_occ, "n_unocc": cfg.n_unocc, "n_pairs": pairs_total, "nG": ng, "n_omega": cfg.n_omega,
                        "atoms_x_proj": [cfg.n_atoms, cfg.n_proj_per_atom], "max_batch_pairs": args.batch or 8192,
@@ -308,18 +347,7 @@ def run_ours(args, cfg):
                                "coefficients, rpa_pw_to_grid (Eq. 10) expands them on the device inside the timed region; "
                                "e2e above uploads the grid orbitals themselves and is PCIe-bound"},
             "gpu_launches": int(launches),
-            "roofline": {"kernel": "rank_k3m_kernel", "bound": "tensor", "achieved": rk_tf, "peak": peak_tf, "unit": "TFLOP/s",
-                         "frac": rk_tf / peak_tf if peak_tf else None, "traffic": RANK_K_DRAM_TRAFFIC_BYTES.get(cfg.index),
-                         "peak_source": "FP64 DMMA issue rate measured live by rpa_probe_fp64_tensor_peak (register-only "
-                                        "mma.sync.m8n8k4.f64, all SMs); MEASURED_PEAKS.json has no FP64 entry",
-                         "peak_alt_tflops_from_bf16": peaks.get("bf16_tflops", 0) * 40.0 / 2250.0,
-                         "note": "achieved = ALGORITHMIC flops (8 per complex multiply-add on one triangle) / time; the "
-                                 "kernel forms the complex product with 3 real multiplications (3M), so it EXECUTES 3/4 of "
-                                 "them: executed_frac = tensor-pipe flops actually issued / peak; one 'launch' here is the rank-K of one "
-                                 "batch of transitions = its whole-wave launch + the K-sliced launch of the last partial wave",
-                         "executed_frac": 0.75 * rk_tf / peak_tf if peak_tf else None,
-                         "flops_per_launch": rk_flops, "ms_per_launch": rk_ms, "launches": rk_launches,
-                         "share_of_step": float(stage_ms[4]) / args.steps / ms_step},
+            "roofline": roofline,
             "stages": {"ms_per_step": {n: float(t) / args.steps for n, t in zip(B.STAGE_NAMES, stage_ms)},
                        "get_all_omega_ms": tail_ms[0] / args.steps, "ec_q_ms": tail_ms[1] / args.steps,
                        "sum_ms": total_stage,
