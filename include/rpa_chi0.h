@@ -29,10 +29,14 @@
  *
  * Internal resources: besides the workspace the handle owns one CUDA stream (high priority, used by rpa_ec_q to factor
  * panels ahead of the trailing updates; ordered with the caller's stream by events) and a few events, all released by
- * rpa_chi0_destroy.  Reproducibility: when the accumulation splits K over several CTAs per tile (small problems, chosen
- * by the library) the tile sums use floating-point atomics, so chi0 is reproducible to rounding (~1e-16 relative), not
- * bitwise, from run to run.  Environment: RPA_RANK_K_4M=1 at rpa_chi0_create selects the 4-multiplication rank-K kernel
- * instead of the default 3-multiplication one (same results to rounding; kept for comparison).
+ * rpa_chi0_destroy.  The rank-K accumulation (Eq. 17) of a batch with ng >= 768 and >= 1024 transitions runs on the
+ * int8 tensor cores: every FP64 operand row is scaled by a power of two and cut into 7 signed 7-bit digits, the digit
+ * products are exact (s32), the recombination is FP64; chi0 then agrees with the FP64 tensor kernel to ~1e-14 relative
+ * Frobenius norm and is bitwise reproducible.  Smaller batches run on the FP64 tensor cores; when that kernel splits K
+ * over several CTAs per tile (chosen by the library) the tile sums use floating-point atomics: reproducible to rounding
+ * (~1e-16 relative), not bitwise.  Environment, read by rpa_chi0_create: RPA_RANK_K_FP64=1 keeps every batch on the FP64
+ * tensor cores (3-multiplication kernel), RPA_RANK_K_4M=1 on the 4-multiplication FP64 kernel; RPA_RANK_K_I8=1 sends
+ * small batches to the int8 kernel too; RPA_RANK_K_I8_DIGITS=6 uses 6 digits (41-bit operands, ~3e-12, 25 % faster).
  *
  * Errors: every int-returning call gives 0 on success or a negative RPA_ERR_* code; rpa_last_error() holds
  * a thread-local message.  Nothing is thrown across the ABI.  A handle is not thread-safe; distinct handles
