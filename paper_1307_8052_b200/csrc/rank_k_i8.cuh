@@ -122,32 +122,36 @@ __global__ void __launch_bounds__(128) rki8_pack_left_kernel(const cd *__restric
     }
 }
 
-// PR[iw][cb][kb][digit][2048]: rows g' = cb 64 + r, value w[iw][p] (a | b) 2^-eR.  grid (nkb, ncb, n_w), block 64.
+// PR[iw][cb][kb][digit][2048]: rows g' = cb 64 + r, value w[iw][p] (a | b) 2^-eR.  The 32 components of a thread are read
+// once and sliced for every frequency of the group.  grid (nkb, ncb), block 64.
 template <int S>
 __global__ void __launch_bounds__(64) rki8_pack_right_kernel(const cd *__restrict__ Nb, int64_t ldn, int Kpad, int ng, int ngp,
-                                                            const double *__restrict__ w, int64_t ldw,
+                                                            const double *__restrict__ w, int64_t ldw, int n_w,
                                                             const double *__restrict__ invR, int8_t *__restrict__ PR) {
-    const int kb = blockIdx.x, cb = blockIdx.y, iw = blockIdx.z, r = threadIdx.x, nkb = gridDim.x, ncb = gridDim.y;
+    const int kb = blockIdx.x, cb = blockIdx.y, r = threadIdx.x, nkb = gridDim.x, ncb = gridDim.y;
     const int g = cb * rki8::CB + r;
     const int k0 = kb * rki8::KB, part = k0 / Kpad, p0 = k0 - part * Kpad;
     const bool valid = g < ng;
-    const double sc = valid ? invR[(size_t)iw * ngp + g] : 0.0;
-    const double *wr = w + (size_t)iw * ldw;
-    int8_t *dst = PR + (((size_t)iw * ncb + cb) * nkb + kb) * S * rki8::B_BYTES + (r % 8) * 16 + (r / 8) * 256;
+    double v[32];
 #pragma unroll
-    for (int c = 0; c < 2; c++) {
-        double x[16];
-#pragma unroll
-        for (int k = 0; k < 16; k++) {
-            double v = 0.0;
-            if (valid) {
-                const int p = p0 + c * 16 + k;
-                const cd z = Nb[(size_t)p * ldn + g];
-                v = (part ? z.y : z.x) * wr[p];
-            }
-            x[k] = v * sc;
+    for (int k = 0; k < 32; k++) {
+        v[k] = 0.0;
+        if (valid) {
+            const cd z = Nb[(size_t)(p0 + k) * ldn + g];
+            v[k] = part ? z.y : z.x;
         }
-        rki8_store_digits<S>(x, dst + c * 128, rki8::B_BYTES);
+    }
+    for (int iw = 0; iw < n_w; iw++) {
+        const double sc = valid ? invR[(size_t)iw * ngp + g] : 0.0;
+        const double *wr = w + (size_t)iw * ldw + p0;
+        int8_t *dst = PR + (((size_t)iw * ncb + cb) * nkb + kb) * S * rki8::B_BYTES + (r % 8) * 16 + (r / 8) * 256;
+#pragma unroll
+        for (int c = 0; c < 2; c++) {
+            double x[16];
+#pragma unroll
+            for (int k = 0; k < 16; k++) x[k] = (v[c * 16 + k] * wr[c * 16 + k]) * sc;
+            rki8_store_digits<S>(x, dst + c * 128, rki8::B_BYTES);
+        }
     }
 }
 

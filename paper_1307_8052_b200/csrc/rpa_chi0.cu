@@ -783,12 +783,12 @@ int add_kpoint_impl(rpa_chi0_t *h, double kweight, int32_t n_occ, const void *ps
                             const double *w0 = w + (size_t)iw0 * L.ldw, *invR0 = invR + (size_t)iw0 * ngp;
                             cd *S0 = h->ptr<cd>(L.S) + (size_t)iw0 * ng * L.ldS;
                             if (SD == 6) {
-                                rki8_pack_right_kernel<6><<<dim3(nkb, ncb, nw), 64, 0, st>>>(Nbuf, L.ldn, Kpad, ng, ngp, w0, L.ldw, invR0, PR);
+                                rki8_pack_right_kernel<6><<<dim3(nkb, ncb), 64, 0, st>>>(Nbuf, L.ldn, Kpad, ng, ngp, w0, L.ldw, nw, invR0, PR);
                                 StageTimer tm5(h, 5, 1);
                                 rank_k_i8_kernel<6><<<dim3(nt, nw), rki8::THREADS, rki8::smem_bytes(6), st>>>(
                                     PL, PR, nkb, ncb, d_tiles, invL, invR0, ng, ngp, S0, L.ldS, (int64_t)ng * L.ldS);
                             } else {
-                                rki8_pack_right_kernel<7><<<dim3(nkb, ncb, nw), 64, 0, st>>>(Nbuf, L.ldn, Kpad, ng, ngp, w0, L.ldw, invR0, PR);
+                                rki8_pack_right_kernel<7><<<dim3(nkb, ncb), 64, 0, st>>>(Nbuf, L.ldn, Kpad, ng, ngp, w0, L.ldw, nw, invR0, PR);
                                 StageTimer tm5(h, 5, 1);
                                 rank_k_i8_kernel<7><<<dim3(nt, nw), rki8::THREADS, rki8::smem_bytes(7), st>>>(
                                     PL, PR, nkb, ncb, d_tiles, invL, invR0, ng, ngp, S0, L.ldS, (int64_t)ng * L.ldS);
