@@ -157,7 +157,10 @@ __global__ void __launch_bounds__(64) rki8_pack_right_kernel(const cd *__restric
 
 // One CTA = tile (rb, cb) of one frequency: tiles[] lists the tiles that meet the lower triangle.
 // grid (n_tiles, n_w), block 192, dynamic shared memory rki8::smem_bytes(S).
-template <int S>
+// CL = 2: launched in clusters of two CTAs (consecutive blockIdx.x) whose tiles share the row block: each CTA fetches
+// half of the row-block digits of a stage and multicasts it to both, so the L2 -> SM traffic of the row operand halves;
+// a stage is released to the producers when the MMAs of BOTH CTAs have read it (multicast commit, barrier count 2).
+template <int S, int CL>
 __global__ void __launch_bounds__(rki8::THREADS, 1)
 rank_k_i8_kernel(const int8_t *__restrict__ PL, const int8_t *__restrict__ PR, int nkb, int ncb, const int2 *__restrict__ tiles,
                  const double *__restrict__ invL, const double *__restrict__ invR, int ng, int ngp, cd *__restrict__ Sacc,
@@ -173,10 +176,12 @@ rank_k_i8_kernel(const int8_t *__restrict__ PL, const int8_t *__restrict__ PR, i
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int2 tile = tiles[blockIdx.x];
     const int rb = tile.x, cb = tile.y, iw = blockIdx.y;
+    uint32_t crank = 0;
+    if constexpr (CL > 1) asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(crank));
     if (tid == 0) {
         for (int s = 0; s < STAGES; s++) {
             mbar_init(&full[s], 1);
-            mbar_init(&empty[s], 1);
+            mbar_init(&empty[s], CL);
         }
         mbar_init(done, 1);
         mbar_fence_init();
@@ -187,19 +192,31 @@ rank_k_i8_kernel(const int8_t *__restrict__ PL, const int8_t *__restrict__ PR, i
     }
     asm volatile("tcgen05.fence::before_thread_sync;");
     __syncthreads();
+    if constexpr (CL > 1) {   // the peer's barriers must be initialised before anything is multicast to them
+        asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+    }
     asm volatile("tcgen05.fence::after_thread_sync;");
     const uint32_t taddr = *tmem_slot;
 
     if (warp == 4) {
         if (lane == 0) {
             const int8_t *srcA = PL + (size_t)rb * nkb * S * A_BYTES;
-            const int8_t *srcB = PR + ((size_t)iw * ncb + cb) * nkb * S * B_BYTES;
+            // a padding tile of an odd row (cb beyond the triangle) computes on the last column block and stores nothing
+            const int8_t *srcB = PR + ((size_t)iw * ncb + min(cb, ncb - 1)) * nkb * S * B_BYTES;
             for (int kb = 0; kb < nkb; kb++) {
                 const int s = kb % STAGES;
                 if (kb >= STAGES) mbar_wait(&empty[s], ((kb / STAGES) - 1) & 1);
                 unsigned char *st = i8_smem + s * STAGE_BYTES;
                 mbar_arrive_expect_tx(&full[s], STAGE_BYTES);
-                bulk_g2s(st, srcA + (size_t)kb * S * A_BYTES, S * A_BYTES, &full[s]);
+                if constexpr (CL > 1) {
+                    constexpr uint32_t PART = S * A_BYTES / CL;
+                    static_assert(PART % 16 == 0, "bulk copies move multiples of 16 bytes");
+                    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster [%0], [%1], %2, [%3], %4;"
+                                 ::"r"(smem_u32(st + crank * PART)), "l"(srcA + (size_t)kb * S * A_BYTES + crank * PART), "r"(PART),
+                                   "r"(smem_u32(&full[s])), "h"((uint16_t)((1u << CL) - 1)) : "memory");
+                } else {
+                    bulk_g2s(st, srcA + (size_t)kb * S * A_BYTES, S * A_BYTES, &full[s]);
+                }
                 bulk_g2s(st + S * A_BYTES, srcB + (size_t)kb * S * B_BYTES, S * B_BYTES, &full[s]);
             }
         }
@@ -210,18 +227,29 @@ rank_k_i8_kernel(const int8_t *__restrict__ PL, const int8_t *__restrict__ PR, i
                 mbar_wait(&full[s], (kb / STAGES) & 1);
                 asm volatile("tcgen05.fence::after_thread_sync;");
                 const uint32_t sa = i8_saddr(i8_smem + s * STAGE_BYTES), sb = sa + S * A_BYTES;
+                // Row digit i meets column digits j = 0 .. S-1-i; their planes are consecutive in shared memory (64 rows =
+                // 8 core-matrix groups each) and their accumulators t = i + j are consecutive in TMEM, so up to 4 of them are
+                // ONE MMA of N = 64 nj columns: the row operand is read 10 times per K block instead of 28 (S = 7), which
+                // keeps the tensor core's shared-memory reads under 128 B/clk.
 #pragma unroll
                 for (int i = 0; i < S; i++) {
                     const uint64_t da = i8_smem_desc(sa + i * A_BYTES, 128, 256);
 #pragma unroll
-                    for (int j = 0; j + i < S; j++) {
-                        const uint64_t db = i8_smem_desc(sb + j * B_BYTES, 128, 256);
-                        // accumulator t = i + j at columns 64 t; the first product into it is (kb, i) = (0, 0)
+                    for (int j0 = 0; j0 + i < S; j0 += 4) {
+                        const int nj = (S - i - j0) < 4 ? (S - i - j0) : 4;
+                        const uint64_t db = i8_smem_desc(sb + j0 * B_BYTES, 128, 256);
+                        const uint32_t idesc = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)((CB * nj) >> 3) << 17) | ((uint32_t)(RB >> 4) << 24);
+                        // the first product into an accumulator is (kb, i) = (0, 0)
                         asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\ntcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n}"
-                                     ::"r"(taddr + (uint32_t)(i + j) * CB), "l"(da), "l"(db), "r"(IDESC), "r"((kb > 0 || i > 0) ? 1 : 0));
+                                     ::"r"(taddr + (uint32_t)(i + j0) * CB), "l"(da), "l"(db), "r"(idesc), "r"((kb > 0 || i > 0) ? 1 : 0));
                     }
                 }
-                i8_commit(&empty[s]);   // arrives when the MMAs above have read this stage
+                if constexpr (CL > 1) {   // arrive on the stage barrier of every CTA of the cluster
+                    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+                                 ::"r"(i8_saddr(&empty[s])), "h"((uint16_t)((1u << CL) - 1)) : "memory");
+                } else {
+                    i8_commit(&empty[s]);   // arrives when the MMAs above have read this stage
+                }
             }
             i8_commit(done);
         }
@@ -267,5 +295,8 @@ rank_k_i8_kernel(const int8_t *__restrict__ PL, const int8_t *__restrict__ PR, i
     }
     asm volatile("tcgen05.fence::before_thread_sync;");
     __syncthreads();
+    if constexpr (CL > 1) {   // no CTA leaves while its peer may still multicast into it or arrive on its barriers
+        asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+    }
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(512));
 }

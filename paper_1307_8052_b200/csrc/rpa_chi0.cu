@@ -213,6 +213,7 @@ struct rpa_chi0 {
     int idx0 = -1;                     // sphere index of G = 0 when q0
     bool use_i8 = false;               // RPA_RANK_K_I8: int8-sliced rank-K on tcgen05 (rank_k_i8.cuh)
     int i8_digits = 7;
+    bool i8_cluster = true;            // clusters of 2 CTAs multicast the row-block digits (RPA_RANK_K_I8_NOCLUSTER=1: off)
     bool i8_force = false;             // RPA_RANK_K_I8=1: also for small batches (tests)
     std::vector<int2> i8_tiles;        // (row block, column block) tiles that meet the lower triangle
     bool use_3m = true;                // rank_k3m_kernel (3-multiplication complex product) for the chi0 accumulation
@@ -297,6 +298,30 @@ int pick_ksplit(int units, int nchunks, int n_sm, double *cost_out = nullptr) {
     }
     if (cost_out) *cost_out = best_cost;   // in units of one full-K item
     return best;
+}
+
+// rank_k_i8_kernel<S, 2> as clusters of two CTAs along x (tiles come in pairs of one row block), or <S, 1> plain
+template <int S>
+cudaError_t launch_i8(bool cluster, dim3 grid, cudaStream_t st, const int8_t *PL, const int8_t *PR, int nkb, int ncb,
+                      const int2 *tiles, const double *invL, const double *invR, int ng, int ngp, cd *Sacc, int64_t ldS,
+                      int64_t strideS) {
+    if (!cluster) {
+        rank_k_i8_kernel<S, 1><<<grid, rki8::THREADS, rki8::smem_bytes(S), st>>>(PL, PR, nkb, ncb, tiles, invL, invR, ng, ngp, Sacc, ldS, strideS);
+        return cudaGetLastError();
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = dim3(rki8::THREADS);
+    cfg.dynamicSmemBytes = rki8::smem_bytes(S);
+    cfg.stream = st;
+    cudaLaunchAttribute attr;
+    attr.id = cudaLaunchAttributeClusterDimension;
+    attr.val.clusterDim.x = 2;
+    attr.val.clusterDim.y = 1;
+    attr.val.clusterDim.z = 1;
+    cfg.attrs = &attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, rank_k_i8_kernel<S, 2>, PL, PR, nkb, ncb, tiles, invL, invR, ng, ngp, Sacc, ldS, strideS);
 }
 
 // Launch plan of the plane kernel: rows per chunk, threads, dynamic shared memory.
@@ -496,18 +521,24 @@ int create_impl(rpa_chi0_t **out, const int32_t grid[3], const double cell[9], c
     // int8-sliced rank-K (rank_k_i8.cuh) unless RPA_RANK_K_FP64 / RPA_RANK_K_4M ask for the FP64 tensor kernels; batches
     // too small to pay for the slicing passes take the FP64 kernel anyway (I8_MIN_NG, I8_MIN_K below)
     h->use_i8 = getenv("RPA_RANK_K_FP64") == nullptr && getenv("RPA_RANK_K_4M") == nullptr;
+    h->i8_cluster = getenv("RPA_RANK_K_I8_NOCLUSTER") == nullptr;
     if (h->use_i8) {
         const int ng_ = h->sp.ng, ngp = (ng_ + rki8::RB - 1) / rki8::RB * rki8::RB;
         for (int rb = 0; rb < 2 * ngp / rki8::RB; rb++) {
             const int g_lo = (rb * rki8::RB) % ngp, g_hi = std::min(g_lo + rki8::RB - 1, ng_ - 1);
             if (g_lo >= ng_) continue;
-            for (int cb = 0; cb * rki8::CB <= g_hi; cb++) h->i8_tiles.push_back(make_int2(rb, cb));
+            int cb = 0;
+            for (; cb * rki8::CB <= g_hi; cb++) h->i8_tiles.push_back(make_int2(rb, cb));
+            // clusters of two CTAs share a row block: an odd row gets a padding tile beyond the triangle (stores nothing)
+            if (h->i8_cluster && (cb & 1)) h->i8_tiles.push_back(make_int2(rb, cb));
         }
         h->i8_force = getenv("RPA_RANK_K_I8") != nullptr;
         const char *dg = getenv("RPA_RANK_K_I8_DIGITS");
         h->i8_digits = (dg && atoi(dg) == 6) ? 6 : 7;
-        if (cudaFuncSetAttribute(rank_k_i8_kernel<6>, cudaFuncAttributeMaxDynamicSharedMemorySize, rki8::smem_bytes(6)) != cudaSuccess ||
-            cudaFuncSetAttribute(rank_k_i8_kernel<7>, cudaFuncAttributeMaxDynamicSharedMemorySize, rki8::smem_bytes(7)) != cudaSuccess)
+        if (cudaFuncSetAttribute(rank_k_i8_kernel<6, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, rki8::smem_bytes(6)) != cudaSuccess ||
+            cudaFuncSetAttribute(rank_k_i8_kernel<7, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, rki8::smem_bytes(7)) != cudaSuccess ||
+            cudaFuncSetAttribute(rank_k_i8_kernel<6, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, rki8::smem_bytes(6)) != cudaSuccess ||
+            cudaFuncSetAttribute(rank_k_i8_kernel<7, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, rki8::smem_bytes(7)) != cudaSuccess)
             h->use_i8 = false;
     }
     CREATE_TRY(cudaFuncSetAttribute(rank_k_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, rk::Cfg<false>::SMEM_BYTES));
@@ -785,13 +816,13 @@ int add_kpoint_impl(rpa_chi0_t *h, double kweight, int32_t n_occ, const void *ps
                             if (SD == 6) {
                                 rki8_pack_right_kernel<6><<<dim3(nkb, ncb), 64, 0, st>>>(Nbuf, L.ldn, Kpad, ng, ngp, w0, L.ldw, nw, invR0, PR);
                                 StageTimer tm5(h, 5, 1);
-                                rank_k_i8_kernel<6><<<dim3(nt, nw), rki8::THREADS, rki8::smem_bytes(6), st>>>(
-                                    PL, PR, nkb, ncb, d_tiles, invL, invR0, ng, ngp, S0, L.ldS, (int64_t)ng * L.ldS);
+                                CUDA_TRY(launch_i8<6>(h->i8_cluster, dim3(nt, nw), st, PL, PR, nkb, ncb, d_tiles, invL, invR0, ng, ngp, S0, L.ldS,
+                                                      (int64_t)ng * L.ldS));
                             } else {
                                 rki8_pack_right_kernel<7><<<dim3(nkb, ncb), 64, 0, st>>>(Nbuf, L.ldn, Kpad, ng, ngp, w0, L.ldw, nw, invR0, PR);
                                 StageTimer tm5(h, 5, 1);
-                                rank_k_i8_kernel<7><<<dim3(nt, nw), rki8::THREADS, rki8::smem_bytes(7), st>>>(
-                                    PL, PR, nkb, ncb, d_tiles, invL, invR0, ng, ngp, S0, L.ldS, (int64_t)ng * L.ldS);
+                                CUDA_TRY(launch_i8<7>(h->i8_cluster, dim3(nt, nw), st, PL, PR, nkb, ncb, d_tiles, invL, invR0, ng, ngp, S0, L.ldS,
+                                                      (int64_t)ng * L.ldS));
                             }
                             h->launches += 1;
                         }
