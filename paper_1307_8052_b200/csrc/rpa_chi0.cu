@@ -45,8 +45,8 @@ int fail(int code, const char *fmt, ...) {
     } while (0)
 
 constexpr int DEFAULT_BATCH = 8192;
-constexpr int MAX_SLOTS = 16;
-constexpr int I8_MIN_NG = 768, I8_MIN_K = 1024;   // below: the FP64 tensor kernel is faster (measured: nG = 401, K = 2400 loses)          // occupied bands per batch
+constexpr int MAX_SLOTS = 16;          // occupied bands per batch
+constexpr int I8_MIN_NG = 768, I8_MIN_K = 1024;  // below: the FP64 tensor kernel is faster (measured: nG = 401, K = 2400 loses)
 constexpr int MAX_BANDS = 1 << 17;     // eps/f scratch
 constexpr int MAX_ATOMS = 4096;
 constexpr int MAX_PROJ = 1 << 16;
