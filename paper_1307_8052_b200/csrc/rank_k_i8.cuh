@@ -5,7 +5,7 @@
 //   Re S[g][g'] = sum_p (a_g)(w a_g') + (b_g)(w b_g'),     Im S[g][g'] = sum_p (b_g)(w a_g') + (-a_g)(w b_g'),
 // i.e. D = L R^T with L = [a | b ; b | -a] (2 ngp "left rows", K' = 2 Kpad columns) and R_w = [w a | w b] (ng rows).
 // Every row of L is scaled by a power of two to (-1, 1) and cut into I8_S signed digits
-//   x = sum_i d_i 2^(-6 - 7 i) + r,   d_i in [-64, 64],   |r| <= 2^(-7 - 7 (S - 1)),
+//   x = sum_i d_i 2^(-6 - 7 i) + r,   d_i in [-64, 64],   |r| <= 2^(-7 - 7 (S - 1))   (one rounding to 6 + 7 (S - 1) bits),
 // likewise every row of R_w (scaled per frequency and row).  The digit products L_i R_j^T with i + j = t share the
 // scale 2^(-12 - 7 t); each t has its own s32 accumulator in TMEM (exact: at most S * K' * 64^2 < 2^31), the pairs with
 // i + j >= S are below the truncation error and are dropped.  The epilogue recombines in FP64:
@@ -69,7 +69,9 @@ __global__ void rki8_scale_finish_kernel(unsigned long long *__restrict__ mx, in
     reinterpret_cast<double *>(mx)[i] = rki8_pow2_scale(m);
 }
 
-// 16 values x (|x| < 1) -> S x 16 digit bytes, written as one 16-byte store per digit plane
+// 16 values x (|x| < 1) -> S x 16 digit bytes, written as one 16-byte store per digit plane.  The value is rounded once to
+// an integer v = rint(x 2^(6 + 7 (S - 1))) (|v| <= 2^48: exact in FP64 and in s64), and v is cut into balanced base-128
+// digits from the least significant end with integer arithmetic: v = sum_i d_i 128^(S-1-i), d_i in [-64, 64].
 template <int S>
 __device__ __forceinline__ void rki8_store_digits(const double (&x)[16], int8_t *dst, int plane_stride) {
     uint32_t pk[S][4];
@@ -77,15 +79,17 @@ __device__ __forceinline__ void rki8_store_digits(const double (&x)[16], int8_t 
     for (int i = 0; i < S; i++)
 #pragma unroll
         for (int q = 0; q < 4; q++) pk[i][q] = 0u;
+    constexpr double SCALE = (double)(1ull << (6 + 7 * (S - 1)));
 #pragma unroll
     for (int k = 0; k < 16; k++) {
-        double y = x[k] * 64.0;
+        long long v = __double2ll_rn(x[k] * SCALE);
 #pragma unroll
-        for (int i = 0; i < S; i++) {
-            const double r = rint(y);
-            pk[i][k >> 2] |= ((uint32_t)(int)r & 0xffu) << (8 * (k & 3));
-            y = (y - r) * 128.0;
+        for (int i = S - 1; i > 0; i--) {
+            const long long d = ((v + 64) & 127) - 64;   // v mod 128 in [-64, 63]
+            pk[i][k >> 2] |= ((uint32_t)d & 0xffu) << (8 * (k & 3));
+            v = (v - d) >> 7;                            // exact: v - d is a multiple of 128
         }
+        pk[0][k >> 2] |= ((uint32_t)v & 0xffu) << (8 * (k & 3));   // |v| <= 64
     }
 #pragma unroll
     for (int i = 0; i < S; i++)
