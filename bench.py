@@ -36,8 +36,8 @@ UNIT = "transitions/s"
 # dram__bytes_write.sum of one batch of 7200 pairs = its two launches (whole waves 2.884 GB + 175.7 MB, K-sliced tail
 # 143.8 MB + 4.5 MB); other configs have no capture
 RANK_K_DRAM_TRAFFIC_BYTES = {1: 3208.2e6}
-# the same for rank_k_i8_kernel (profiles/r1h_bench_cfg1.md): DRAM bytes of one launch (a group of frequencies)
-RANK_K_I8_DRAM_TRAFFIC_BYTES = {1: 4549.1e6}   # 4.395 GB read + 154 MB written per launch of 8 frequencies
+# the same for rank_k_i8_kernel (profiles/r1i_bench_cfg1.md): DRAM bytes of one launch (a group of frequencies)
+RANK_K_I8_DRAM_TRAFFIC_BYTES = {1: 4455.9e6}   # 4.304 GB read + 152 MB written per launch of 8 frequencies
 
 def rank_k_useful_flops(ng, n_omega, n_pairs):
     """8 flop per complex MAC on one triangle: 4 nG (nG+1) n_omega per pair."""
