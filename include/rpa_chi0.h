@@ -36,7 +36,8 @@
  * over several CTAs per tile (chosen by the library) the tile sums use floating-point atomics: reproducible to rounding
  * (~1e-16 relative), not bitwise.  Environment, read by rpa_chi0_create: RPA_RANK_K_FP64=1 keeps every batch on the FP64
  * tensor cores (3-multiplication kernel), RPA_RANK_K_4M=1 on the 4-multiplication FP64 kernel; RPA_RANK_K_I8=1 sends
- * small batches to the int8 kernel too; RPA_RANK_K_I8_DIGITS=6 uses 6 digits (41-bit operands, ~3e-12, 25 % faster).
+ * small batches to the int8 kernel too; RPA_RANK_K_I8_DIGITS=6 uses 6 digits (41-bit operands, ~3e-12, 25 % fewer MMAs);
+ * RPA_RANK_K_I8_NOCLUSTER=1 launches the int8 kernel without thread-block clusters.
  *
  * Errors: every int-returning call gives 0 on success or a negative RPA_ERR_* code; rpa_last_error() holds
  * a thread-local message.  Nothing is thrown across the ABI.  A handle is not thread-safe; distinct handles
