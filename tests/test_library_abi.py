@@ -45,7 +45,7 @@ def test_library_is_sm100a_with_dmma_and_bulk_copies():
     assert body.count("DMMA") >= 256   # 8 k-steps x 32 DMMA.8x8x4, fully unrolled
     assert "UBLKCP" in body            # cp.async.bulk on the TMA engine
     i8 = out.stdout.split("rank_k_i8_kernel", 1)[1].split("Function :", 1)[0]
-    assert i8.count("UTCIMMA") >= 21   # tcgen05.mma.kind::i8: one per digit pair of a K block
+    assert i8.count("UTCIMMA") >= 8    # tcgen05.mma.kind::i8: 8 (6 digits) or 10 (7 digits) wide MMAs per K block
     assert "UBLKCP" in i8
 
 
