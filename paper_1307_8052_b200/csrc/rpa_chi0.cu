@@ -1022,7 +1022,7 @@ int ec_q_impl(rpa_chi0_t *h, const double *v_G, int iw_begin, int iw_end, double
                 // on the caller's stream after it
                 cudaStream_t ps = p == 0 ? h->side : st;
                 if (p > 0) h->launches += update(st, Lt, p * CH_NB, c0, 1, c0 + CH_NB);
-                chol_panel_kernel<<<dim3(std::max(1, (rest + 127) / 128), nm), 128, 0, ps>>>(
+                chol_panel_kernel<<<dim3(std::max(1, (rest + 127) / 128), nm), CH_THREADS, 0, ps>>>(
                     M, ng, c0, Lt + (size_t)p * CH_NB * L.ldn, L.ldn, lt_mat, d_flag, d_ld);
                 h->launches += 1;
                 if (p == 0) {
