@@ -219,6 +219,8 @@ struct rpa_chi0 {
     bool use_3m = true;                // rank_k3m_kernel (3-multiplication complex product) for the chi0 accumulation
     cudaStream_t side = nullptr;       // panel factorisations of rpa_ec_q run here, ahead of the trailing updates
     cudaEvent_t ev_panel[2] = {nullptr, nullptr}, ev_col = nullptr, ev_fork = nullptr;
+    cudaStream_t main2 = nullptr, side2 = nullptr;   // second lane of rpa_ec_q (half of the matrices of a group)
+    cudaEvent_t ev_panel2[2] = {nullptr, nullptr}, ev_col2 = nullptr, ev_join = nullptr;
     size_t zy_smem = 0;
     unsigned char *ws;
     // profiling
@@ -505,7 +507,10 @@ int create_impl(rpa_chi0_t **out, const int32_t grid[3], const double cell[9], c
         int prio_lo = 0, prio_hi = 0;
         CREATE_TRY(cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi));
         CREATE_TRY(cudaStreamCreateWithPriority(&h->side, cudaStreamNonBlocking, prio_hi));
-        for (cudaEvent_t *e : {&h->ev_panel[0], &h->ev_panel[1], &h->ev_col, &h->ev_fork})
+        CREATE_TRY(cudaStreamCreateWithPriority(&h->side2, cudaStreamNonBlocking, prio_hi));
+        CREATE_TRY(cudaStreamCreateWithPriority(&h->main2, cudaStreamNonBlocking, prio_lo));
+        for (cudaEvent_t *e : {&h->ev_panel[0], &h->ev_panel[1], &h->ev_col, &h->ev_fork, &h->ev_panel2[0], &h->ev_panel2[1],
+                               &h->ev_col2, &h->ev_join})
             CREATE_TRY(cudaEventCreateWithFlags(e, cudaEventDisableTiming));
     }
     if (h->zy_kernel) {
@@ -996,47 +1001,71 @@ int ec_q_impl(rpa_chi0_t *h, const double *v_G, int iw_begin, int iw_end, double
         // (0.37 GB for cfg 1, beyond L2) happens once per 128 columns instead of once per 32.
         // Look-ahead: the first panel of the next block needs only the first tile column of that big update; it runs on
         // the high-priority side stream while the rest of the update proceeds.  Two block buffers of Lt alternate.
+        // Two lanes: the group's matrices are split in halves that run the same schedule on their own pair of streams.
+        // The panel steps are latency-bound (one warp factors the diagonal block, few CTAs), the trailing updates are
+        // throughput-bound: with two independent halves in flight one half's updates fill the SMs while the other
+        // half is in its panel steps.  `RPA_EC_LANES=1` keeps everything on one lane.
         const int64_t lt_mat = (int64_t)CH_P * CH_NB * L.ldn;          // per matrix
         const size_t lt_block = (size_t)L.ec_group * lt_mat;           // per block buffer
         const double *wneg = h->ptr<double>(L.wneg);
-        auto update = [&](cudaStream_t s_, cd *Lt, int K, int g0, int mode, int col_limit) {
+        const char *lanes_env = getenv("RPA_EC_LANES");
+        const int n_lanes = (nm >= 2 && !(lanes_env && atoi(lanes_env) == 1)) ? 2 : 1;
+        struct Lane {
+            cudaStream_t main, side;
+            cudaEvent_t *ev_panel, ev_col;
+            int m0, nm;
+        } lanes[2] = {{st, h->side, h->ev_panel, h->ev_col, 0, n_lanes == 2 ? (nm + 1) / 2 : nm},
+                      {h->main2, h->side2, h->ev_panel2, h->ev_col2, (nm + 1) / 2, nm / 2}};
+        auto update = [&](const Lane &ln, cudaStream_t s_, cd *Lt, int K, int g0, int mode, int col_limit) {
             const int rest = ng - g0;
             if (rest <= 0) return 0;
             const int nt = (rest + rk::T - 1) / rk::T;
             const int tiles = mode == 1 ? nt : (mode == 2 ? ntiles_lower(rest, rk::T) - nt : ntiles_lower(rest, rk::T));
             if (tiles <= 0) return 0;
-            rank_k_kernel<false><<<dim3(tiles, nm), rk::Cfg<false>::THREADS, rk::Cfg<false>::SMEM_BYTES, s_>>>(
-                Lt, L.ldn, lt_mat, K, wneg, CH_P * CH_NB, M, ng, (int64_t)ng * ng, ng, g0, nm, mode, col_limit);
+            rank_k_kernel<false><<<dim3(tiles, ln.nm), rk::Cfg<false>::THREADS, rk::Cfg<false>::SMEM_BYTES, s_>>>(
+                Lt, L.ldn, lt_mat, K, wneg, CH_P * CH_NB, M + (size_t)ln.m0 * ng * ng, ng, (int64_t)ng * ng, ng, g0, ln.nm, mode,
+                col_limit);
             return 1;
         };
         CUDA_TRY(cudaEventRecord(h->ev_fork, st));
-        CUDA_TRY(cudaStreamWaitEvent(h->side, h->ev_fork, 0));
+        for (int l = 0; l < n_lanes; l++) {
+            CUDA_TRY(cudaStreamWaitEvent(lanes[l].side, h->ev_fork, 0));
+            if (l > 0) CUDA_TRY(cudaStreamWaitEvent(lanes[l].main, h->ev_fork, 0));
+        }
         int blk = 0;
         for (int kb = 0; kb < ng; kb += CH_P * CH_NB, blk++) {
-            cd *Lt = h->ptr<cd>(L.Lt) + (size_t)(blk & 1) * lt_block;
-            int np = 0;   // panels of this block
-            for (int p = 0; p < CH_P && kb + p * CH_NB < ng; p++, np++) {
-                const int c0 = kb + p * CH_NB;
-                const int rest = ng - (c0 + CH_NB);
-                // panel 0 of a block runs on the side stream (ahead of the rest of the previous big update), the others
-                // on the caller's stream after it
-                cudaStream_t ps = p == 0 ? h->side : st;
-                if (p > 0) h->launches += update(st, Lt, p * CH_NB, c0, 1, c0 + CH_NB);
-                chol_panel_kernel<<<dim3(std::max(1, (rest + 127) / 128), nm), CH_THREADS, 0, ps>>>(
-                    M, ng, c0, Lt + (size_t)p * CH_NB * L.ldn, L.ldn, lt_mat, d_flag, d_ld);
-                h->launches += 1;
-                if (p == 0) {
-                    CUDA_TRY(cudaEventRecord(h->ev_panel[blk & 1], h->side));
-                    CUDA_TRY(cudaStreamWaitEvent(st, h->ev_panel[blk & 1], 0));
+            for (int l = 0; l < n_lanes; l++) {
+                const Lane &ln = lanes[l];
+                cd *Lt = h->ptr<cd>(L.Lt) + (size_t)(blk & 1) * lt_block + (size_t)ln.m0 * lt_mat;
+                int np = 0;   // panels of this block
+                for (int p = 0; p < CH_P && kb + p * CH_NB < ng; p++, np++) {
+                    const int c0 = kb + p * CH_NB;
+                    const int rest = ng - (c0 + CH_NB);
+                    // panel 0 of a block runs on the side stream (ahead of the rest of the previous big update), the
+                    // others on the lane's main stream after it
+                    cudaStream_t ps = p == 0 ? ln.side : ln.main;
+                    if (p > 0) h->launches += update(ln, ln.main, Lt, p * CH_NB, c0, 1, c0 + CH_NB);
+                    chol_panel_kernel<<<dim3(std::max(1, (rest + 127) / 128), ln.nm), CH_THREADS, 0, ps>>>(
+                        M + (size_t)ln.m0 * ng * ng, ng, c0, Lt + (size_t)p * CH_NB * L.ldn, L.ldn, lt_mat, d_flag + ln.m0,
+                        d_ld + ln.m0);
+                    h->launches += 1;
+                    if (p == 0) {
+                        CUDA_TRY(cudaEventRecord(ln.ev_panel[blk & 1], ln.side));
+                        CUDA_TRY(cudaStreamWaitEvent(ln.main, ln.ev_panel[blk & 1], 0));
+                    }
+                }
+                const int g0 = kb + np * CH_NB;
+                if (g0 < ng) {
+                    h->launches += update(ln, ln.main, Lt, np * CH_NB, g0, 1, ng);
+                    CUDA_TRY(cudaEventRecord(ln.ev_col, ln.main));
+                    CUDA_TRY(cudaStreamWaitEvent(ln.side, ln.ev_col, 0));
+                    h->launches += update(ln, ln.main, Lt, np * CH_NB, g0, 2, ng);
                 }
             }
-            const int g0 = kb + np * CH_NB;
-            if (g0 < ng) {
-                h->launches += update(st, Lt, np * CH_NB, g0, 1, ng);
-                CUDA_TRY(cudaEventRecord(h->ev_col, st));
-                CUDA_TRY(cudaStreamWaitEvent(h->side, h->ev_col, 0));
-                h->launches += update(st, Lt, np * CH_NB, g0, 2, ng);
-            }
+        }
+        if (n_lanes == 2) {   // join: the caller's stream continues after the second lane
+            CUDA_TRY(cudaEventRecord(h->ev_join, lanes[1].main));
+            CUDA_TRY(cudaStreamWaitEvent(st, h->ev_join, 0));
         }
         CUDA_TRY(cudaGetLastError());
         ec_collect_kernel<<<1, 32, 0, st>>>(d_ld, d_tr, nm, iw0, d_e);
@@ -1120,8 +1149,10 @@ int rpa_chi0_accumulators(const rpa_chi0_t *h, void **S, size_t *bytes) {
 
 void rpa_chi0_destroy(rpa_chi0_t *h) {
     if (!h) return;
-    if (h->side) cudaStreamDestroy(h->side);
-    for (cudaEvent_t e : {h->ev_panel[0], h->ev_panel[1], h->ev_col, h->ev_fork})
+    for (cudaStream_t s_ : {h->side, h->side2, h->main2})
+        if (s_) cudaStreamDestroy(s_);
+    for (cudaEvent_t e : {h->ev_panel[0], h->ev_panel[1], h->ev_col, h->ev_fork, h->ev_panel2[0], h->ev_panel2[1], h->ev_col2,
+                          h->ev_join})
         if (e) cudaEventDestroy(e);
     for (auto &ev : h->events) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
     for (auto &e : h->pool) cudaEventDestroy(e);
