@@ -154,9 +154,10 @@ rank_k_kernel(const cd *__restrict__ Nb, int64_t ldn, int64_t strideN, int Kpad,
     const int g = lane >> 2, kq = lane & 3, pp = kq >> 1, c = kq & 1;
     const int wsel = warp >> 2, quad = warp & 3;
     const int rowoff = (quad >> 1) * 32, coloff = (quad & 1) * 32;
-    // a warp whose sub-tile lies strictly above the diagonal or wholly beyond the matrix edge, or whose frequency does
-    // not exist, only keeps the barriers moving
-    const bool active = (wsel < n_om) && !(ti == tj && coloff > rowoff) && row0 + rowoff < ng && col0 + coloff < ng;
+    // a warp whose sub-tile lies strictly above the diagonal, wholly beyond the matrix edge or the column limit, or whose
+    // frequency does not exist, only keeps the barriers moving
+    // (col_limit: a Cholesky strip update writes only 32 of the tile's 64 columns)
+    const bool active = (wsel < n_om) && !(ti == tj && coloff > rowoff) && row0 + rowoff < ng && col0 + coloff < min(ng, col_limit);
 
     if (!SHARED_N && active) {   // short K: pull this warp's part of the accumulator tile towards L2 while the K loop runs
         const cd *Sp = S + (size_t)(om0 + wsel) * strideS;
