@@ -96,19 +96,25 @@ rank_k_kernel(const cd *__restrict__ Nb, int64_t ldn, int64_t strideN, int Kpad,
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     // lower-triangle tile (ti >= tj) from the linear index
     // tile_mode 0: all lower tiles; 1: only the first tile column (tj = 0, blockIdx.x = ti); 2: all the others
-    // (the lower tiles of the triangle shifted by one tile) -- the blocked Cholesky of rpa_ec_q uses 1 and 2.
+    // (the lower tiles of the triangle shifted by one tile); 3: the first two tile columns; 4: all the others (shifted by
+    // two tiles) -- the blocked Cholesky of rpa_ec_q uses 1 (strips), 3 and 4.
     // Columns >= col_limit (<= ng) are not written (a strip update inside a Cholesky block touches one 32-column panel).
     const int t = blockIdx.x;
     int ti, tj;
     if (tile_mode == 1) {
         ti = t;
         tj = 0;
+    } else if (tile_mode == 3) {
+        const int nt = (ng - g0 + T - 1) / T;
+        ti = t < nt ? t : t - nt + 1;
+        tj = t < nt ? 0 : 1;
     } else {
         ti = (int)((sqrt(8.0 * (double)t + 1.0) - 1.0) * 0.5);
         while ((ti + 1) * (ti + 2) / 2 <= t) ti++;
         while (ti * (ti + 1) / 2 > t) ti--;
         tj = t - ti * (ti + 1) / 2;
         if (tile_mode == 2) { ti++; tj++; }
+        if (tile_mode == 4) { ti += 2; tj += 2; }
     }
     const int row0 = g0 + ti * T, col0 = g0 + tj * T;
     const int om0 = blockIdx.y * NW;

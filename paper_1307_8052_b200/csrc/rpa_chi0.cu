@@ -999,8 +999,10 @@ int ec_q_impl(rpa_chi0_t *h, const double *v_G, int iw_begin, int iw_end, double
         // column of rank_k_kernel<false>, K = 32 p, columns limited to the panel), is factored and solved, and only after
         // the last panel is the trailing matrix updated, once, with K = 128: the read-modify-write of the trailing matrix
         // (0.37 GB for cfg 1, beyond L2) happens once per 128 columns instead of once per 32.
-        // Look-ahead: the first panel of the next block needs only the first tile column of that big update; it runs on
-        // the high-priority side stream while the rest of the update proceeds.  Two block buffers of Lt alternate.
+        // Look-ahead: the next block needs only the first two tile columns (128 columns) of that big update; they are
+        // updated on the high-priority side stream, which then runs the whole next block (panels and strips: the serial,
+        // latency-bound chain) while the rest of the update proceeds on the main stream.  Two block buffers of Lt alternate
+        // (block b + 2 starts after the look-ahead of block b + 1, which waits for the big update of block b).
         // Two lanes: the group's matrices are split in halves that run the same schedule on their own pair of streams.
         // The panel steps are latency-bound (one warp factors the diagonal block, few CTAs), the trailing updates are
         // throughput-bound: with two independent halves in flight one half's updates fill the SMs while the other
@@ -1020,7 +1022,11 @@ int ec_q_impl(rpa_chi0_t *h, const double *v_G, int iw_begin, int iw_end, double
             const int rest = ng - g0;
             if (rest <= 0) return 0;
             const int nt = (rest + rk::T - 1) / rk::T;
-            const int tiles = mode == 1 ? nt : (mode == 2 ? ntiles_lower(rest, rk::T) - nt : ntiles_lower(rest, rk::T));
+            const int tiles = mode == 1   ? nt
+                              : mode == 2 ? ntiles_lower(rest, rk::T) - nt
+                              : mode == 3 ? nt + std::max(nt - 1, 0)
+                              : mode == 4 ? (nt > 2 ? (nt - 2) * (nt - 1) / 2 : 0)
+                                          : ntiles_lower(rest, rk::T);
             if (tiles <= 0) return 0;
             rank_k_kernel<false><<<dim3(tiles, ln.nm), rk::Cfg<false>::THREADS, rk::Cfg<false>::SMEM_BYTES, s_>>>(
                 Lt, L.ldn, lt_mat, K, wneg, CH_P * CH_NB, M + (size_t)ln.m0 * ng * ng, ng, (int64_t)ng * ng, ng, g0, ln.nm, mode,
@@ -1037,29 +1043,27 @@ int ec_q_impl(rpa_chi0_t *h, const double *v_G, int iw_begin, int iw_end, double
             for (int l = 0; l < n_lanes; l++) {
                 const Lane &ln = lanes[l];
                 cd *Lt = h->ptr<cd>(L.Lt) + (size_t)(blk & 1) * lt_block + (size_t)ln.m0 * lt_mat;
+                // the block's panels and strips: the serial chain, all on the high-priority side stream
                 int np = 0;   // panels of this block
                 for (int p = 0; p < CH_P && kb + p * CH_NB < ng; p++, np++) {
                     const int c0 = kb + p * CH_NB;
                     const int rest = ng - (c0 + CH_NB);
-                    // panel 0 of a block runs on the side stream (ahead of the rest of the previous big update), the
-                    // others on the lane's main stream after it
-                    cudaStream_t ps = p == 0 ? ln.side : ln.main;
-                    if (p > 0) h->launches += update(ln, ln.main, Lt, p * CH_NB, c0, 1, c0 + CH_NB);
-                    chol_panel_kernel<<<dim3(std::max(1, (rest + 127) / 128), ln.nm), CH_THREADS, 0, ps>>>(
+                    if (p > 0) h->launches += update(ln, ln.side, Lt, p * CH_NB, c0, 1, c0 + CH_NB);
+                    chol_panel_kernel<<<dim3(std::max(1, (rest + 127) / 128), ln.nm), CH_THREADS, 0, ln.side>>>(
                         M + (size_t)ln.m0 * ng * ng, ng, c0, Lt + (size_t)p * CH_NB * L.ldn, L.ldn, lt_mat, d_flag + ln.m0,
                         d_ld + ln.m0);
                     h->launches += 1;
-                    if (p == 0) {
-                        CUDA_TRY(cudaEventRecord(ln.ev_panel[blk & 1], ln.side));
-                        CUDA_TRY(cudaStreamWaitEvent(ln.main, ln.ev_panel[blk & 1], 0));
-                    }
                 }
+                CUDA_TRY(cudaEventRecord(ln.ev_panel[blk & 1], ln.side));
+                CUDA_TRY(cudaStreamWaitEvent(ln.main, ln.ev_panel[blk & 1], 0));
                 const int g0 = kb + np * CH_NB;
                 if (g0 < ng) {
-                    h->launches += update(ln, ln.main, Lt, np * CH_NB, g0, 1, ng);
+                    // look-ahead: the first two tile columns (= the next block's 128 columns) on the side stream, after
+                    // the previous block's big update; the rest of the trailing matrix on the main stream meanwhile
+                    if (blk > 0) CUDA_TRY(cudaStreamWaitEvent(ln.side, ln.ev_col, 0));
+                    h->launches += update(ln, ln.side, Lt, np * CH_NB, g0, 3, ng);
+                    h->launches += update(ln, ln.main, Lt, np * CH_NB, g0, 4, ng);
                     CUDA_TRY(cudaEventRecord(ln.ev_col, ln.main));
-                    CUDA_TRY(cudaStreamWaitEvent(ln.side, ln.ev_col, 0));
-                    h->launches += update(ln, ln.main, Lt, np * CH_NB, g0, 2, ng);
                 }
             }
         }
