@@ -27,9 +27,10 @@
  * may return before the device work finishes; device inputs must stay alive until the stream reaches that
  * point.  Host input arrays are consumed before the call returns.  rpa_ec_q and rpa_chi0_sync block.
  *
- * Internal resources: besides the workspace the handle owns three CUDA streams (used by rpa_ec_q: two of high priority
- * to factor panels ahead of the trailing updates, one for the second half of the matrices, which is factorised
- * concurrently with the first; all ordered with the caller's stream by events) and a few events, all released by
+ * Internal resources: besides the workspace the handle owns seven CUDA streams (used by rpa_ec_q: a high-priority
+ * stream per lane for the look-ahead update, panels and strips, which run ahead of the big trailing updates, and a
+ * main stream for each lane but the first, which uses the caller's; a lane factorises its share of the frequencies
+ * concurrently with the others; all ordered with the caller's stream by events) and a few events, all released by
  * rpa_chi0_destroy.  The rank-K accumulation (Eq. 17) of a batch with ng >= 768 and >= 1024 transitions runs on the
  * int8 tensor cores: every FP64 operand row is scaled by a power of two and cut into 7 signed 7-bit digits, the digit
  * products are exact (s32), the recombination is FP64; chi0 then agrees with the FP64 tensor kernel to ~1e-14 relative
@@ -38,8 +39,8 @@
  * (~1e-16 relative), not bitwise.  Environment, read by rpa_chi0_create: RPA_RANK_K_FP64=1 keeps every batch on the FP64
  * tensor cores (3-multiplication kernel), RPA_RANK_K_4M=1 on the 4-multiplication FP64 kernel; RPA_RANK_K_I8=1 sends
  * small batches to the int8 kernel too; RPA_RANK_K_I8_DIGITS=6 uses 6 digits (41-bit operands, ~3e-12, 25 % fewer MMAs);
- * RPA_RANK_K_I8_NOCLUSTER=1 launches the int8 kernel without thread-block clusters.  Read by rpa_ec_q: RPA_EC_LANES=1
- * factorises all frequencies of a group in one lane (default: two concurrent halves).
+ * RPA_RANK_K_I8_NOCLUSTER=1 launches the int8 kernel without thread-block clusters.  Read by rpa_ec_q: RPA_EC_LANES=n
+ * (1 ... 4) factorises the frequencies of a group in n concurrent lanes (default 2).
  *
  * Errors: every int-returning call gives 0 on success or a negative RPA_ERR_* code; rpa_last_error() holds
  * a thread-local message.  Nothing is thrown across the ABI.  A handle is not thread-safe; distinct handles

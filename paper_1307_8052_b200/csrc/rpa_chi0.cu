@@ -50,6 +50,8 @@ constexpr int I8_MIN_NG = 768, I8_MIN_K = 1024;  // below: the FP64 tensor kerne
 constexpr int MAX_BANDS = 1 << 17;     // eps/f scratch
 constexpr int MAX_ATOMS = 4096;
 constexpr int MAX_PROJ = 1 << 16;
+constexpr int EC_DEFAULT_LANES = 2;
+constexpr int EC_MAX_LANES = 4;       // concurrent shares of a group in rpa_ec_q
 constexpr int EC_GROUP = 16;           // frequencies factorised together in rpa_ec_q
 constexpr size_t I_BUDGET = (size_t)4 << 30; // pruned intermediate of a whole batch when it fits (fewer, larger launches beat L2 residency)
 constexpr int NSTAGE = 6;
@@ -219,8 +221,9 @@ struct rpa_chi0 {
     bool use_3m = true;                // rank_k3m_kernel (3-multiplication complex product) for the chi0 accumulation
     cudaStream_t side = nullptr;       // panel factorisations of rpa_ec_q run here, ahead of the trailing updates
     cudaEvent_t ev_panel[2] = {nullptr, nullptr}, ev_col = nullptr, ev_fork = nullptr;
-    cudaStream_t main2 = nullptr, side2 = nullptr;   // second lane of rpa_ec_q (half of the matrices of a group)
-    cudaEvent_t ev_panel2[2] = {nullptr, nullptr}, ev_col2 = nullptr, ev_join = nullptr;
+    // further lanes of rpa_ec_q (each factorises its share of the matrices of a group on its own stream pair)
+    cudaStream_t xmain[EC_MAX_LANES - 1] = {}, xside[EC_MAX_LANES - 1] = {};
+    cudaEvent_t xev_panel[EC_MAX_LANES - 1][2] = {}, xev_col[EC_MAX_LANES - 1] = {}, xev_join[EC_MAX_LANES - 1] = {};
     size_t zy_smem = 0;
     unsigned char *ws;
     // profiling
@@ -507,11 +510,14 @@ int create_impl(rpa_chi0_t **out, const int32_t grid[3], const double cell[9], c
         int prio_lo = 0, prio_hi = 0;
         CREATE_TRY(cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi));
         CREATE_TRY(cudaStreamCreateWithPriority(&h->side, cudaStreamNonBlocking, prio_hi));
-        CREATE_TRY(cudaStreamCreateWithPriority(&h->side2, cudaStreamNonBlocking, prio_hi));
-        CREATE_TRY(cudaStreamCreateWithPriority(&h->main2, cudaStreamNonBlocking, prio_lo));
-        for (cudaEvent_t *e : {&h->ev_panel[0], &h->ev_panel[1], &h->ev_col, &h->ev_fork, &h->ev_panel2[0], &h->ev_panel2[1],
-                               &h->ev_col2, &h->ev_join})
+        for (cudaEvent_t *e : {&h->ev_panel[0], &h->ev_panel[1], &h->ev_col, &h->ev_fork})
             CREATE_TRY(cudaEventCreateWithFlags(e, cudaEventDisableTiming));
+        for (int l = 0; l < EC_MAX_LANES - 1; l++) {
+            CREATE_TRY(cudaStreamCreateWithPriority(&h->xside[l], cudaStreamNonBlocking, prio_hi));
+            CREATE_TRY(cudaStreamCreateWithPriority(&h->xmain[l], cudaStreamNonBlocking, prio_lo));
+            for (cudaEvent_t *e : {&h->xev_panel[l][0], &h->xev_panel[l][1], &h->xev_col[l], &h->xev_join[l]})
+                CREATE_TRY(cudaEventCreateWithFlags(e, cudaEventDisableTiming));
+        }
     }
     if (h->zy_kernel) {
         CREATE_TRY(cudaFuncSetAttribute(h->zy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->zy_smem));
@@ -1003,21 +1009,29 @@ int ec_q_impl(rpa_chi0_t *h, const double *v_G, int iw_begin, int iw_end, double
         // updated on the high-priority side stream, which then runs the whole next block (panels and strips: the serial,
         // latency-bound chain) while the rest of the update proceeds on the main stream.  Two block buffers of Lt alternate
         // (block b + 2 starts after the look-ahead of block b + 1, which waits for the big update of block b).
-        // Two lanes: the group's matrices are split in halves that run the same schedule on their own pair of streams.
+        // Lanes: the group's matrices are split in shares that run the same schedule on their own pair of streams.
         // The panel steps are latency-bound (one warp factors the diagonal block, few CTAs), the trailing updates are
-        // throughput-bound: with two independent halves in flight one half's updates fill the SMs while the other
-        // half is in its panel steps.  `RPA_EC_LANES=1` keeps everything on one lane.
+        // throughput-bound: with independent shares in flight one share's updates fill the SMs while another is in
+        // its panel steps.  Two lanes by default; `RPA_EC_LANES=n` (1 ... 4) chooses (measured on 16 matrices of 1200
+        // with the whole-block look-ahead: 2.68 / 2.66 / 2.64 / 2.63 ms for 1 / 2 / 3 / 4 lanes: the chain of a lane
+        // does not get shorter, so more lanes add little).
         const int64_t lt_mat = (int64_t)CH_P * CH_NB * L.ldn;          // per matrix
         const size_t lt_block = (size_t)L.ec_group * lt_mat;           // per block buffer
         const double *wneg = h->ptr<double>(L.wneg);
         const char *lanes_env = getenv("RPA_EC_LANES");
-        const int n_lanes = (nm >= 2 && !(lanes_env && atoi(lanes_env) == 1)) ? 2 : 1;
+        const int want = lanes_env ? atoi(lanes_env) : EC_DEFAULT_LANES;
+        const int n_lanes = std::max(1, std::min({want, EC_MAX_LANES, nm}));
         struct Lane {
             cudaStream_t main, side;
             cudaEvent_t *ev_panel, ev_col;
             int m0, nm;
-        } lanes[2] = {{st, h->side, h->ev_panel, h->ev_col, 0, n_lanes == 2 ? (nm + 1) / 2 : nm},
-                      {h->main2, h->side2, h->ev_panel2, h->ev_col2, (nm + 1) / 2, nm / 2}};
+        } lanes[EC_MAX_LANES];
+        for (int l = 0, m0 = 0; l < n_lanes; l++) {   // matrices dealt as evenly as possible
+            const int cnt = nm / n_lanes + (l < nm % n_lanes ? 1 : 0);
+            if (l == 0) lanes[l] = {st, h->side, h->ev_panel, h->ev_col, m0, cnt};
+            else lanes[l] = {h->xmain[l - 1], h->xside[l - 1], h->xev_panel[l - 1], h->xev_col[l - 1], m0, cnt};
+            m0 += cnt;
+        }
         auto update = [&](const Lane &ln, cudaStream_t s_, cd *Lt, int K, int g0, int mode, int col_limit) {
             const int rest = ng - g0;
             if (rest <= 0) return 0;
@@ -1067,9 +1081,9 @@ int ec_q_impl(rpa_chi0_t *h, const double *v_G, int iw_begin, int iw_end, double
                 }
             }
         }
-        if (n_lanes == 2) {   // join: the caller's stream continues after the second lane
-            CUDA_TRY(cudaEventRecord(h->ev_join, lanes[1].main));
-            CUDA_TRY(cudaStreamWaitEvent(st, h->ev_join, 0));
+        for (int l = 1; l < n_lanes; l++) {   // join: the caller's stream continues after the other lanes
+            CUDA_TRY(cudaEventRecord(h->xev_join[l - 1], lanes[l].main));
+            CUDA_TRY(cudaStreamWaitEvent(st, h->xev_join[l - 1], 0));
         }
         CUDA_TRY(cudaGetLastError());
         ec_collect_kernel<<<1, 32, 0, st>>>(d_ld, d_tr, nm, iw0, d_e);
@@ -1153,11 +1167,15 @@ int rpa_chi0_accumulators(const rpa_chi0_t *h, void **S, size_t *bytes) {
 
 void rpa_chi0_destroy(rpa_chi0_t *h) {
     if (!h) return;
-    for (cudaStream_t s_ : {h->side, h->side2, h->main2})
-        if (s_) cudaStreamDestroy(s_);
-    for (cudaEvent_t e : {h->ev_panel[0], h->ev_panel[1], h->ev_col, h->ev_fork, h->ev_panel2[0], h->ev_panel2[1], h->ev_col2,
-                          h->ev_join})
+    if (h->side) cudaStreamDestroy(h->side);
+    for (cudaEvent_t e : {h->ev_panel[0], h->ev_panel[1], h->ev_col, h->ev_fork})
         if (e) cudaEventDestroy(e);
+    for (int l = 0; l < EC_MAX_LANES - 1; l++) {
+        for (cudaStream_t s_ : {h->xside[l], h->xmain[l]})
+            if (s_) cudaStreamDestroy(s_);
+        for (cudaEvent_t e : {h->xev_panel[l][0], h->xev_panel[l][1], h->xev_col[l], h->xev_join[l]})
+            if (e) cudaEventDestroy(e);
+    }
     for (auto &ev : h->events) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
     for (auto &e : h->pool) cudaEventDestroy(e);
     delete h;
