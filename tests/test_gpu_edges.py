@@ -203,6 +203,36 @@ def test_ec_q_range_partial_sums_and_isolation():
         h.close()
 
 
+def test_ec_q_lanes_give_the_same_numbers(monkeypatch):
+    """rpa_ec_q factorises the frequencies of a group in 1 ... 4 concurrent lanes (include/rpa_chi0.h, RPA_EC_LANES):
+    every matrix goes through the same arithmetic whichever lane it is in, so e(omega) must agree bit for bit, for an
+    even split, a ragged one (8 frequencies in 3 lanes) and more lanes than frequencies (a range of 2).  nG = 401
+    (configs[2]) spans four 128-column blocks with a ragged last one: look-ahead and big updates both run."""
+    import torch
+    from paper_1307_8052_b200 import binding as B
+    for cfg, n_unocc in ((W.CONFIGS[0], None), (W.CONFIGS[2], 24)):
+        h = _handle(cfg)
+        try:
+            kd = W.kpoint(cfg, 0) if n_unocc is None else W.kpoint(cfg, 0, unocc=range(n_unocc))
+            g, K2 = B.rpa_chi0_gvectors(h)
+            Qd = torch.from_numpy(W.paw_Q(cfg, K2)).to("cuda:0")
+            B.add_kpoint_host(h, kd, cfg.n_proj, Qd, W.atom_positions(cfg))
+            v = W.coulomb(K2)
+            ref = None
+            for lanes in ("1", "2", "3", "4"):
+                monkeypatch.setenv("RPA_EC_LANES", lanes)
+                ec, e = B.rpa_ec_q(h, v)
+                ec2, e2 = B.rpa_ec_q_range(h, v, 1, 3)
+                if ref is None:
+                    ref = (ec, e, ec2, e2)
+                    assert np.all(np.isfinite(e)) and np.all(e < 0.0)
+                else:
+                    assert ec == ref[0] and np.array_equal(e, ref[1])
+                    assert ec2 == ref[2] and np.array_equal(e2, ref[3])
+        finally:
+            h.close()
+
+
 def test_int8_tcgen05_probe_self_check():
     """rpa_probe_int8_tensor_peak: the TMEM read-back of one tcgen05.mma.kind::i8 equals the host product bit for bit,
     and the issue rate is in the range of a Blackwell int8 tensor pipe (legacy mma.sync reaches 1.1 Pop/s)."""
