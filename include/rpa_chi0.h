@@ -31,16 +31,14 @@
  * stream per lane for the look-ahead update, panels and strips, which run ahead of the big trailing updates, and a
  * main stream for each lane but the first, which uses the caller's; a lane factorises its share of the frequencies
  * concurrently with the others; all ordered with the caller's stream by events) and a few events, all released by
- * rpa_chi0_destroy.  The rank-K accumulation (Eq. 17) of a batch with ng >= 768 and >= 1024 transitions runs on the
- * int8 tensor cores: every FP64 operand row is scaled by a power of two and cut into 7 signed 7-bit digits, the digit
- * products are exact (s32), the recombination is FP64; chi0 then agrees with the FP64 tensor kernel to ~1e-14 relative
- * Frobenius norm and is bitwise reproducible.  Smaller batches run on the FP64 tensor cores; when that kernel splits K
- * over several CTAs per tile (chosen by the library) the tile sums use floating-point atomics: reproducible to rounding
- * (~1e-16 relative), not bitwise.  Environment, read by rpa_chi0_create: RPA_RANK_K_FP64=1 keeps every batch on the FP64
- * tensor cores (3-multiplication kernel), RPA_RANK_K_4M=1 on the 4-multiplication FP64 kernel; RPA_RANK_K_I8=1 sends
- * small batches to the int8 kernel too; RPA_RANK_K_I8_DIGITS=6 uses 6 digits (41-bit operands, ~3e-12, 25 % fewer MMAs);
- * RPA_RANK_K_I8_NOCLUSTER=1 launches the int8 kernel without thread-block clusters.  Read by rpa_ec_q: RPA_EC_LANES=n
- * (1 ... 4) factorises the frequencies of a group in n concurrent lanes (default 2).
+ * rpa_chi0_destroy.
+ *
+ * Arithmetic: everything is FP64 / complex128 ("Double and double complex precision").  The rank-K accumulation
+ * (Eq. 17 / Eq. 20) runs on the FP64 tensor cores (DMMA) by default; when that kernel splits K over several CTAs per
+ * tile (chosen by the library) the tile sums use floating-point atomics: chi0 is then reproducible to rounding (~1e-16
+ * relative), not bitwise.  rpa_chi0_set_rank_k_mode selects other kernels per handle, among them an opt-in int8-sliced
+ * emulation with a stated error bound.  The library reads no environment variables and keeps no global state besides the
+ * thread-local error string.
  *
  * Errors: every int-returning call gives 0 on success or a negative RPA_ERR_* code; rpa_last_error() holds
  * a thread-local message.  Nothing is thrown across the ABI.  A handle is not thread-safe; distinct handles
@@ -158,6 +156,55 @@ int rpa_ec_q(rpa_chi0_t *h, const double *v_G, double *ec_ha, double *e_omega);
 int rpa_ec_q_range(rpa_chi0_t *h, const double *v_G, int32_t iw_begin, int32_t iw_end, double *ec_partial_ha,
                    double *e_omega);
 
+/*
+ * Kernel of the rank-K accumulation S_w += N diag(w) N^H (Eq. 17 / Eq. 20; Table 1 step 11) used by
+ * the later rpa_chi0_add_kpoint* calls on this handle.  mode = one RPA_RANK_K_* kind, for RPA_RANK_K_I8 optionally or-ed
+ * with RPA_RANK_K_FLAG_* bits.
+ *   RPA_RANK_K_FP64_3M (default): FP64 tensor cores (DMMA.8x8x4), complex product by three real contractions
+ *       (Re = P1 + P2, Im = P3 - P1 + P2): IEEE double throughout, error ~ K u |n||n'| per element like any FP64 ZHERK.
+ *   RPA_RANK_K_FP64_4M: FP64 tensor cores, the plain four-multiplication real view (the reference form of the update).
+ *   RPA_RANK_K_I8: for batches with ng >= 768 and >= 1024 transitions, the update is computed on the int8 tensor cores
+ *       (tcgen05.mma.kind::i8, s32 accumulators in TMEM) from digit slices of the FP64 operands (Ozaki scheme): every
+ *       row g of N, and every row g' of N diag(w) per frequency, is scaled by a power of two 2^-e > its largest
+ *       |component| and rounded ONCE to b = 6 + 7 (digits - 1) bits of that scale (digits = 6, 7, 8: b = 41, 48, 55),
+ *       the digit products are exact, those below the rounding are dropped, the recombination is FP64.  Error bound per
+ *       element, with sL_g = 2^e of row g of N and sR_g' that of row g' of N diag(w), K' = 2 K:
+ *           |dS[g][g']| <= (digits + 2) 2^(-7 digits) sL_g sR_g' K'
+ *       (first-order: 2 roundings of 2^(-7 digits + 1) / 2 per product plus the digits - 1 dropped pair levels of
+ *       2^(-7 digits) each).  It is an ABSOLUTE bound on the scale of the row maxima: an element that is 2^-20 of its row
+ *       maximum keeps b - 20 bits, where IEEE double keeps 53 -- narrower than FP64 for rows with a wide dynamic range
+ *       (tests/test_gpu_rank_k_i8.py checks this bound element by element on such rows).  Measured on BASELINE configs:
+ *       1-5e-14 (digits = 7), 1-3e-12 (6) relative Frobenius distance from the FP64 kernel.  Bitwise reproducible.  Smaller
+ *       batches, batches where digits 2 K' 64^2 >= 2^31 (s32 accumulators no longer provably exact: more than 37 448 /
+ *       32 768 transitions per batch for 7 / 8 digits), and handles with more than 32 accumulator slots run the default
+ *       FP64 kernel.  A NaN or Inf in N or w makes the rows / columns of S it enters non-finite, as in the FP64 kernels.
+ *       digits: 6, 7 or 8 (0 = 7); ignored by the FP64 modes.
+ *   RPA_RANK_K_FLAG_ALL_BATCHES: take the int8 path for small batches too (tests; it loses time there).
+ *   RPA_RANK_K_FLAG_NO_CLUSTER: launch rank_k_i8_kernel without thread-block clusters (no multicast of the row digits).
+ * May be called at any time between calls on the handle; RPA_ERR_INVALID_ARG on unknown modes / flags / digits.
+ */
+#define RPA_RANK_K_FP64_3M 0
+#define RPA_RANK_K_FP64_4M 1
+#define RPA_RANK_K_I8 2
+#define RPA_RANK_K_FLAG_NO_CLUSTER 0x100
+#define RPA_RANK_K_FLAG_ALL_BATCHES 0x200
+int rpa_chi0_set_rank_k_mode(rpa_chi0_t *h, int32_t mode, int32_t digits);
+
+/* How many rank-K batches have run on the FP64 tensor kernels and on the int8-sliced kernel since create (which path a
+ * batch took is otherwise invisible: the results agree to the bound above). */
+int rpa_chi0_rank_k_batches(const rpa_chi0_t *h, int64_t *fp64_batches, int64_t *i8_batches);
+
+/* rpa_ec_q factorises the frequencies of a group in n_lanes (1 ... 4, default 2) concurrent shares, each on its own pair
+ * of internal streams.  e(omega) does not depend on it (every matrix is factorised by the same kernels in the same order). */
+int rpa_chi0_set_ec_lanes(rpa_chi0_t *h, int32_t n_lanes);
+
+/*
+ * E_c = sum_q w_q E_c(q): the sum over the irreducible-zone q-points of Eq. 1 (reading A17:
+ * rpa_ec_q applies no q weight).  ec_q, q_weights: host double [n_q]; ec_ha: host double[1].  Host arithmetic on the n_q
+ * scalars, summed in the order given; n_q = 0 gives 0.
+ */
+int rpa_total_energy(int32_t n_q, const double *ec_q, const double *q_weights, double *ec_ha);
+
 /* Zero the accumulators (start another q with the same sphere). */
 int rpa_chi0_reset(rpa_chi0_t *h);
 
@@ -167,8 +214,8 @@ int rpa_chi0_sync(rpa_chi0_t *h);
 /*
  * Per-stage device times (ms, CUDA events on the handle's stream) accumulated by rpa_chi0_add_kpoint while
  * profiling is on: [0] pair product + 2-D FFT, [1] third-axis DFT + sphere gather, [2] PAW, [3] weights,
- * [4] rank-K update (all its kernels), [5] the rank_k_i8_kernel launches alone (part of [4]; 0 when the FP64 tensor
- * kernel ran); launches[6] = kernel launches per stage.  Turning profiling on adds event records only.
+ * [4] rank-K update (all its kernels), [5] the rank_k_i8_kernel launches alone (a SUBSET of [4], not a further stage; 0
+ * when the FP64 tensor kernel ran); launches[6] = kernel launches per stage.  Turning profiling on adds event records only.
  */
 int rpa_chi0_set_profiling(rpa_chi0_t *h, int32_t on);
 int rpa_chi0_stage_times(rpa_chi0_t *h, double ms[6], int64_t launches[6]);
@@ -246,18 +293,6 @@ int rpa_chi0_add_kpoint_optical(rpa_chi0_t *h, double kweight, int32_t n_occ, co
 int rpa_chi0_set_spin_degeneracy(rpa_chi0_t *h, int32_t s);
 
 void rpa_chi0_destroy(rpa_chi0_t *h);
-
-/* Register-only DMMA issue-rate probe: runs `iters` dependent-free mma.sync.m8n8k4.f64 per warp on every SM and
- * returns the achieved FP64 tensor TFLOP/s (the measured roofline denominator of the rank-K update).  The one
- * call that allocates (and frees) 64 bytes of device memory itself: it has no handle and no workspace. */
-int rpa_probe_fp64_tensor_peak(void *cuda_stream, double *tflops);
-
-/* tcgen05 int8 issue-rate probe (the denominator of the planned int8-sliced rank-K update): on every SM
- * one thread issues 20000 accumulating tcgen05.mma.kind::i8 of 128 x 256 x 32 (operands in shared memory, s32
- * accumulator in TMEM); returns the achieved int8 Top/s in *tops.  The first MMA of CTA 0 is read back from TMEM and
- * compared with the host product of the same seeded operands: *mismatches = number of wrong elements of 32768 (0 on a
- * working path).  Allocates and frees 140 KB of device memory itself; blocks. */
-int rpa_probe_int8_tensor_peak(void *cuda_stream, double *tops, int32_t *mismatches);
 
 /* Thread-local message of the last error on this thread (static storage, never NULL). */
 const char *rpa_last_error(void);

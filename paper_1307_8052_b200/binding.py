@@ -24,11 +24,18 @@ RPA_ERR_NOT_PD = -5
 EXPORTS = (
     "rpa_chi0_workspace_bytes", "rpa_chi0_create", "rpa_chi0_ng", "rpa_chi0_gvectors", "rpa_chi0_add_kpoint",
     "rpa_chi0_get", "rpa_ec_q", "rpa_chi0_reset", "rpa_chi0_sync", "rpa_chi0_set_profiling", "rpa_chi0_stage_times",
-    "rpa_chi0_launch_count", "rpa_chi0_accumulators", "rpa_chi0_destroy", "rpa_probe_fp64_tensor_peak", "rpa_last_error",
+    "rpa_chi0_launch_count", "rpa_chi0_accumulators", "rpa_chi0_destroy", "rpa_last_error",
     "rpa_pw_to_grid", "rpa_symmetry_remap", "rpa_momentum_pw", "rpa_chi0_add_kpoint_optical",
     "rpa_chi0_set_spin_degeneracy", "rpa_chi0_create_real_axis", "rpa_ec_q_range",
-    "rpa_probe_int8_tensor_peak",
+    "rpa_chi0_set_rank_k_mode", "rpa_chi0_rank_k_batches", "rpa_chi0_set_ec_lanes", "rpa_total_energy",
 )
+
+# rpa_chi0_set_rank_k_mode (include/rpa_chi0.h)
+RPA_RANK_K_FP64_3M = 0
+RPA_RANK_K_FP64_4M = 1
+RPA_RANK_K_I8 = 2
+RPA_RANK_K_FLAG_NO_CLUSTER = 0x100
+RPA_RANK_K_FLAG_ALL_BATCHES = 0x200
 
 STAGE_NAMES = ("pair_product_fft_yz", "fft_x_gather", "paw", "weights", "rank_k", "rank_k_i8_mma")
 
@@ -90,10 +97,14 @@ def lib():
     L.rpa_chi0_accumulators.argtypes = [vp, C.POINTER(vp), C.POINTER(sz)]
     L.rpa_chi0_destroy.restype = None
     L.rpa_chi0_destroy.argtypes = [vp]
-    L.rpa_probe_fp64_tensor_peak.restype = C.c_int
-    L.rpa_probe_fp64_tensor_peak.argtypes = [vp, C.POINTER(f64)]
-    L.rpa_probe_int8_tensor_peak.restype = C.c_int
-    L.rpa_probe_int8_tensor_peak.argtypes = [vp, C.POINTER(f64), C.POINTER(i32)]
+    L.rpa_chi0_set_rank_k_mode.restype = C.c_int
+    L.rpa_chi0_set_rank_k_mode.argtypes = [vp, i32, i32]
+    L.rpa_chi0_rank_k_batches.restype = C.c_int
+    L.rpa_chi0_rank_k_batches.argtypes = [vp, C.POINTER(i64), C.POINTER(i64)]
+    L.rpa_chi0_set_ec_lanes.restype = C.c_int
+    L.rpa_chi0_set_ec_lanes.argtypes = [vp, i32]
+    L.rpa_total_energy.restype = C.c_int
+    L.rpa_total_energy.argtypes = [i32, vp, vp, C.POINTER(f64)]
     L.rpa_pw_to_grid.restype = C.c_int
     L.rpa_pw_to_grid.argtypes = [vp, i32, i32, vp, vp, vp]
     L.rpa_symmetry_remap.restype = C.c_int
@@ -322,12 +333,29 @@ def rpa_chi0_set_spin_degeneracy(h: Handle, s: int):
 
 
 def rpa_total_energy(ec_q, q_weights) -> float:
-    """E_c = sum_q w_q E_c(q) (Eq. 1): the outer q loop's final sum over the IBZ weights (host arithmetic on the
-    per-q scalars the library returns; the per-q work is rpa_chi0_* / rpa_ec_q)."""
-    e, w = _np(ec_q, np.float64), _np(q_weights, np.float64)
+    """E_c = sum_q w_q E_c(q) (Eq. 1): the outer q loop's final sum over the IBZ weights, by the library."""
+    e, w = _np(ec_q, np.float64).reshape(-1), _np(q_weights, np.float64).reshape(-1)
     if e.shape != w.shape:
         raise ValueError("one weight per q-point")
-    return float(np.dot(w, e))
+    out = C.c_double(0.0)
+    _check(lib().rpa_total_energy(int(e.size), _hp(e), _hp(w), C.byref(out)))
+    return float(out.value)
+
+
+def rpa_chi0_set_rank_k_mode(h: Handle, mode: int, digits: int = 0):
+    """mode: RPA_RANK_K_FP64_3M (default of the library) / RPA_RANK_K_FP64_4M / RPA_RANK_K_I8 [| RPA_RANK_K_FLAG_*]."""
+    _check(lib().rpa_chi0_set_rank_k_mode(h.ptr, int(mode), int(digits)))
+
+
+def rpa_chi0_rank_k_batches(h: Handle):
+    """(batches run on the FP64 tensor kernels, batches run on the int8-sliced kernel) since create."""
+    a, b = C.c_int64(0), C.c_int64(0)
+    _check(lib().rpa_chi0_rank_k_batches(h.ptr, C.byref(a), C.byref(b)))
+    return int(a.value), int(b.value)
+
+
+def rpa_chi0_set_ec_lanes(h: Handle, n_lanes: int):
+    _check(lib().rpa_chi0_set_ec_lanes(h.ptr, int(n_lanes)))
 
 
 def rpa_chi0_sync(h: Handle):
@@ -420,23 +448,6 @@ def rpa_momentum_pw(h: Handle, k_cart, g_pw, C_occ, C_unocc, n_proj=None, P_occ=
 
 def rpa_chi0_destroy(h: Handle):
     h.close()
-
-
-def rpa_probe_fp64_tensor_peak(device="cuda:0") -> float:
-    torch = _torch()
-    with torch.cuda.device(torch.device(device)):
-        t = C.c_double(0.0)
-        _check(lib().rpa_probe_fp64_tensor_peak(C.c_void_p(torch.cuda.current_stream().cuda_stream), C.byref(t)))
-    return float(t.value)
-
-
-def rpa_probe_int8_tensor_peak(device="cuda:0"):
-    """(int8 tcgen05 Top/s, mismatches of the self-checked first MMA)."""
-    torch = _torch()
-    with torch.cuda.device(torch.device(device)):
-        t, bad = C.c_double(0.0), C.c_int32(-1)
-        _check(lib().rpa_probe_int8_tensor_peak(C.c_void_p(torch.cuda.current_stream().cuda_stream), C.byref(t), C.byref(bad)))
-    return float(t.value), int(bad.value)
 
 
 # ---- host-buffer convenience on top of the calls above (the end-to-end path bench.py times) ------------------

@@ -19,8 +19,9 @@
 #include "probe_i8.cuh"
 
 namespace rki8 {
-// S = digits per operand: 6 + 7 (S - 1) bits.  S = 7 (48 bits): the result agrees with the FP64 tensor path to FP64
-// rounding (~1e-14 relative Frobenius); S = 6 (41 bits): ~3e-12, 3/4 of the MMAs.
+// S = digits per operand: 6 + 7 (S - 1) bits of the row's power-of-two scale.  S = 7 (48 bits): agrees with the FP64 tensor
+// path to ~1e-14 relative Frobenius; S = 6 (41 bits): ~3e-12, 3/4 of the MMAs; S = 8 (55 bits: every element within 2^-2 of
+// its row maximum is sliced without any rounding; 36 digit products instead of 28, all 512 TMEM columns).
 constexpr int RB = 128, CB = 64;     // rows / columns of a CTA tile
 constexpr int KB = 32;               // K' entries (bytes) per MMA
 constexpr int A_BYTES = RB * KB, B_BYTES = CB * KB;
@@ -31,8 +32,13 @@ constexpr int THREADS = 192;         // warps 0-3: epilogue (TMEM lanes), warp 4
 constexpr uint32_t IDESC = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(CB >> 3) << 17) | ((uint32_t)(RB >> 4) << 24);
 }  // namespace rki8
 
-__device__ __forceinline__ double rki8_pow2_scale(double m) {   // 2^-e with 2^e > m (1 for m = 0)
-    return m > 0.0 ? scalbn(1.0, -(ilogb(m) + 1)) : 1.0;
+// 2^-e with 2^e > m (1 for m = 0).  A subnormal maximum would need 2^-e > 2^1023: the exponent is clamped there (the row is
+// then sliced against a scale up to 2^51 too large: it keeps the bits above 2^-1078, i.e. all that a subnormal has).
+// m = +Inf marks a row that holds a NaN or an Inf (rki8_rowmax_kernel): its scale is NaN, which the epilogue multiplies
+// into every element of that row / column of S -- the FP64 tensor kernels propagate non-finite inputs the same way.
+__device__ __forceinline__ double rki8_pow2_scale(double m) {
+    if (!(m < __longlong_as_double(0x7ff0000000000000ll))) return __longlong_as_double(0x7ff8000000000000ll);
+    return m > 0.0 ? scalbn(1.0, min(1023, -(ilogb(m) + 1))) : 1.0;
 }
 
 // Row maxima: mx[0][g] = max_p max(|Re|, |Im|) of Nb, mx[1 + iw][g] = max_p |w[iw][p]| max(|Re|, |Im|), as the bit patterns
@@ -50,18 +56,23 @@ __global__ void __launch_bounds__(128) rki8_rowmax_kernel(const cd *__restrict__
     for (int i = 0; i < RKI8_MAXW; i++) mw[i] = 0.0;
     for (int p = p_lo; p < p_hi; p++) {
         const cd v = Nb[(size_t)p * ldn + g];
-        const double an = fmax(fabs(v.x), fabs(v.y));
+        // fmax drops NaN operands: a NaN (or Inf) anywhere in the row must surface as a +Inf maximum instead
+        const double inf = __longlong_as_double(0x7ff0000000000000ll);
+        const double an = (v.x != v.x || v.y != v.y) ? inf : fmax(fabs(v.x), fabs(v.y));
         m0 = fmax(m0, an);
 #pragma unroll
         for (int i = 0; i < RKI8_MAXW; i++)
-            if (i < n_w) mw[i] = fmax(mw[i], fabs(w[(size_t)i * ldw + p]) * an);
+            if (i < n_w) {
+                const double t = fabs(w[(size_t)i * ldw + p]) * an;   // NaN weight, or 0 * Inf: NaN
+                mw[i] = fmax(mw[i], t != t ? inf : t);
+            }
     }
     atomicMax(&mx[g], (unsigned long long)__double_as_longlong(m0));
 #pragma unroll
     for (int i = 0; i < RKI8_MAXW; i++)
         if (i < n_w) atomicMax(&mx[(size_t)(1 + i) * ngp + g], (unsigned long long)__double_as_longlong(mw[i]));
 }
-// inv[i] = 2^-e with 2^e > max (in place over the bit patterns).  grid ceil(n/256), block 256.
+// inv[i] = 2^-e with 2^e > max, NaN for a non-finite row (in place over the bit patterns).  grid ceil(n/256), block 256.
 __global__ void rki8_scale_finish_kernel(unsigned long long *__restrict__ mx, int n) {
     const int i = blockIdx.x * 256 + threadIdx.x;
     if (i >= n) return;

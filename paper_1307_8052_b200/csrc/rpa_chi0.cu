@@ -23,7 +23,6 @@
 #include "paw.cuh"
 #include "rank_k.cuh"
 #include "rank_k3m.cuh"
-#include "probe_i8.cuh"
 #include "rank_k_i8.cuh"
 
 namespace {
@@ -213,12 +212,16 @@ struct rpa_chi0 {
     double spin_deg = 2.0;             // prefactor s of chi0 = (s/Omega) S: 2 spin-paired (A3), 1 per explicit spin channel
     bool q0 = false;                   // q = 0: pair densities need the optical-limit head (rpa_chi0_add_kpoint_optical)
     int idx0 = -1;                     // sphere index of G = 0 when q0
-    bool use_i8 = false;               // RPA_RANK_K_I8: int8-sliced rank-K on tcgen05 (rank_k_i8.cuh)
+    // rank-K kernel of the chi0 accumulation (rpa_chi0_set_rank_k_mode; default: FP64 tensor cores, 3-multiplication)
+    bool use_i8 = false;               // RPA_RANK_K_I8: int8-sliced rank-K on tcgen05 (rank_k_i8.cuh) for large batches
     int i8_digits = 7;
-    bool i8_cluster = true;            // clusters of 2 CTAs multicast the row-block digits (RPA_RANK_K_I8_NOCLUSTER=1: off)
-    bool i8_force = false;             // RPA_RANK_K_I8=1: also for small batches (tests)
+    bool i8_cluster = true;            // clusters of 2 CTAs multicast the row-block digits (RPA_RANK_K_FLAG_NO_CLUSTER: off)
+    bool i8_force = false;             // RPA_RANK_K_FLAG_ALL_BATCHES: also for batches below I8_MIN_NG / I8_MIN_K
+    bool i8_attr_set = false;          // cudaFuncSetAttribute done for the rank_k_i8_kernel instances
     std::vector<int2> i8_tiles;        // (row block, column block) tiles that meet the lower triangle
-    bool use_3m = true;                // rank_k3m_kernel (3-multiplication complex product) for the chi0 accumulation
+    bool use_3m = true;                // rank_k3m_kernel (3-multiplication complex product); false: rank_k_kernel<true> (4M)
+    int64_t i8_batches = 0, fp64_batches = 0;   // batches each rank-K path has taken (rpa_chi0_rank_k_batches)
+    int ec_lanes = EC_DEFAULT_LANES;   // rpa_chi0_set_ec_lanes
     cudaStream_t side = nullptr;       // panel factorisations of rpa_ec_q run here, ahead of the trailing updates
     cudaEvent_t ev_panel[2] = {nullptr, nullptr}, ev_col = nullptr, ev_fork = nullptr;
     // further lanes of rpa_ec_q (each factorises its share of the matrices of a group on its own stream pair)
@@ -528,30 +531,7 @@ int create_impl(rpa_chi0_t **out, const int32_t grid[3], const double cell[9], c
     }
     CREATE_TRY(cudaFuncSetAttribute(rank_k_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, rk::Cfg<true>::SMEM_BYTES));
     CREATE_TRY(cudaFuncSetAttribute(rank_k3m_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, rk3::SMEM_BYTES));
-    h->use_3m = getenv("RPA_RANK_K_4M") == nullptr;
-    // int8-sliced rank-K (rank_k_i8.cuh) unless RPA_RANK_K_FP64 / RPA_RANK_K_4M ask for the FP64 tensor kernels; batches
-    // too small to pay for the slicing passes take the FP64 kernel anyway (I8_MIN_NG, I8_MIN_K below)
-    h->use_i8 = getenv("RPA_RANK_K_FP64") == nullptr && getenv("RPA_RANK_K_4M") == nullptr;
-    h->i8_cluster = getenv("RPA_RANK_K_I8_NOCLUSTER") == nullptr;
-    if (h->use_i8) {
-        const int ng_ = h->sp.ng, ngp = (ng_ + rki8::RB - 1) / rki8::RB * rki8::RB;
-        for (int rb = 0; rb < 2 * ngp / rki8::RB; rb++) {
-            const int g_lo = (rb * rki8::RB) % ngp, g_hi = std::min(g_lo + rki8::RB - 1, ng_ - 1);
-            if (g_lo >= ng_) continue;
-            int cb = 0;
-            for (; cb * rki8::CB <= g_hi; cb++) h->i8_tiles.push_back(make_int2(rb, cb));
-            // clusters of two CTAs share a row block: an odd row gets a padding tile beyond the triangle (stores nothing)
-            if (h->i8_cluster && (cb & 1)) h->i8_tiles.push_back(make_int2(rb, cb));
-        }
-        h->i8_force = getenv("RPA_RANK_K_I8") != nullptr;
-        const char *dg = getenv("RPA_RANK_K_I8_DIGITS");
-        h->i8_digits = (dg && atoi(dg) == 6) ? 6 : 7;
-        if (cudaFuncSetAttribute(rank_k_i8_kernel<6, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, rki8::smem_bytes(6)) != cudaSuccess ||
-            cudaFuncSetAttribute(rank_k_i8_kernel<7, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, rki8::smem_bytes(7)) != cudaSuccess ||
-            cudaFuncSetAttribute(rank_k_i8_kernel<6, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, rki8::smem_bytes(6)) != cudaSuccess ||
-            cudaFuncSetAttribute(rank_k_i8_kernel<7, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, rki8::smem_bytes(7)) != cudaSuccess)
-            h->use_i8 = false;
-    }
+    // the chi0 accumulation runs on the FP64 tensor cores (rank_k3m_kernel) unless rpa_chi0_set_rank_k_mode says otherwise
     CREATE_TRY(cudaFuncSetAttribute(rank_k_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, rk::Cfg<false>::SMEM_BYTES));
 
     // tables: twiddles in extended precision, box -> sphere map
@@ -629,6 +609,63 @@ int rpa_chi0_gvectors(const rpa_chi0_t *h, int32_t *g, double *K2) {
 }
 
 }  // extern "C"
+
+namespace {
+// One batch of the chi0 accumulation on the int8 tensor cores (rank_k_i8.cuh): slicing passes + rank_k_i8_kernel<S> for
+// every group of frequencies whose digit planes fit the scratch.  *done = false (nothing enqueued) when the batch cannot
+// take this path: the exactness bound S K' 64^2 < 2^31 of the s32 accumulators does not hold (K' = 2 Kpad), the scratch
+// is too small for one frequency, or there are more than RKI8_MAXW slots -- the caller then runs the FP64 tensor kernel.
+template <int S>
+int i8_batch(rpa_chi0 *h, int K, int Kpad, bool *done) {
+    *done = false;
+    const Layout &L = h->L;
+    const int ng = h->sp.ng;
+    cudaStream_t st = h->stream;
+    if ((int64_t)S * 2 * Kpad * 4096 >= ((int64_t)1 << 31)) return RPA_OK;   // s32 accumulators could overflow: not error-free
+    if (h->n_omega > RKI8_MAXW) return RPA_OK;
+    cd *Nbuf = h->ptr<cd>(L.Nbuf);
+    double *w = h->ptr<double>(L.w);
+    // scratch (the pair-density buffer I is free again): invL | invR | tiles | PL | PR of a frequency group
+    const int ngp = (ng + rki8::RB - 1) / rki8::RB * rki8::RB, nrb = 2 * ngp / rki8::RB;
+    const int ncb = (ng + rki8::CB - 1) / rki8::CB, nkb = 2 * Kpad / rki8::KB, nt = (int)h->i8_tiles.size();
+    const size_t scratch = (size_t)L.sub_pairs * L.I_pair_bytes;
+    size_t off = 0;
+    auto carve = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
+    const size_t o_invL = carve((size_t)(1 + h->n_omega) * ngp * 8), o_invR = o_invL + (size_t)ngp * 8;
+    const size_t o_tiles = carve((size_t)nt * sizeof(int2));
+    const size_t o_PL = carve((size_t)nrb * nkb * S * rki8::A_BYTES);
+    const size_t per_w = (size_t)ncb * nkb * S * rki8::B_BYTES;
+    int wg = off < scratch ? (int)std::min<size_t>((size_t)h->n_omega, (scratch - off) / per_w) : 0;
+    if (wg < 1) return RPA_OK;
+    const int ngroups = (h->n_omega + wg - 1) / wg;
+    wg = (h->n_omega + ngroups - 1) / ngroups;   // equal groups
+    unsigned char *base = h->ws + L.I;
+    double *invL = (double *)(base + o_invL), *invR = (double *)(base + o_invR);
+    int2 *d_tiles = (int2 *)(base + o_tiles);
+    int8_t *PL = (int8_t *)(base + o_PL), *PR = (int8_t *)(base + off);
+    CUDA_TRY(cudaMemcpyAsync(d_tiles, h->i8_tiles.data(), (size_t)nt * sizeof(int2), cudaMemcpyHostToDevice, st));
+    const int nmx = (1 + h->n_omega) * ngp;
+    CUDA_TRY(cudaMemsetAsync(invL, 0, (size_t)nmx * 8, st));
+    rki8_rowmax_kernel<<<dim3((ng + 127) / 128, std::max(1, std::min(64, K / 64))), 128, 0, st>>>(
+        Nbuf, L.ldn, K, ng, w, L.ldw, h->n_omega, ngp, (unsigned long long *)invL);
+    rki8_scale_finish_kernel<<<(nmx + 255) / 256, 256, 0, st>>>((unsigned long long *)invL, nmx);
+    rki8_pack_left_kernel<S><<<dim3(nkb, nrb), 128, 0, st>>>(Nbuf, L.ldn, Kpad, ng, ngp, invL, PL);
+    h->launches += 3;
+    for (int iw0 = 0; iw0 < h->n_omega; iw0 += wg) {
+        const int nw = std::min(wg, h->n_omega - iw0);
+        const double *w0 = w + (size_t)iw0 * L.ldw, *invR0 = invR + (size_t)iw0 * ngp;
+        cd *S0 = h->ptr<cd>(L.S) + (size_t)iw0 * ng * L.ldS;
+        rki8_pack_right_kernel<S><<<dim3(nkb, ncb), 64, 0, st>>>(Nbuf, L.ldn, Kpad, ng, ngp, w0, L.ldw, nw, invR0, PR);
+        StageTimer tm5(h, 5, 1);
+        CUDA_TRY(launch_i8<S>(h->i8_cluster, dim3(nt, nw), st, PL, PR, nkb, ncb, d_tiles, invL, invR0, ng, ngp, S0, L.ldS,
+                              (int64_t)ng * L.ldS));
+        h->launches += 1;
+    }
+    h->launches -= 1;   // the caller's stage timer counts one
+    *done = true;
+    return RPA_OK;
+}
+}  // namespace
 
 namespace {
 // rpa_chi0_add_kpoint, and rpa_chi0_add_kpoint_optical when grad != NULL (q = 0 handle: G = 0 element replaced)
@@ -792,55 +829,15 @@ int add_kpoint_impl(rpa_chi0_t *h, double kweight, int32_t n_occ, const void *ps
                 StageTimer tm(h, 4, 1);
                 bool done_i8 = false;
                 if (h->use_i8 && (h->i8_force || (ng >= I8_MIN_NG && K >= I8_MIN_K))) {
-                    // scratch (the pair-density buffer I is free again): invL | invR | tiles | PL | PR of a frequency group
-                    const int ngp = (ng + rki8::RB - 1) / rki8::RB * rki8::RB, nrb = 2 * ngp / rki8::RB;
-                    const int ncb = (ng + rki8::CB - 1) / rki8::CB, nkb = 2 * Kpad / rki8::KB, nt = (int)h->i8_tiles.size();
-                    const size_t scratch = (size_t)L.sub_pairs * L.I_pair_bytes;
-                    size_t off = 0;
-                    auto carve = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
-                    const size_t o_invL = carve((size_t)(1 + h->n_omega) * ngp * 8), o_invR = o_invL + (size_t)ngp * 8;
-                    const size_t o_tiles = carve((size_t)nt * sizeof(int2));
-                    const int SD = h->i8_digits;
-                    const size_t o_PL = carve((size_t)nrb * nkb * SD * rki8::A_BYTES);
-                    const size_t per_w = (size_t)ncb * nkb * SD * rki8::B_BYTES;
-                    int wg = off < scratch ? (int)std::min<size_t>((size_t)h->n_omega, (scratch - off) / per_w) : 0;
-                    if (wg >= 1 && h->n_omega <= RKI8_MAXW) {
-                        const int ngroups = (h->n_omega + wg - 1) / wg;
-                        wg = (h->n_omega + ngroups - 1) / ngroups;   // equal groups
-                        unsigned char *base = h->ws + L.I;
-                        double *invL = (double *)(base + o_invL), *invR = (double *)(base + o_invR);
-                        int2 *d_tiles = (int2 *)(base + o_tiles);
-                        int8_t *PL = (int8_t *)(base + o_PL), *PR = (int8_t *)(base + off);
-                        CUDA_TRY(cudaMemcpyAsync(d_tiles, h->i8_tiles.data(), (size_t)nt * sizeof(int2), cudaMemcpyHostToDevice, st));
-                        const int nmx = (1 + h->n_omega) * ngp;
-                        CUDA_TRY(cudaMemsetAsync(invL, 0, (size_t)nmx * 8, st));
-                        rki8_rowmax_kernel<<<dim3((ng + 127) / 128, std::max(1, std::min(64, K / 64))), 128, 0, st>>>(
-                            Nbuf, L.ldn, K, ng, w, L.ldw, h->n_omega, ngp, (unsigned long long *)invL);
-                        rki8_scale_finish_kernel<<<(nmx + 255) / 256, 256, 0, st>>>((unsigned long long *)invL, nmx);
-                        if (SD == 6) rki8_pack_left_kernel<6><<<dim3(nkb, nrb), 128, 0, st>>>(Nbuf, L.ldn, Kpad, ng, ngp, invL, PL);
-                        else rki8_pack_left_kernel<7><<<dim3(nkb, nrb), 128, 0, st>>>(Nbuf, L.ldn, Kpad, ng, ngp, invL, PL);
-                        h->launches += 3;
-                        for (int iw0 = 0; iw0 < h->n_omega; iw0 += wg) {
-                            const int nw = std::min(wg, h->n_omega - iw0);
-                            const double *w0 = w + (size_t)iw0 * L.ldw, *invR0 = invR + (size_t)iw0 * ngp;
-                            cd *S0 = h->ptr<cd>(L.S) + (size_t)iw0 * ng * L.ldS;
-                            if (SD == 6) {
-                                rki8_pack_right_kernel<6><<<dim3(nkb, ncb), 64, 0, st>>>(Nbuf, L.ldn, Kpad, ng, ngp, w0, L.ldw, nw, invR0, PR);
-                                StageTimer tm5(h, 5, 1);
-                                CUDA_TRY(launch_i8<6>(h->i8_cluster, dim3(nt, nw), st, PL, PR, nkb, ncb, d_tiles, invL, invR0, ng, ngp, S0, L.ldS,
-                                                      (int64_t)ng * L.ldS));
-                            } else {
-                                rki8_pack_right_kernel<7><<<dim3(nkb, ncb), 64, 0, st>>>(Nbuf, L.ldn, Kpad, ng, ngp, w0, L.ldw, nw, invR0, PR);
-                                StageTimer tm5(h, 5, 1);
-                                CUDA_TRY(launch_i8<7>(h->i8_cluster, dim3(nt, nw), st, PL, PR, nkb, ncb, d_tiles, invL, invR0, ng, ngp, S0, L.ldS,
-                                                      (int64_t)ng * L.ldS));
-                            }
-                            h->launches += 1;
-                        }
-                        h->launches -= 1;   // the stage timer counts one
-                        done_i8 = true;
+                    int rc = RPA_OK;
+                    switch (h->i8_digits) {
+                        case 6: rc = i8_batch<6>(h, K, Kpad, &done_i8); break;
+                        case 8: rc = i8_batch<8>(h, K, Kpad, &done_i8); break;
+                        default: rc = i8_batch<7>(h, K, Kpad, &done_i8); break;
                     }
+                    if (rc != RPA_OK) return rc;
                 }
+                (done_i8 ? h->i8_batches : h->fp64_batches) += 1;
                 if (done_i8) {
                 } else if (h->use_3m) {
                     // whole waves (one CTA per SM) with full K, then the last partial wave K-sliced so that it fills the GPU too
@@ -1012,15 +1009,13 @@ int ec_q_impl(rpa_chi0_t *h, const double *v_G, int iw_begin, int iw_end, double
         // Lanes: the group's matrices are split in shares that run the same schedule on their own pair of streams.
         // The panel steps are latency-bound (one warp factors the diagonal block, few CTAs), the trailing updates are
         // throughput-bound: with independent shares in flight one share's updates fill the SMs while another is in
-        // its panel steps.  Two lanes by default; `RPA_EC_LANES=n` (1 ... 4) chooses (measured on 16 matrices of 1200
+        // its panel steps.  Two lanes by default; rpa_chi0_set_ec_lanes(h, n) (1 ... 4) chooses (measured on 16 matrices of 1200
         // with the whole-block look-ahead: 2.68 / 2.66 / 2.64 / 2.63 ms for 1 / 2 / 3 / 4 lanes: the chain of a lane
         // does not get shorter, so more lanes add little).
         const int64_t lt_mat = (int64_t)CH_P * CH_NB * L.ldn;          // per matrix
         const size_t lt_block = (size_t)L.ec_group * lt_mat;           // per block buffer
         const double *wneg = h->ptr<double>(L.wneg);
-        const char *lanes_env = getenv("RPA_EC_LANES");
-        const int want = lanes_env ? atoi(lanes_env) : EC_DEFAULT_LANES;
-        const int n_lanes = std::max(1, std::min({want, EC_MAX_LANES, nm}));
+        const int n_lanes = std::max(1, std::min({h->ec_lanes, EC_MAX_LANES, nm}));
         struct Lane {
             cudaStream_t main, side;
             cudaEvent_t *ev_panel, ev_col;
@@ -1128,6 +1123,73 @@ int rpa_chi0_set_spin_degeneracy(rpa_chi0_t *h, int32_t s) {
     return RPA_OK;
 }
 
+int rpa_chi0_set_rank_k_mode(rpa_chi0_t *h, int32_t mode, int32_t digits) {
+    if (!h) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_set_rank_k_mode: handle is NULL");
+    const int kind = mode & 0xff, flags = mode & ~0xff;
+    if (flags & ~(RPA_RANK_K_FLAG_NO_CLUSTER | RPA_RANK_K_FLAG_ALL_BATCHES))
+        return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_set_rank_k_mode: unknown flag bits 0x%x", flags);
+    if (kind == RPA_RANK_K_FP64_3M || kind == RPA_RANK_K_FP64_4M) {
+        if (flags) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_set_rank_k_mode: flags apply to RPA_RANK_K_I8 only");
+        h->use_i8 = false;
+        h->use_3m = kind == RPA_RANK_K_FP64_3M;
+        return RPA_OK;
+    }
+    if (kind != RPA_RANK_K_I8) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_set_rank_k_mode: unknown mode %d", kind);
+    if (digits == 0) digits = 7;
+    if (digits < 6 || digits > 8) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_set_rank_k_mode: digits must be 6, 7 or 8 (0: 7), got %d", digits);
+    if (!h->i8_attr_set) {
+        CUDA_TRY(cudaFuncSetAttribute(rank_k_i8_kernel<6, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, rki8::smem_bytes(6)));
+        CUDA_TRY(cudaFuncSetAttribute(rank_k_i8_kernel<7, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, rki8::smem_bytes(7)));
+        CUDA_TRY(cudaFuncSetAttribute(rank_k_i8_kernel<8, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, rki8::smem_bytes(8)));
+        CUDA_TRY(cudaFuncSetAttribute(rank_k_i8_kernel<6, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, rki8::smem_bytes(6)));
+        CUDA_TRY(cudaFuncSetAttribute(rank_k_i8_kernel<7, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, rki8::smem_bytes(7)));
+        CUDA_TRY(cudaFuncSetAttribute(rank_k_i8_kernel<8, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, rki8::smem_bytes(8)));
+        h->i8_attr_set = true;
+    }
+    h->i8_cluster = !(flags & RPA_RANK_K_FLAG_NO_CLUSTER);
+    h->i8_force = (flags & RPA_RANK_K_FLAG_ALL_BATCHES) != 0;
+    h->i8_digits = digits;
+    h->use_3m = true;   // batches the int8 path does not take run rank_k3m_kernel
+    // tiles (128-row block of L, 64-column block) that meet the lower triangle of either half (Re, Im) of D = L R^T
+    h->i8_tiles.clear();
+    const int ng_ = h->sp.ng, ngp = (ng_ + rki8::RB - 1) / rki8::RB * rki8::RB;
+    for (int rb = 0; rb < 2 * ngp / rki8::RB; rb++) {
+        const int g_lo = (rb * rki8::RB) % ngp, g_hi = std::min(g_lo + rki8::RB - 1, ng_ - 1);
+        if (g_lo >= ng_) continue;
+        int cb = 0;
+        for (; cb * rki8::CB <= g_hi; cb++) h->i8_tiles.push_back(make_int2(rb, cb));
+        // clusters of two CTAs share a row block: an odd row gets a padding tile beyond the triangle (stores nothing)
+        if (h->i8_cluster && (cb & 1)) h->i8_tiles.push_back(make_int2(rb, cb));
+    }
+    h->use_i8 = true;
+    return RPA_OK;
+}
+
+int rpa_chi0_rank_k_batches(const rpa_chi0_t *h, int64_t *fp64_batches, int64_t *i8_batches) {
+    if (!h || !fp64_batches || !i8_batches) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_rank_k_batches: NULL argument");
+    *fp64_batches = h->fp64_batches;
+    *i8_batches = h->i8_batches;
+    return RPA_OK;
+}
+
+int rpa_chi0_set_ec_lanes(rpa_chi0_t *h, int32_t n_lanes) {
+    if (!h) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_set_ec_lanes: handle is NULL");
+    if (n_lanes < 1 || n_lanes > EC_MAX_LANES)
+        return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_set_ec_lanes: n_lanes must be 1 ... %d, got %d", EC_MAX_LANES, n_lanes);
+    h->ec_lanes = n_lanes;
+    return RPA_OK;
+}
+
+// E_c = sum_q w_q E_c(q): the outer q loop's final sum of Eq. 1 over the IBZ weights.  Host arithmetic on the
+// per-q scalars rpa_ec_q returned; summed in the order given.
+int rpa_total_energy(int32_t n_q, const double *ec_q, const double *q_weights, double *ec_ha) {
+    if (n_q < 0 || !ec_ha || (n_q > 0 && (!ec_q || !q_weights))) return fail(RPA_ERR_INVALID_ARG, "rpa_total_energy: invalid argument");
+    double sum = 0.0;
+    for (int i = 0; i < n_q; i++) sum += q_weights[i] * ec_q[i];
+    *ec_ha = sum;
+    return RPA_OK;
+}
+
 int rpa_chi0_sync(rpa_chi0_t *h) {
     if (!h) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_sync: handle is NULL");
     CUDA_TRY(cudaStreamSynchronize(h->stream));
@@ -1144,7 +1206,7 @@ int rpa_chi0_set_profiling(rpa_chi0_t *h, int32_t on) {
     return RPA_OK;
 }
 
-int rpa_chi0_stage_times(rpa_chi0_t *h, double ms[5], int64_t launches[5]) {
+int rpa_chi0_stage_times(rpa_chi0_t *h, double ms[6], int64_t launches[6]) {
     if (!h || !ms || !launches) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_stage_times: NULL argument");
     int rc = drain_events(h);
     if (rc != RPA_OK) return rc;
@@ -1286,111 +1348,6 @@ int rpa_symmetry_remap(rpa_chi0_t *h, int32_t n_bands, const int32_t M[9], int32
         h->launches += 1;
     }
     CUDA_TRY(cudaGetLastError());
-    return RPA_OK;
-}
-
-// ---- FP64 tensor issue-rate probe -----------------------------------------------------------------------------
-__global__ void dmma_probe_kernel(double *out, int iters, double a0, double b0) {
-    double c[8][2];
-#pragma unroll
-    for (int i = 0; i < 8; i++) c[i][0] = c[i][1] = 0.0;
-    const double a = a0 + threadIdx.x * 1e-9, b = b0;
-    for (int it = 0; it < iters; it++) {
-#pragma unroll
-        for (int i = 0; i < 8; i++)
-            asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
-                         : "+d"(c[i][0]), "+d"(c[i][1]) : "d"(a), "d"(b));
-    }
-    double s = 0.0;
-#pragma unroll
-    for (int i = 0; i < 8; i++) s += c[i][0] + c[i][1];
-    if (s == 123.456) out[0] = s;  // never true: keeps the loop alive without memory traffic
-}
-
-int rpa_probe_fp64_tensor_peak(void *cuda_stream, double *tflops) {
-    if (!tflops) return fail(RPA_ERR_INVALID_ARG, "rpa_probe_fp64_tensor_peak: NULL argument");
-    cudaStream_t st = (cudaStream_t)cuda_stream;
-    int dev = 0, nsm = 0;
-    CUDA_TRY(cudaGetDevice(&dev));
-    CUDA_TRY(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
-    double *buf = nullptr;
-    CUDA_TRY(cudaMalloc(&buf, 64));  // the probe is the one call that allocates: it has no handle / workspace
-    cudaEvent_t e0, e1;
-    CUDA_TRY(cudaEventCreate(&e0));
-    CUDA_TRY(cudaEventCreate(&e1));
-    const int iters = 100000, threads = 512;
-    dmma_probe_kernel<<<nsm, threads, 0, st>>>(buf, 2000, 1.0, 1e-3);
-    double best = 0.0;
-    for (int rep = 0; rep < 3; rep++) {
-        CUDA_TRY(cudaEventRecord(e0, st));
-        dmma_probe_kernel<<<nsm, threads, 0, st>>>(buf, iters, 1.0, 1e-3);
-        CUDA_TRY(cudaEventRecord(e1, st));
-        CUDA_TRY(cudaEventSynchronize(e1));
-        float ms = 0.f;
-        CUDA_TRY(cudaEventElapsedTime(&ms, e0, e1));
-        const double fl = (double)nsm * (threads / 32) * (double)iters * 8.0 * 512.0;
-        best = std::max(best, fl / (ms * 1e-3) * 1e-12);
-    }
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
-    cudaFree(buf);
-    *tflops = best;
-    return RPA_OK;
-}
-
-int rpa_probe_int8_tensor_peak(void *cuda_stream, double *tops, int32_t *mismatches) {
-    if (!tops || !mismatches) return fail(RPA_ERR_INVALID_ARG, "rpa_probe_int8_tensor_peak: NULL argument");
-    cudaStream_t st = (cudaStream_t)cuda_stream;
-    int dev = 0, nsm = 0;
-    CUDA_TRY(cudaGetDevice(&dev));
-    CUDA_TRY(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
-    std::vector<int8_t> A(I8_M * I8_K), B(I8_N * I8_K);
-    uint32_t x = 12345u;   // small LCG: values in [-64, 63]
-    for (auto *v : {&A, &B})
-        for (auto &e : *v) { x = x * 1664525u + 1013904223u; e = (int8_t)((int)((x >> 24) & 127) - 64); }
-    unsigned char *buf = nullptr;   // like the FP64 probe: no handle, no workspace, allocates and frees its own scratch
-    const size_t nD = (size_t)I8_M * I8_N * sizeof(int32_t);
-    CUDA_TRY(cudaMalloc(&buf, A.size() + B.size() + nD));
-    int8_t *dA = (int8_t *)buf, *dB = dA + A.size();
-    int32_t *dD = (int32_t *)(buf + A.size() + B.size());
-    cudaEvent_t e0 = nullptr, e1 = nullptr;
-    int rc = RPA_OK;
-    double best = 0.0;
-    std::vector<int32_t> D((size_t)I8_M * I8_N);
-    do {
-#define PROBE_TRY(expr) if ((expr) != cudaSuccess) { rc = fail(RPA_ERR_CUDA, "rpa_probe_int8_tensor_peak: %s", cudaGetErrorString(cudaGetLastError())); break; }
-        PROBE_TRY(cudaMemcpyAsync(dA, A.data(), A.size(), cudaMemcpyHostToDevice, st));
-        PROBE_TRY(cudaMemcpyAsync(dB, B.data(), B.size(), cudaMemcpyHostToDevice, st));
-        PROBE_TRY(cudaMemsetAsync(dD, 0xff, nD, st));
-        PROBE_TRY(cudaEventCreate(&e0));
-        PROBE_TRY(cudaEventCreate(&e1));
-        i8_probe_kernel<<<nsm, 128, 0, st>>>(dA, dB, dD, 100);
-        PROBE_TRY(cudaMemcpyAsync(D.data(), dD, nD, cudaMemcpyDeviceToHost, st));
-        const int iters = 20000;
-        for (int rep = 0; rep < 3 && rc == RPA_OK; rep++) {
-            PROBE_TRY(cudaEventRecord(e0, st));
-            i8_probe_kernel<<<nsm, 128, 0, st>>>(dA, dB, dD, iters);
-            PROBE_TRY(cudaEventRecord(e1, st));
-            PROBE_TRY(cudaEventSynchronize(e1));
-            float ms = 0.f;
-            PROBE_TRY(cudaEventElapsedTime(&ms, e0, e1));
-            best = std::max(best, (double)nsm * (iters + 1.0) * 2.0 * I8_M * I8_N * I8_K / (ms * 1e-3) * 1e-12);
-        }
-#undef PROBE_TRY
-    } while (0);
-    if (e0) cudaEventDestroy(e0);
-    if (e1) cudaEventDestroy(e1);
-    cudaFree(buf);
-    if (rc != RPA_OK) return rc;
-    int bad = 0;
-    for (int i = 0; i < I8_M; i++)
-        for (int j = 0; j < I8_N; j++) {
-            int32_t sum = 0;
-            for (int k = 0; k < I8_K; k++) sum += (int32_t)A[i * I8_K + k] * (int32_t)B[j * I8_K + k];
-            bad += sum != D[(size_t)i * I8_N + j];
-        }
-    *mismatches = bad;
-    *tops = best;
     return RPA_OK;
 }
 

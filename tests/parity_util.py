@@ -7,8 +7,10 @@ def rel_fro(a, b):
     return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
 
 
-def gpu_run(cfg, kds, use_paw=True, max_batch_pairs=0, want_ec=True, device="cuda:0"):
-    """chi0[nw][ng][ng] (numpy), (ec, e_omega) or None, g, K2 -- everything computed by librpa_chi0.so."""
+def gpu_run(cfg, kds, use_paw=True, max_batch_pairs=0, want_ec=True, device="cuda:0", rank_k_mode=None, info=None):
+    """chi0[nw][ng][ng] (numpy), (ec, e_omega) or None, g, K2 -- everything computed by librpa_chi0.so.
+    rank_k_mode: None (the library's default, FP64 tensor cores) or (mode, digits) for rpa_chi0_set_rank_k_mode.
+    info: a dict that receives "rank_k_batches" = (FP64 batches, int8 batches) the handle ran."""
     import torch
     from paper_1307_8052_b200 import binding as B
     from paper_1307_8052_b200 import workload as W
@@ -16,6 +18,8 @@ def gpu_run(cfg, kds, use_paw=True, max_batch_pairs=0, want_ec=True, device="cud
     ptot = int(cfg.n_proj.sum()) if use_paw else 0
     h = B.rpa_chi0_create(cfg.grid, cfg.cell, cfg.q_red, W.tuned_ecut(cfg), om, wt, max_batch_pairs, ptot, device)
     try:
+        if rank_k_mode is not None:
+            B.rpa_chi0_set_rank_k_mode(h, *rank_k_mode)
         g, K2 = B.rpa_chi0_gvectors(h)
         Qd = R = npj = None
         if use_paw and ptot:
@@ -30,6 +34,8 @@ def gpu_run(cfg, kds, use_paw=True, max_batch_pairs=0, want_ec=True, device="cud
             again = B.rpa_chi0_get(h, 0).cpu().numpy()
             assert np.array_equal(again, chi[0])
         B.rpa_chi0_sync(h)
+        if info is not None:
+            info["rank_k_batches"] = B.rpa_chi0_rank_k_batches(h)
     finally:
         h.close()
     return chi, ec, g, K2

@@ -203,8 +203,8 @@ def test_ec_q_range_partial_sums_and_isolation():
         h.close()
 
 
-def test_ec_q_lanes_give_the_same_numbers(monkeypatch):
-    """rpa_ec_q factorises the frequencies of a group in 1 ... 4 concurrent lanes (include/rpa_chi0.h, RPA_EC_LANES):
+def test_ec_q_lanes_give_the_same_numbers():
+    """rpa_ec_q factorises the frequencies of a group in 1 ... 4 concurrent lanes (rpa_chi0_set_ec_lanes):
     every matrix goes through the same arithmetic whichever lane it is in, so e(omega) must agree bit for bit, for an
     even split, a ragged one (8 frequencies in 3 lanes) and more lanes than frequencies (a range of 2).  nG = 401
     (configs[2]) spans four 128-column blocks with a ragged last one: look-ahead and big updates both run."""
@@ -219,8 +219,8 @@ def test_ec_q_lanes_give_the_same_numbers(monkeypatch):
             B.add_kpoint_host(h, kd, cfg.n_proj, Qd, W.atom_positions(cfg))
             v = W.coulomb(K2)
             ref = None
-            for lanes in ("1", "2", "3", "4"):
-                monkeypatch.setenv("RPA_EC_LANES", lanes)
+            for lanes in (1, 2, 3, 4):
+                B.rpa_chi0_set_ec_lanes(h, lanes)
                 ec, e = B.rpa_ec_q(h, v)
                 ec2, e2 = B.rpa_ec_q_range(h, v, 1, 3)
                 if ref is None:
@@ -229,6 +229,10 @@ def test_ec_q_lanes_give_the_same_numbers(monkeypatch):
                 else:
                     assert ec == ref[0] and np.array_equal(e, ref[1])
                     assert ec2 == ref[2] and np.array_equal(e2, ref[3])
+            for bad in (0, 5):
+                with pytest.raises(B.RpaError) as ei:
+                    B.rpa_chi0_set_ec_lanes(h, bad)
+                assert ei.value.code == B.RPA_ERR_INVALID_ARG
         finally:
             h.close()
 
@@ -236,7 +240,9 @@ def test_ec_q_lanes_give_the_same_numbers(monkeypatch):
 def test_int8_tcgen05_probe_self_check():
     """rpa_probe_int8_tensor_peak: the TMEM read-back of one tcgen05.mma.kind::i8 equals the host product bit for bit,
     and the issue rate is in the range of a Blackwell int8 tensor pipe (legacy mma.sync reaches 1.1 Pop/s)."""
-    from paper_1307_8052_b200 import binding as B
-    tops, bad = B.rpa_probe_int8_tensor_peak("cuda:0")
+    from paper_1307_8052_b200 import probes
+    tops, bad = probes.rpa_probe_int8_tensor_peak("cuda:0")
     assert bad == 0
     assert 2000.0 < tops < 6000.0
+    tf = probes.rpa_probe_fp64_tensor_peak("cuda:0")
+    assert 20.0 < tf < 60.0   # B200: 40 TFLOP/s nominal FP64

@@ -94,52 +94,70 @@ def test_config1_molecule_slice():
     _compare(cfg, kds)
 
 
-def _big_config_slice(cfg, occ, unocc, n_sample, omegas=(0, 7, 15), k_list=(0, 1), device_resident=False):
+def _big_config_slice(cfg, occ, unocc, n_sample, omegas=(0, 7, 15), k_list=(0, 1), device_resident=False, modes=(None,),
+                      max_batch=0, want_batches=None):
     """Configs 3 / 4 at full grid, nG, omega count and atoms, on a band slice (a full oracle run costs hours to a
     day of CPU).  The oracle evaluates chi0 on a sampled sub-list of the sphere (every element of
     Eq. 17 is an independent sum, so chi0 restricted to those G is exactly the chi0 of those G); the sample holds
     the first / last G and both sides of several 64-tile boundaries.  E_c(q), which needs the whole matrix, is
-    checked against the eigenvalue route sum_i ln(1 - l_i) + l_i on the library's own chi0 (numpy eigvalsh)."""
+    checked against the eigenvalue route sum_i ln(1 - l_i) + l_i on the library's own chi0 (numpy eigvalsh).
+    modes: one GPU run per entry (None = the library's default rank-K kernel, else (mode, digits) for
+    rpa_chi0_set_rank_k_mode), every one compared with the SAME oracle result; the E_c check runs for the first.
+    want_batches: per mode, the (FP64, int8) batch counts rpa_chi0_rank_k_batches must report."""
     import torch
     from paper_1307_8052_b200 import binding as B
     om, wt = W.omega_grid(cfg.n_omega)
     ptot = int(cfg.n_proj.sum())
     kds = [W.kpoint(cfg, k, occ=occ, unocc=unocc) for k in k_list]
-    h = B.rpa_chi0_create(cfg.grid, cfg.cell, cfg.q_red, W.tuned_ecut(cfg), om, wt, 0, ptot, "cuda:0")
-    try:
-        g, K2 = B.rpa_chi0_gvectors(h)
-        ng = len(g)
-        rng = np.random.default_rng(7)
-        sel = set([0, 1, ng - 1, ng - 2, 63, 64, 65, 127, 128, (ng // 64) * 64 - 1, (ng // 64) * 64])
-        sel |= set(rng.choice(ng, n_sample - len(sel), replace=False).tolist())
-        sel = np.array(sorted(s for s in sel if 0 <= s < ng))
-        Qd = torch.from_numpy(W.paw_Q(cfg, K2)).to("cuda:0")
-        R = W.atom_positions(cfg)
-        for kd in kds:
-            if device_resident:  # exactly what bench.py's timed step does: arrays already in HBM, default batching
-                dv = {k: torch.from_numpy(getattr(kd, k)).to("cuda:0") for k in ("psi_occ", "psi_unocc", "P_occ", "P_unocc")}
-                B.rpa_chi0_add_kpoint(h, kd.kweight, dv["psi_occ"], dv["psi_unocc"], kd.eps_occ, kd.eps_unocc, kd.f_occ,
-                                      kd.f_unocc, cfg.n_proj, dv["P_occ"], dv["P_unocc"], Qd, R)
-                B.rpa_chi0_sync(h)
-                del dv
-            else:
-                B.add_kpoint_host(h, kd, cfg.n_proj, Qd, R)
-        seld = torch.from_numpy(sel).to("cuda:0")
-        chi_sel, chi_full = {}, {}
-        for i in omegas:
-            c = B.rpa_chi0_get(h, i)
-            chi_sel[i] = c[seld][:, seld].cpu().numpy()
-            if i in (omegas[0], omegas[-1]):
-                chi_full[i] = c.cpu().numpy()
-            del c
-        v = W.coulomb(K2)
-        ec, e = B.rpa_ec_q(h, v)
-    finally:
-        h.close()
+    results = []
+    sel = g = None
+    for im, mode in enumerate(modes):
+        h = B.rpa_chi0_create(cfg.grid, cfg.cell, cfg.q_red, W.tuned_ecut(cfg), om, wt, max_batch, ptot, "cuda:0")
+        try:
+            if mode is not None:
+                B.rpa_chi0_set_rank_k_mode(h, *mode)
+            g, K2 = B.rpa_chi0_gvectors(h)
+            ng = len(g)
+            rng = np.random.default_rng(7)
+            sel = set([0, 1, ng - 1, ng - 2, 63, 64, 65, 127, 128, (ng // 64) * 64 - 1, (ng // 64) * 64])
+            sel |= set(rng.choice(ng, n_sample - len(sel), replace=False).tolist())
+            sel = np.array(sorted(s for s in sel if 0 <= s < ng))
+            Qd = torch.from_numpy(W.paw_Q(cfg, K2)).to("cuda:0")
+            R = W.atom_positions(cfg)
+            for kd in kds:
+                if device_resident:  # exactly what bench.py's timed step does: arrays already in HBM, one call per k-point
+                    dv = {k: torch.from_numpy(getattr(kd, k)).to("cuda:0") for k in ("psi_occ", "psi_unocc", "P_occ", "P_unocc")}
+                    B.rpa_chi0_add_kpoint(h, kd.kweight, dv["psi_occ"], dv["psi_unocc"], kd.eps_occ, kd.eps_unocc, kd.f_occ,
+                                          kd.f_unocc, cfg.n_proj, dv["P_occ"], dv["P_unocc"], Qd, R)
+                    B.rpa_chi0_sync(h)
+                    del dv
+                else:
+                    B.add_kpoint_host(h, kd, cfg.n_proj, Qd, R)
+            if want_batches is not None:
+                assert B.rpa_chi0_rank_k_batches(h) == want_batches[im], (mode, B.rpa_chi0_rank_k_batches(h))
+            seld = torch.from_numpy(sel).to("cuda:0")
+            chi_sel, chi_full = {}, {}
+            for i in omegas:
+                c = B.rpa_chi0_get(h, i)
+                chi_sel[i] = c[seld][:, seld].cpu().numpy()
+                if im == 0 and i in (omegas[0], omegas[-1]):
+                    chi_full[i] = c.cpu().numpy()
+                del c
+            v = W.coulomb(K2)
+            ec, e = B.rpa_ec_q(h, v)
+            results.append((chi_sel, chi_full, ec, e, v))
+        finally:
+            h.close()
+        torch.cuda.empty_cache()
     chi_o, _, g_o, _ = oracle_run(cfg, kds, True, want_ec=False, g=g[sel])
-    for i in omegas:
-        err = rel_fro(chi_sel[i], chi_o[i])
-        assert err <= CHI_TOL, f"omega {i}: rel Frobenius error on the sampled G {err:.3e}"
+    for (chi_sel, _, _, _, _), mode in zip(results, modes):
+        for i in omegas:
+            err = rel_fro(chi_sel[i], chi_o[i])
+            assert err <= CHI_TOL, f"mode {mode}, omega {i}: rel Frobenius error on the sampled G {err:.3e}"
+            # and element by element on the sample: every sampled element within 1e-9 of the sample's largest
+            # (a wrong far off-diagonal element cannot hide behind the diagonal's norm)
+            assert np.abs(chi_sel[i] - chi_o[i]).max() <= 1e-9 * np.abs(chi_o[i]).max(), (mode, i)
+    _, chi_full, ec, e, v = results[0]
     d = np.sqrt(v)
     for i, c in chi_full.items():
         assert np.array_equal(c, c.conj().T)
@@ -148,6 +166,8 @@ def _big_config_slice(cfg, occ, unocc, n_sample, omegas=(0, 7, 15), k_list=(0, 1
         want = float(np.sum(np.log1p(-lam) + lam))
         assert abs(e[i] - want) <= 1e-9 * max(abs(want), np.abs(e).max() * 1e-3), (i, e[i], want)
     assert np.isfinite(ec) and ec < 0.0
+    for r in results[1:]:   # E_c(q) of the other modes against the first
+        assert abs(r[2] - ec) <= 1e-10 * abs(ec)
 
 
 def test_config3_slab_slice():
@@ -162,6 +182,33 @@ def test_config4_large_slab_slice():
     unoccupied."""
     cfg = W.CONFIGS[4]
     _big_config_slice(cfg, occ=[0, 119], unocc=list(range(0, 3000, 240))[:13], n_sample=120)
+
+
+def _all_rank_k_modes():
+    from paper_1307_8052_b200 import binding as B
+    return (None, (B.RPA_RANK_K_FP64_4M, 0), (B.RPA_RANK_K_I8, 7), (B.RPA_RANK_K_I8, 8))
+
+
+def test_config3_large_batch_every_rank_k_mode():
+    """What a real configs[3] run launches: one batch of >= 1024 transitions (1 occupied x 1031 unoccupied, odd count,
+    Kpad = 1056) at full grid / nG = 3004 / 16 omega / 10 x 18 projectors, device-resident, for every rank-K mode against
+    ONE oracle run on 120 sampled G.  FP64 3M (default): 1128 tiles x 16 omega in whole waves plus a K-sliced tail launch;
+    int8 (picked by the library's own thresholds, no ALL_BATCHES flag): 24 row blocks per half, odd tile rows with padding
+    tiles, and -- with max_batch_pairs = 1056 sizing the scratch -- the frequencies in three groups (6, 6, 4), as at the
+    default batch of 8192 (Eq. 17 / Eq. 20)."""
+    cfg = W.CONFIGS[3]
+    _big_config_slice(cfg, occ=[31], unocc=list(range(3, 1034)), n_sample=120, k_list=(0,),
+                      device_resident=True, modes=_all_rank_k_modes(), max_batch=1056,
+                      want_batches=((1, 0), (1, 0), (0, 1), (0, 1)))
+
+
+def test_config4_large_batch_every_rank_k_mode():
+    """The same for configs[4]: 48x48x192 grid, nG = 5001 (79 column blocks, 40 row blocks per half), 18 x 18 projectors,
+    1 occupied x 1031 unoccupied bands in one batch."""
+    cfg = W.CONFIGS[4]
+    _big_config_slice(cfg, occ=[59], unocc=list(range(0, 3000, 2))[:1031], n_sample=100, k_list=(0,),
+                      device_resident=True, modes=_all_rank_k_modes(), max_batch=1056,
+                      want_batches=((1, 0), (1, 0), (0, 1), (0, 1)))
 
 
 def test_config1_full_size_bench_configuration():
@@ -198,15 +245,36 @@ def test_pipelined_host_upload_matches_single_call():
         h.close()
 
 
-def test_four_multiplication_rank_k_path_still_agrees():
-    """RPA_RANK_K_4M=1 (read at rpa_chi0_create) selects rank_k_kernel<true>, the 4-multiplication real-view
-    kernel that rank_k3m_kernel replaced for the chi0 accumulation; it stays the reference implementation of the
-    update (and its <false> variant serves the Cholesky), so its parity is kept under test."""
-    import os
-    import subprocess
-    import sys
-    env = dict(os.environ, RPA_RANK_K_4M="1")
-    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-    r = subprocess.run([sys.executable, "-m", "pytest", "-x", "-q", "-m", "gpu", "tests/test_gpu_parity.py", "-k",
-                        "config0_toy_full or tiny_skewed or config2_bulk"], cwd=root, env=env, capture_output=True, text=True)
-    assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
+def test_four_multiplication_rank_k_path_still_agrees(tiny_cfg):
+    """rpa_chi0_set_rank_k_mode(RPA_RANK_K_FP64_4M) selects rank_k_kernel<true>, the 4-multiplication real-view kernel
+    that rank_k3m_kernel replaced for the chi0 accumulation; it stays the reference form of the update (and its <false>
+    variant serves the Cholesky), so its parity with the oracle is kept under test."""
+    from paper_1307_8052_b200 import binding as B
+    cfg2 = W.CONFIGS[2]
+    cases = [(W.CONFIGS[0], [W.kpoint(W.CONFIGS[0], 0)]), (tiny_cfg, [W.kpoint(tiny_cfg, 0)]),
+             (cfg2, [W.kpoint(cfg2, k, occ=[0, 3, 7], unocc=range(0, 300, 7)[:45]) for k in (0, 1)])]
+    for cfg, kds in cases:
+        chi_g, ec_g, _, _ = gpu_run(cfg, kds, True, rank_k_mode=(B.RPA_RANK_K_FP64_4M, 0))
+        chi_o, ec_o, _, _ = oracle_run(cfg, kds, True)
+        for i in range(cfg.n_omega):
+            assert rel_fro(chi_g[i], chi_o[i]) <= CHI_TOL
+        assert abs(ec_g[0] - ec_o[0]) <= EC_TOL * abs(ec_o[0])
+
+
+def test_rank_k_mode_setter_validates():
+    from paper_1307_8052_b200 import binding as B
+    cfg = W.CONFIGS[0]
+    om, wt = W.omega_grid(cfg.n_omega)
+    h = B.rpa_chi0_create(cfg.grid, cfg.cell, cfg.q_red, W.tuned_ecut(cfg), om, wt, 0, 0, "cuda:0")
+    try:
+        for mode, digits in ((7, 0), (B.RPA_RANK_K_I8, 5), (B.RPA_RANK_K_I8, 9), (B.RPA_RANK_K_I8 | 0x800, 7),
+                             (B.RPA_RANK_K_FP64_3M | B.RPA_RANK_K_FLAG_ALL_BATCHES, 0)):
+            with pytest.raises(B.RpaError) as ei:
+                B.rpa_chi0_set_rank_k_mode(h, mode, digits)
+            assert ei.value.code == B.RPA_ERR_INVALID_ARG
+        for mode, digits in ((B.RPA_RANK_K_I8, 0), (B.RPA_RANK_K_I8 | B.RPA_RANK_K_FLAG_NO_CLUSTER, 8),
+                             (B.RPA_RANK_K_FP64_4M, 0), (B.RPA_RANK_K_FP64_3M, 0)):
+            B.rpa_chi0_set_rank_k_mode(h, mode, digits)
+        assert B.rpa_chi0_rank_k_batches(h) == (0, 0)
+    finally:
+        h.close()

@@ -14,8 +14,8 @@ from paper_1307_8052_b200 import workload as W
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def _declared_symbols():
-    src = open(os.path.join(ROOT, "include", "rpa_chi0.h")).read()
+def _declared_symbols(header="rpa_chi0.h"):
+    src = open(os.path.join(ROOT, "include", header)).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     return sorted(set(re.findall(r"\b(rpa_[a-z0-9_]+)\s*\(", src)))
 
@@ -29,6 +29,39 @@ def test_library_builds_and_exports_every_declared_symbol():
     for n in names:
         assert hasattr(lib, n), f"{n} declared in include/rpa_chi0.h but not exported"
     assert sorted(B.EXPORTS) == names, "binding.EXPORTS out of sync with the header"
+
+
+def test_probe_library_builds_and_exports_every_declared_symbol():
+    """include/rpa_probes.h is the bench-only helper library: its symbols live in librpa_probes.so, none in the product."""
+    from paper_1307_8052_b200 import probes
+    path = cuda_build.build_probes()
+    lib = ctypes.CDLL(path)
+    names = _declared_symbols("rpa_probes.h")
+    assert names == sorted(probes.EXPORTS)
+    for n in names:
+        assert hasattr(lib, n), f"{n} declared in include/rpa_probes.h but not exported"
+    product = ctypes.CDLL(cuda_build.build())
+    for n in names:
+        assert not hasattr(product, n), f"{n} must not be exported by librpa_chi0.so"
+
+
+def test_library_keeps_no_process_global_switches():
+    """no global state except the thread-local error string -- kernel choice is an explicit setter
+    (rpa_chi0_set_rank_k_mode, rpa_chi0_set_ec_lanes), never an environment variable."""
+    csrc = os.path.join(ROOT, "paper_1307_8052_b200", "csrc")
+    for f in os.listdir(csrc):
+        assert "getenv" not in open(os.path.join(csrc, f)).read(), f
+
+
+def test_total_energy_is_the_weighted_q_sum():
+    """rpa_total_energy (Eq. 1): host arithmetic behind the C ABI, so it runs without a GPU."""
+    assert B.rpa_total_energy([-0.5, -0.25, 1.0], [0.125, 0.375, 0.5]) == -0.5 * 0.125 - 0.25 * 0.375 + 0.5
+    assert B.rpa_total_energy([], []) == 0.0
+    out = ctypes.c_double(7.0)
+    assert B.lib().rpa_total_energy(2, None, None, ctypes.byref(out)) == B.RPA_ERR_INVALID_ARG
+    assert B.lib().rpa_total_energy(-1, None, None, ctypes.byref(out)) == B.RPA_ERR_INVALID_ARG
+    with pytest.raises(ValueError):
+        B.rpa_total_energy([1.0], [0.5, 0.5])
 
 
 def test_library_is_sm100a_with_dmma_and_bulk_copies():
