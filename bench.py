@@ -443,6 +443,8 @@ def per_config_block(args, dev, peak_tf, peaks, peak_kind, main_line, main_cfg):
     out = {}
     steps, n_warm = 3, 2
     for idx, (n_o, n_u) in PER_CONFIG_PLAN.items():
+        if idx == main_cfg.index:
+            continue
         cfg = W.CONFIGS[idx]
         t_wall = time.perf_counter()
         om, wt = W.omega_grid(cfg.n_omega)
@@ -502,8 +504,8 @@ def per_config_block(args, dev, peak_tf, peaks, peak_kind, main_line, main_cfg):
                      "rank_k_tflops": rep["rank_k"]["tflops"], "rank_k_frac": rep["rank_k"]["frac"],
                      "rank_k_ms": rep["rank_k"]["ms_per_step"],
                      "pair_density_gbs": rep["pair_density"]["achieved"], "pair_density_frac": rep["pair_density"]["frac"],
-                     "pair_density_ms": rep["pair_density"]["ms_per_step"], "paw_ms": rep["ms_per_step"]["paw"],
-                     "ec_q_ms": tail[0] / steps, "ec_q_ha": ec}
+                     "pair_density_ms": rep["pair_density"]["ms_per_step"], "stage_ms": rep["ms_per_step"],
+                     "paw_ms": rep["ms_per_step"]["paw"], "ec_q_ms": tail[0] / steps, "ec_q_ha": ec}
             if idx == 0:
                 entry["note"] = "launch/latency-bound (8.7e7 flop in total): throughput only, no roofline claim"
         finally:
@@ -546,9 +548,15 @@ def main():
     ap.add_argument("--exchange", default="allreduce", choices=["allreduce", "reduce_scatter"],
                     help="N > 1: all-reduce of S (every rank reads out and factorises all frequencies) or reduce-scatter "
                          "by frequency (every rank reads out and factorises its own, scalar all-reduce of E_c)")
+    ap.add_argument("--bands", default="", help="OxU: time only the first O occupied and U unoccupied bands per k-point "
+                                                "(profiling runs of the big configs; named in config.workload)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
     cfg = W.CONFIGS[args.config]
+    if args.bands:
+        import dataclasses
+        n_o, n_u = (int(x) for x in args.bands.lower().split("x"))
+        cfg = dataclasses.replace(cfg, n_occ=n_o, n_unocc=n_u, name=f"{cfg.name} (band slice {n_o} x {n_u})")
     if args.impl == "reference":
         run_reference(args, cfg)
     else:

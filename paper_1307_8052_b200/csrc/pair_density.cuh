@@ -281,13 +281,17 @@ __global__ void __launch_bounds__(128) pd_xaxis_kernel(const cd *__restrict__ I,
 // Dynamic shared memory: N1 * PD_X8_ND * sizeof(cd) (twiddle products per (j, kept-frequency slot)).  Same arguments
 // as pd_xaxis_kernel.
 #define PD_X8_ND_MAX 3
-template <int PD_X8_ND>   // kept-frequency slots per residue mod 8 (2 when the box needs no more: fewer registers)
+// NBT > 0: N1 = 8 NBT known at compile time (short x axes: the 24^3 and 16^3 grids): the j loop is unrolled, so all 8 NBT
+// loads of a column are in flight together.  grid (ceil(nb2 / 128), pairs handled concurrently): a block walks over the
+// pairs pl = blockIdx.y, blockIdx.y + gridDim.y, ... of the launch, so the twiddle table, the kept-slot mask and the
+// column's scatter indices are set up once per block and not once per pair.
+template <int PD_X8_ND, int NBT>   // PD_X8_ND: kept-frequency slots per residue mod 8 (2 when the box needs no more: fewer registers)
 __global__ void __launch_bounds__(128) pd_xaxis8_kernel(const cd *__restrict__ I, cd *__restrict__ Nbuf, int64_t ldn,
                                                        const cd *__restrict__ tw1, const int32_t *__restrict__ box2s,
-                                                       int N1, int nb2, int g1min, int ng1, int p_begin, double inv_n) {
+                                                       int N1, int nb2, int g1min, int ng1, int p_begin, int p_count, double inv_n) {
     extern __shared__ __align__(16) unsigned char pd_smem[];
     cd *twt = reinterpret_cast<cd *>(pd_smem);   // [j][slot], slot = k1 PD_X8_ND + d: W_N1^(j f_slot)
-    const int NB = N1 >> 3;
+    const int NB = NBT > 0 ? NBT : (N1 >> 3);
     // kept frequencies of residue k1: f = k1 + 8 (dlo + d), box index f - g1min (the same for every thread)
     const int dlo = (g1min >= 0 ? g1min : g1min - 7) / 8;
     for (int i = threadIdx.x; i < NB * 8 * PD_X8_ND; i += blockDim.x) {
@@ -306,35 +310,56 @@ __global__ void __launch_bounds__(128) pd_xaxis8_kernel(const cd *__restrict__ I
     __syncthreads();
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= nb2) return;
-    const int pl = blockIdx.y;
-    const cd *Ip = I + (size_t)pl * N1 * nb2 + b;
-    cd acc[8][PD_X8_ND];
-#pragma unroll
-    for (int k1 = 0; k1 < 8; k1++)
-#pragma unroll
-        for (int d = 0; d < PD_X8_ND; d++) acc[k1][d] = cmake(0.0, 0.0);
-    for (int j = 0; j < NB; j++) {
-        cd v[8];
-#pragma unroll
-        for (int s = 0; s < 8; s++) v[s] = Ip[(size_t)(j + NB * s) * nb2];
-        Bfly<8>::run(v);
-        const cd *tj = twt + j * 8 * PD_X8_ND;
+    // short axes: the sphere index of every kept slot of this column (-1: outside the sphere) is the same for all pairs
+    int sidx[NBT > 0 ? 8 : 1][PD_X8_ND];
+    if constexpr (NBT > 0) {
 #pragma unroll
         for (int k1 = 0; k1 < 8; k1++)
 #pragma unroll
-            for (int d = 0; d < PD_X8_ND; d++)
-                if (mask & (1u << (k1 * PD_X8_ND + d))) acc[k1][d] = cfma(tj[k1 * PD_X8_ND + d], v[k1], acc[k1][d]);
-    }
-    cd *out = Nbuf + (size_t)(p_begin + pl) * ldn;
-#pragma unroll
-    for (int k1 = 0; k1 < 8; k1++)
-#pragma unroll
-        for (int d = 0; d < PD_X8_ND; d++)
-            if (mask & (1u << (k1 * PD_X8_ND + d))) {
-                const int gi = k1 + 8 * (dlo + d) - g1min;
-                const int s = box2s[(size_t)gi * nb2 + b];
-                if (s >= 0) out[s] = cscale(inv_n, acc[k1][d]);
+            for (int d = 0; d < PD_X8_ND; d++) {
+                sidx[k1][d] = -1;
+                if (mask & (1u << (k1 * PD_X8_ND + d))) sidx[k1][d] = box2s[(size_t)(k1 + 8 * (dlo + d) - g1min) * nb2 + b];
             }
+    }
+    for (int pl = blockIdx.y; pl < p_count; pl += gridDim.y) {
+        const cd *Ip = I + (size_t)pl * N1 * nb2 + b;
+        cd acc[8][PD_X8_ND];
+#pragma unroll
+        for (int k1 = 0; k1 < 8; k1++)
+#pragma unroll
+            for (int d = 0; d < PD_X8_ND; d++) acc[k1][d] = cmake(0.0, 0.0);
+        auto body = [&](int j) {
+            cd v[8];
+#pragma unroll
+            for (int s = 0; s < 8; s++) v[s] = Ip[(size_t)(j + NB * s) * nb2];
+            Bfly<8>::run(v);
+            const cd *tj = twt + j * 8 * PD_X8_ND;
+#pragma unroll
+            for (int k1 = 0; k1 < 8; k1++)
+#pragma unroll
+                for (int d = 0; d < PD_X8_ND; d++)
+                    if (mask & (1u << (k1 * PD_X8_ND + d))) acc[k1][d] = cfma(tj[k1 * PD_X8_ND + d], v[k1], acc[k1][d]);
+        };
+        if constexpr (NBT > 0) {
+#pragma unroll
+            for (int j = 0; j < NBT; j++) body(j);
+        } else {
+#pragma unroll 1
+            for (int j = 0; j < NB; j++) body(j);
+        }
+        cd *out = Nbuf + (size_t)(p_begin + pl) * ldn;
+#pragma unroll
+        for (int k1 = 0; k1 < 8; k1++)
+#pragma unroll
+            for (int d = 0; d < PD_X8_ND; d++) {
+                if constexpr (NBT > 0) {
+                    if (sidx[k1][d] >= 0) out[sidx[k1][d]] = cscale(inv_n, acc[k1][d]);
+                } else if (mask & (1u << (k1 * PD_X8_ND + d))) {
+                    const int s = box2s[(size_t)(k1 + 8 * (dlo + d) - g1min) * nb2 + b];
+                    if (s >= 0) out[s] = cscale(inv_n, acc[k1][d]);
+                }
+            }
+    }
 }
 // can pd_xaxis8_kernel serve this x axis?  (every kept frequency must fall in one of its PD_X8_ND slots per residue)
 // returns the number of slots needed (2 or 3), or 0 if the kernel cannot serve this x axis

@@ -113,6 +113,11 @@ struct PdZyParams {
     int n0, mlen, m0;               // pair p of the batch -> band n = n0 + p / mlen, m = m0 + p % mlen
     int p_begin, p_count;           // pairs of the batch handled by this launch
     int n_units;                    // groups of <= G consecutive pairs with the same occupied band
+    // closed-form unit -> pair map (pdzy_plan_units): the launch's first row (pairs of one occupied band) may start in its
+    // middle and holds nu0 units; every later row starts a fresh unit and holds upr = ceil(mlen / G) units, the last one
+    // possibly cut short by the end of the launch.  Divisions by N1 and upr are multiplications by 2^64 / d rounded up.
+    int row0, nu0, upr;
+    unsigned long long magic_n1, magic_upr;
     int g2min, ng2, g3min, ng3;
 };
 
@@ -124,7 +129,7 @@ struct PdZy {
     // enumerating the quarter-warp bank groups of the pass-A stores (k1 fixed) and pass-B loads (j fixed) of this lane
     // layout: conflict-free for NB3 = 2, 3, 8, 16, 10 % over the minimum for NB3 = 14
     static constexpr int XP = NB3 == 2 ? 3 : NB3 == 3 ? 9 : NB3 == 14 ? 17 : NB3 + ((NB3 & 1) ? 0 : 1);
-    static constexpr int XLINE = NB3 == 2 ? 26 : NB3 == 3 ? 75 : NB3 == 14 ? 206 : NA3 * XP;
+        static constexpr int XLINE = NB3 == 2 ? 26 : NB3 == 3 ? 75 : NB3 == 14 ? 206 : NA3 * XP;
     static_assert(XLINE >= (NA3 - 1) * XP + NB3, "exchange line too short");
     static constexpr int ROWS = NW * LPW;                 // z lines per chunk
     static constexpr int NCH = (N2 + ROWS - 1) / ROWS;
@@ -144,35 +149,41 @@ struct PdZy {
     static bool box_ok(int g3min, int ng3) { return g3min >= NA3 * DLO && g3min + ng3 <= NA3 * (DHI + 1); }
 };
 
-// unit u of the launch -> first pair p (relative to the batch) and the number of pairs cnt <= G, all in one row.
-template <int G>
-__device__ __forceinline__ void pdzy_unit(const PdZyParams &P, int u, int &p, int &cnt) {
-    p = P.p_begin;
-    const int p_end = P.p_begin + P.p_count;
-    while (true) {
-        const int row = p / P.mlen;
-        const int rend = min((row + 1) * P.mlen, p_end);
-        const int nu = (rend - p + G - 1) / G;
-        if (u < nu) {
-            p += u * G;
-            cnt = min(G, rend - p);
-            return;
-        }
-        u -= nu;
-        p = rend;
-    }
+// x / d for any 0 <= x < 2^31, d >= 1 as the high half of a 64 x 64 multiplication: magic = floor((2^64 - 1) / d) + 1, so
+// magic d = 2^64 + e with 0 < e <= d and x magic / 2^64 = x / d + x e / (d 2^64), whose excess stays below 1 / d.
+// d = 1 has no 64-bit magic: it is encoded as 0.
+static inline unsigned long long pdzy_magic(int d) { return d <= 1 ? 0ull : ~0ull / (unsigned long long)d + 1ull; }
+__device__ __forceinline__ int pdzy_fastdiv(int x, unsigned long long magic) {
+    return magic ? (int)__umul64hi((unsigned long long)(unsigned)x, magic) : x;
 }
 
-static inline int pdzy_count_units(int p_begin, int p_count, int mlen, int G) {
-    int p = p_begin, n = 0;
-    const int p_end = p_begin + p_count;
-    while (p < p_end) {
-        const int row = p / mlen;
-        const int rend = std::min((row + 1) * mlen, p_end);
-        n += (rend - p + G - 1) / G;
-        p = rend;
+// unit u of the launch -> first pair p (relative to the batch) and the number of pairs cnt <= G, all in one row r.
+template <int G>
+__device__ __forceinline__ void pdzy_unit(const PdZyParams &P, int u, int &p, int &cnt, int &r) {
+    if (u < P.nu0) {
+        r = P.row0;
+        p = P.p_begin + u * G;
+    } else {
+        const int u2 = u - P.nu0, q = pdzy_fastdiv(u2, P.magic_upr);
+        r = P.row0 + 1 + q;
+        p = r * P.mlen + (u2 - q * P.upr) * G;
     }
-    return n;
+    cnt = min(G, min((r + 1) * P.mlen, P.p_begin + P.p_count) - p);
+}
+
+// host: fills n_units, row0, nu0, upr and the division constants of a launch over pairs [p_begin, p_begin + p_count)
+template <class Params>
+static inline void pdzy_plan_units(Params &P, int G) {
+    const int p_end = P.p_begin + P.p_count;
+    P.row0 = P.p_begin / P.mlen;
+    const int first_end = std::min((P.row0 + 1) * P.mlen, p_end);
+    P.nu0 = (first_end - P.p_begin + G - 1) / G;
+    P.upr = (P.mlen + G - 1) / G;
+    int n = P.nu0;
+    for (int p = first_end; p < p_end; p += P.mlen) n += (std::min(p + P.mlen, p_end) - p + G - 1) / G;
+    P.n_units = n;
+    P.magic_n1 = pdzy_magic(P.N1);
+    P.magic_upr = pdzy_magic(P.upr);
 }
 
 
@@ -244,11 +255,12 @@ __global__ void __launch_bounds__(NW * 32, MINB) pd_zy_kernel(const __grid_const
         k.g = 0;
         k.cnt = 0;
         if (k.w < n_items) {
-            const int u = k.w / P.N1;
+            const int u = pdzy_fastdiv(k.w, P.magic_n1);
+            int r;
             k.j1 = k.w - u * P.N1;
-            pdzy_unit<G>(P, u, k.p0, k.cnt);
-            k.n = P.n0 + k.p0 / P.mlen;
-            k.m = P.m0 + k.p0 % P.mlen;
+            pdzy_unit<G>(P, u, k.p0, k.cnt, r);
+            k.n = P.n0 + r;
+            k.m = P.m0 + k.p0 - r * P.mlen;
         }
     };
     auto advance = [&](PdZyCursor &k) {

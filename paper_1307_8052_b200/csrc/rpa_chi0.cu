@@ -358,7 +358,9 @@ void plan_zy_kernel(rpa_chi0 *h) {
     try_zy<PdZy<N3_, NA3_, DLO_, DHI_, N2_, NA2_, NW_, LPW_, G_>>(                     \
         h, pd_zy_kernel<N3_, NA3_, DLO_, DHI_, N2_, NA2_, NW_, LPW_, G_, MINB_, ##__VA_ARGS__>, G_, MINB_)
     if (N2 == 60 && N3 == 64) ZY(64, 8, -1, 0, 60, 12, 4, 4, 4, 2, true);
-    else if (N2 == 24 && N3 == 24) ZY(24, 8, -1, 0, 24, 8, 3, 8, 4, 3);
+    // 24-point lines as 6 x 4 (4 lanes per line, 8 lines per warp: every lane busy, 64 contiguous bytes per line and load
+    // instruction) and 12 x 2 in y: 1.58 -> 1.33 ms per 8 k-points of configs[2] against the 8 x 3 / 8 x 3 split
+    else if (N2 == 24 && N3 == 24) ZY(24, 6, -1, 0, 24, 12, 3, 8, 4, 3);
     else if (N2 == 16 && N3 == 16) ZY(16, 8, -1, 0, 16, 8, 1, 16, 4, 8);
     else if (N2 == 40 && N3 == 168) ZY(168, 12, -2, 1, 40, 8, 4, 2, 1, 2);
     else if (N2 == 48 && N3 == 192) ZY(192, 12, -3, 2, 48, 12, 8, 2, 2, 1, true);
@@ -761,7 +763,7 @@ int add_kpoint_impl(rpa_chi0_t *h, double kweight, int32_t n_occ, const void *ps
                     P.N1 = N1;
                     P.n0 = n0; P.mlen = mlen; P.m0 = m0;
                     P.p_begin = p0; P.p_count = pc;
-                    P.n_units = pdzy_count_units(p0, pc, mlen, h->zy_G);
+                    pdzy_plan_units(P, h->zy_G);
                     P.g2min = sp.gmin[1]; P.ng2 = ng2; P.g3min = sp.gmin[2]; P.ng3 = ng3;
                     // persistent 1-D grid: one CTA per resident slot, work items (unit, plane) dealt round-robin
                     const int nctas = std::max(1, std::min(P.n_units * N1, h->n_sm * h->zy_ctas_per_sm));
@@ -785,12 +787,21 @@ int add_kpoint_impl(rpa_chi0_t *h, double kweight, int32_t n_occ, const void *ps
                 {
                     StageTimer tm(h, 1, 1);
                     const int xslots = pd_xaxis8_slots(N1, sp.gmin[0], ng1);
-                    if (xslots == 2)
-                        pd_xaxis8_kernel<2><<<dim3((nb2 + 127) / 128, pc), 128, (size_t)N1 * 2 * sizeof(cd), st>>>(
-                            h->ptr<cd>(L.I), Nbuf, L.ldn, h->ptr<cd>(L.tw1), h->ptr<int32_t>(L.box2s), N1, nb2, sp.gmin[0], ng1, p0, inv_n);
+                    const int xbx = (nb2 + 127) / 128;
+                    // short x axes (compile-time N1): blocks walk over the pairs, as many as keep every SM busy with ~8 blocks;
+                    // long axes: one block per (column block, pair) as before (measured: the walk loses 4-5 % there)
+                    const bool xshort = xslots == 2 && (N1 == 24 || N1 == 16);
+                    const int xby = xshort ? std::max(1, std::min(pc, (h->n_sm * 8 + xbx - 1) / xbx)) : pc;
+#define X8_ARGS h->ptr<cd>(L.I), Nbuf, L.ldn, h->ptr<cd>(L.tw1), h->ptr<int32_t>(L.box2s), N1, nb2, sp.gmin[0], ng1, p0, pc, inv_n
+                    if (xslots == 2 && N1 == 24)
+                        pd_xaxis8_kernel<2, 3><<<dim3(xbx, xby), 128, (size_t)N1 * 2 * sizeof(cd), st>>>(X8_ARGS);
+                    else if (xslots == 2 && N1 == 16)
+                        pd_xaxis8_kernel<2, 2><<<dim3(xbx, xby), 128, (size_t)N1 * 2 * sizeof(cd), st>>>(X8_ARGS);
+                    else if (xslots == 2)
+                        pd_xaxis8_kernel<2, 0><<<dim3(xbx, xby), 128, (size_t)N1 * 2 * sizeof(cd), st>>>(X8_ARGS);
                     else if (xslots == 3)
-                        pd_xaxis8_kernel<3><<<dim3((nb2 + 127) / 128, pc), 128, (size_t)N1 * 3 * sizeof(cd), st>>>(
-                            h->ptr<cd>(L.I), Nbuf, L.ldn, h->ptr<cd>(L.tw1), h->ptr<int32_t>(L.box2s), N1, nb2, sp.gmin[0], ng1, p0, inv_n);
+                        pd_xaxis8_kernel<3, 0><<<dim3(xbx, xby), 128, (size_t)N1 * 3 * sizeof(cd), st>>>(X8_ARGS);
+#undef X8_ARGS
                     else
                         pd_xaxis_kernel<<<dim3((nb2 + 127) / 128, pc), 128, (size_t)N1 * PD_G1_BLOCK * sizeof(cd), st>>>(
                             h->ptr<cd>(L.I), Nbuf, L.ldn, h->ptr<cd>(L.tw1), h->ptr<int32_t>(L.box2s), N1, nb2, sp.gmin[0], ng1, p0, inv_n);

@@ -246,3 +246,79 @@ def test_int8_tcgen05_probe_self_check():
     assert 2000.0 < tops < 6000.0
     tf = probes.rpa_probe_fp64_tensor_peak("cuda:0")
     assert 20.0 < tf < 60.0   # B200: 40 TFLOP/s nominal FP64
+
+
+def test_nothing_is_written_outside_the_workspace_and_the_outputs():
+    """A write-bounds check of every kernel of the path (compute-sanitizer is closed on this GPU pool, see
+    profiles/r2_sanitizer.md): the workspace, chi0_out and psi_out sit between 8 MB guard bands filled with a byte
+    pattern; after add_kpoint (PAW, both FP64 kernels, the int8 kernel with and without clusters, 6 / 7 / 8 digits),
+    get, ec_q (Cholesky), pw_to_grid and symmetry_remap on configs[0] and on a ragged skewed-cell grid the bands must be
+    untouched and the workspace bytes beyond what rpa_chi0_workspace_bytes reported must be too."""
+    import ctypes as C
+    import torch
+    from paper_1307_8052_b200 import binding as B
+    GUARD = 8 << 20
+
+    def guarded(nbytes):
+        buf = torch.full((GUARD + nbytes + 256 + GUARD,), 0xA5, dtype=torch.uint8, device="cuda:0")
+        off = GUARD + (-(buf.data_ptr() + GUARD)) % 256
+        return buf, off
+
+    def check(buf, off, nbytes, what):
+        assert bool((buf[:off] == 0xA5).all()), f"{what}: bytes before the buffer were overwritten"
+        assert bool((buf[off + nbytes:] == 0xA5).all()), f"{what}: bytes after the buffer were overwritten"
+
+    cell = np.array([[6.0, 0.2, 0.0], [0.1, 5.0, 0.3], [0.0, -0.2, 7.0]])
+    ragged = W.custom_config(777, cell, (12, 10, 14), (0.25, 0.0, 0.5), n_occ=3, n_unocc=7, ng_target=33, n_omega=5, n_atoms=2,
+                             n_proj_per_atom=3, orb_ecut_ha=2.0)
+    modes = [(B.RPA_RANK_K_FP64_3M, 0), (B.RPA_RANK_K_FP64_4M, 0)]
+    for digits in (6, 7, 8):
+        modes.append((B.RPA_RANK_K_I8 | B.RPA_RANK_K_FLAG_ALL_BATCHES, digits))
+    modes.append((B.RPA_RANK_K_I8 | B.RPA_RANK_K_FLAG_ALL_BATCHES | B.RPA_RANK_K_FLAG_NO_CLUSTER, 7))
+    for cfg in (W.CONFIGS[0], ragged):
+        om, wt = W.omega_grid(cfg.n_omega)
+        ptot = int(cfg.n_proj.sum())
+        nbytes = B.rpa_chi0_workspace_bytes(cfg.grid, cfg.cell, cfg.q_red, W.tuned_ecut(cfg), cfg.n_omega, 48, ptot)
+        ws, ws_off = guarded(nbytes)
+        g32, c64, q64 = np.asarray(cfg.grid, np.int32), np.ascontiguousarray(cfg.cell, np.float64).reshape(9), np.asarray(cfg.q_red, np.float64)
+        out = C.c_void_p()
+        stream = torch.cuda.current_stream()
+        rc = B.lib().rpa_chi0_create(C.byref(out), g32.ctypes.data_as(C.c_void_p), c64.ctypes.data_as(C.c_void_p),
+                                     q64.ctypes.data_as(C.c_void_p), W.tuned_ecut(cfg), cfg.n_omega, om.ctypes.data_as(C.c_void_p),
+                                     wt.ctypes.data_as(C.c_void_p), 48, ptot, C.c_void_p(ws.data_ptr() + ws_off), C.c_size_t(nbytes),
+                                     C.c_void_p(stream.cuda_stream))
+        assert rc == 0, B.rpa_last_error()
+        h = B.Handle(out, ws, torch.device("cuda", 0), stream, g32, cfg.n_omega)
+        try:
+            g, K2 = B.rpa_chi0_gvectors(h)
+            ng = len(g)
+            kd = W.kpoint(cfg, 0)
+            d = _dev(kd)
+            Qd = torch.from_numpy(W.paw_Q(cfg, K2)).to("cuda:0")
+            chi_buf, chi_off = guarded(ng * ng * 16)
+            chi = chi_buf[chi_off:chi_off + ng * ng * 16].view(torch.complex128).view(ng, ng)
+            for mode in modes:
+                B.rpa_chi0_set_rank_k_mode(h, *mode)
+                B.rpa_chi0_add_kpoint(h, 1.0, d["psi_occ"], d["psi_unocc"], kd.eps_occ, kd.eps_unocc, kd.f_occ, kd.f_unocc,
+                                      cfg.n_proj, d["P_occ"], d["P_unocc"], Qd, W.atom_positions(cfg))
+                for i in range(cfg.n_omega):
+                    B.rpa_chi0_get(h, i, chi)
+                B.rpa_ec_q(h, W.coulomb(K2))
+                B.rpa_chi0_sync(h)
+                check(ws, ws_off, nbytes, f"workspace, mode {mode}")
+                check(chi_buf, chi_off, ng * ng * 16, f"chi0_out, mode {mode}")
+            # Table 1 steps 3-4
+            g_pw, C_o, _ = W.kpoint_coefficients(cfg, 0, occ=range(cfg.n_occ), unocc=[])
+            N = int(np.prod(cfg.grid))
+            psi_buf, psi_off = guarded(cfg.n_occ * N * 16)
+            psi = psi_buf[psi_off:psi_off + cfg.n_occ * N * 16].view(torch.complex128).view((cfg.n_occ,) + tuple(cfg.grid))
+            B.rpa_pw_to_grid(h, g_pw, torch.from_numpy(C_o).to("cuda:0"), psi)
+            B.rpa_chi0_sync(h)
+            check(psi_buf, psi_off, cfg.n_occ * N * 16, "psi_out of rpa_pw_to_grid")
+            check(ws, ws_off, nbytes, "workspace after rpa_pw_to_grid")
+            src = psi.clone()
+            B.rpa_symmetry_remap(h, src, np.diag([-1, -1, -1]), True, psi)
+            B.rpa_chi0_sync(h)
+            check(psi_buf, psi_off, cfg.n_occ * N * 16, "psi_out of rpa_symmetry_remap")
+        finally:
+            h.close()
