@@ -222,6 +222,9 @@ struct rpa_chi0 {
     bool use_3m = true;                // rank_k3m_kernel (3-multiplication complex product); false: rank_k_kernel<true> (4M)
     int64_t i8_batches = 0, fp64_batches = 0;   // batches each rank-K path has taken (rpa_chi0_rank_k_batches)
     int ec_lanes = EC_DEFAULT_LANES;   // rpa_chi0_set_ec_lanes
+    struct EcGraph { int nm, lanes; cudaGraphExec_t exec; int64_t launches; };
+    std::vector<EcGraph> ec_graphs;    // captured factorisations of rpa_ec_q, one per (matrices in the group, lanes)
+    bool ec_use_graph = true;
     cudaStream_t side = nullptr;       // panel factorisations of rpa_ec_q run here, ahead of the trailing updates
     cudaEvent_t ev_panel[2] = {nullptr, nullptr}, ev_col = nullptr, ev_fork = nullptr;
     // further lanes of rpa_ec_q (each factorises its share of the matrices of a group on its own stream pair)
@@ -982,6 +985,128 @@ int rpa_chi0_get(rpa_chi0_t *h, int32_t i_omega, void *chi0_out) {
 }  // extern "C"
 
 namespace {
+// The blocked Cholesky of the nm matrices of a group (M[0 .. nm), in place; ln det into logdet, flags on a non-positive
+// pivot), enqueued on the caller's stream and the handle's side streams: everything between the fork event on the caller's
+// stream and the join back onto it.  *launches receives the number of kernels enqueued.
+int ec_enqueue_factorization(rpa_chi0 *h, int nm, int n_lanes, int64_t *launches) {
+    const Layout &L = h->L;
+    const int ng = h->sp.ng;
+    cudaStream_t st = h->stream;
+    cd *M = h->ptr<cd>(L.M);
+    int *d_flag = h->ptr<int>(L.flag);
+    double *d_ld = h->ptr<double>(L.logdet);
+    const int64_t lt_mat = (int64_t)CH_P * CH_NB * L.ldn;          // per matrix
+    const size_t lt_block = (size_t)L.ec_group * lt_mat;           // per block buffer
+    const double *wneg = h->ptr<double>(L.wneg);
+    struct Lane {
+        cudaStream_t main, side;
+        cudaEvent_t *ev_panel, ev_col;
+        int m0, nm;
+    } lanes[EC_MAX_LANES];
+    for (int l = 0, m0 = 0; l < n_lanes; l++) {   // matrices dealt as evenly as possible
+        const int cnt = nm / n_lanes + (l < nm % n_lanes ? 1 : 0);
+        if (l == 0) lanes[l] = {st, h->side, h->ev_panel, h->ev_col, m0, cnt};
+        else lanes[l] = {h->xmain[l - 1], h->xside[l - 1], h->xev_panel[l - 1], h->xev_col[l - 1], m0, cnt};
+        m0 += cnt;
+    }
+    auto update = [&](const Lane &ln, cudaStream_t s_, cd *Lt, int K, int g0, int mode, int col_limit) {
+        const int rest = ng - g0;
+        if (rest <= 0) return 0;
+        const int nt = (rest + rk::T - 1) / rk::T;
+        const int tiles = mode == 1   ? nt
+                          : mode == 2 ? ntiles_lower(rest, rk::T) - nt
+                          : mode == 3 ? nt + std::max(nt - 1, 0)
+                          : mode == 4 ? (nt > 2 ? (nt - 2) * (nt - 1) / 2 : 0)
+                                      : ntiles_lower(rest, rk::T);
+        if (tiles <= 0) return 0;
+        rank_k_kernel<false><<<dim3(tiles, ln.nm), rk::Cfg<false>::THREADS, rk::Cfg<false>::SMEM_BYTES, s_>>>(
+            Lt, L.ldn, lt_mat, K, wneg, CH_P * CH_NB, M + (size_t)ln.m0 * ng * ng, ng, (int64_t)ng * ng, ng, g0, ln.nm, mode,
+            col_limit);
+        return 1;
+    };
+    CUDA_TRY(cudaEventRecord(h->ev_fork, st));
+    for (int l = 0; l < n_lanes; l++) {
+        CUDA_TRY(cudaStreamWaitEvent(lanes[l].side, h->ev_fork, 0));
+        if (l > 0) CUDA_TRY(cudaStreamWaitEvent(lanes[l].main, h->ev_fork, 0));
+    }
+    int blk = 0;
+    for (int kb = 0; kb < ng; kb += CH_P * CH_NB, blk++) {
+        for (int l = 0; l < n_lanes; l++) {
+            const Lane &ln = lanes[l];
+            cd *Lt = h->ptr<cd>(L.Lt) + (size_t)(blk & 1) * lt_block + (size_t)ln.m0 * lt_mat;
+            // the block's panels and strips: the serial chain, all on the high-priority side stream
+            int np = 0;   // panels of this block
+            for (int p = 0; p < CH_P && kb + p * CH_NB < ng; p++, np++) {
+                const int c0 = kb + p * CH_NB;
+                const int rest = ng - (c0 + CH_NB);
+                if (p > 0) *launches += update(ln, ln.side, Lt, p * CH_NB, c0, 1, c0 + CH_NB);
+                chol_panel_kernel<<<dim3(std::max(1, (rest + 127) / 128), ln.nm), CH_THREADS, 0, ln.side>>>(
+                    M + (size_t)ln.m0 * ng * ng, ng, c0, Lt + (size_t)p * CH_NB * L.ldn, L.ldn, lt_mat, d_flag + ln.m0,
+                    d_ld + ln.m0);
+                *launches += 1;
+            }
+            CUDA_TRY(cudaEventRecord(ln.ev_panel[blk & 1], ln.side));
+            CUDA_TRY(cudaStreamWaitEvent(ln.main, ln.ev_panel[blk & 1], 0));
+            const int g0 = kb + np * CH_NB;
+            if (g0 < ng) {
+                // look-ahead: the first two tile columns (= the next block's 128 columns) on the side stream, after
+                // the previous block's big update; the rest of the trailing matrix on the main stream meanwhile
+                if (blk > 0) CUDA_TRY(cudaStreamWaitEvent(ln.side, ln.ev_col, 0));
+                *launches += update(ln, ln.side, Lt, np * CH_NB, g0, 3, ng);
+                *launches += update(ln, ln.main, Lt, np * CH_NB, g0, 4, ng);
+                CUDA_TRY(cudaEventRecord(ln.ev_col, ln.main));
+            }
+        }
+    }
+    for (int l = 1; l < n_lanes; l++) {   // join: the caller's stream continues after the other lanes
+        CUDA_TRY(cudaEventRecord(h->xev_join[l - 1], lanes[l].main));
+        CUDA_TRY(cudaStreamWaitEvent(st, h->xev_join[l - 1], 0));
+    }
+    CUDA_TRY(cudaGetLastError());
+    return RPA_OK;
+}
+
+// The same through a CUDA graph: the factorisation of a group is ~170 (1 lane) to ~600 (4 lanes) small dependent launches
+// on up to eight streams, and issuing them costs the host more than the device needs to run them (every lane adds its own
+// launches and event operations to the one issuing thread).  The launch sequence depends only on (nm, n_lanes) -- all
+// pointers lie in the caller's workspace -- so it is captured once per handle and shape and replayed with one
+// cudaGraphLaunch.  Falls back to direct launches if capture or instantiation fails.
+int ec_factorize(rpa_chi0 *h, int nm, int n_lanes) {
+    if (h->ec_use_graph) {
+        for (auto &g : h->ec_graphs)
+            if (g.nm == nm && g.lanes == n_lanes) {
+                CUDA_TRY(cudaGraphLaunch(g.exec, h->stream));
+                h->launches += g.launches;
+                return RPA_OK;
+            }
+        if (h->ec_graphs.size() < 16) {
+            int64_t n = 0;
+            cudaGraph_t graph = nullptr;
+            cudaGraphExec_t exec = nullptr;
+            bool ok = cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+            if (ok) {
+                const int rc = ec_enqueue_factorization(h, nm, n_lanes, &n);
+                const cudaError_t e = cudaStreamEndCapture(h->stream, &graph);
+                ok = rc == RPA_OK && e == cudaSuccess && graph != nullptr;
+            }
+            if (ok) ok = cudaGraphInstantiate(&exec, graph, 0) == cudaSuccess;
+            if (graph) cudaGraphDestroy(graph);
+            if (ok) {
+                h->ec_graphs.push_back({nm, n_lanes, exec, n});
+                CUDA_TRY(cudaGraphLaunch(exec, h->stream));
+                h->launches += n;
+                return RPA_OK;
+            }
+            cudaGetLastError();          // clear the capture error
+            h->ec_use_graph = false;     // and stay on direct launches
+        }
+    }
+    int64_t n = 0;
+    const int rc = ec_enqueue_factorization(h, nm, n_lanes, &n);
+    h->launches += n;
+    return rc;
+}
+
 // e(omega_i) for i in [iw_begin, iw_end) and ec = (1/2pi) sum over that range of wt_i e_i
 int ec_q_impl(rpa_chi0_t *h, const double *v_G, int iw_begin, int iw_end, double *ec_ha, double *e_omega) {
     if (!h || !v_G || !ec_ha) return fail(RPA_ERR_INVALID_ARG, "rpa_ec_q: NULL argument");
@@ -1023,73 +1148,10 @@ int ec_q_impl(rpa_chi0_t *h, const double *v_G, int iw_begin, int iw_end, double
         // its panel steps.  Two lanes by default; rpa_chi0_set_ec_lanes(h, n) (1 ... 4) chooses (measured on 16 matrices of 1200
         // with the whole-block look-ahead: 2.68 / 2.66 / 2.64 / 2.63 ms for 1 / 2 / 3 / 4 lanes: the chain of a lane
         // does not get shorter, so more lanes add little).
-        const int64_t lt_mat = (int64_t)CH_P * CH_NB * L.ldn;          // per matrix
-        const size_t lt_block = (size_t)L.ec_group * lt_mat;           // per block buffer
-        const double *wneg = h->ptr<double>(L.wneg);
         const int n_lanes = std::max(1, std::min({h->ec_lanes, EC_MAX_LANES, nm}));
-        struct Lane {
-            cudaStream_t main, side;
-            cudaEvent_t *ev_panel, ev_col;
-            int m0, nm;
-        } lanes[EC_MAX_LANES];
-        for (int l = 0, m0 = 0; l < n_lanes; l++) {   // matrices dealt as evenly as possible
-            const int cnt = nm / n_lanes + (l < nm % n_lanes ? 1 : 0);
-            if (l == 0) lanes[l] = {st, h->side, h->ev_panel, h->ev_col, m0, cnt};
-            else lanes[l] = {h->xmain[l - 1], h->xside[l - 1], h->xev_panel[l - 1], h->xev_col[l - 1], m0, cnt};
-            m0 += cnt;
-        }
-        auto update = [&](const Lane &ln, cudaStream_t s_, cd *Lt, int K, int g0, int mode, int col_limit) {
-            const int rest = ng - g0;
-            if (rest <= 0) return 0;
-            const int nt = (rest + rk::T - 1) / rk::T;
-            const int tiles = mode == 1   ? nt
-                              : mode == 2 ? ntiles_lower(rest, rk::T) - nt
-                              : mode == 3 ? nt + std::max(nt - 1, 0)
-                              : mode == 4 ? (nt > 2 ? (nt - 2) * (nt - 1) / 2 : 0)
-                                          : ntiles_lower(rest, rk::T);
-            if (tiles <= 0) return 0;
-            rank_k_kernel<false><<<dim3(tiles, ln.nm), rk::Cfg<false>::THREADS, rk::Cfg<false>::SMEM_BYTES, s_>>>(
-                Lt, L.ldn, lt_mat, K, wneg, CH_P * CH_NB, M + (size_t)ln.m0 * ng * ng, ng, (int64_t)ng * ng, ng, g0, ln.nm, mode,
-                col_limit);
-            return 1;
-        };
-        CUDA_TRY(cudaEventRecord(h->ev_fork, st));
-        for (int l = 0; l < n_lanes; l++) {
-            CUDA_TRY(cudaStreamWaitEvent(lanes[l].side, h->ev_fork, 0));
-            if (l > 0) CUDA_TRY(cudaStreamWaitEvent(lanes[l].main, h->ev_fork, 0));
-        }
-        int blk = 0;
-        for (int kb = 0; kb < ng; kb += CH_P * CH_NB, blk++) {
-            for (int l = 0; l < n_lanes; l++) {
-                const Lane &ln = lanes[l];
-                cd *Lt = h->ptr<cd>(L.Lt) + (size_t)(blk & 1) * lt_block + (size_t)ln.m0 * lt_mat;
-                // the block's panels and strips: the serial chain, all on the high-priority side stream
-                int np = 0;   // panels of this block
-                for (int p = 0; p < CH_P && kb + p * CH_NB < ng; p++, np++) {
-                    const int c0 = kb + p * CH_NB;
-                    const int rest = ng - (c0 + CH_NB);
-                    if (p > 0) h->launches += update(ln, ln.side, Lt, p * CH_NB, c0, 1, c0 + CH_NB);
-                    chol_panel_kernel<<<dim3(std::max(1, (rest + 127) / 128), ln.nm), CH_THREADS, 0, ln.side>>>(
-                        M + (size_t)ln.m0 * ng * ng, ng, c0, Lt + (size_t)p * CH_NB * L.ldn, L.ldn, lt_mat, d_flag + ln.m0,
-                        d_ld + ln.m0);
-                    h->launches += 1;
-                }
-                CUDA_TRY(cudaEventRecord(ln.ev_panel[blk & 1], ln.side));
-                CUDA_TRY(cudaStreamWaitEvent(ln.main, ln.ev_panel[blk & 1], 0));
-                const int g0 = kb + np * CH_NB;
-                if (g0 < ng) {
-                    // look-ahead: the first two tile columns (= the next block's 128 columns) on the side stream, after
-                    // the previous block's big update; the rest of the trailing matrix on the main stream meanwhile
-                    if (blk > 0) CUDA_TRY(cudaStreamWaitEvent(ln.side, ln.ev_col, 0));
-                    h->launches += update(ln, ln.side, Lt, np * CH_NB, g0, 3, ng);
-                    h->launches += update(ln, ln.main, Lt, np * CH_NB, g0, 4, ng);
-                    CUDA_TRY(cudaEventRecord(ln.ev_col, ln.main));
-                }
-            }
-        }
-        for (int l = 1; l < n_lanes; l++) {   // join: the caller's stream continues after the other lanes
-            CUDA_TRY(cudaEventRecord(h->xev_join[l - 1], lanes[l].main));
-            CUDA_TRY(cudaStreamWaitEvent(st, h->xev_join[l - 1], 0));
+        {
+            const int rc = ec_factorize(h, nm, n_lanes);
+            if (rc != RPA_OK) return rc;
         }
         CUDA_TRY(cudaGetLastError());
         ec_collect_kernel<<<1, 32, 0, st>>>(d_ld, d_tr, nm, iw0, d_e);
@@ -1249,6 +1311,7 @@ void rpa_chi0_destroy(rpa_chi0_t *h) {
         for (cudaEvent_t e : {h->xev_panel[l][0], h->xev_panel[l][1], h->xev_col[l], h->xev_join[l]})
             if (e) cudaEventDestroy(e);
     }
+    for (auto &g : h->ec_graphs) cudaGraphExecDestroy(g.exec);
     for (auto &ev : h->events) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
     for (auto &e : h->pool) cudaEventDestroy(e);
     delete h;
