@@ -9,37 +9,67 @@
 // for the same result (the cancellation in Im S is against terms of the size of |S|, i.e. an absolute error of a few
 // ulp of |S|, far inside the 1e-10 relative Frobenius tolerance of the path).
 //
-// One CTA = one 64 x 64 complex tile of the lower triangle, ONE frequency; 8 consumer warps, each 32 rows x 16 columns
-// (3 x 4 x 2 DMMA accumulators = 96 registers) + a TMA producer warp with a 3-stage ring of 32-pair chunks.  A DMMA
-// k-step covers 4 pairs; a lane loads its (row, pair) / (column, pair) element with one LDS.128 (row pitch = 32 mod
-// 128 bytes: the 8 lanes of a quarter-warp hit 8 distinct 16-byte bank groups) and forms a + b, w c, w d, w (c - d)
-// on the FP64 ALU (10 operations per 24 DMMA).
+// One CTA = one 64 x 64 complex tile of the lower triangle, ONE frequency; EIGHT warps, all of them consumers, each
+// 32 rows x 16 columns (3 x 4 x 2 DMMA accumulators = 96 registers).  A DMMA k-step covers 4 pairs; a lane loads its
+// (row, pair) / (column, pair) element with one LDS.128 (row pitch = 32 mod 128 bytes: the 8 lanes of a quarter-warp hit
+// 8 distinct 16-byte bank groups) and forms a + b, w c, w d, w (c - d) on the FP64 ALU (10 operations per 24 DMMA).
+//
+// Why eight warps and no producer warp (round 2).  The SM's register file is split over its four schedulers, so a CTA of
+// nine warps (8 consumers + a TMA producer, round 1) puts three warps on one scheduler and caps EVERY thread at 168
+// registers; with 96 accumulator registers that left no room to fetch the operands of the next k-step early, and ncu
+// (profiles/r2c_rank_k3m.md) showed the result: the two warps of a scheduler interleave their 24 DMMAs one to one, finish
+// together, and both sit in their LDS + operand-preparation bubble while the tensor pipe idles (DMMA sub-pipe 83.7 %
+// busy, top stall samples on the operand-preparation instructions).  With exactly eight warps the cap is 255 registers:
+// the operands of k-step ks + 1 are loaded (LDS first, preparation between the two halves of the DMMAs) into a second
+// register set while the DMMAs of k-step ks issue, also across stage boundaries.  The stage refills are issued by the
+// consumer warps themselves, in turn -- which is only affordable because a refill is now THREE instructions: the row
+// tile and the column tile of a 32-pair chunk are one cp.async.bulk.tensor each (a 2-D tensor map over the N buffer, box
+// 32 pairs x 66 G: the 2 extra columns give the 1056-byte row pitch the bank-conflict-free LDS.128 pattern needs, and
+// out-of-range columns of ragged edge tiles arrive as zeros), plus one bulk copy of the 32 weights.  (One 1-KB bulk copy
+// per pair row and operand, 65 per chunk, kept the round-1 producer warp 2/3 busy just issuing them: measured 60 cycles
+// per copy; folded into the consumers that cost 25 % of the kernel.)
 #pragma once
+#include <cuda.h>
 #include "rank_k.cuh"
 
 namespace rk3 {
 constexpr int T = 64;
 constexpr int KC = 32;                      // pairs per stage
 constexpr int STAGES = 3;
-#ifndef RK3_MI
-#define RK3_MI 4
-#endif
-constexpr int MI = RK3_MI;                  // 8-row blocks per warp: warp tile (8 MI) x 16
-constexpr int CONSUMER_WARPS = 4 * (T / (8 * MI));
-constexpr int THREADS = (CONSUMER_WARPS + 1) * 32;
+constexpr int MI = 4;                       // 8-row blocks per warp: warp tile 32 x 16
+constexpr int WARPS = 4 * (T / (8 * MI));   // 8
+constexpr int THREADS = WARPS * 32;
 constexpr int PITCH = T * 16 + 32;          // bytes per pair row (= 32 mod 128)
-constexpr int TILE_BYTES = KC * PITCH;      // 16896
+constexpr int BOX_DOUBLES = PITCH / 8;      // inner extent of the tensor-map box: 66 complex = 132 doubles
+constexpr int TILE_BYTES = KC * PITCH;      // 33792
 constexpr int W_BYTES = KC * 8;
 constexpr int STAGE_BYTES = 2 * TILE_BYTES + W_BYTES;
 constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 2 * STAGES * 8;
+static_assert(WARPS == 8 && KC == 32, "one pair row per lane in a refill; eight warps = 255 registers per thread");
+
+// operands of one k-step (4 pairs) of a warp: as loaded, and ready for the DMMAs
+struct Raw {
+    cd a[MI], b[2];
+    double wv;
+};
+struct Operands {
+    double are[MI], aim[MI], asum[MI], bre[2], bim[2], bdif[2];
+};
 }  // namespace rk3
 
-// Nb[Kpad][ldn] (rows >= K zero), w[n_omega][ldw], S[n_omega][ng][ldS] (lower triangle accumulated), Kpad % 32 == 0.
+// 2-D tiled bulk tensor copy global -> shared (TMA, UTMALDG in SASS): box of the tensor map at element coordinates (x, y)
+__device__ __forceinline__ void tma_load_2d(void *dst_smem, const CUtensorMap *map, int x, int y, uint64_t *bar) {
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+                 ::"r"(smem_u32(dst_smem)), "l"(map), "r"(x), "r"(y), "r"(smem_u32(bar)) : "memory");
+}
+
+// Nb[Kpad][ldn] (rows >= K zero) through nmap: a 2-D FP64 tensor map over it, dims (2 ldn, Kmax), box (132, 32);
+// w[n_omega][ldw], S[n_omega][ng][ldS] (lower triangle accumulated), Kpad % 32 == 0.
 // Work items (tile, frequency) are numbered item = iw * ntiles + tile; grid = (n_items_of_this_launch, 1, ksplit), the
 // launch covers items item_off .. item_off + gridDim.x - 1; ksplit as in rank_k_kernel (atomic tile adds when > 1).
 // The host issues the whole waves with ksplit = 1 and the last partial wave K-sliced so that it also fills the GPU.
 __global__ void __launch_bounds__(rk3::THREADS, 1)
-rank_k3m_kernel(const cd *__restrict__ Nb, int64_t ldn, int Kpad, const double *__restrict__ w, int64_t ldw,
+rank_k3m_kernel(const __grid_constant__ CUtensorMap nmap, int Kpad, const double *__restrict__ w, int64_t ldw,
                 cd *__restrict__ S, int64_t ldS, int64_t strideS, int ng, int ntiles, int item_off) {
     using namespace rk3;
     extern __shared__ __align__(128) unsigned char rk_smem[];
@@ -53,16 +83,11 @@ rank_k3m_kernel(const cd *__restrict__ Nb, int64_t ldn, int Kpad, const double *
     while (ti * (ti + 1) / 2 > t) ti--;
     const int tj = t - ti * (ti + 1) / 2;
     const int row0 = ti * T, col0 = tj * T;
-    const uint32_t rowbytes = (uint32_t)min(T, ng - row0) * 16u, colbytes = (uint32_t)min(T, ng - col0) * 16u;
-    const uint32_t stage_tx = KC * (rowbytes + colbytes) + KC * 8u;
-
-    // zero the ring once so that the never-copied tail columns of edge tiles hold finite numbers
-    for (int i = tid; i < STAGES * STAGE_BYTES / 16; i += THREADS)
-        reinterpret_cast<double2 *>(rk_smem)[i] = make_double2(0.0, 0.0);
+    constexpr uint32_t stage_tx = 2 * TILE_BYTES + KC * 8u;   // two whole boxes (out-of-range parts arrive as zeros) + weights
     if (tid == 0) {
         for (int s = 0; s < STAGES; s++) {
             mbar_init(&full[s], 1);
-            mbar_init(&empty[s], CONSUMER_WARPS);
+            mbar_init(&empty[s], WARPS);
         }
         mbar_fence_init();
     }
@@ -72,26 +97,24 @@ rank_k3m_kernel(const cd *__restrict__ Nb, int64_t ldn, int Kpad, const double *
     const int nk_all = Kpad / KC, ksplit = (int)gridDim.z;
     const int it0 = (int)(((int64_t)nk_all * blockIdx.z) / ksplit), it1 = (int)(((int64_t)nk_all * (blockIdx.z + 1)) / ksplit);
     const int nk = it1 - it0;
-    if (warp == CONSUMER_WARPS) {
-        // ---- producer warp: one 16-byte-aligned bulk copy per pair row and operand, plus the 16 weights ------------
-        for (int it = 0; it < nk; it++) {
-            const int s = it % STAGES;
-            if (it >= STAGES) mbar_wait(&empty[s], ((it / STAGES) - 1) & 1);
-            unsigned char *st = rk_smem + s * STAGE_BYTES;
-            if (lane == 0) mbar_arrive_expect_tx(&full[s], stage_tx);
-            __syncwarp();
-            const cd *Nw = Nb + ((size_t)(it0 + it) * KC + lane) * ldn;   // KC = 32: one pair row per lane
-            bulk_g2s(st + lane * PITCH, Nw + row0, rowbytes, &full[s]);
-            bulk_g2s(st + TILE_BYTES + lane * PITCH, Nw + col0, colbytes, &full[s]);
-            if (lane == 0) bulk_g2s(st + 2 * TILE_BYTES, w + (size_t)iw * ldw + (size_t)(it0 + it) * KC, KC * 8, &full[s]);
-        }
-        return;
-    }
+
+    // chunk `it` of this CTA's K slice -> its ring slot: the row tile and the column tile as one tensor copy each, plus
+    // the 32 weights.  Called by one lane.
+    auto refill = [&](int it) {
+        const int s = it % STAGES;
+        unsigned char *st = rk_smem + s * STAGE_BYTES;
+        mbar_arrive_expect_tx(&full[s], stage_tx);
+        tma_load_2d(st, &nmap, 2 * row0, (it0 + it) * KC, &full[s]);
+        tma_load_2d(st + TILE_BYTES, &nmap, 2 * col0, (it0 + it) * KC, &full[s]);
+        bulk_g2s(st + 2 * TILE_BYTES, w + (size_t)iw * ldw + (size_t)(it0 + it) * KC, KC * 8, &full[s]);
+    };
+    if (warp < STAGES && warp < nk && lane == 0) refill(warp);   // the first chunks: warps 0 .. STAGES-1
 
     const int g = lane >> 2, kq = lane & 3;
     const int rowoff = (warp >> 2) * (8 * MI), coloff = (warp & 3) * 16;
     // a warp whose sub-tile lies strictly above the diagonal, or wholly beyond the matrix edge (ragged last tile row /
-    // column), only keeps the barriers moving: the warp sharing its scheduler then has the tensor pipe to itself
+    // column), only keeps the barriers moving and takes its refill turns: the warp sharing its scheduler then has the
+    // tensor pipe to itself
     const bool active = !(ti == tj && coloff > rowoff + 8 * MI - 1) && row0 + rowoff < ng && col0 + coloff < ng;
 
     double p1[MI][2][2], p2[MI][2][2], p3[MI][2][2];
@@ -108,45 +131,86 @@ rank_k3m_kernel(const cd *__restrict__ Nb, int64_t ldn, int Kpad, const double *
     const uint32_t b_off = TILE_BYTES + kq * PITCH + (coloff + g) * 16;
     const uint32_t w_off = 2 * TILE_BYTES + kq * 8;
 
-    for (int it = 0; it < nk; it++) {
-        const int s = it % STAGES;
-        mbar_wait(&full[s], (it / STAGES) & 1);
-        if (active) {
-            const unsigned char *st = rk_smem + s * STAGE_BYTES;
+    auto load_raw = [&](Raw &r, const unsigned char *st, int ks) {
+        const uint32_t ko = ks * 4 * PITCH;
+        r.wv = *reinterpret_cast<const double *>(st + w_off + ks * 32);
 #pragma unroll
-            for (int ks = 0; ks < KC / 4; ks++) {
-                const uint32_t ko = ks * 4 * PITCH;
-                const double wv = *reinterpret_cast<const double *>(st + w_off + ks * 32);
-                double are[MI], aim[MI], asum[MI], bre[2], bim[2], bdif[2];
+        for (int mi = 0; mi < MI; mi++) r.a[mi] = *reinterpret_cast<const cd *>(st + a_off + ko + mi * 128);
 #pragma unroll
-                for (int mi = 0; mi < MI; mi++) {
-                    const cd a = *reinterpret_cast<const cd *>(st + a_off + ko + mi * 128);
-                    are[mi] = a.x;
-                    aim[mi] = a.y;
-                    asum[mi] = a.x + a.y;
-                }
+        for (int ni = 0; ni < 2; ni++) r.b[ni] = *reinterpret_cast<const cd *>(st + b_off + ko + ni * 128);
+    };
+    auto prep = [&](Operands &o, const Raw &r) {
+#pragma unroll
+        for (int mi = 0; mi < MI; mi++) {
+            o.are[mi] = r.a[mi].x;
+            o.aim[mi] = r.a[mi].y;
+            o.asum[mi] = r.a[mi].x + r.a[mi].y;
+        }
+#pragma unroll
+        for (int ni = 0; ni < 2; ni++) {
+            o.bre[ni] = r.wv * r.b[ni].x;
+            o.bim[ni] = r.wv * r.b[ni].y;
+            o.bdif[ni] = o.bre[ni] - o.bim[ni];
+        }
+    };
+    auto mma_half = [&](const Operands &o, int half) {   // 8-row blocks 2 half, 2 half + 1
+#pragma unroll
+        for (int m2 = 0; m2 < MI / 2; m2++) {
+            const int mi = half * (MI / 2) + m2;
+            if (mi < mi_valid) {   // warp-uniform
 #pragma unroll
                 for (int ni = 0; ni < 2; ni++) {
-                    const cd b = *reinterpret_cast<const cd *>(st + b_off + ko + ni * 128);
-                    bre[ni] = wv * b.x;
-                    bim[ni] = wv * b.y;
-                    bdif[ni] = bre[ni] - bim[ni];
-                }
-#pragma unroll
-                for (int mi = 0; mi < MI; mi++) {
-                    if (mi < mi_valid) {   // warp-uniform
-#pragma unroll
-                        for (int ni = 0; ni < 2; ni++) {
-                            dmma(p1[mi][ni][0], p1[mi][ni][1], are[mi], bre[ni]);
-                            dmma(p2[mi][ni][0], p2[mi][ni][1], aim[mi], bim[ni]);
-                            dmma(p3[mi][ni][0], p3[mi][ni][1], asum[mi], bdif[ni]);
-                        }
-                    }
+                    dmma(p1[mi][ni][0], p1[mi][ni][1], o.are[mi], o.bre[ni]);
+                    dmma(p2[mi][ni][0], p2[mi][ni][1], o.aim[mi], o.bim[ni]);
+                    dmma(p3[mi][ni][0], p3[mi][ni][1], o.asum[mi], o.bdif[ni]);
                 }
             }
         }
+    };
+    // one k-step: the loads of the next k-step first, its FP64-ALU preparation between the two halves of the DMMAs
+    auto step = [&](const Operands &cur, Operands &nxt, const unsigned char *st_next, int ks_next) {
+        Raw r;
+        load_raw(r, st_next, ks_next);
+        mma_half(cur, 0);
+        prep(nxt, r);
+        mma_half(cur, 1);
+    };
+
+    Operands oa, ob;
+    if (nk > 0) {
+        mbar_wait(&full[0], 0);
+        if (active) {
+            Raw r;
+            load_raw(r, rk_smem, 0);
+            prep(oa, r);
+        }
+    }
+    for (int it = 0; it < nk; it++) {
+        const int s = it % STAGES;
+        const unsigned char *st = rk_smem + s * STAGE_BYTES;
+        if (active) {
+#pragma unroll
+            for (int ks = 0; ks < KC / 4 - 2; ks += 2) {
+                step(oa, ob, st, ks + 1);
+                step(ob, oa, st, ks + 2);
+            }
+            step(oa, ob, st, KC / 4 - 1);   // k-step 6 under the loads of k-step 7: the chunk is now all in registers
+        }
         __syncwarp();
-        if (lane == 0) mbar_arrive(&empty[s]);
+        if (lane == 0) mbar_arrive(&empty[s]);   // release the slot
+        if (it + 1 < nk) {                        // k-step 7 under the loads of k-step 0 of the next chunk
+            const int s1 = (it + 1) % STAGES;
+            mbar_wait(&full[s1], ((it + 1) / STAGES) & 1);
+            if (active) step(ob, oa, rk_smem + s1 * STAGE_BYTES, 0);
+        } else if (active) {
+            mma_half(ob, 0);
+            mma_half(ob, 1);
+        }
+        // refill turn: chunk it + STAGES goes into the slot just released, once all eight warps have released it
+        if (it + STAGES < nk && (it & (WARPS - 1)) == warp && lane == 0) {
+            mbar_wait(&empty[s], (it / STAGES) & 1);
+            refill(it + STAGES);
+        }
     }
 
     if (!active) return;

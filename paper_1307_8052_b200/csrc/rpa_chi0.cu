@@ -1,6 +1,7 @@
 // librpa_chi0.so -- host orchestration and C ABI of the chi0 / RPA hot path (include/rpa_chi0.h).
 // Everything on the path runs in the kernels of pair_density.cuh, paw.cuh, rank_k.cuh and energy.cuh; this file
 // builds the sphere tables, carves the caller's workspace, plans the batches and enqueues the launches.
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdarg.h>
@@ -219,6 +220,7 @@ struct rpa_chi0 {
     bool i8_force = false;             // RPA_RANK_K_FLAG_ALL_BATCHES: also for batches below I8_MIN_NG / I8_MIN_K
     bool i8_attr_set = false;          // cudaFuncSetAttribute done for the rank_k_i8_kernel instances
     std::vector<int2> i8_tiles;        // (row block, column block) tiles that meet the lower triangle
+    CUtensorMap nmap;                  // 2-D FP64 tensor map over the N buffer for rank_k3m_kernel: dims (2 ldn, Kmax), box (132, 32)
     bool use_3m = true;                // rank_k3m_kernel (3-multiplication complex product); false: rank_k_kernel<true> (4M)
     int64_t i8_batches = 0, fp64_batches = 0;   // batches each rank-K path has taken (rpa_chi0_rank_k_batches)
     int ec_lanes = EC_DEFAULT_LANES;   // rpa_chi0_set_ec_lanes
@@ -536,6 +538,25 @@ int create_impl(rpa_chi0_t **out, const int32_t grid[3], const double cell[9], c
     }
     CREATE_TRY(cudaFuncSetAttribute(rank_k_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, rk::Cfg<true>::SMEM_BYTES));
     CREATE_TRY(cudaFuncSetAttribute(rank_k3m_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, rk3::SMEM_BYTES));
+    {
+        // tensor map of the N buffer ([pair][ldn] complex = [pair][2 ldn] doubles): the driver entry point is fetched through
+        // the runtime, so the library links against nothing but cudart
+        typedef CUresult (*EncodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                        const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                        CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        CREATE_TRY(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+        if (!fn || qres != cudaDriverEntryPointSuccess) { delete h; return fail(RPA_ERR_CUDA, "rpa_chi0_create: cuTensorMapEncodeTiled unavailable"); }
+        const cuuint64_t gdim[2] = {(cuuint64_t)(2 * h->L.ldn), (cuuint64_t)h->L.Kmax};
+        const cuuint64_t gstride[1] = {(cuuint64_t)(h->L.ldn * sizeof(cd))};
+        const cuuint32_t box[2] = {(cuuint32_t)rk3::BOX_DOUBLES, (cuuint32_t)rk3::KC};
+        const cuuint32_t estr[2] = {1, 1};
+        const CUresult cr = ((EncodeTiled)fn)(&h->nmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, h->ws + h->L.Nbuf, gdim, gstride, box, estr,
+                                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                                              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (cr != CUDA_SUCCESS) { delete h; return fail(RPA_ERR_CUDA, "rpa_chi0_create: cuTensorMapEncodeTiled failed (%d)", (int)cr); }
+    }
     // the chi0 accumulation runs on the FP64 tensor cores (rank_k3m_kernel) unless rpa_chi0_set_rank_k_mode says otherwise
     CREATE_TRY(cudaFuncSetAttribute(rank_k_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, rk::Cfg<false>::SMEM_BYTES));
 
@@ -860,7 +881,7 @@ int add_kpoint_impl(rpa_chi0_t *h, double kweight, int32_t n_occ, const void *ps
                     const int tail = units - whole;
                     auto launch = [&](int off, int count, int ksplit) {
                         rank_k3m_kernel<<<dim3(count, 1, ksplit), rk3::THREADS, rk3::SMEM_BYTES, st>>>(
-                            Nbuf, L.ldn, Kpad, w, L.ldw, h->ptr<cd>(L.S), L.ldS, (int64_t)ng * L.ldS, ng, ntiles, off);
+                            h->nmap, Kpad, w, L.ldw, h->ptr<cd>(L.S), L.ldS, (int64_t)ng * L.ldS, ng, ntiles, off);
                     };
                     double c_single = 0.0, c_tail = 0.0;
                     const int s_single = pick_ksplit(units, nchunks, h->n_sm, &c_single);
