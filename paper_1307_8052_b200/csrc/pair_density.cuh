@@ -17,7 +17,9 @@
 
 struct PdPlaneParams {
     const cd *psi_occ, *psi_unocc;  // [band][N1][N2][N3]
-    cd *I;                          // [pair - p_begin][N1][ng2][ng3]
+    cd *I;                          // [pair - p_begin][N1][ncols]: only the (g2, g3) columns that hold sphere points
+    const int32_t *coltab;          // [ncols]: (g2i << 16) | g3i of column c
+    int ncols;
     const cd *tw3, *tw2;            // exp(-2 pi i t/N3), exp(-2 pi i t/N2)
     int N1, N2, N3;
     int n0, mlen, m0;               // pair p of the batch -> band n = n0 + p / mlen, m = m0 + p % mlen
@@ -210,8 +212,11 @@ __global__ void __launch_bounds__(256) pd_plane_kernel(const __grid_constant__ P
             }
         }
         const cd *out = Y + (size_t)(npy & 1) * ysz;
-        cd *Io = P.I + ((size_t)(p - P.p_begin) * P.N1 + j1) * nb2;
-        for (int i = tid; i < nb2; i += nth) Io[i] = out[i];
+        cd *Io = P.I + ((size_t)(p - P.p_begin) * P.N1 + j1) * P.ncols;   // only the columns that hold sphere points
+        for (int i = tid; i < P.ncols; i += nth) {
+            const int oc = P.coltab[i];
+            Io[i] = out[(oc >> 16) * ng3 + (oc & 0xffff)];
+        }
         // the next pair's first z pass writes zbuf / Y only after the __syncthreads at the top of the loop
     }
 }
@@ -219,7 +224,7 @@ __global__ void __launch_bounds__(256) pd_plane_kernel(const __grid_constant__ P
 typedef void (*PdPlaneKernel)(const PdPlaneParams);
 
 // x axis + gather.  Thread (pair, b) with b = g2i*ng3 + g3i a column of the pruned box; tw1[t] = exp(-2 pi i t/N1).
-// box2s[g1i*nb2 + b] = index of (g1min+g1i, ., .) in the sphere list, or -1 outside the sphere.
+// box2s[g1i*nb2 + b] = index of (g1min+g1i, column b) in the sphere list, or -1 outside the sphere; nb2 = kept (g2, g3) columns.
 // The (ng1 x N1) DFT matrix of the kept frequencies is tabulated in shared memory ([j1][g1i], read as a warp-wide
 // broadcast); a thread keeps PD_G1_BLOCK accumulators, so a sphere with ng1 <= PD_G1_BLOCK reads I once, and the
 // loads of four x planes are issued together to cover the L2 latency.

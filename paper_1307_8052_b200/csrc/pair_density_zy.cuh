@@ -107,7 +107,10 @@ struct PrunedDft {
 
 struct PdZyParams {
     const cd *psi_occ, *psi_unocc;  // [band][N1][N2][N3]
-    cd *I;                          // [pair - p_begin][N1][ng2][ng3]
+    cd *I;                          // [pair - p_begin][N1][ncols]: only the (g2, g3) columns that hold sphere points
+    const int32_t *coltab;          // [ncols]: (g2i << 16) | g3i of column c, ascending in g2i ng3 + g3i
+    const int32_t *rowtab;          // [ng2 + 1]: first column of every g2i
+    int ncols;
     const cd *tw3, *tw2;            // exp(-2 pi i t/N3), exp(-2 pi i t/N2)
     int N1;
     int n0, mlen, m0;               // pair p of the batch -> band n = n0 + p / mlen, m = m0 + p % mlen
@@ -211,17 +214,14 @@ __global__ void __launch_bounds__(NW * 32, MINB) pd_zy_kernel(const __grid_const
                   NTH = C::NTH;
     extern __shared__ __align__(16) unsigned char pd_smem[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int ng2 = P.ng2, ng3 = P.ng3, nb2 = ng2 * ng3;
+    const int ng2 = P.ng2, ng3 = P.ng3, nb2 = P.ncols;   // nb2: columns kept (pitch of I), <= ng2 ng3
     cd *tw2s = reinterpret_cast<cd *>(pd_smem);
     cd *X = tw2s + N2;
     cd *UN = X + NW * LPW * XLINE;
     cd *Y = UN + NA3 * NTH;
     int32_t *otab = reinterpret_cast<int32_t *>(Y + (size_t)N2 * G * ng3);
     for (int i = tid; i < N2; i += NTH) tw2s[i] = P.tw2[i];
-    for (int i = tid; i < nb2; i += NTH) {
-        const int o = i / ng3;
-        otab[i] = (o << 16) | (i - o * ng3);
-    }
+    for (int i = tid; i < nb2; i += NTH) otab[i] = P.coltab[i];
 
     // ---- this thread's z role: line lw of the warp, butterfly / pass-B slot j ------------------------------------
     const int lw = lane / NB3, j = lane - lw * NB3;
@@ -304,9 +304,13 @@ __global__ void __launch_bounds__(NW * 32, MINB) pd_zy_kernel(const __grid_const
     // rows NB2 (f mod NA2) + j2 and its twiddles W_N2^(j2 f) never change
     const int yb_tpo = max(1, NTH / ng2);
     const int yb_o = (tid / yb_tpo < ng2) ? tid / yb_tpo : -1, yb_c0 = tid % yb_tpo;
-    int yb_row = 0;
+    int yb_row = 0, yb_rs = 0, yb_rc = 0;   // YROW: source row block, first kept column of the row, kept columns in it
     cd ytw[(YROW && NB2 > 1) ? NB2 - 1 : 1];
     if constexpr (YROW) {
+        if (yb_o >= 0) {
+            yb_rs = P.rowtab[yb_o];
+            yb_rc = P.rowtab[yb_o + 1] - yb_rs;
+        }
         int f = P.g2min + (yb_o >= 0 ? yb_o : 0);
         f %= N2;
         if (f < 0) f += N2;
@@ -370,20 +374,22 @@ __global__ void __launch_bounds__(NW * 32, MINB) pd_zy_kernel(const __grid_const
             }
         }
         __syncthreads();
-        if constexpr (YROW) {   // pass B, this thread's output row: columns gc = gg ng3 + col with stride yb_tpo
+        if constexpr (YROW) {   // pass B, this thread's output row: its kept columns, yb_tpo threads per row, for every pair
             if (yb_o >= 0) {
-                cd *Io = P.I + ((size_t)(p0 - P.p_begin) * P.N1 + j1) * nb2 + yb_o * ng3;
+                cd *Io = P.I + ((size_t)(p0 - P.p_begin) * P.N1 + j1) * nb2 + yb_rs;
                 const cd *src = Y + (size_t)yb_row * pitch;
-                int gg = 0, col = yb_c0;
-                while (col >= ng3) { col -= ng3; gg++; }
+                // (pair, kept column of the row) flattened, yb_tpo threads per row
+                int gg = 0, idx = yb_c0;
+                while (idx >= yb_rc && gg < cnt) { idx -= yb_rc; gg++; }
                 while (gg < cnt) {
+                    const int col = otab[yb_rs + idx] & 0xffff;
                     const cd *sp = src + gg * ng3 + col;
                     cd acc = sp[0];
 #pragma unroll
                     for (int j2 = 1; j2 < NB2; j2++) acc = cfma(ytw[j2 - 1], sp[j2 * pitch], acc);
-                    Io[(size_t)gg * P.N1 * nb2 + col] = acc;
-                    col += yb_tpo;
-                    while (col >= ng3) { col -= ng3; gg++; }
+                    Io[(size_t)gg * P.N1 * nb2 + idx] = acc;
+                    idx += yb_tpo;
+                    while (idx >= yb_rc && gg < cnt) { idx -= yb_rc; gg++; }
                 }
             }
         } else {   // pass B: out[g][o][g3i] = sum_j2 W_N2^(j2 f) A[j2 + NB2 (f mod NA2)][g][g3i]

@@ -66,6 +66,11 @@ struct Sphere {
     std::vector<double> K2;    // |q+G|^2
     std::vector<double> Kc;    // [ng][3] Cartesian q+G
     int gmin[3] = {0, 0, 0}, gmax[3] = {0, 0, 0};
+    // the (g2, g3) columns of the bounding box that hold at least one sphere point, ascending in g2i ng3 + g3i: the pruned
+    // transforms keep only these after the y axis (configs[2]: 73 of 121, configs[1]: 147 of 195)
+    std::vector<int32_t> coltab;   // (g2i << 16) | g3i
+    std::vector<int32_t> rowtab;   // [ng2 + 1]: first column of every g2i
+    int ncols = 0;
 };
 
 void recip_lattice(const double A[9], double B[9], double *vol) {
@@ -117,10 +122,24 @@ void build_sphere(const int32_t grid[3], const double B[9], const double q[3], d
             }
         }
     }
+    if (sp->ng > 0) {
+        const int ng2 = sp->gmax[1] - sp->gmin[1] + 1, ng3 = sp->gmax[2] - sp->gmin[2] + 1;
+        std::vector<char> used((size_t)ng2 * ng3, 0);
+        for (int s = 0; s < sp->ng; s++) used[(size_t)(sp->g[3 * s + 1] - sp->gmin[1]) * ng3 + (sp->g[3 * s + 2] - sp->gmin[2])] = 1;
+        sp->coltab.clear();
+        sp->rowtab.assign(ng2 + 1, 0);
+        for (int o = 0; o < ng2; o++) {
+            sp->rowtab[o] = (int32_t)sp->coltab.size();
+            for (int c = 0; c < ng3; c++)
+                if (used[(size_t)o * ng3 + c]) sp->coltab.push_back((o << 16) | c);
+        }
+        sp->rowtab[ng2] = (int32_t)sp->coltab.size();
+        sp->ncols = (int)sp->coltab.size();
+    }
 }
 
 struct Layout {
-    size_t S, Nbuf, w, I, T, M, Lt, wneg, tw1, tw2, tw3, box2s, Kc, omega, wt, band, R, aj_atom, aj_j, atom_poff, atom_ni,
+    size_t S, Nbuf, w, I, T, M, Lt, wneg, tw1, tw2, tw3, box2s, coltab, rowtab, Kc, omega, wt, band, R, aj_atom, aj_j, atom_poff, atom_ni,
         atom_qoff, v, e, tr, logdet, flag, ec, total;
     int64_t ldS, ldn, ldw;
     int Kmax, sub_pairs, ec_group;
@@ -166,6 +185,8 @@ void make_layout(const int32_t grid[3], const Sphere &sp, int n_omega, int max_b
     L->tw2 = take((size_t)grid[1] * sizeof(cd));
     L->tw3 = take((size_t)grid[2] * sizeof(cd));
     L->box2s = take((size_t)ng1 * nb2 * sizeof(int32_t));
+    L->coltab = take((size_t)nb2 * sizeof(int32_t));
+    L->rowtab = take((size_t)(sp.gmax[1] - sp.gmin[1] + 2) * sizeof(int32_t));
     L->Kc = take((size_t)ng * 3 * sizeof(double));
     L->omega = take((size_t)n_omega * sizeof(double));
     L->wt = take((size_t)n_omega * sizeof(double));
@@ -576,12 +597,17 @@ int create_impl(rpa_chi0_t **out, const int32_t grid[3], const double cell[9], c
         CREATE_TRY(cudaStreamSynchronize(h->stream));
     }
     const int ng1 = sp.gmax[0] - sp.gmin[0] + 1, ng2 = sp.gmax[1] - sp.gmin[1] + 1, ng3 = sp.gmax[2] - sp.gmin[2] + 1;
-    std::vector<int32_t> box2s((size_t)ng1 * ng2 * ng3, -1);
+    // (x frequency, kept column) -> sphere index or -1
+    std::vector<int32_t> colof((size_t)ng2 * ng3, -1);
+    for (int c = 0; c < sp.ncols; c++) colof[(size_t)(sp.coltab[c] >> 16) * ng3 + (sp.coltab[c] & 0xffff)] = c;
+    std::vector<int32_t> box2s((size_t)ng1 * sp.ncols, -1);
     for (int s = 0; s < sp.ng; s++) {
         const int a = sp.g[3 * s] - sp.gmin[0], b = sp.g[3 * s + 1] - sp.gmin[1], c = sp.g[3 * s + 2] - sp.gmin[2];
-        box2s[((size_t)a * ng2 + b) * ng3 + c] = s;
+        box2s[(size_t)a * sp.ncols + colof[(size_t)b * ng3 + c]] = s;
     }
     CREATE_TRY(cudaMemcpyAsync(h->ws + L.box2s, box2s.data(), box2s.size() * sizeof(int32_t), cudaMemcpyHostToDevice, h->stream));
+    CREATE_TRY(cudaMemcpyAsync(h->ws + L.coltab, sp.coltab.data(), sp.coltab.size() * sizeof(int32_t), cudaMemcpyHostToDevice, h->stream));
+    CREATE_TRY(cudaMemcpyAsync(h->ws + L.rowtab, sp.rowtab.data(), sp.rowtab.size() * sizeof(int32_t), cudaMemcpyHostToDevice, h->stream));
     CREATE_TRY(cudaMemcpyAsync(h->ws + L.Kc, sp.Kc.data(), sp.Kc.size() * sizeof(double), cudaMemcpyHostToDevice, h->stream));
     CREATE_TRY(cudaMemcpyAsync(h->ws + L.omega, h->omega.data(), n_omega * sizeof(double), cudaMemcpyHostToDevice, h->stream));
     CREATE_TRY(cudaMemcpyAsync(h->ws + L.wt, h->wt.data(), n_omega * sizeof(double), cudaMemcpyHostToDevice, h->stream));
@@ -783,6 +809,7 @@ int add_kpoint_impl(rpa_chi0_t *h, double kweight, int32_t n_occ, const void *ps
                     PdZyParams P;
                     P.psi_occ = (const cd *)psi_occ; P.psi_unocc = (const cd *)psi_unocc;
                     P.I = h->ptr<cd>(L.I);
+                    P.coltab = h->ptr<int32_t>(L.coltab); P.rowtab = h->ptr<int32_t>(L.rowtab); P.ncols = sp.ncols;
                     P.tw3 = h->ptr<cd>(L.tw3); P.tw2 = h->ptr<cd>(L.tw2);
                     P.N1 = N1;
                     P.n0 = n0; P.mlen = mlen; P.m0 = m0;
@@ -798,6 +825,7 @@ int add_kpoint_impl(rpa_chi0_t *h, double kweight, int32_t n_occ, const void *ps
                     PdPlaneParams P;
                     P.psi_occ = (const cd *)psi_occ; P.psi_unocc = (const cd *)psi_unocc;
                     P.I = h->ptr<cd>(L.I);
+                    P.coltab = h->ptr<int32_t>(L.coltab); P.ncols = sp.ncols;
                     P.tw3 = h->ptr<cd>(L.tw3); P.tw2 = h->ptr<cd>(L.tw2);
                     P.N1 = N1; P.N2 = N2; P.N3 = N3;
                     P.n0 = n0; P.mlen = mlen; P.m0 = m0;
@@ -811,12 +839,13 @@ int add_kpoint_impl(rpa_chi0_t *h, double kweight, int32_t n_occ, const void *ps
                 {
                     StageTimer tm(h, 1, 1);
                     const int xslots = pd_xaxis8_slots(N1, sp.gmin[0], ng1);
-                    const int xbx = (nb2 + 127) / 128;
+                    const int ncols = sp.ncols;   // the x transform runs on the kept (g2, g3) columns only
+                    const int xbx = (ncols + 127) / 128;
                     // short x axes (compile-time N1): blocks walk over the pairs, as many as keep every SM busy with ~8 blocks;
                     // long axes: one block per (column block, pair) as before (measured: the walk loses 4-5 % there)
                     const bool xshort = xslots == 2 && (N1 == 24 || N1 == 16);
                     const int xby = xshort ? std::max(1, std::min(pc, (h->n_sm * 8 + xbx - 1) / xbx)) : pc;
-#define X8_ARGS h->ptr<cd>(L.I), Nbuf, L.ldn, h->ptr<cd>(L.tw1), h->ptr<int32_t>(L.box2s), N1, nb2, sp.gmin[0], ng1, p0, pc, inv_n
+#define X8_ARGS h->ptr<cd>(L.I), Nbuf, L.ldn, h->ptr<cd>(L.tw1), h->ptr<int32_t>(L.box2s), N1, ncols, sp.gmin[0], ng1, p0, pc, inv_n
                     if (xslots == 2 && N1 == 24)
                         pd_xaxis8_kernel<2, 3><<<dim3(xbx, xby), 128, (size_t)N1 * 2 * sizeof(cd), st>>>(X8_ARGS);
                     else if (xslots == 2 && N1 == 16)
@@ -827,8 +856,8 @@ int add_kpoint_impl(rpa_chi0_t *h, double kweight, int32_t n_occ, const void *ps
                         pd_xaxis8_kernel<3, 0><<<dim3(xbx, xby), 128, (size_t)N1 * 3 * sizeof(cd), st>>>(X8_ARGS);
 #undef X8_ARGS
                     else
-                        pd_xaxis_kernel<<<dim3((nb2 + 127) / 128, pc), 128, (size_t)N1 * PD_G1_BLOCK * sizeof(cd), st>>>(
-                            h->ptr<cd>(L.I), Nbuf, L.ldn, h->ptr<cd>(L.tw1), h->ptr<int32_t>(L.box2s), N1, nb2, sp.gmin[0], ng1, p0, inv_n);
+                        pd_xaxis_kernel<<<dim3(xbx, pc), 128, (size_t)N1 * PD_G1_BLOCK * sizeof(cd), st>>>(
+                            h->ptr<cd>(L.I), Nbuf, L.ldn, h->ptr<cd>(L.tw1), h->ptr<int32_t>(L.box2s), N1, ncols, sp.gmin[0], ng1, p0, inv_n);
                     CUDA_TRY(cudaGetLastError());
                 }
             }
