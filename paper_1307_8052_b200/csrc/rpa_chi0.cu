@@ -840,23 +840,24 @@ int add_kpoint_impl(rpa_chi0_t *h, double kweight, int32_t n_occ, const void *ps
                     StageTimer tm(h, 1, 1);
                     const int xslots = pd_xaxis8_slots(N1, sp.gmin[0], ng1);
                     const int ncols = sp.ncols;   // the x transform runs on the kept (g2, g3) columns only
-                    const int xbx = (ncols + 127) / 128;
+                    const int xth = std::min(128, (ncols + 31) / 32 * 32);   // 73 kept columns (configs[2]): 96 threads, not 128
+                    const int xbx = (ncols + xth - 1) / xth;
                     // short x axes (compile-time N1): blocks walk over the pairs, as many as keep every SM busy with ~8 blocks;
                     // long axes: one block per (column block, pair) as before (measured: the walk loses 4-5 % there)
                     const bool xshort = xslots == 2 && (N1 == 24 || N1 == 16);
                     const int xby = xshort ? std::max(1, std::min(pc, (h->n_sm * 8 + xbx - 1) / xbx)) : pc;
 #define X8_ARGS h->ptr<cd>(L.I), Nbuf, L.ldn, h->ptr<cd>(L.tw1), h->ptr<int32_t>(L.box2s), N1, ncols, sp.gmin[0], ng1, p0, pc, inv_n
                     if (xslots == 2 && N1 == 24)
-                        pd_xaxis8_kernel<2, 3><<<dim3(xbx, xby), 128, (size_t)N1 * 2 * sizeof(cd), st>>>(X8_ARGS);
+                        pd_xaxis8_kernel<2, 3><<<dim3(xbx, xby), xth, (size_t)N1 * 2 * sizeof(cd), st>>>(X8_ARGS);
                     else if (xslots == 2 && N1 == 16)
-                        pd_xaxis8_kernel<2, 2><<<dim3(xbx, xby), 128, (size_t)N1 * 2 * sizeof(cd), st>>>(X8_ARGS);
+                        pd_xaxis8_kernel<2, 2><<<dim3(xbx, xby), xth, (size_t)N1 * 2 * sizeof(cd), st>>>(X8_ARGS);
                     else if (xslots == 2)
-                        pd_xaxis8_kernel<2, 0><<<dim3(xbx, xby), 128, (size_t)N1 * 2 * sizeof(cd), st>>>(X8_ARGS);
+                        pd_xaxis8_kernel<2, 0><<<dim3(xbx, xby), xth, (size_t)N1 * 2 * sizeof(cd), st>>>(X8_ARGS);
                     else if (xslots == 3)
-                        pd_xaxis8_kernel<3, 0><<<dim3(xbx, xby), 128, (size_t)N1 * 3 * sizeof(cd), st>>>(X8_ARGS);
+                        pd_xaxis8_kernel<3, 0><<<dim3(xbx, xby), xth, (size_t)N1 * 3 * sizeof(cd), st>>>(X8_ARGS);
 #undef X8_ARGS
                     else
-                        pd_xaxis_kernel<<<dim3(xbx, pc), 128, (size_t)N1 * PD_G1_BLOCK * sizeof(cd), st>>>(
+                        pd_xaxis_kernel<<<dim3((ncols + 127) / 128, pc), 128, (size_t)N1 * PD_G1_BLOCK * sizeof(cd), st>>>(
                             h->ptr<cd>(L.I), Nbuf, L.ldn, h->ptr<cd>(L.tw1), h->ptr<int32_t>(L.box2s), N1, ncols, sp.gmin[0], ng1, p0, inv_n);
                     CUDA_TRY(cudaGetLastError());
                 }
