@@ -845,7 +845,19 @@ int add_kpoint_impl(rpa_chi0_t *h, double kweight, int32_t n_occ, const void *ps
                     // short x axes (compile-time N1): blocks walk over the pairs, as many as keep every SM busy with ~8 blocks;
                     // long axes: one block per (column block, pair) as before (measured: the walk loses 4-5 % there)
                     const bool xshort = xslots == 2 && (N1 == 24 || N1 == 16);
-                    const int xby = xshort ? std::max(1, std::min(pc, (h->n_sm * 8 + xbx - 1) / xbx)) : pc;
+                    int xby = pc;
+                    if (xshort) {
+                        // every block resident at once and the same number of pairs for each: ceil(pc xbx / slots) rounds of
+                        // the pair loop (2400 pairs of a configs[2] k-point on 740 slots: 600 blocks x 4 pairs, not 1184 x 2-3 in
+                        // two waves)
+                        int per_sm = 0;
+                        const void *xk = N1 == 24 ? (const void *)pd_xaxis8_kernel<2, 3> : (const void *)pd_xaxis8_kernel<2, 2>;
+                        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, xk, xth, (size_t)N1 * 2 * sizeof(cd)) != cudaSuccess || per_sm < 1)
+                            per_sm = 4;
+                        const int slots = std::max(1, h->n_sm * per_sm / xbx);
+                        const int rounds = (pc + slots - 1) / slots;
+                        xby = (pc + rounds - 1) / rounds;
+                    }
 #define X8_ARGS h->ptr<cd>(L.I), Nbuf, L.ldn, h->ptr<cd>(L.tw1), h->ptr<int32_t>(L.box2s), N1, ncols, sp.gmin[0], ng1, p0, pc, inv_n
                     if (xslots == 2 && N1 == 24)
                         pd_xaxis8_kernel<2, 3><<<dim3(xbx, xby), xth, (size_t)N1 * 2 * sizeof(cd), st>>>(X8_ARGS);
