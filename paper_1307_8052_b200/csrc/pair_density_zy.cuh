@@ -132,7 +132,9 @@ struct PdZy {
     // enumerating the quarter-warp bank groups of the pass-A stores (k1 fixed) and pass-B loads (j fixed) of this lane
     // layout: conflict-free for NB3 = 2, 3, 8, 16, 10 % over the minimum for NB3 = 14
     static constexpr int XP = NB3 == 2 ? 3 : NB3 == 3 ? 9 : NB3 == 14 ? 17 : NB3 + ((NB3 & 1) ? 0 : 1);
-        static constexpr int XLINE = NB3 == 2 ? 26 : NB3 == 3 ? 75 : NB3 == 14 ? 206 : NA3 * XP;
+        // NB3 = 4 (two lines per quarter-warp): stores hit lw XLINE + j, loads lw XLINE + j XP: XP = 5 and XLINE = 4 mod 8 make
+    // both sets {0..7} (XLINE = NA3 XP = 30 gave two-way conflicts on both: 27 % of the kernel's wavefronts on configs[2])
+    static constexpr int XLINE = NB3 == 2 ? 26 : NB3 == 3 ? 75 : NB3 == 14 ? 206 : NB3 == 4 ? ((NA3 - 1) * XP + NB3 + 7) / 8 * 8 + 4 : NA3 * XP;
     static_assert(XLINE >= (NA3 - 1) * XP + NB3, "exchange line too short");
     static constexpr int ROWS = NW * LPW;                 // z lines per chunk
     static constexpr int NCH = (N2 + ROWS - 1) / ROWS;
