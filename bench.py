@@ -4,8 +4,9 @@
 A step is one pass of the whole hot path over the workload (S1 = create is done
 once, untimed): reset, rpa_chi0_add_kpoint for every k-point of the rank, rpa_chi0_get for every omega and
 rpa_ec_q.  `value` = transitions of all ranks / max-over-ranks device time, inputs resident in HBM.
-`e2e` = the same pass with the k-point arrays starting in pinned HOST memory (H2D inside the timed region)
-and E_c(q) / e(omega) read back to the host.  Everything is FP64 / complex128; `roofline` is the FP64
+`e2e` = the same pass in the paper's data flow: plane-wave coefficients and projections start in pinned HOST memory,
+are copied and expanded on the device (Eq. 10) inside the timed region, and E_c(q) / e(omega) are read back to the
+host; `e2e_grid` = the same with grid orbitals uploaded instead (20x the bytes, PCIe-bound).  Everything is FP64 / complex128; `roofline` is the FP64
 tensor-core rank-K kernel (rank_k3m_kernel) in TFLOP/s.  Extra blocks of the same JSON line: `rank_k_i8` (the
 opt-in int8-sliced arm, timed in the same run and compared with the FP64 result), `per_config` (configs 0 and 2
 in full, configs 3 and 4 on one 8192-transition batch at full grid / nG), `cpu_baseline` (the oracle).
@@ -387,13 +388,19 @@ def run_ours(args, cfg):
             "dtype": "f64 (complex128)", "data": "synthetic",
             "config": config_dict(cfg, ng, world, args.batch, args.exchange),
             "clocks": clocks,
-            "e2e": {"value": pairs_total / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e,
-                    "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": 8 * (1 + cfg.n_omega) + 16},
-            "e2e_pw": {"value": pairs_total / (ms_pw * 1e-3), "unit": UNIT, "ms_per_step": ms_pw,
-                       "h2d_bytes_per_step": int(h2d_pw), "d2h_bytes_per_step": 8 * (1 + cfg.n_omega) + 16,
-                       "note": "same step fed the way the paper's pipeline is (Table 1 step 3): the host holds plane-wave "
-                               "coefficients, rpa_pw_to_grid (Eq. 10) expands them on the device inside the timed region; "
-                               "e2e above uploads the grid orbitals themselves and is PCIe-bound"},
+            # end to end in the paper's own data flow (Table 1 steps 3 and 5-13): the host holds the orbitals as
+            # plane-wave coefficients; every step copies them (and the projections) from pinned host memory, expands them on
+            # the device with rpa_pw_to_grid (Eq. 10, inside the timed region), adds the k-point, reads chi0 out for every
+            # omega and reads E_c(q), e(omega) back to the host
+            "e2e": {"value": pairs_total / (ms_pw * 1e-3), "unit": UNIT, "ms_per_step": ms_pw,
+                    "h2d_bytes_per_step": int(h2d_pw), "d2h_bytes_per_step": 8 * (1 + cfg.n_omega) + 16,
+                    "input": "plane-wave coefficients C_n(Q) + PAW projections in pinned host memory -> "
+                             "binding.add_kpoint_host_pw (rpa_pw_to_grid + rpa_chi0_add_kpoint) -> rpa_chi0_get x n_omega -> rpa_ec_q"},
+            # the same step when the caller holds the orbitals on the real-space grid in host memory (20x the bytes): the
+            # upload of 2.1 GB per k-point at PCIe speed bounds it, whatever the kernels do
+            "e2e_grid": {"value": pairs_total / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e,
+                         "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": 8 * (1 + cfg.n_omega) + 16,
+                         "input": "grid orbitals u(r) in pinned host memory -> binding.add_kpoint_host (sliced, pipelined upload)"},
             "gpu_launches": int(launches),
             "roofline": roofline,
             "stages": {"ms_per_step": rep["ms_per_step"], "get_all_omega_ms": tail_ms[0] / args.steps,
