@@ -12,7 +12,10 @@
 // One CTA = one 64 x 64 complex tile of the lower triangle, ONE frequency; EIGHT warps, all of them consumers, each
 // 32 rows x 16 columns (3 x 4 x 2 DMMA accumulators = 96 registers).  A DMMA k-step covers 4 pairs; a lane loads its
 // (row, pair) / (column, pair) element with one LDS.128 (row pitch = 32 mod 128 bytes: the 8 lanes of a quarter-warp hit
-// 8 distinct 16-byte bank groups) and forms a + b, w c, w d, w (c - d) on the FP64 ALU (10 operations per 24 DMMA).
+// 8 distinct 16-byte bank groups) and forms w c, w d, w (c - d) on the FP64 ALU (6 operations per 24 DMMA).  The row
+// operand's a + b comes ready-made from a third plane, NS[pair][g] = Re + Im of N (rk3_rowsum_kernel, one pass over N per
+// batch): an FP64-ALU instruction interleaved with DMMAs costs the shared FP64 datapath about three times its nominal two
+// cycles (timing experiment, profiles/r2c_rank_k3m.md: -4.6 % without the four additions per k-step), an LDS.64 does not.
 //
 // Why eight warps and no producer warp (round 2).  The SM's register file is split over its four schedulers, so a CTA of
 // nine warps (8 consumers + a TMA producer, round 1) puts three warps on one scheduler and caps EVERY thread at 168
@@ -22,35 +25,41 @@
 // busy, top stall samples on the operand-preparation instructions).  With exactly eight warps the cap is 255 registers:
 // the operands of k-step ks + 1 are loaded (LDS first, preparation between the two halves of the DMMAs) into a second
 // register set while the DMMAs of k-step ks issue, also across stage boundaries.  The stage refills are issued by the
-// consumer warps themselves, in turn -- which is only affordable because a refill is now THREE instructions: the row
-// tile and the column tile of a 32-pair chunk are one cp.async.bulk.tensor each (a 2-D tensor map over the N buffer, box
-// 32 pairs x 66 G: the 2 extra columns give the 1056-byte row pitch the bank-conflict-free LDS.128 pattern needs, and
-// out-of-range columns of ragged edge tiles arrive as zeros), plus one bulk copy of the 32 weights.  (One 1-KB bulk copy
-// per pair row and operand, 65 per chunk, kept the round-1 producer warp 2/3 busy just issuing them: measured 60 cycles
-// per copy; folded into the consumers that cost 25 % of the kernel.)
+// consumer warps themselves, in turn -- which is only affordable because a refill is now FOUR instructions: the row
+// tile, the column tile and the row-sum tile of a 16-pair chunk are one cp.async.bulk.tensor each (2-D tensor maps over
+// the N and NS buffers, boxes 16 pairs x 66 G / 68 doubles: the extra columns give the 1056- / 544-byte row pitches the
+// bank-conflict-free LDS patterns need, and out-of-range columns of ragged edge tiles arrive as zeros), plus one bulk copy
+// of the 16 weights.  (One 1-KB bulk copy per pair row and operand, 65 per 32-pair chunk, kept the round-1 producer warp
+// 2/3 busy just issuing them: measured 60 cycles per copy; folded into the consumers that cost 25 % of the kernel.)
+// Chunks of 16 pairs in a ring of 5 (213 KB) instead of 32 in a ring of 3: the third plane would not fit otherwise.
 #pragma once
 #include <cuda.h>
 #include "rank_k.cuh"
 
 namespace rk3 {
 constexpr int T = 64;
-constexpr int KC = 32;                      // pairs per stage
-constexpr int STAGES = 3;
+constexpr int KC = 16;                      // pairs per stage
+constexpr int STAGES = 5;
 constexpr int MI = 4;                       // 8-row blocks per warp: warp tile 32 x 16
 constexpr int WARPS = 4 * (T / (8 * MI));   // 8
 constexpr int THREADS = WARPS * 32;
 constexpr int PITCH = T * 16 + 32;          // bytes per pair row (= 32 mod 128)
-constexpr int BOX_DOUBLES = PITCH / 8;      // inner extent of the tensor-map box: 66 complex = 132 doubles
-constexpr int TILE_BYTES = KC * PITCH;      // 33792
+constexpr int BOX_DOUBLES = PITCH / 8;      // inner extent of the tensor-map box over N: 66 complex = 132 doubles
+constexpr int TILE_BYTES = KC * PITCH;      // 16896
+constexpr int SPITCH = T * 8 + 32;          // bytes per pair row of the row-sum tile (= 32 mod 128: conflict-free LDS.64)
+constexpr int SBOX_DOUBLES = SPITCH / 8;    // 68
+constexpr int STILE_BYTES = KC * SPITCH;    // 8704
 constexpr int W_BYTES = KC * 8;
-constexpr int STAGE_BYTES = 2 * TILE_BYTES + W_BYTES;
+constexpr int STAGE_BYTES = 2 * TILE_BYTES + STILE_BYTES + W_BYTES;   // 42624
 constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 2 * STAGES * 8;
-static_assert(WARPS == 8 && KC == 32, "one pair row per lane in a refill; eight warps = 255 registers per thread");
+static_assert(WARPS == 8, "eight warps = 255 registers per thread");
+static_assert(TILE_BYTES % 128 == 0 && STILE_BYTES % 128 == 0 && STAGE_BYTES % 128 == 0, "TMA destinations are 128-byte aligned");
+static_assert(KC % 8 == 0 && KC / 4 >= 4 && (KC / 4) % 2 == 0, "k-steps of a chunk come in pairs, at least two pairs");
 
 // operands of one k-step (4 pairs) of a warp: as loaded, and ready for the DMMAs
 struct Raw {
     cd a[MI], b[2];
-    double wv;
+    double s[MI], wv;
 };
 struct Operands {
     double are[MI], aim[MI], asum[MI], bre[2], bim[2], bdif[2];
@@ -63,13 +72,24 @@ __device__ __forceinline__ void tma_load_2d(void *dst_smem, const CUtensorMap *m
                  ::"r"(smem_u32(dst_smem)), "l"(map), "r"(x), "r"(y), "r"(smem_u32(bar)) : "memory");
 }
 
-// Nb[Kpad][ldn] (rows >= K zero) through nmap: a 2-D FP64 tensor map over it, dims (2 ldn, Kmax), box (132, 32);
-// w[n_omega][ldw], S[n_omega][ng][ldS] (lower triangle accumulated), Kpad % 32 == 0.
+// NS[p][g] = Re N[p][g] + Im N[p][g] for p < rows, g < ldn: the third operand plane of the 3M product.
+// grid (rows, ceil(ldn / 256)), block 256.
+__global__ void __launch_bounds__(256) rk3_rowsum_kernel(const cd *__restrict__ Nb, int64_t ldn, double *__restrict__ NS) {
+    const int g = blockIdx.y * 256 + threadIdx.x;
+    if (g >= ldn) return;
+    const cd v = Nb[(size_t)blockIdx.x * ldn + g];
+    NS[(size_t)blockIdx.x * ldn + g] = v.x + v.y;
+}
+
+// Nb[Kpad][ldn] (rows >= K zero) through nmap: a 2-D FP64 tensor map over it, dims (2 ldn, Kmax), box (132, 16); its row
+// sums NS[Kpad][ldn] through smap: dims (ldn, Kmax), box (68, 16);
+// w[n_omega][ldw], S[n_omega][ng][ldS] (lower triangle accumulated), Kpad % 16 == 0.
 // Work items (tile, frequency) are numbered item = iw * ntiles + tile; grid = (n_items_of_this_launch, 1, ksplit), the
 // launch covers items item_off .. item_off + gridDim.x - 1; ksplit as in rank_k_kernel (atomic tile adds when > 1).
 // The host issues the whole waves with ksplit = 1 and the last partial wave K-sliced so that it also fills the GPU.
 __global__ void __launch_bounds__(rk3::THREADS, 1)
-rank_k3m_kernel(const __grid_constant__ CUtensorMap nmap, int Kpad, const double *__restrict__ w, int64_t ldw,
+rank_k3m_kernel(const __grid_constant__ CUtensorMap nmap, const __grid_constant__ CUtensorMap smap, int Kpad,
+                const double *__restrict__ w, int64_t ldw,
                 cd *__restrict__ S, int64_t ldS, int64_t strideS, int ng, int ntiles, int item_off) {
     using namespace rk3;
     extern __shared__ __align__(128) unsigned char rk_smem[];
@@ -83,7 +103,7 @@ rank_k3m_kernel(const __grid_constant__ CUtensorMap nmap, int Kpad, const double
     while (ti * (ti + 1) / 2 > t) ti--;
     const int tj = t - ti * (ti + 1) / 2;
     const int row0 = ti * T, col0 = tj * T;
-    constexpr uint32_t stage_tx = 2 * TILE_BYTES + KC * 8u;   // two whole boxes (out-of-range parts arrive as zeros) + weights
+    constexpr uint32_t stage_tx = 2 * TILE_BYTES + STILE_BYTES + KC * 8u;   // three whole boxes (out-of-range parts arrive as zeros) + weights
     if (tid == 0) {
         for (int s = 0; s < STAGES; s++) {
             mbar_init(&full[s], 1);
@@ -98,15 +118,16 @@ rank_k3m_kernel(const __grid_constant__ CUtensorMap nmap, int Kpad, const double
     const int it0 = (int)(((int64_t)nk_all * blockIdx.z) / ksplit), it1 = (int)(((int64_t)nk_all * (blockIdx.z + 1)) / ksplit);
     const int nk = it1 - it0;
 
-    // chunk `it` of this CTA's K slice -> its ring slot: the row tile and the column tile as one tensor copy each, plus
-    // the 32 weights.  Called by one lane.
+    // chunk `it` of this CTA's K slice -> its ring slot: the row tile, the column tile and the row-sum tile as one tensor
+    // copy each, plus the weights.  Called by one lane.
     auto refill = [&](int it) {
         const int s = it % STAGES;
         unsigned char *st = rk_smem + s * STAGE_BYTES;
         mbar_arrive_expect_tx(&full[s], stage_tx);
         tma_load_2d(st, &nmap, 2 * row0, (it0 + it) * KC, &full[s]);
         tma_load_2d(st + TILE_BYTES, &nmap, 2 * col0, (it0 + it) * KC, &full[s]);
-        bulk_g2s(st + 2 * TILE_BYTES, w + (size_t)iw * ldw + (size_t)(it0 + it) * KC, KC * 8, &full[s]);
+        tma_load_2d(st + 2 * TILE_BYTES, &smap, row0, (it0 + it) * KC, &full[s]);
+        bulk_g2s(st + 2 * TILE_BYTES + STILE_BYTES, w + (size_t)iw * ldw + (size_t)(it0 + it) * KC, KC * 8, &full[s]);
     };
     if (warp < STAGES && warp < nk && lane == 0) refill(warp);   // the first chunks: warps 0 .. STAGES-1
 
@@ -129,13 +150,17 @@ rank_k3m_kernel(const __grid_constant__ CUtensorMap nmap, int Kpad, const double
     const int mi_valid = min(MI, (ng - (row0 + rowoff) + 7) / 8);
     const uint32_t a_off = kq * PITCH + (rowoff + g) * 16;
     const uint32_t b_off = TILE_BYTES + kq * PITCH + (coloff + g) * 16;
-    const uint32_t w_off = 2 * TILE_BYTES + kq * 8;
+    const uint32_t s_off = 2 * TILE_BYTES + kq * SPITCH + (rowoff + g) * 8;
+    const uint32_t w_off = 2 * TILE_BYTES + STILE_BYTES + kq * 8;
 
     auto load_raw = [&](Raw &r, const unsigned char *st, int ks) {
         const uint32_t ko = ks * 4 * PITCH;
         r.wv = *reinterpret_cast<const double *>(st + w_off + ks * 32);
 #pragma unroll
-        for (int mi = 0; mi < MI; mi++) r.a[mi] = *reinterpret_cast<const cd *>(st + a_off + ko + mi * 128);
+        for (int mi = 0; mi < MI; mi++) {
+            r.a[mi] = *reinterpret_cast<const cd *>(st + a_off + ko + mi * 128);
+            r.s[mi] = *reinterpret_cast<const double *>(st + s_off + ks * 4 * SPITCH + mi * 64);
+        }
 #pragma unroll
         for (int ni = 0; ni < 2; ni++) r.b[ni] = *reinterpret_cast<const cd *>(st + b_off + ko + ni * 128);
     };
@@ -144,7 +169,7 @@ rank_k3m_kernel(const __grid_constant__ CUtensorMap nmap, int Kpad, const double
         for (int mi = 0; mi < MI; mi++) {
             o.are[mi] = r.a[mi].x;
             o.aim[mi] = r.a[mi].y;
-            o.asum[mi] = r.a[mi].x + r.a[mi].y;
+            o.asum[mi] = r.s[mi];
         }
 #pragma unroll
         for (int ni = 0; ni < 2; ni++) {
@@ -194,11 +219,11 @@ rank_k3m_kernel(const __grid_constant__ CUtensorMap nmap, int Kpad, const double
                 step(oa, ob, st, ks + 1);
                 step(ob, oa, st, ks + 2);
             }
-            step(oa, ob, st, KC / 4 - 1);   // k-step 6 under the loads of k-step 7: the chunk is now all in registers
+            step(oa, ob, st, KC / 4 - 1);   // the last k-step but one under the loads of the last: the chunk is now all in registers
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty[s]);   // release the slot
-        if (it + 1 < nk) {                        // k-step 7 under the loads of k-step 0 of the next chunk
+        if (it + 1 < nk) {                        // the last k-step under the loads of k-step 0 of the next chunk
             const int s1 = (it + 1) % STAGES;
             mbar_wait(&full[s1], ((it + 1) / STAGES) & 1);
             if (active) step(ob, oa, rk_smem + s1 * STAGE_BYTES, 0);

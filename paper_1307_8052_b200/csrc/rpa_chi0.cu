@@ -139,7 +139,7 @@ void build_sphere(const int32_t grid[3], const double B[9], const double q[3], d
 }
 
 struct Layout {
-    size_t S, Nbuf, w, I, T, M, Lt, wneg, tw1, tw2, tw3, box2s, coltab, rowtab, Kc, omega, wt, band, R, aj_atom, aj_j, atom_poff, atom_ni,
+    size_t S, Nbuf, NS, w, I, T, M, Lt, wneg, tw1, tw2, tw3, box2s, coltab, rowtab, Kc, omega, wt, band, R, aj_atom, aj_j, atom_poff, atom_ni,
         atom_qoff, v, e, tr, logdet, flag, ec, total;
     int64_t ldS, ldn, ldw;
     int Kmax, sub_pairs, ec_group;
@@ -175,6 +175,7 @@ void make_layout(const int32_t grid[3], const Sphere &sp, int n_omega, int max_b
     };
     L->S = take((size_t)n_omega * ng * L->ldS * sizeof(cd));
     L->Nbuf = take((size_t)Kmax * L->ldn * sizeof(cd));
+    L->NS = take((size_t)Kmax * L->ldn * sizeof(double));   // Re + Im of N: third operand plane of rank_k3m_kernel
     L->w = take((size_t)n_omega * L->ldw * sizeof(double));
     L->I = take((size_t)L->sub_pairs * L->I_pair_bytes);
     L->T = take((size_t)MAX_SLOTS * std::max(max_proj, 0) * L->ldn * sizeof(cd));
@@ -241,7 +242,7 @@ struct rpa_chi0 {
     bool i8_force = false;             // RPA_RANK_K_FLAG_ALL_BATCHES: also for batches below I8_MIN_NG / I8_MIN_K
     bool i8_attr_set = false;          // cudaFuncSetAttribute done for the rank_k_i8_kernel instances
     std::vector<int2> i8_tiles;        // (row block, column block) tiles that meet the lower triangle
-    CUtensorMap nmap;                  // 2-D FP64 tensor map over the N buffer for rank_k3m_kernel: dims (2 ldn, Kmax), box (132, 32)
+    CUtensorMap nmap, smap;            // 2-D FP64 tensor maps for rank_k3m_kernel over N (dims (2 ldn, Kmax), box (132, 16)) and NS ((ldn, Kmax), (68, 16))
     bool use_3m = true;                // rank_k3m_kernel (3-multiplication complex product); false: rank_k_kernel<true> (4M)
     int64_t i8_batches = 0, fp64_batches = 0;   // batches each rank-K path has taken (rpa_chi0_rank_k_batches)
     int ec_lanes = EC_DEFAULT_LANES;   // rpa_chi0_set_ec_lanes
@@ -321,11 +322,11 @@ int ntiles_lower(int n, int t) {
 
 // K slices of the rank-K launch: one CTA per SM, `units` equal work items (tile x frequency pair).  With s slices
 // the grid needs ceil(units s / n_sm) rounds of 1/s of an item each; take the s that minimises that time, charging
-// 1 % per extra slice for its prologue / atomic epilogue, and keep at least 16 chunks (256 pairs) per slice.
-int pick_ksplit(int units, int nchunks, int n_sm, double *cost_out = nullptr) {
+// 1 % per extra slice for its prologue / atomic epilogue, and keep at least min_chunks chunks (512 pairs) per slice.
+int pick_ksplit(int units, int nchunks, int n_sm, double *cost_out = nullptr, int min_chunks = 16) {
     int best = 1;
     double best_cost = 1e300;
-    for (int s = 1; s <= 8 && nchunks / s >= 16; s++) {
+    for (int s = 1; s <= 8 && nchunks / s >= min_chunks; s++) {
         const double rounds = (double)(((int64_t)units * s + n_sm - 1) / n_sm) / s;
         const double cost = rounds * (1.0 + 0.01 * (s - 1));
         if (cost < best_cost * (1.0 - 1e-9)) { best_cost = cost; best = s; }
@@ -577,6 +578,13 @@ int create_impl(rpa_chi0_t **out, const int32_t grid[3], const double cell[9], c
                                               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                                               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (cr != CUDA_SUCCESS) { delete h; return fail(RPA_ERR_CUDA, "rpa_chi0_create: cuTensorMapEncodeTiled failed (%d)", (int)cr); }
+        const cuuint64_t sdim[2] = {(cuuint64_t)h->L.ldn, (cuuint64_t)h->L.Kmax};
+        const cuuint64_t sstride[1] = {(cuuint64_t)(h->L.ldn * sizeof(double))};
+        const cuuint32_t sbox[2] = {(cuuint32_t)rk3::SBOX_DOUBLES, (cuuint32_t)rk3::KC};
+        const CUresult cs = ((EncodeTiled)fn)(&h->smap, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, h->ws + h->L.NS, sdim, sstride, sbox, estr,
+                                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                                              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (cs != CUDA_SUCCESS) { delete h; return fail(RPA_ERR_CUDA, "rpa_chi0_create: cuTensorMapEncodeTiled (row sums) failed (%d)", (int)cs); }
     }
     // the chi0 accumulation runs on the FP64 tensor cores (rank_k3m_kernel) unless rpa_chi0_set_rank_k_mode says otherwise
     CREATE_TRY(cudaFuncSetAttribute(rank_k_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, rk::Cfg<false>::SMEM_BYTES));
@@ -923,11 +931,14 @@ int add_kpoint_impl(rpa_chi0_t *h, double kweight, int32_t n_occ, const void *ps
                     const int tail = units - whole;
                     auto launch = [&](int off, int count, int ksplit) {
                         rank_k3m_kernel<<<dim3(count, 1, ksplit), rk3::THREADS, rk3::SMEM_BYTES, st>>>(
-                            h->nmap, Kpad, w, L.ldw, h->ptr<cd>(L.S), L.ldS, (int64_t)ng * L.ldS, ng, ntiles, off);
+                            h->nmap, h->smap, Kpad, w, L.ldw, h->ptr<cd>(L.S), L.ldS, (int64_t)ng * L.ldS, ng, ntiles, off);
                     };
+                    // third operand plane of the 3M product: NS = Re N + Im N, one pass over the batch's N
+                    rk3_rowsum_kernel<<<dim3(Kpad, (unsigned)((L.ldn + 255) / 256)), 256, 0, st>>>(Nbuf, L.ldn, h->ptr<double>(L.NS));
+                    h->launches += 1;
                     double c_single = 0.0, c_tail = 0.0;
-                    const int s_single = pick_ksplit(units, nchunks, h->n_sm, &c_single);
-                    const int s_tail = tail > 0 ? pick_ksplit(tail, nchunks, h->n_sm, &c_tail) : 1;
+                    const int s_single = pick_ksplit(units, nchunks, h->n_sm, &c_single, 512 / rk3::KC);
+                    const int s_tail = tail > 0 ? pick_ksplit(tail, nchunks, h->n_sm, &c_tail, 512 / rk3::KC) : 1;
                     // two launches only if the model says they save at least a tenth of an item
                     if (whole > 0 && tail > 0 && whole / h->n_sm + c_tail + 0.1 < c_single) {
                         launch(0, whole, 1);
