@@ -30,8 +30,9 @@
  * Internal resources: besides the workspace the handle owns seven CUDA streams (used by rpa_ec_q: a high-priority
  * stream per lane for the look-ahead update, panels and strips, which run ahead of the big trailing updates, and a
  * main stream for each lane but the first, which uses the caller's; a lane factorises its share of the frequencies
- * concurrently with the others; all ordered with the caller's stream by events) and a few events, all released by
- * rpa_chi0_destroy.
+ * concurrently with the others; all ordered with the caller's stream by events), a few events, two tensor maps over its
+ * own workspace, and the CUDA graphs rpa_ec_q captures on first use (one per number of matrices in a group and lanes: the
+ * factorisation is a few hundred small dependent launches, replayed with one launch), all released by rpa_chi0_destroy.
  *
  * Arithmetic: everything is FP64 / complex128 ("Double and double complex precision").  The rank-K accumulation
  * (Eq. 17 / Eq. 20) runs on the FP64 tensor cores (DMMA) by default; when that kernel splits K over several CTAs per
