@@ -158,13 +158,17 @@ struct PdZy {
 // magic d = 2^64 + e with 0 < e <= d and x magic / 2^64 = x / d + x e / (d 2^64), whose excess stays below 1 / d.
 // d = 1 has no 64-bit magic: it is encoded as 0.
 static inline unsigned long long pdzy_magic(int d) { return d <= 1 ? 0ull : ~0ull / (unsigned long long)d + 1ull; }
-__device__ __forceinline__ int pdzy_fastdiv(int x, unsigned long long magic) {
+__host__ __device__ __forceinline__ int pdzy_fastdiv(int x, unsigned long long magic) {
+#ifdef __CUDA_ARCH__
     return magic ? (int)__umul64hi((unsigned long long)(unsigned)x, magic) : x;
+#else   // the host copy exists for tests/host/unit_map_check.cu
+    return magic ? (int)(((unsigned __int128)(unsigned)x * magic) >> 64) : x;
+#endif
 }
 
 // unit u of the launch -> first pair p (relative to the batch) and the number of pairs cnt <= G, all in one row r.
 template <int G>
-__device__ __forceinline__ void pdzy_unit(const PdZyParams &P, int u, int &p, int &cnt, int &r) {
+__host__ __device__ __forceinline__ void pdzy_unit(const PdZyParams &P, int u, int &p, int &cnt, int &r) {
     if (u < P.nu0) {
         r = P.row0;
         p = P.p_begin + u * G;
@@ -173,7 +177,8 @@ __device__ __forceinline__ void pdzy_unit(const PdZyParams &P, int u, int &p, in
         r = P.row0 + 1 + q;
         p = r * P.mlen + (u2 - q * P.upr) * G;
     }
-    cnt = min(G, min((r + 1) * P.mlen, P.p_begin + P.p_count) - p);
+    const int rest = ((r + 1) * P.mlen < P.p_begin + P.p_count ? (r + 1) * P.mlen : P.p_begin + P.p_count) - p;
+    cnt = rest < G ? rest : G;
 }
 
 // host: fills n_units, row0, nu0, upr and the division constants of a launch over pairs [p_begin, p_begin + p_count)

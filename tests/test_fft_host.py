@@ -25,3 +25,18 @@ def test_butterflies_and_lines_match_direct_dft(tmp_path):
         assert err >= 0.0, (kind, n)
         tol = 1e-14 * max(4.0, float(n))
         assert err < tol, (kind, n, err)
+
+
+@pytest.mark.skipif(not (os.path.exists(NVCC) or shutil.which("nvcc")), reason="nvcc not available")
+def test_work_item_map_of_the_pair_density_kernel_matches_a_plain_walk(tmp_path):
+    """pdzy_plan_units / pdzy_unit / pdzy_fastdiv (csrc/pair_density_zy.cuh): closed-form unit -> (row, first pair, count)
+    map with magic-number divisions, against a walk over the pairs, for 60 000 random launches (starting mid-row, ending
+    mid-row, single pairs, G = 1, 2, 4) and the launch shapes of the BASELINE configs."""
+    exe = str(tmp_path / "unit_map_check")
+    src = os.path.join(HERE, "host", "unit_map_check.cu")
+    r = subprocess.run([NVCC, "-O1", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-diag-suppress", "20208", "-o", exe, src],
+                       capture_output=True, text=True)
+    assert r.returncode == 0, r.stderr
+    out = subprocess.run([exe], capture_output=True, text=True)
+    cases, bad = (int(x) for x in out.stdout.split())
+    assert out.returncode == 0 and bad == 0 and cases == 60000, out.stdout
