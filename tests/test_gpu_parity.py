@@ -278,3 +278,43 @@ def test_rank_k_mode_setter_validates():
         assert B.rpa_chi0_rank_k_batches(h) == (0, 0)
     finally:
         h.close()
+
+
+def test_config4_batch_spanning_two_pair_density_launches():
+    """A default-size batch of configs[4] (8 x 1024 = 8192 transitions, 48x48x192 grid) needs 5 GB of pair-density scratch, more
+    than the 4 GB the library gives it, so the batch is transformed by TWO launches of the z/y and x kernels, the second
+    starting in the middle of an occupied row (pair 7050 = row 6, column 906).  The same k-point added with
+    max_batch_pairs = 4096 (two batches of four whole rows, one launch each) must give the same chi0 to rounding; that
+    configuration's kernels are compared with the oracle by test_config4_large_batch_every_rank_k_mode."""
+    import torch
+    from paper_1307_8052_b200 import binding as B
+    cfg = W.CONFIGS[4]
+    om, wt = W.omega_grid(cfg.n_omega)
+    ptot = int(cfg.n_proj.sum())
+    occ, unocc = list(range(8)), list(range(1024))
+    g_pw, C_o, C_u = W.kpoint_coefficients(cfg, 0, occ, unocc)
+    eps, f = W.eigenvalues(cfg, 0)
+    P = W.projections(cfg, 0)
+    bo, bu = np.asarray(occ), np.asarray(unocc) + cfg.n_occ
+    c = np.ascontiguousarray
+    out = []
+    for batch in (0, 4096):
+        h = B.rpa_chi0_create(cfg.grid, cfg.cell, cfg.q_red, W.tuned_ecut(cfg), om, wt, batch, ptot, "cuda:0")
+        try:
+            g, K2 = B.rpa_chi0_gvectors(h)
+            psi_o = B.rpa_pw_to_grid(h, g_pw, torch.from_numpy(C_o).to("cuda:0"))
+            psi_u = B.rpa_pw_to_grid(h, g_pw, torch.from_numpy(C_u).to("cuda:0"))
+            Qd = torch.from_numpy(W.paw_Q(cfg, K2)).to("cuda:0")
+            B.rpa_chi0_add_kpoint(h, 0.125, psi_o, psi_u, c(eps[bo]), c(eps[bu]), c(f[bo]), c(f[bu]), cfg.n_proj,
+                                  torch.from_numpy(c(P[bo])).to("cuda:0"), torch.from_numpy(c(P[bu])).to("cuda:0"), Qd,
+                                  W.atom_positions(cfg))
+            assert B.rpa_chi0_rank_k_batches(h)[0] == (1 if batch == 0 else 2)
+            chi = B.rpa_chi0_get(h, 5)
+            sel = torch.arange(0, chi.shape[0], 7, device="cuda:0")
+            out.append(chi[sel][:, sel].cpu().numpy())
+            del chi, psi_o, psi_u, Qd
+        finally:
+            h.close()
+        torch.cuda.empty_cache()
+    assert rel_fro(out[0], out[1]) <= 1e-12
+    assert np.abs(out[0] - out[1]).max() <= 1e-11 * np.abs(out[1]).max()
