@@ -22,6 +22,10 @@ def _compare(cfg, kds, use_paw=True, max_batch_pairs=0):
     for i in range(cfg.n_omega):
         err = rel_fro(chi_g[i], chi_o[i])
         assert err <= CHI_TOL, f"omega {i}: rel Frobenius error {err:.3e}"
+        # and element by element: no element (far off-diagonal ones included) further from the oracle than 1e-10 of the
+        # largest element -- a norm dominated by the diagonal cannot hide a wrong small element behind it
+        worst = float(np.abs(chi_g[i] - chi_o[i]).max() / np.abs(chi_o[i]).max())
+        assert worst <= CHI_TOL, f"omega {i}: largest element error {worst:.3e} of the largest element"
     assert abs(ec_g[0] - ec_o[0]) <= EC_TOL * abs(ec_o[0]), (ec_g[0], ec_o[0])
     # e(omega) = ln det + Tr is a cancelling difference at large omega: compare on the scale of the largest term
     assert np.allclose(ec_g[1], ec_o[1], rtol=EC_TOL, atol=1e-12 * np.abs(ec_o[1]).max())

@@ -99,9 +99,10 @@ def _element_bound_case(cfg, kd, digits, use_paw=True):
     return worst_i8, worst_fp
 
 
-@pytest.mark.parametrize("digits", [6, 7, 8])
+@pytest.mark.parametrize("digits", [0, 6, 7, 8])
 def test_element_bound_ordinary_rows(digits):
-    """configs[0] as generated: all transitions of a row have comparable size."""
+    """configs[0] as generated: all transitions of a row have comparable size.  digits = 0: the default FP64 kernel, every
+    element within the rounding of an FP64 sum of its own terms (8 K u sum_p |w| |n_g| |n_g'|)."""
     cfg = W.CONFIGS[0]
     _element_bound_case(cfg, W.kpoint(cfg, 0), digits)
 
