@@ -291,7 +291,7 @@ __global__ void __launch_bounds__(128) pd_xaxis_kernel(const cd *__restrict__ I,
 // pairs pl = blockIdx.y, blockIdx.y + gridDim.y, ... of the launch, so the twiddle table, the kept-slot mask and the
 // column's scatter indices are set up once per block and not once per pair.
 template <int PD_X8_ND, int NBT>   // PD_X8_ND: kept-frequency slots per residue mod 8 (2 when the box needs no more: fewer registers)
-__global__ void __launch_bounds__(128) pd_xaxis8_kernel(const cd *__restrict__ I, cd *__restrict__ Nbuf, int64_t ldn,
+__global__ void __launch_bounds__(128, 4) pd_xaxis8_kernel(const cd *__restrict__ I, cd *__restrict__ Nbuf, int64_t ldn,
                                                        const cd *__restrict__ tw1, const int32_t *__restrict__ box2s,
                                                        int N1, int nb2, int g1min, int ng1, int p_begin, int p_count, double inv_n) {
     extern __shared__ __align__(16) unsigned char pd_smem[];
