@@ -322,3 +322,59 @@ def test_config4_batch_spanning_two_pair_density_launches():
         torch.cuda.empty_cache()
     assert rel_fro(out[0], out[1]) <= 1e-12
     assert np.abs(out[0] - out[1]).max() <= 1e-11 * np.abs(out[1]).max()
+
+
+def _full_config_every_element(cfg, k_list):
+    """A BASELINE config at FULL size -- every k-point in k_list with all its bands, default batching, device-resident
+    arrays, one rpa_chi0_add_kpoint per k-point: the launch configuration bench.py times -- against a FULL oracle run:
+    every element of every frequency (relative Frobenius <= 1e-10 and largest element error <= 1e-10 of the largest
+    element) and E_c(q), e(omega) against the oracle's own unblocked Cholesky."""
+    import torch
+    from paper_1307_8052_b200 import binding as B
+    import oracle
+    om, wt = W.omega_grid(cfg.n_omega)
+    ptot = int(cfg.n_proj.sum())
+    h = B.rpa_chi0_create(cfg.grid, cfg.cell, cfg.q_red, W.tuned_ecut(cfg), om, wt, 0, ptot, "cuda:0")
+    orc = oracle.Chi0Oracle(cfg.grid, cfg.cell, cfg.q_red, W.tuned_ecut(cfg), om, wt)
+    try:
+        g, K2 = B.rpa_chi0_gvectors(h)
+        assert (g == orc.g).all()
+        Q = W.paw_Q(cfg, K2)
+        Qd = torch.from_numpy(Q).to("cuda:0")
+        R = W.atom_positions(cfg)
+        for k in k_list:
+            kd = W.kpoint(cfg, k)
+            dv = {n: torch.from_numpy(getattr(kd, n)).to("cuda:0") for n in ("psi_occ", "psi_unocc", "P_occ", "P_unocc")}
+            B.rpa_chi0_add_kpoint(h, kd.kweight, dv["psi_occ"], dv["psi_unocc"], kd.eps_occ, kd.eps_unocc, kd.f_occ, kd.f_unocc,
+                                  cfg.n_proj, dv["P_occ"], dv["P_unocc"], Qd, R)
+            orc.add_kpoint(kd, cfg.n_proj, Q, R)   # the CPU works while the GPU does
+            B.rpa_chi0_sync(h)
+            del dv
+        assert B.rpa_chi0_rank_k_batches(h)[1] == 0   # the default FP64 kernel
+        chi_o = orc.get()
+        for i in range(cfg.n_omega):
+            c = B.rpa_chi0_get(h, i).cpu().numpy()
+            err = rel_fro(c, chi_o[i])
+            assert err <= CHI_TOL, f"omega {i}: rel Frobenius error {err:.3e}"
+            worst = float(np.abs(c - chi_o[i]).max() / np.abs(chi_o[i]).max())
+            assert worst <= CHI_TOL, f"omega {i}: largest element error {worst:.3e}"
+        v = W.coulomb(K2)
+        ec, e = B.rpa_ec_q(h, v)
+        ec_o, e_o = orc.ec_q(v)
+        assert abs(ec - ec_o) <= EC_TOL * abs(ec_o), (ec, ec_o)
+        assert np.allclose(e, e_o, rtol=EC_TOL, atol=1e-12 * np.abs(e_o).max())
+    finally:
+        h.close()
+
+
+def test_config1_full_size_every_element():
+    """configs[1] in full (7200 transitions, 56x60x64 grid, nG = 1200, 16 omega, PAW): all 16 x 1200 x 1200 elements and E_c(q)
+    against a full oracle run (about half a minute of CPU)."""
+    _full_config_every_element(W.CONFIGS[1], [0])
+
+
+def test_config2_full_every_kpoint_every_element():
+    """configs[2] in full: all 64 k-points x 8 x 300 bands = 153 600 transitions (24^3 grid, nG = 401, 16 omega, PAW): all
+    elements and E_c(q) against a full oracle run (about a minute of CPU)."""
+    cfg = W.CONFIGS[2]
+    _full_config_every_element(cfg, list(range(cfg.n_k)))
