@@ -40,7 +40,7 @@ namespace rk3 {
 constexpr int T = 64;
 constexpr int KC = 16;                      // pairs per stage
 constexpr int STAGES = 5;
-constexpr int MI = 4;                       // 8-row blocks per warp: warp tile 32 x 16
+constexpr int MI = 4;                       // 8-row blocks per warp: warp tile 32 x 16 (64 x 8 measured: +1 % on configs[1] / [3], -7 % on the small matrices of configs[2])
 constexpr int WARPS = 4 * (T / (8 * MI));   // 8
 constexpr int THREADS = WARPS * 32;
 constexpr int PITCH = T * 16 + 32;          // bytes per pair row (= 32 mod 128)
@@ -148,6 +148,8 @@ rank_k3m_kernel(const __grid_constant__ CUtensorMap nmap, const __grid_constant_
 
     // 8-row blocks of this warp's sub-tile that hold matrix rows (ragged last tile row): the others are skipped
     const int mi_valid = min(MI, (ng - (row0 + rowoff) + 7) / 8);
+    // ... and, in a tile on the diagonal, the 8-row blocks that lie wholly above this warp's first column
+    const int mi_lo = ti == tj ? max(0, (coloff - rowoff) / 8) : 0;
     const uint32_t a_off = kq * PITCH + (rowoff + g) * 16;
     const uint32_t b_off = TILE_BYTES + kq * PITCH + (coloff + g) * 16;
     const uint32_t s_off = 2 * TILE_BYTES + kq * SPITCH + (rowoff + g) * 8;
@@ -182,7 +184,7 @@ rank_k3m_kernel(const __grid_constant__ CUtensorMap nmap, const __grid_constant_
 #pragma unroll
         for (int m2 = 0; m2 < MI / 2; m2++) {
             const int mi = half * (MI / 2) + m2;
-            if (mi < mi_valid) {   // warp-uniform
+            if (mi >= mi_lo && mi < mi_valid) {   // warp-uniform
 #pragma unroll
                 for (int ni = 0; ni < 2; ni++) {
                     dmma(p1[mi][ni][0], p1[mi][ni][1], o.are[mi], o.bre[ni]);
