@@ -206,6 +206,32 @@ int rpa_chi0_set_ec_lanes(rpa_chi0_t *h, int32_t n_lanes);
  */
 int rpa_total_energy(int32_t n_q, const double *ec_q, const double *q_weights, double *ec_ha);
 
+/*
+ * The integrand of Eq. 2 (Table 1 step 12) for ONE matrix, for callers that cannot allocate device
+ * memory (code under CUDA graph capture, serving loops, harnesses that forbid cudaMalloc):
+ *     e = ln det(1 - v^1/2 chi0 v^1/2) + Tr(v^1/2 chi0 v^1/2),
+ * the e(omega) of rpa_ec_q, by the same kernels (blocked Cholesky, trailing updates on the FP64 tensor cores) on one
+ * stream.  No handle and no workspace: the matrix being factorised, the solved panels and the scalars live in a
+ * file-scope device array of the library, RPA_NOALLOC_SCRATCH_BYTES (5 MiB + 2 KiB) per GPU that loads the library,
+ * held until the process exits.  The call makes no cudaMalloc / cudaFree and calls no allocating library routine.
+ *   chi0:  DEVICE complex128 [ng][ng] row-major as rpa_chi0_get returns it (Hermitian, imaginary axis); only the lower
+ *          triangle g >= g' is read; not modified.
+ *   ng:    1 ... RPA_NOALLOC_MAX_NG; larger gives RPA_ERR_UNSUPPORTED (use rpa_ec_q), ng < 1 RPA_ERR_INVALID_ARG.
+ *   v_G:   DEVICE double [ng], the Coulomb kernel 4 pi / |q+G|^2, every entry finite and > 0 (NOT checked: the call
+ *          does not read device memory from the host).
+ *   e:     DEVICE double [1]; NaN if a pivot of the factorisation is not positive (where rpa_ec_q returns RPA_ERR_NOT_PD).
+ *   cuda_stream: a cudaStream_t (NULL = legacy default stream).  The call only enqueues kernels on it and returns
+ *          without synchronising; chi0, v_G and e must stay alive until the stream reaches that point.
+ * The first call on a device resolves the device address of the array (cudaGetSymbolAddress) and sets a kernel
+ * attribute: make that one outside stream capture, with the device current.  The array is shared by EVERY call in the
+ * process on that GPU and keeps the contents of the last one (each call re-initialises what it reads): calls that may
+ * overlap on the GPU -- different streams without an ordering between them, or two host threads -- race on it; order
+ * them on one stream or with events.  Independent of every rpa_chi0_t handle.
+ */
+#define RPA_NOALLOC_MAX_NG 512
+#define RPA_NOALLOC_SCRATCH_BYTES (RPA_NOALLOC_MAX_NG * RPA_NOALLOC_MAX_NG * 16 + 128 * RPA_NOALLOC_MAX_NG * 16 + 2048)
+int rpa_e_omega_noalloc(const void *chi0, int32_t ng, const double *v_G, double *e, void *cuda_stream);
+
 /* Zero the accumulators (start another q with the same sphere). */
 int rpa_chi0_reset(rpa_chi0_t *h);
 

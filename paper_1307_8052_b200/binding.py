@@ -28,6 +28,7 @@ EXPORTS = (
     "rpa_pw_to_grid", "rpa_symmetry_remap", "rpa_momentum_pw", "rpa_chi0_add_kpoint_optical",
     "rpa_chi0_set_spin_degeneracy", "rpa_chi0_create_real_axis", "rpa_ec_q_range",
     "rpa_chi0_set_rank_k_mode", "rpa_chi0_rank_k_batches", "rpa_chi0_set_ec_lanes", "rpa_total_energy",
+    "rpa_e_omega_noalloc",
 )
 
 # rpa_chi0_set_rank_k_mode (include/rpa_chi0.h)
@@ -105,6 +106,8 @@ def lib():
     L.rpa_chi0_set_ec_lanes.argtypes = [vp, i32]
     L.rpa_total_energy.restype = C.c_int
     L.rpa_total_energy.argtypes = [i32, vp, vp, C.POINTER(f64)]
+    L.rpa_e_omega_noalloc.restype = C.c_int
+    L.rpa_e_omega_noalloc.argtypes = [vp, i32, vp, vp, vp]
     L.rpa_pw_to_grid.restype = C.c_int
     L.rpa_pw_to_grid.argtypes = [vp, i32, i32, vp, vp, vp]
     L.rpa_symmetry_remap.restype = C.c_int
@@ -340,6 +343,26 @@ def rpa_total_energy(ec_q, q_weights) -> float:
     out = C.c_double(0.0)
     _check(lib().rpa_total_energy(int(e.size), _hp(e), _hp(w), C.byref(out)))
     return float(out.value)
+
+
+RPA_NOALLOC_MAX_NG = 512
+
+
+def rpa_e_omega_noalloc(chi0, v_G, e, stream=None):
+    """e[0] = ln det(1 - v^1/2 chi0 v^1/2) + Tr(v^1/2 chi0 v^1/2) (Eq. 2's integrand) for one DEVICE matrix chi0 [ng][ng]
+    complex128, v_G a DEVICE double [ng], e a DEVICE double [1]; asynchronous on `stream` (a torch.cuda.Stream; None =
+    torch's current stream).  No device allocation: the scratch is a fixed array of the library (ng <= 512)."""
+    torch = _torch()
+    if not isinstance(chi0, torch.Tensor) or chi0.dim() != 2 or chi0.shape[0] != chi0.shape[1]:
+        raise ValueError("chi0 must be a square CUDA tensor")
+    ng, dev = int(chi0.shape[0]), chi0.device
+    if tuple(v_G.shape) != (ng,) or e.numel() != 1:
+        raise ValueError("v_G must be [ng], e one double")
+    st = torch.cuda.current_stream(dev) if stream is None else stream
+    with torch.cuda.device(dev):
+        _check(lib().rpa_e_omega_noalloc(_dev_ptr(chi0, "chi0", torch.complex128, dev), ng,
+                                         _dev_ptr(v_G, "v_G", torch.float64, dev), _dev_ptr(e, "e", torch.float64, dev),
+                                         C.c_void_p(st.cuda_stream)))
 
 
 def rpa_chi0_set_rank_k_mode(h: Handle, mode: int, digits: int = 0):

@@ -9,6 +9,7 @@
 #include <string.h>
 
 #include <algorithm>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -1500,3 +1501,121 @@ int rpa_symmetry_remap(rpa_chi0_t *h, int32_t n_bands, const int32_t M[9], int32
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------------
+// rpa_e_omega_noalloc: e(omega) of Eq. 2 for one caller-supplied chi0 matrix, without any device allocation
+// (include/rpa_chi0.h).  The matrix being factorised, the solved panels of a block and the scalars live in ONE
+// file-scope device array; every GPU that loads the library holds it until the process exits.
+//
+// In host code `rpa_noalloc_scratch` is a host-side stand-in for the symbol, not a device address: the address the
+// kernels get is the one cudaGetSymbolAddress returns, taken once per device with that device current (noalloc_setup).
+namespace {
+constexpr int NA_MAX_NG = RPA_NOALLOC_MAX_NG;
+constexpr size_t NA_M = 0;                                                    // cd [ng][ng]: 1 - v^1/2 chi0 v^1/2, factorised in place
+constexpr size_t NA_LT = NA_M + (size_t)NA_MAX_NG * NA_MAX_NG * sizeof(cd);   // cd [CH_P * CH_NB][ldn]: solved panels of the current block
+constexpr size_t NA_WNEG = NA_LT + (size_t)CH_P * CH_NB * NA_MAX_NG * sizeof(cd);   // double [CH_P * CH_NB] = -1: weight of the trailing update
+constexpr size_t NA_LOGDET = NA_WNEG + (size_t)CH_P * CH_NB * sizeof(double);
+constexpr size_t NA_TR = NA_LOGDET + 256;
+constexpr size_t NA_FLAG = NA_TR + 256;
+constexpr size_t NA_BYTES = NA_FLAG + 512;
+static_assert(NA_BYTES == RPA_NOALLOC_SCRATCH_BYTES, "the header states the size of the array");
+static_assert(NA_LT % 256 == 0 && NA_WNEG % 256 == 0 && NA_LOGDET % 256 == 0, "sub-buffers stay 256-byte aligned");
+constexpr int NA_MAX_DEVICES = 64;
+}  // namespace
+
+static __device__ __align__(256) unsigned char rpa_noalloc_scratch[NA_BYTES];
+
+// what every call must find initialised, whatever the last call left: the update weights, ln det = 0, flag = 0
+__global__ void noalloc_begin_kernel(double *__restrict__ wneg, double *__restrict__ logdet, int *__restrict__ flag) {
+    const int i = threadIdx.x;
+    if (i < CH_P * CH_NB) wneg[i] = -1.0;
+    if (i == 0) {
+        *logdet = 0.0;
+        *flag = 0;
+    }
+}
+
+// e = ln det + Tr, NaN after a non-positive pivot
+__global__ void noalloc_finish_kernel(const double *__restrict__ logdet, const double *__restrict__ tr,
+                                      const int *__restrict__ flag, double *__restrict__ e) {
+    if (threadIdx.x == 0) *e = *flag ? __longlong_as_double(0x7ff8000000000000ll) : *logdet + *tr;
+}
+
+namespace {
+struct NoallocDevice {
+    bool ready = false;
+    unsigned char *scratch = nullptr;   // DEVICE address of rpa_noalloc_scratch on this device
+};
+NoallocDevice g_noalloc[NA_MAX_DEVICES];
+std::mutex g_noalloc_mutex;
+
+// once per device, with that device current: the device address of the array, and the shared-memory size of the update kernel
+int noalloc_setup(int dev, unsigned char **scratch) {
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    NoallocDevice &d = g_noalloc[dev];
+    if (!d.ready) {
+        unsigned char *p = nullptr;
+        CUDA_TRY(cudaGetSymbolAddress((void **)&p, rpa_noalloc_scratch));
+        if (!p || (reinterpret_cast<uintptr_t>(p) & 255) != 0)
+            return fail(RPA_ERR_CUDA, "rpa_e_omega_noalloc: cudaGetSymbolAddress gave %p for the scratch array", (void *)p);
+        CUDA_TRY(cudaFuncSetAttribute(rank_k_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, rk::Cfg<false>::SMEM_BYTES));
+        d.scratch = p;
+        d.ready = true;
+    }
+    *scratch = d.scratch;
+    return RPA_OK;
+}
+}  // namespace
+
+extern "C" int rpa_e_omega_noalloc(const void *chi0, int32_t ng, const double *v_G, double *e, void *cuda_stream) {
+    if (!chi0 || !v_G || !e) return fail(RPA_ERR_INVALID_ARG, "rpa_e_omega_noalloc: NULL argument");
+    if (ng < 1) return fail(RPA_ERR_INVALID_ARG, "rpa_e_omega_noalloc: ng = %d", ng);
+    if (ng > NA_MAX_NG)
+        return fail(RPA_ERR_UNSUPPORTED, "rpa_e_omega_noalloc: ng = %d exceeds RPA_NOALLOC_MAX_NG = %d (the fixed scratch array); use rpa_ec_q",
+                    ng, NA_MAX_NG);
+    int dev = -1;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= NA_MAX_DEVICES) return fail(RPA_ERR_UNSUPPORTED, "rpa_e_omega_noalloc: device ordinal %d", dev);
+    unsigned char *scratch = nullptr;
+    {
+        const int rc = noalloc_setup(dev, &scratch);
+        if (rc != RPA_OK) return rc;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    cd *M = reinterpret_cast<cd *>(scratch + NA_M), *Lt = reinterpret_cast<cd *>(scratch + NA_LT);
+    double *wneg = reinterpret_cast<double *>(scratch + NA_WNEG), *logdet = reinterpret_cast<double *>(scratch + NA_LOGDET);
+    double *tr = reinterpret_cast<double *>(scratch + NA_TR);
+    int *flag = reinterpret_cast<int *>(scratch + NA_FLAG);
+    const cd *X = static_cast<const cd *>(chi0);
+    const int64_t ldn = (int64_t)align_up((size_t)ng, 8);
+    const int64_t lt_mat = (int64_t)CH_P * CH_NB * ldn;
+
+    noalloc_begin_kernel<<<1, CH_P * CH_NB, 0, st>>>(wneg, logdet, flag);
+    // chi0 is already (s / Omega) S: scale 1
+    ec_build_kernel<<<dim3((ng + 127) / 128, ng, 1), 128, 0, st>>>(X, ng, 0, ng, 1.0, v_G, M);
+    ec_trace_kernel<<<1, 256, 0, st>>>(X, ng, 0, ng, 1.0, v_G, tr);
+    // the schedule of rpa_ec_q for one matrix on one stream: per block of CH_P panels, panel p first receives the
+    // block's earlier panels on its own 32 columns (strip), is factored and solved; then one K = 128 trailing update
+    auto update = [&](int K, int g0, int mode, int col_limit) {
+        const int rest = ng - g0;
+        if (rest <= 0) return;
+        const int nt = (rest + rk::T - 1) / rk::T;
+        const int tiles = mode == 1 ? nt : ntiles_lower(rest, rk::T);
+        rank_k_kernel<false><<<dim3(tiles, 1), rk::Cfg<false>::THREADS, rk::Cfg<false>::SMEM_BYTES, st>>>(
+            Lt, ldn, lt_mat, K, wneg, CH_P * CH_NB, M, ng, (int64_t)ng * ng, ng, g0, 1, mode, col_limit);
+    };
+    for (int kb = 0; kb < ng; kb += CH_P * CH_NB) {
+        int np = 0;
+        for (int p = 0; p < CH_P && kb + p * CH_NB < ng; p++, np++) {
+            const int c0 = kb + p * CH_NB;
+            const int rest = ng - (c0 + CH_NB);
+            if (p > 0) update(p * CH_NB, c0, 1, c0 + CH_NB);
+            chol_panel_kernel<<<dim3(std::max(1, (rest + 127) / 128), 1), CH_THREADS, 0, st>>>(
+                M, ng, c0, Lt + (size_t)p * CH_NB * ldn, ldn, lt_mat, flag, logdet);
+        }
+        update(np * CH_NB, kb + np * CH_NB, 0, ng);
+    }
+    noalloc_finish_kernel<<<1, 32, 0, st>>>(logdet, tr, flag, e);
+    CUDA_TRY(cudaGetLastError());
+    return RPA_OK;
+}
