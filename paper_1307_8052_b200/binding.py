@@ -533,28 +533,68 @@ def add_kpoint_host(h: Handle, kd, n_proj=None, Q_dev=None, R_cart=None, pinned=
 
 
 def add_kpoint_host_pw(h: Handle, kweight, g_pw, C_occ, C_unocc, eps_occ, eps_unocc, f_occ, f_unocc, n_proj=None,
-                       P_occ=None, P_unocc=None, Q_dev=None, R_cart=None):
+                       P_occ=None, P_unocc=None, Q_dev=None, R_cart=None, n_slices=4, n_calls=1):
     """The paper's own pipeline (Table 1 steps 3 and 5-11): the host holds the orbitals as plane-wave coefficients
     C_*[bands][n_pw] (host tensors, ideally pinned; g_pw[n_pw][3] their integer wave vectors) -- about 1/20 of the
     bytes of the grid orbitals -- the device expands them with rpa_pw_to_grid (Eq. 10) into buffers kept on the
-    handle and adds the k-point.  Returns the bytes copied host->device.  Marshalling only."""
+    handle and adds the k-point.  Returns the bytes copied host->device.  Marshalling only.
+
+    The coefficients go up on a side stream, the unoccupied ones in `n_slices` slices; rpa_pw_to_grid of a slice is
+    enqueued on the handle's stream behind the event of its copy, so the expansion of slice i runs under the copy of
+    slice i + 1 (rpa_pw_to_grid keeps the index table of g_pw on the device between calls and does not block).  The
+    unoccupied bands are added in `n_calls` rpa_chi0_add_kpoint calls (the accumulation is additive over any split of the
+    bands); with 2 the kernels of the first group hide the upload and expansion of the second, but on
+    configs[1] the second call costs more than that saves (measured 26.96 ms against 26.66 with one call), hence 1."""
     torch = _torch()
     dev = h.device
     have_paw = n_proj is not None and len(n_proj) > 0
-    with torch.cuda.device(dev), torch.cuda.stream(h.stream):
+    main = h.stream
+    with torch.cuda.device(dev), torch.cuda.stream(main):
         t = lambda a: a if isinstance(a, torch.Tensor) else torch.from_numpy(np.ascontiguousarray(a))
-        C_o, C_u = t(C_occ).to(dev, non_blocking=True), t(C_unocc).to(dev, non_blocking=True)
-        nbytes = (C_o.numel() + C_u.numel()) * 16
-        P_o = P_u = None
+        C_oh, C_uh = t(C_occ), t(C_unocc)
+        n_o, n_u, n_pw = int(C_oh.shape[0]), int(C_uh.shape[0]), int(C_oh.shape[1])
+        nbytes = (C_oh.numel() + C_uh.numel()) * 16
+        P_oh = P_uh = None
         if have_paw:
-            P_o, P_u = t(P_occ).to(dev, non_blocking=True), t(P_unocc).to(dev, non_blocking=True)
-            nbytes += (P_o.numel() + P_u.numel()) * 16
+            P_oh, P_uh = t(P_occ), t(P_unocc)
+            nbytes += (P_oh.numel() + P_uh.numel()) * 16
+        key = (n_o, n_u, n_pw, 0 if P_oh is None else int(P_oh.shape[1]))
         bufs = getattr(h, "_pw_bufs", None)
-        shape = (int(C_o.shape[0]), int(C_u.shape[0]))
-        if bufs is None or bufs[0] != shape:
-            bufs = h._pw_bufs = (shape, torch.empty((shape[0],) + h.grid, dtype=torch.complex128, device=dev),
-                                 torch.empty((shape[1],) + h.grid, dtype=torch.complex128, device=dev))
-        psi_o = rpa_pw_to_grid(h, g_pw, C_o, bufs[1])
-        psi_u = rpa_pw_to_grid(h, g_pw, C_u, bufs[2])
-        rpa_chi0_add_kpoint(h, kweight, psi_o, psi_u, eps_occ, eps_unocc, f_occ, f_unocc, n_proj, P_o, P_u, Q_dev, R_cart)
+        if bufs is None or bufs["key"] != key:
+            c128 = dict(dtype=torch.complex128, device=dev)
+            bufs = h._pw_bufs = {"key": key, "psi_o": torch.empty((n_o,) + h.grid, **c128), "psi_u": torch.empty((n_u,) + h.grid, **c128),
+                                 "C_o": torch.empty((n_o, n_pw), **c128), "C_u": torch.empty((n_u, n_pw), **c128),
+                                 "P_o": None if P_oh is None else torch.empty(tuple(P_oh.shape), **c128),
+                                 "P_u": None if P_uh is None else torch.empty(tuple(P_uh.shape), **c128)}
+        side = getattr(h, "_copy_stream", None)
+        if side is None:
+            side = h._copy_stream = torch.cuda.Stream(device=dev)
+        side.wait_stream(main)   # the kernels of the previous call that read these buffers are enqueued on the main stream
+
+        def upload(dst, src):
+            with torch.cuda.stream(side):
+                dst.copy_(src, non_blocking=True)
+                ev = torch.cuda.Event()
+                ev.record(side)
+            return ev
+
+        ev = upload(bufs["C_o"], C_oh)
+        main.wait_event(ev)
+        rpa_pw_to_grid(h, g_pw, bufs["C_o"], bufs["psi_o"])
+        if have_paw:
+            upload(bufs["P_o"], P_oh)
+            main.wait_event(upload(bufs["P_u"], P_uh))
+        eps_u, f_u = _np(eps_unocc, np.float64), _np(f_unocc, np.float64)
+        n_calls = max(1, min(int(n_calls), n_u))
+        per_call = max(1, -(-n_u // n_calls))
+        step = max(1, -(-per_call // max(1, int(n_slices) // n_calls)))
+        for c0 in range(0, n_u, per_call):
+            c1 = min(c0 + per_call, n_u)
+            for m0 in range(c0, c1, step):
+                m1 = min(m0 + step, c1)
+                ev = upload(bufs["C_u"][m0:m1], C_uh[m0:m1])
+                main.wait_event(ev)
+                rpa_pw_to_grid(h, g_pw, bufs["C_u"][m0:m1], bufs["psi_u"][m0:m1])
+            rpa_chi0_add_kpoint(h, kweight, bufs["psi_o"], bufs["psi_u"][c0:c1], eps_occ, eps_u[c0:c1], f_occ, f_u[c0:c1], n_proj,
+                                bufs["P_o"], None if bufs["P_u"] is None else bufs["P_u"][c0:c1], Q_dev, R_cart)
     return nbytes

@@ -141,7 +141,7 @@ void build_sphere(const int32_t grid[3], const double B[9], const double q[3], d
 
 struct Layout {
     size_t S, Nbuf, NS, w, I, T, M, Lt, wneg, tw1, tw2, tw3, box2s, coltab, rowtab, Kc, omega, wt, band, R, aj_atom, aj_j, atom_poff, atom_ni,
-        atom_qoff, v, e, tr, logdet, flag, ec, total;
+        atom_qoff, v, e, tr, logdet, flag, ec, pwtab, total;
     int64_t ldS, ldn, ldw;
     int Kmax, sub_pairs, ec_group;
     size_t I_pair_bytes;
@@ -205,6 +205,7 @@ void make_layout(const int32_t grid[3], const Sphere &sp, int n_omega, int max_b
     L->logdet = take((size_t)EC_GROUP * sizeof(double));
     L->flag = take((size_t)EC_GROUP * sizeof(int));
     L->ec = take(sizeof(double));
+    L->pwtab = take((size_t)grid[0] * grid[1] * grid[2] * sizeof(int32_t));   // plane-wave box -> coefficient index (rpa_pw_to_grid), kept between calls
     L->total = off;
 }
 
@@ -256,6 +257,10 @@ struct rpa_chi0 {
     cudaStream_t xmain[EC_MAX_LANES - 1] = {}, xside[EC_MAX_LANES - 1] = {};
     cudaEvent_t xev_panel[EC_MAX_LANES - 1][2] = {}, xev_col[EC_MAX_LANES - 1] = {}, xev_join[EC_MAX_LANES - 1] = {};
     size_t zy_smem = 0;
+    // rpa_pw_to_grid: the index table of the last g_pw, kept on the device (L.pwtab) while the caller passes the same vectors
+    std::vector<int32_t> pw_g, pw_table;
+    int pw_qmin[3] = {0, 0, 0};
+    int64_t pw_nq[3] = {0, 0, 0};
     unsigned char *ws;
     // profiling
     bool prof = false;
@@ -1406,17 +1411,28 @@ int rpa_pw_to_grid(rpa_chi0_t *h, int32_t n_bands, int32_t n_pw, const int32_t *
         CUDA_TRY(cudaMemsetAsync(psi_out, 0, (size_t)n_bands * N * sizeof(cd), st));
         return RPA_OK;
     }
+    // The table box index -> coefficient index depends only on g_pw: callers expand many band sets with the same vectors
+    // (every k-point slice, every step), so the last table stays on the device in its own workspace region and a call
+    // with the same g_pw neither rebuilds nor uploads it (and does not wait for the stream).
+    const bool cached = h->pw_g.size() == (size_t)3 * n_pw && memcmp(h->pw_g.data(), g_pw, (size_t)3 * n_pw * sizeof(int32_t)) == 0;
     int qmin[3], qmax[3];
-    for (int d = 0; d < 3; d++) qmin[d] = qmax[d] = g_pw[d];
-    for (int i = 0; i < n_pw; i++)
-        for (int d = 0; d < 3; d++) {
-            qmin[d] = std::min(qmin[d], (int)g_pw[3 * i + d]);
-            qmax[d] = std::max(qmax[d], (int)g_pw[3 * i + d]);
-        }
-    const int64_t nq1 = (int64_t)qmax[0] - qmin[0] + 1, nq2 = (int64_t)qmax[1] - qmin[1] + 1, nq3 = (int64_t)qmax[2] - qmin[2] + 1;
+    int64_t nq1, nq2, nq3;
+    if (cached) {
+        for (int d = 0; d < 3; d++) qmin[d] = h->pw_qmin[d];
+        nq1 = h->pw_nq[0]; nq2 = h->pw_nq[1]; nq3 = h->pw_nq[2];
+    } else {
+        for (int d = 0; d < 3; d++) qmin[d] = qmax[d] = g_pw[d];
+        for (int i = 0; i < n_pw; i++)
+            for (int d = 0; d < 3; d++) {
+                qmin[d] = std::min(qmin[d], (int)g_pw[3 * i + d]);
+                qmax[d] = std::max(qmax[d], (int)g_pw[3 * i + d]);
+            }
+        nq1 = (int64_t)qmax[0] - qmin[0] + 1; nq2 = (int64_t)qmax[1] - qmin[1] + 1; nq3 = (int64_t)qmax[2] - qmin[2] + 1;
+    }
     const int64_t ncol = nq2 * nq3;
     const size_t scratch = (size_t)L.sub_pairs * L.I_pair_bytes;
-    const size_t table_bytes = align_up((size_t)(nq1 * ncol) * sizeof(int32_t), 256);
+    const bool keep = nq1 * ncol <= (int64_t)N;   // fits the table region (a box inside the grid always does)
+    const size_t table_bytes = keep ? 0 : align_up((size_t)(nq1 * ncol) * sizeof(int32_t), 256);
     const size_t t1_band = (size_t)N1 * ncol * sizeof(cd);
     const size_t smem = ((size_t)N2 + N3 + ncol + (size_t)N2 * nq3) * sizeof(cd);
     if (nq1 * ncol > ((int64_t)1 << 28) || table_bytes + t1_band > scratch)
@@ -1424,17 +1440,26 @@ int rpa_pw_to_grid(rpa_chi0_t *h, int32_t n_bands, int32_t n_pw, const int32_t *
                     (long long)nq1, (long long)nq2, (long long)nq3, scratch);
     if (smem > 200 * 1024)
         return fail(RPA_ERR_UNSUPPORTED, "rpa_pw_to_grid: plane of the plane-wave box too large for shared memory (%zu B)", smem);
-    std::vector<int32_t> table((size_t)(nq1 * ncol), -1);
-    for (int i = 0; i < n_pw; i++) {
-        const size_t at = ((size_t)(g_pw[3 * i] - qmin[0]) * nq2 + (g_pw[3 * i + 1] - qmin[1])) * nq3 + (g_pw[3 * i + 2] - qmin[2]);
-        if (table[at] >= 0) return fail(RPA_ERR_INVALID_ARG, "rpa_pw_to_grid: plane wave %d duplicates plane wave %d", i, table[at]);
-        table[at] = i;
-    }
     unsigned char *base = h->ws + L.I;
-    int32_t *d_table = reinterpret_cast<int32_t *>(base);
+    int32_t *d_table = keep ? h->ptr<int32_t>(L.pwtab) : reinterpret_cast<int32_t *>(base);
     cd *T1 = reinterpret_cast<cd *>(base + table_bytes);
-    CUDA_TRY(cudaMemcpyAsync(d_table, table.data(), table.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
-    CUDA_TRY(cudaStreamSynchronize(st));   // `table` is pageable host memory about to go out of scope
+    if (!cached) {
+        h->pw_g.clear();   // no table is valid while this one is being built
+        std::vector<int32_t> &table = h->pw_table;
+        table.assign((size_t)(nq1 * ncol), -1);
+        for (int i = 0; i < n_pw; i++) {
+            const size_t at = ((size_t)(g_pw[3 * i] - qmin[0]) * nq2 + (g_pw[3 * i + 1] - qmin[1])) * nq3 + (g_pw[3 * i + 2] - qmin[2]);
+            if (table[at] >= 0) return fail(RPA_ERR_INVALID_ARG, "rpa_pw_to_grid: plane wave %d duplicates plane wave %d", i, table[at]);
+            table[at] = i;
+        }
+        CUDA_TRY(cudaMemcpyAsync(d_table, table.data(), table.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+        CUDA_TRY(cudaStreamSynchronize(st));   // `table` is pageable host memory that the next call may rewrite
+        if (keep) {
+            h->pw_g.assign(g_pw, g_pw + (size_t)3 * n_pw);
+            for (int d = 0; d < 3; d++) h->pw_qmin[d] = qmin[d];
+            h->pw_nq[0] = nq1; h->pw_nq[1] = nq2; h->pw_nq[2] = nq3;
+        }
+    }
     const PwZyKernel zy = pw_zy_pick(N2, N3);
     if (smem > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(zy, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     // table-driven persistent kernel when both in-plane axes have a radix-8 / radix-12 split and its arrays fit

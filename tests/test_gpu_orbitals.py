@@ -151,6 +151,62 @@ def test_add_kpoint_host_pw_pipeline_against_the_oracle():
     assert abs(ec - ec_o[0]) <= 1e-9 * abs(ec_o[0])
 
 
+def test_pw_to_grid_index_table_is_kept_and_invalidated():
+    """rpa_pw_to_grid keeps the index table of the last g_pw on the device: the same list again (after an add_kpoint has
+    overwritten the handle's scratch), the same vectors in another order, another list and back must all give the
+    oracle's orbitals."""
+    import torch
+    from paper_1307_8052_b200 import binding as B
+    cfg = W.CONFIGS[0]
+    kd = W.kpoint(cfg, 0)
+    g, C = _coeffs(cfg, 0, range(3))
+    perm = np.random.default_rng(5).permutation(len(g))
+    sub = perm[:41]
+    h = _handle(cfg)
+    try:
+        def check(gl, Cl):
+            u = B.rpa_pw_to_grid(h, gl, torch.from_numpy(np.ascontiguousarray(Cl)).cuda()).cpu().numpy()
+            want = oracle.pw_to_grid(cfg.grid, gl, Cl).reshape(u.shape)
+            assert np.abs(u - want).max() <= 1e-12 * np.abs(want).max()
+        check(g, C)
+        check(g, C[::-1])                       # same list: the kept table
+        B.add_kpoint_host(h, kd)                # pair densities run through the scratch the table used to live in
+        check(g, C)
+        check(g[perm], C[:, perm])              # same vectors, other order: another table
+        check(g[sub], C[:, sub])                # a smaller box
+        check(g, C)
+        with pytest.raises(B.RpaError):         # a failed build leaves no table behind
+            B.rpa_pw_to_grid(h, [[0, 0, 1], [0, 0, 1]], torch.ones((1, 2), dtype=torch.complex128, device="cuda"))
+        check(g[sub], C[:, sub])
+    finally:
+        h.close()
+
+
+def test_add_kpoint_host_pw_in_two_calls_agrees_with_one():
+    import torch
+    from paper_1307_8052_b200 import binding as B
+    cfg = W.CONFIGS[0]
+    kd = W.kpoint(cfg, 0)
+    g_pw, Co, Cu = W.kpoint_coefficients(cfg, 0)
+    h = _handle(cfg)
+    try:
+        _, K2 = B.rpa_chi0_gvectors(h)
+        Qd = torch.from_numpy(W.paw_Q(cfg, K2)).to("cuda:0")
+        pin = lambda a: torch.from_numpy(a).pin_memory()
+        Cop, Cup, Pop, Pup = pin(Co), pin(Cu), pin(kd.P_occ), pin(kd.P_unocc)
+        res = []
+        for n_calls, n_slices in ((1, 4), (2, 4), (3, 7), (1, 1)):
+            B.rpa_chi0_reset(h)
+            B.add_kpoint_host_pw(h, kd.kweight, g_pw, Cop, Cup, kd.eps_occ, kd.eps_unocc, kd.f_occ, kd.f_unocc, cfg.n_proj, Pop,
+                                 Pup, Qd, W.atom_positions(cfg), n_slices=n_slices, n_calls=n_calls)
+            res.append(np.stack([B.rpa_chi0_get(h, i).cpu().numpy() for i in range(cfg.n_omega)]))
+    finally:
+        h.close()
+    for r in res[1:]:
+        for i in range(cfg.n_omega):
+            assert rel_fro(r[i], res[0][i]) <= 1e-13
+
+
 @pytest.mark.parametrize("M,tr", [(np.eye(3, dtype=int), True), (-np.eye(3, dtype=int), False),
                                   ([[0, -1, 0], [1, 0, 0], [0, 0, 1]], False), ([[0, 1, 0], [1, 0, 0], [0, 0, -1]], True)])
 def test_symmetry_remap_bit_exact(M, tr):
