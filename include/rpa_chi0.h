@@ -197,6 +197,9 @@ int rpa_chi0_rank_k_batches(const rpa_chi0_t *h, int64_t *fp64_batches, int64_t 
 
 /* rpa_ec_q factorises the frequencies of a group in n_lanes (1 ... 4, default 2) concurrent shares, each on its own pair
  * of internal streams.  e(omega) does not depend on it (every matrix is factorised by the same kernels in the same order). */
+#define RPA_EC_FLAG_WIDE_TILES 0x100 /* or-ed into n_lanes: the updates on the serial chain of the factorisation (strips,
+                                       * look-ahead columns) in the 64 x 64 tiles of the big trailing updates instead of
+                                       * their own 32 x 32-tile kernel; same results to rounding, for comparison only */
 int rpa_chi0_set_ec_lanes(rpa_chi0_t *h, int32_t n_lanes);
 
 /*

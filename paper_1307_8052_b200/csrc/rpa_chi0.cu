@@ -251,6 +251,7 @@ struct rpa_chi0 {
     struct EcGraph { int nm, lanes; cudaGraphExec_t exec; int64_t launches; };
     std::vector<EcGraph> ec_graphs;    // captured factorisations of rpa_ec_q, one per (matrices in the group, lanes)
     bool ec_use_graph = true;
+    bool ec_tile32 = true;             // chain updates of rpa_ec_q by chol_update32_kernel (RPA_EC_FLAG_WIDE_TILES: rank_k_kernel<false>)
     cudaStream_t side = nullptr;       // panel factorisations of rpa_ec_q run here, ahead of the trailing updates
     cudaEvent_t ev_panel[2] = {nullptr, nullptr}, ev_col = nullptr, ev_fork = nullptr;
     // further lanes of rpa_ec_q (each factorises its share of the matrices of a group on its own stream pair)
@@ -594,6 +595,7 @@ int create_impl(rpa_chi0_t **out, const int32_t grid[3], const double cell[9], c
     }
     // the chi0 accumulation runs on the FP64 tensor cores (rank_k3m_kernel) unless rpa_chi0_set_rank_k_mode says otherwise
     CREATE_TRY(cudaFuncSetAttribute(rank_k_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, rk::Cfg<false>::SMEM_BYTES));
+    CREATE_TRY(cudaFuncSetAttribute(chol_update32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, cu32::smem_bytes(CH_P * CH_NB)));
 
     // tables: twiddles in extended precision, box -> sphere map
     const Sphere &sp = h->sp;
@@ -1104,6 +1106,16 @@ int ec_enqueue_factorization(rpa_chi0 *h, int nm, int n_lanes, int64_t *launches
             col_limit);
         return 1;
     };
+    // the updates on the serial chain (strips, look-ahead columns) in 32 x 32 tiles: ncolt column tiles from column g0
+    auto update32 = [&](const Lane &ln, cudaStream_t s_, cd *Lt, int K, int g0, int ncolt) {
+        const int nt = (ng - g0 + cu32::T - 1) / cu32::T;
+        int tiles = 0;
+        for (int tj = 0; tj < ncolt; tj++) tiles += std::max(nt - tj, 0);
+        if (tiles <= 0) return 0;
+        chol_update32_kernel<<<dim3(tiles, ln.nm), cu32::THREADS, cu32::smem_bytes(K), s_>>>(Lt, L.ldn, lt_mat, K,
+                                                                                             M + (size_t)ln.m0 * ng * ng, ng, g0, ncolt);
+        return 1;
+    };
     CUDA_TRY(cudaEventRecord(h->ev_fork, st));
     for (int l = 0; l < n_lanes; l++) {
         CUDA_TRY(cudaStreamWaitEvent(lanes[l].side, h->ev_fork, 0));
@@ -1119,7 +1131,8 @@ int ec_enqueue_factorization(rpa_chi0 *h, int nm, int n_lanes, int64_t *launches
             for (int p = 0; p < CH_P && kb + p * CH_NB < ng; p++, np++) {
                 const int c0 = kb + p * CH_NB;
                 const int rest = ng - (c0 + CH_NB);
-                if (p > 0) *launches += update(ln, ln.side, Lt, p * CH_NB, c0, 1, c0 + CH_NB);
+                if (p > 0)
+                    *launches += h->ec_tile32 ? update32(ln, ln.side, Lt, p * CH_NB, c0, 1) : update(ln, ln.side, Lt, p * CH_NB, c0, 1, c0 + CH_NB);
                 chol_panel_kernel<<<dim3(std::max(1, (rest + 127) / 128), ln.nm), CH_THREADS, 0, ln.side>>>(
                     M + (size_t)ln.m0 * ng * ng, ng, c0, Lt + (size_t)p * CH_NB * L.ldn, L.ldn, lt_mat, d_flag + ln.m0,
                     d_ld + ln.m0);
@@ -1132,7 +1145,7 @@ int ec_enqueue_factorization(rpa_chi0 *h, int nm, int n_lanes, int64_t *launches
                 // look-ahead: the first two tile columns (= the next block's 128 columns) on the side stream, after
                 // the previous block's big update; the rest of the trailing matrix on the main stream meanwhile
                 if (blk > 0) CUDA_TRY(cudaStreamWaitEvent(ln.side, ln.ev_col, 0));
-                *launches += update(ln, ln.side, Lt, np * CH_NB, g0, 3, ng);
+                *launches += h->ec_tile32 ? update32(ln, ln.side, Lt, np * CH_NB, g0, 2 * rk::T / cu32::T) : update(ln, ln.side, Lt, np * CH_NB, g0, 3, ng);
                 *launches += update(ln, ln.main, Lt, np * CH_NB, g0, 4, ng);
                 CUDA_TRY(cudaEventRecord(ln.ev_col, ln.main));
             }
@@ -1327,8 +1340,15 @@ int rpa_chi0_rank_k_batches(const rpa_chi0_t *h, int64_t *fp64_batches, int64_t 
 
 int rpa_chi0_set_ec_lanes(rpa_chi0_t *h, int32_t n_lanes) {
     if (!h) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_set_ec_lanes: handle is NULL");
+    const bool wide = (n_lanes & RPA_EC_FLAG_WIDE_TILES) != 0;
+    n_lanes &= ~RPA_EC_FLAG_WIDE_TILES;
     if (n_lanes < 1 || n_lanes > EC_MAX_LANES)
         return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_set_ec_lanes: n_lanes must be 1 ... %d, got %d", EC_MAX_LANES, n_lanes);
+    if (h->ec_tile32 == wide) {   // the captured graphs hold the other kernels
+        for (auto &g : h->ec_graphs) cudaGraphExecDestroy(g.exec);
+        h->ec_graphs.clear();
+    }
+    h->ec_tile32 = !wide;
     h->ec_lanes = n_lanes;
     return RPA_OK;
 }
