@@ -37,6 +37,7 @@ RPA_RANK_K_FP64_4M = 1
 RPA_RANK_K_I8 = 2
 RPA_RANK_K_FLAG_NO_CLUSTER = 0x100
 RPA_RANK_K_FLAG_ALL_BATCHES = 0x200
+RPA_EC_FLAG_WIDE_TILES = 0x100   # rpa_chi0_set_ec_lanes
 
 STAGE_NAMES = ("pair_product_fft_yz", "fft_x_gather", "paw", "weights", "rank_k", "rank_k_i8_mma")
 

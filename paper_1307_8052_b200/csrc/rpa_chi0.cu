@@ -1116,6 +1116,15 @@ int ec_enqueue_factorization(rpa_chi0 *h, int nm, int n_lanes, int64_t *launches
                                                                                              M + (size_t)ln.m0 * ng * ng, ng, g0, ncolt);
         return 1;
     };
+    // which kernel for an update on the chain (ncols64 tile columns of 64 from column g0, all nm matrices of the group):
+    // while its 64 x 64 tiles alone fill the GPU the factorisation is throughput-bound and the wide tiles are more
+    // efficient (two CTAs per SM, operands through a ring); once they no longer do, the 32 x 32 tiles finish sooner
+    auto small_grid = [&](int g0, int ncols64) {
+        const int nt = (ng - g0 + rk::T - 1) / rk::T;
+        int tiles = 0;
+        for (int tj = 0; tj < ncols64; tj++) tiles += std::max(nt - tj, 0);
+        return h->ec_tile32 && tiles * nm < 2 * h->n_sm;   // measured on 16 matrices of 401 / 1200 / 3004: 1, 2, 3, 4 x n_sm
+    };
     CUDA_TRY(cudaEventRecord(h->ev_fork, st));
     for (int l = 0; l < n_lanes; l++) {
         CUDA_TRY(cudaStreamWaitEvent(lanes[l].side, h->ev_fork, 0));
@@ -1132,7 +1141,7 @@ int ec_enqueue_factorization(rpa_chi0 *h, int nm, int n_lanes, int64_t *launches
                 const int c0 = kb + p * CH_NB;
                 const int rest = ng - (c0 + CH_NB);
                 if (p > 0)
-                    *launches += h->ec_tile32 ? update32(ln, ln.side, Lt, p * CH_NB, c0, 1) : update(ln, ln.side, Lt, p * CH_NB, c0, 1, c0 + CH_NB);
+                    *launches += small_grid(c0, 1) ? update32(ln, ln.side, Lt, p * CH_NB, c0, 1) : update(ln, ln.side, Lt, p * CH_NB, c0, 1, c0 + CH_NB);
                 chol_panel_kernel<<<dim3(std::max(1, (rest + 127) / 128), ln.nm), CH_THREADS, 0, ln.side>>>(
                     M + (size_t)ln.m0 * ng * ng, ng, c0, Lt + (size_t)p * CH_NB * L.ldn, L.ldn, lt_mat, d_flag + ln.m0,
                     d_ld + ln.m0);
@@ -1145,7 +1154,7 @@ int ec_enqueue_factorization(rpa_chi0 *h, int nm, int n_lanes, int64_t *launches
                 // look-ahead: the first two tile columns (= the next block's 128 columns) on the side stream, after
                 // the previous block's big update; the rest of the trailing matrix on the main stream meanwhile
                 if (blk > 0) CUDA_TRY(cudaStreamWaitEvent(ln.side, ln.ev_col, 0));
-                *launches += h->ec_tile32 ? update32(ln, ln.side, Lt, np * CH_NB, g0, 2 * rk::T / cu32::T) : update(ln, ln.side, Lt, np * CH_NB, g0, 3, ng);
+                *launches += small_grid(g0, 2) ? update32(ln, ln.side, Lt, np * CH_NB, g0, 2 * rk::T / cu32::T) : update(ln, ln.side, Lt, np * CH_NB, g0, 3, ng);
                 *launches += update(ln, ln.main, Lt, np * CH_NB, g0, 4, ng);
                 CUDA_TRY(cudaEventRecord(ln.ev_col, ln.main));
             }

@@ -219,7 +219,9 @@ def test_ec_q_lanes_give_the_same_numbers():
             B.add_kpoint_host(h, kd, cfg.n_proj, Qd, W.atom_positions(cfg))
             v = W.coulomb(K2)
             ref = None
-            for lanes in (1, 2, 3, 4):
+            # RPA_EC_FLAG_WIDE_TILES: the chain updates in the 64 x 64 tiles of the big updates instead of their own
+            # 32 x 32-tile kernel -- the same sums in the same order, so also bit for bit
+            for lanes in (1, 2, 3, 4, 2 | B.RPA_EC_FLAG_WIDE_TILES, 3 | B.RPA_EC_FLAG_WIDE_TILES):
                 B.rpa_chi0_set_ec_lanes(h, lanes)
                 ec, e = B.rpa_ec_q(h, v)
                 ec2, e2 = B.rpa_ec_q_range(h, v, 1, 3)
@@ -229,7 +231,7 @@ def test_ec_q_lanes_give_the_same_numbers():
                 else:
                     assert ec == ref[0] and np.array_equal(e, ref[1])
                     assert ec2 == ref[2] and np.array_equal(e2, ref[3])
-            for bad in (0, 5):
+            for bad in (0, 5, B.RPA_EC_FLAG_WIDE_TILES, 0x200 | 2):
                 with pytest.raises(B.RpaError) as ei:
                     B.rpa_chi0_set_ec_lanes(h, bad)
                 assert ei.value.code == B.RPA_ERR_INVALID_ARG
