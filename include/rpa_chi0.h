@@ -134,6 +134,30 @@ int rpa_chi0_add_kpoint(rpa_chi0_t *h, double kweight, int32_t n_occ, const void
                         const double *f_unocc, int32_t n_atoms, const int32_t *n_proj, const void *P_occ,
                         const void *P_unocc, const void *Q, const double *R_cart);
 
+/*
+ * The same k-point in three steps, for unoccupied orbitals that are still being produced on the handle's stream while the
+ * first pair densities are computed -- the paper's own pipeline, where every orbital is expanded from its plane-wave
+ * coefficients just before use (Table 1 steps 3-5): uploads and rpa_pw_to_grid calls of later bands go between
+ * the steps, and the copies hide under the pair densities of the earlier bands.  Same result as ONE rpa_chi0_add_kpoint
+ * call, bit for bit (the same pair densities meet in the same rank-K update).
+ *   rpa_chi0_add_kpoint_begin: arguments as rpa_chi0_add_kpoint.  psi_unocc and P_unocc are the full [n_unocc] arrays;
+ *     band m of psi_unocc is read by the rpa_chi0_add_kpoint_pairs call that covers m (stream order), P_unocc by
+ *     rpa_chi0_add_kpoint_end.  The transitions must fit ONE batch: n_occ n_unocc <= max_batch_pairs of the handle and
+ *     n_occ <= 16, else RPA_ERR_UNSUPPORTED and nothing is open (use rpa_chi0_add_kpoint).  Not for q = 0 handles.
+ *   rpa_chi0_add_kpoint_pairs(m_begin, m_end): pair densities (S2 + S3) of every occupied band with the unoccupied bands
+ *     [m_begin, m_end).  Slices must follow one another: the first starts at 0, each at the end of the one before.
+ *   rpa_chi0_add_kpoint_end: PAW correction, weights and the rank-K update of the whole k-point (S4 - S6).
+ *     RPA_ERR_INVALID_ARG, nothing added, if the slices did not reach n_unocc.  Closes the k-point in every case.
+ * Between begin and end the handle accepts rpa_pw_to_grid, rpa_symmetry_remap, rpa_chi0_get, rpa_ec_q, rpa_chi0_sync;
+ * rpa_chi0_add_kpoint* return RPA_ERR_INVALID_ARG.
+ */
+int rpa_chi0_add_kpoint_begin(rpa_chi0_t *h, double kweight, int32_t n_occ, const void *psi_occ, int32_t n_unocc,
+                              const void *psi_unocc, const double *eps_occ, const double *eps_unocc, const double *f_occ,
+                              const double *f_unocc, int32_t n_atoms, const int32_t *n_proj, const void *P_occ,
+                              const void *P_unocc, const void *Q, const double *R_cart);
+int rpa_chi0_add_kpoint_pairs(rpa_chi0_t *h, int32_t m_begin, int32_t m_end);
+int rpa_chi0_add_kpoint_end(rpa_chi0_t *h);
+
 /* chi0(i omega_i) = (2/Omega) S_i as a full Hermitian matrix, dev cdouble [ng][ng] row-major (Eq. 3 prefactor,
  * P:L56; spin-paired, reading A3).  Stream-ordered; does not modify the accumulators. */
 int rpa_chi0_get(rpa_chi0_t *h, int32_t i_omega, void *chi0_out);

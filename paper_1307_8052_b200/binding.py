@@ -28,7 +28,7 @@ EXPORTS = (
     "rpa_pw_to_grid", "rpa_symmetry_remap", "rpa_momentum_pw", "rpa_chi0_add_kpoint_optical",
     "rpa_chi0_set_spin_degeneracy", "rpa_chi0_create_real_axis", "rpa_ec_q_range",
     "rpa_chi0_set_rank_k_mode", "rpa_chi0_rank_k_batches", "rpa_chi0_set_ec_lanes", "rpa_total_energy",
-    "rpa_e_omega_noalloc",
+    "rpa_e_omega_noalloc", "rpa_chi0_add_kpoint_begin", "rpa_chi0_add_kpoint_pairs", "rpa_chi0_add_kpoint_end",
 )
 
 # rpa_chi0_set_rank_k_mode (include/rpa_chi0.h)
@@ -80,6 +80,12 @@ def lib():
     L.rpa_chi0_gvectors.argtypes = [vp, vp, vp]
     L.rpa_chi0_add_kpoint.restype = C.c_int
     L.rpa_chi0_add_kpoint.argtypes = [vp, f64, i32, vp, i32, vp, vp, vp, vp, vp, i32, vp, vp, vp, vp, vp]
+    L.rpa_chi0_add_kpoint_begin.restype = C.c_int
+    L.rpa_chi0_add_kpoint_begin.argtypes = L.rpa_chi0_add_kpoint.argtypes
+    L.rpa_chi0_add_kpoint_pairs.restype = C.c_int
+    L.rpa_chi0_add_kpoint_pairs.argtypes = [vp, i32, i32]
+    L.rpa_chi0_add_kpoint_end.restype = C.c_int
+    L.rpa_chi0_add_kpoint_end.argtypes = [vp]
     L.rpa_chi0_get.restype = C.c_int
     L.rpa_chi0_get.argtypes = [vp, i32, vp]
     L.rpa_ec_q.restype = C.c_int
@@ -252,7 +258,7 @@ def rpa_chi0_gvectors(h: Handle):
 
 def rpa_chi0_add_kpoint(h: Handle, kweight, psi_occ, psi_unocc, eps_occ, eps_unocc, f_occ, f_unocc,
                         n_proj: Optional[Sequence[int]] = None, P_occ=None, P_unocc=None, Q=None, R_cart=None,
-                        qdir_cart=None, grad=None):
+                        qdir_cart=None, grad=None, _begin=False):
     """psi_*, P_*, Q: CUDA complex128 tensors (layouts of include/rpa_chi0.h); eps_*, f_*, n_proj, R_cart: host.
     With qdir_cart and grad (CUDA [3][n_occ][n_unocc]) this is rpa_chi0_add_kpoint_optical (q = 0 handles)."""
     torch = _torch()
@@ -285,7 +291,9 @@ def rpa_chi0_add_kpoint(h: Handle, kweight, psi_occ, psi_unocc, eps_occ, eps_uno
         args = (0, None, None, None, None, None)
     common = (h.ptr, float(kweight), n_occ, _dev_ptr(psi_occ, "psi_occ", c128, h.device) if n_occ else None, n_unocc,
               _dev_ptr(psi_unocc, "psi_unocc", c128, h.device) if n_unocc else None, _hp(eo), _hp(eu), _hp(fo), _hp(fu), *args)
-    if grad is None and qdir_cart is None:
+    if _begin:
+        rc = lib().rpa_chi0_add_kpoint_begin(*common)
+    elif grad is None and qdir_cart is None:
         rc = lib().rpa_chi0_add_kpoint(*common)
     else:
         if grad is None or qdir_cart is None or grad.numel() != 3 * n_occ * n_unocc:
@@ -293,6 +301,23 @@ def rpa_chi0_add_kpoint(h: Handle, kweight, psi_occ, psi_unocc, eps_occ, eps_uno
         qd = _np(qdir_cart, np.float64).reshape(3)
         rc = lib().rpa_chi0_add_kpoint_optical(*common, _hp(qd), _dev_ptr(grad, "grad", c128, h.device))
     _check(rc)
+
+
+def rpa_chi0_add_kpoint_begin(h: Handle, kweight, psi_occ, psi_unocc, eps_occ, eps_unocc, f_occ, f_unocc, n_proj=None,
+                              P_occ=None, P_unocc=None, Q=None, R_cart=None):
+    """Open a k-point whose unoccupied orbitals (rows of psi_unocc) are still being produced on the handle's stream:
+    followed by rpa_chi0_add_kpoint_pairs for consecutive band slices and rpa_chi0_add_kpoint_end.  RpaError with code
+    RPA_ERR_UNSUPPORTED when the transitions do not fit one batch (then use rpa_chi0_add_kpoint)."""
+    rpa_chi0_add_kpoint(h, kweight, psi_occ, psi_unocc, eps_occ, eps_unocc, f_occ, f_unocc, n_proj, P_occ, P_unocc, Q, R_cart,
+                        _begin=True)
+
+
+def rpa_chi0_add_kpoint_pairs(h: Handle, m_begin: int, m_end: int):
+    _check(lib().rpa_chi0_add_kpoint_pairs(h.ptr, int(m_begin), int(m_end)))
+
+
+def rpa_chi0_add_kpoint_end(h: Handle):
+    _check(lib().rpa_chi0_add_kpoint_end(h.ptr))
 
 
 def rpa_chi0_get(h: Handle, i_omega: int, out=None):
@@ -534,7 +559,7 @@ def add_kpoint_host(h: Handle, kd, n_proj=None, Q_dev=None, R_cart=None, pinned=
 
 
 def add_kpoint_host_pw(h: Handle, kweight, g_pw, C_occ, C_unocc, eps_occ, eps_unocc, f_occ, f_unocc, n_proj=None,
-                       P_occ=None, P_unocc=None, Q_dev=None, R_cart=None, n_slices=4, n_calls=1):
+                       P_occ=None, P_unocc=None, Q_dev=None, R_cart=None, n_slices=8, n_calls=1, streamed=True):
     """The paper's own pipeline (Table 1 steps 3 and 5-11): the host holds the orbitals as plane-wave coefficients
     C_*[bands][n_pw] (host tensors, ideally pinned; g_pw[n_pw][3] their integer wave vectors) -- about 1/20 of the
     bytes of the grid orbitals -- the device expands them with rpa_pw_to_grid (Eq. 10) into buffers kept on the
@@ -542,10 +567,12 @@ def add_kpoint_host_pw(h: Handle, kweight, g_pw, C_occ, C_unocc, eps_occ, eps_un
 
     The coefficients go up on a side stream, the unoccupied ones in `n_slices` slices; rpa_pw_to_grid of a slice is
     enqueued on the handle's stream behind the event of its copy, so the expansion of slice i runs under the copy of
-    slice i + 1 (rpa_pw_to_grid keeps the index table of g_pw on the device between calls and does not block).  The
-    unoccupied bands are added in `n_calls` rpa_chi0_add_kpoint calls (the accumulation is additive over any split of the
-    bands); with 2 the kernels of the first group hide the upload and expansion of the second, but on
-    configs[1] the second call costs more than that saves (measured 26.96 ms against 26.66 with one call), hence 1."""
+    slice i + 1 (rpa_pw_to_grid keeps the index table of g_pw on the device between calls and does not block).  When the
+    transitions fit one batch the k-point is added with rpa_chi0_add_kpoint_begin / _pairs / _end: the pair densities of a
+    slice are enqueued right behind its expansion, so the remaining uploads hide under them and only the first slice's
+    copy is exposed; the result is that of one rpa_chi0_add_kpoint call, bit for bit.  Otherwise (or with n_calls > 1)
+    the unoccupied bands are added in `n_calls` rpa_chi0_add_kpoint calls after their slices have arrived (the accumulation
+    is additive over any split of the bands)."""
     torch = _torch()
     dev = h.device
     have_paw = n_proj is not None and len(n_proj) > 0
@@ -587,6 +614,16 @@ def add_kpoint_host_pw(h: Handle, kweight, g_pw, C_occ, C_unocc, eps_occ, eps_un
             main.wait_event(upload(bufs["P_u"], P_uh))
         eps_u, f_u = _np(eps_unocc, np.float64), _np(f_unocc, np.float64)
         n_calls = max(1, min(int(n_calls), n_u))
+        want_streamed, streamed = bool(streamed), False
+        if want_streamed and n_calls == 1 and n_u > 1:
+            # one k-point, its pair densities slice by slice as the orbitals arrive (rpa_chi0_add_kpoint_begin / _pairs / _end)
+            try:
+                rpa_chi0_add_kpoint_begin(h, kweight, bufs["psi_o"], bufs["psi_u"], eps_occ, eps_u, f_occ, f_u, n_proj, bufs["P_o"],
+                                          bufs["P_u"], Q_dev, R_cart)
+                streamed = True
+            except RpaError as e:
+                if e.code != RPA_ERR_UNSUPPORTED:
+                    raise
         per_call = max(1, -(-n_u // n_calls))
         step = max(1, -(-per_call // max(1, int(n_slices) // n_calls)))
         for c0 in range(0, n_u, per_call):
@@ -596,6 +633,11 @@ def add_kpoint_host_pw(h: Handle, kweight, g_pw, C_occ, C_unocc, eps_occ, eps_un
                 ev = upload(bufs["C_u"][m0:m1], C_uh[m0:m1])
                 main.wait_event(ev)
                 rpa_pw_to_grid(h, g_pw, bufs["C_u"][m0:m1], bufs["psi_u"][m0:m1])
-            rpa_chi0_add_kpoint(h, kweight, bufs["psi_o"], bufs["psi_u"][c0:c1], eps_occ, eps_u[c0:c1], f_occ, f_u[c0:c1], n_proj,
-                                bufs["P_o"], None if bufs["P_u"] is None else bufs["P_u"][c0:c1], Q_dev, R_cart)
+                if streamed:
+                    rpa_chi0_add_kpoint_pairs(h, m0, m1)
+            if streamed:
+                rpa_chi0_add_kpoint_end(h)
+            else:
+                rpa_chi0_add_kpoint(h, kweight, bufs["psi_o"], bufs["psi_u"][c0:c1], eps_occ, eps_u[c0:c1], f_occ, f_u[c0:c1], n_proj,
+                                    bufs["P_o"], None if bufs["P_u"] is None else bufs["P_u"][c0:c1], Q_dev, R_cart)
     return nbytes

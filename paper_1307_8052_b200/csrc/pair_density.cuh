@@ -229,17 +229,28 @@ typedef void (*PdPlaneKernel)(const PdPlaneParams);
 // broadcast); a thread keeps PD_G1_BLOCK accumulators, so a sphere with ng1 <= PD_G1_BLOCK reads I once, and the
 // loads of four x planes are issued together to cover the L2 latency.
 // Dynamic shared memory: N1 * PD_G1_BLOCK * sizeof(cd).
+// Row of the N buffer that pair pl of a launch goes to.  A plain launch covers the batch's pairs p_begin, p_begin + 1, ...
+// (win.len = INT_MAX: row = p_begin + pl).  A window launch (streamed k-point: some unoccupied bands of every occupied row)
+// numbers its pairs row by row over the window, p' = p_begin + pl = r win.len + j, and they belong to the batch's rows
+// r win.stride + win.off + j.
+struct PdRowWindow {
+    int len, stride, off;
+};
+__device__ __forceinline__ size_t pd_out_row(int p, PdRowWindow win) {
+    const int r = p / win.len;
+    return (size_t)r * win.stride + win.off + (p - r * win.len);
+}
 #define PD_G1_BLOCK 16
 __global__ void __launch_bounds__(128) pd_xaxis_kernel(const cd *__restrict__ I, cd *__restrict__ Nbuf, int64_t ldn,
                                                       const cd *__restrict__ tw1, const int32_t *__restrict__ box2s,
-                                                      int N1, int nb2, int g1min, int ng1, int p_begin, double inv_n) {
+                                                      int N1, int nb2, int g1min, int ng1, int p_begin, double inv_n, PdRowWindow win) {
     extern __shared__ __align__(16) unsigned char pd_smem[];
     cd *twt = reinterpret_cast<cd *>(pd_smem);   // [j1][t]
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     const bool act = b < nb2;
     const int pl = blockIdx.y;
     const cd *Ip = I + (size_t)pl * N1 * nb2 + (act ? b : 0);
-    cd *out = Nbuf + (size_t)(p_begin + pl) * ldn;
+    cd *out = Nbuf + pd_out_row(p_begin + pl, win) * ldn;
     for (int gc = 0; gc < ng1; gc += PD_G1_BLOCK) {
         __syncthreads();
         for (int i = threadIdx.x; i < N1 * PD_G1_BLOCK; i += blockDim.x) {
@@ -293,7 +304,7 @@ __global__ void __launch_bounds__(128) pd_xaxis_kernel(const cd *__restrict__ I,
 template <int PD_X8_ND, int NBT>   // PD_X8_ND: kept-frequency slots per residue mod 8 (2 when the box needs no more: fewer registers)
 __global__ void __launch_bounds__(128, 4) pd_xaxis8_kernel(const cd *__restrict__ I, cd *__restrict__ Nbuf, int64_t ldn,
                                                        const cd *__restrict__ tw1, const int32_t *__restrict__ box2s,
-                                                       int N1, int nb2, int g1min, int ng1, int p_begin, int p_count, double inv_n) {
+                                                       int N1, int nb2, int g1min, int ng1, int p_begin, int p_count, double inv_n, PdRowWindow win) {
     extern __shared__ __align__(16) unsigned char pd_smem[];
     cd *twt = reinterpret_cast<cd *>(pd_smem);   // [j][slot], slot = k1 PD_X8_ND + d: W_N1^(j f_slot)
     const int NB = NBT > 0 ? NBT : (N1 >> 3);
@@ -352,7 +363,7 @@ __global__ void __launch_bounds__(128, 4) pd_xaxis8_kernel(const cd *__restrict_
 #pragma unroll 1
             for (int j = 0; j < NB; j++) body(j);
         }
-        cd *out = Nbuf + (size_t)(p_begin + pl) * ldn;
+        cd *out = Nbuf + pd_out_row(p_begin + pl, win) * ldn;
 #pragma unroll
         for (int k1 = 0; k1 < 8; k1++)
 #pragma unroll

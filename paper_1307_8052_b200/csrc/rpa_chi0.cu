@@ -3,6 +3,7 @@
 // builds the sphere tables, carves the caller's workspace, plans the batches and enqueues the launches.
 #include <cuda.h>
 #include <cuda_runtime.h>
+#include <limits.h>
 #include <math.h>
 #include <stdarg.h>
 #include <stdio.h>
@@ -216,6 +217,21 @@ struct StageEvent {
 
 }  // namespace
 
+// One call's arguments (rpa_chi0_add_kpoint, rpa_chi0_add_kpoint_optical when grad != NULL, or the streamed variant)
+struct AddArgs {
+    double kweight;
+    int32_t n_occ;
+    const void *psi_occ;
+    int32_t n_unocc;
+    const void *psi_unocc;
+    const double *eps_occ, *eps_unocc, *f_occ, *f_unocc;
+    int32_t n_atoms;
+    const int32_t *n_proj;
+    const void *P_occ, *P_unocc, *Q;
+    const double *R_cart, *qdir;
+    const void *grad;
+};
+
 struct rpa_chi0 {
     cudaStream_t stream = nullptr;
     int32_t grid[3];
@@ -262,6 +278,11 @@ struct rpa_chi0 {
     std::vector<int32_t> pw_g, pw_table;
     int pw_qmin[3] = {0, 0, 0};
     int64_t pw_nq[3] = {0, 0, 0};
+    // streamed k-point (rpa_chi0_add_kpoint_begin / _pairs / _end): the open call's arguments (the host arrays among them are
+    // not used after _begin), its projector count and the first unoccupied band not yet given to _pairs
+    bool pend_open = false;
+    AddArgs pend = {};
+    int pend_ptot = 0, pend_m_next = 0;
     unsigned char *ws;
     // profiling
     bool prof = false;
@@ -736,24 +757,29 @@ int i8_batch(rpa_chi0 *h, int K, int Kpad, bool *done) {
 }  // namespace
 
 namespace {
-// rpa_chi0_add_kpoint, and rpa_chi0_add_kpoint_optical when grad != NULL (q = 0 handle: G = 0 element replaced)
-int add_kpoint_impl(rpa_chi0_t *h, double kweight, int32_t n_occ, const void *psi_occ, int32_t n_unocc,
-                    const void *psi_unocc, const double *eps_occ, const double *eps_unocc, const double *f_occ,
-                    const double *f_unocc, int32_t n_atoms, const int32_t *n_proj, const void *P_occ,
-                    const void *P_unocc, const void *Q, const double *R_cart, const double *qdir, const void *grad) {
+#define ADD_ARGS_LOCALS                                                                                                  \
+    const double kweight = A.kweight; const int32_t n_occ = A.n_occ, n_unocc = A.n_unocc, n_atoms = A.n_atoms;            \
+    const void *psi_occ = A.psi_occ, *psi_unocc = A.psi_unocc, *P_occ = A.P_occ, *P_unocc = A.P_unocc, *Q = A.Q, *grad = A.grad; \
+    const double *eps_occ = A.eps_occ, *eps_unocc = A.eps_unocc, *f_occ = A.f_occ, *f_unocc = A.f_unocc, *R_cart = A.R_cart, *qdir = A.qdir; \
+    const int32_t *n_proj = A.n_proj;                                                                                    \
+    (void)kweight; (void)n_occ; (void)n_unocc; (void)n_atoms; (void)psi_occ; (void)psi_unocc; (void)P_occ; (void)P_unocc; (void)Q; \
+    (void)grad; (void)eps_occ; (void)eps_unocc; (void)f_occ; (void)f_unocc; (void)R_cart; (void)qdir; (void)n_proj;     \
+    const Layout &L = h->L; const Sphere &sp = h->sp; const int ng = sp.ng; cudaStream_t st = h->stream;                 \
+    (void)L; (void)sp; (void)ng; (void)st
+
+// validation, PAW metadata and band energies / occupations to the device; *ptot_out = sum of n_proj.
+// Returns 1 (not an error code) when the band set is empty: nothing to add.
+int add_setup(rpa_chi0_t *h, const AddArgs &A, int *ptot_out) {
     if (!h) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_add_kpoint: handle is NULL");
-    if (h->q0 && !grad)
+    if (h->q0 && !A.grad)
         return fail(RPA_ERR_UNSUPPORTED, "rpa_chi0_add_kpoint: the handle has q = 0: use rpa_chi0_add_kpoint_optical (P:L113-134)");
-    if (!h->q0 && grad) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_add_kpoint_optical: the handle has q != 0");
-    if (n_occ < 0 || n_unocc < 0 || n_atoms < 0) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_add_kpoint: negative count");
-    if (n_occ == 0 || n_unocc == 0) return RPA_OK;  // empty band set: nothing to add
-    if (!psi_occ || !psi_unocc || !eps_occ || !eps_unocc || !f_occ || !f_unocc)
+    if (!h->q0 && A.grad) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_add_kpoint_optical: the handle has q != 0");
+    if (A.n_occ < 0 || A.n_unocc < 0 || A.n_atoms < 0) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_add_kpoint: negative count");
+    if (A.n_occ == 0 || A.n_unocc == 0) return 1;  // empty band set: nothing to add
+    if (!A.psi_occ || !A.psi_unocc || !A.eps_occ || !A.eps_unocc || !A.f_occ || !A.f_unocc)
         return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_add_kpoint: NULL band array");
-    if ((int64_t)n_occ + n_unocc > MAX_BANDS) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_add_kpoint: more than %d bands", MAX_BANDS);
-    const Layout &L = h->L;
-    const Sphere &sp = h->sp;
-    const int ng = sp.ng;
-    cudaStream_t st = h->stream;
+    if ((int64_t)A.n_occ + A.n_unocc > MAX_BANDS) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_add_kpoint: more than %d bands", MAX_BANDS);
+    ADD_ARGS_LOCALS;
 
     // ---- PAW metadata ----------------------------------------------------------------------------------
     int ptot = 0;
@@ -791,179 +817,221 @@ int add_kpoint_impl(rpa_chi0_t *h, double kweight, int32_t n_occ, const void *ps
     CUDA_TRY(cudaMemcpyAsync(d_eu, eps_unocc, n_unocc * sizeof(double), cudaMemcpyHostToDevice, st));
     CUDA_TRY(cudaMemcpyAsync(d_fu, f_unocc, n_unocc * sizeof(double), cudaMemcpyHostToDevice, st));
 
-    // ---- batches: either several whole occupied rows, or a slice of one row ---------------------------------
-    const int Kmax = L.Kmax;
-    int rows_per_batch = 1, mchunk = n_unocc;
-    if (n_unocc >= Kmax) {
-        const int nch = (n_unocc + Kmax - 1) / Kmax;
-        mchunk = (int)align_up((size_t)(n_unocc + nch - 1) / nch, K_ALIGN);
-        mchunk = std::min(mchunk, Kmax);
-    } else {
-        rows_per_batch = std::max(1, std::min(MAX_SLOTS, Kmax / n_unocc));
-    }
+    *ptot_out = ptot;
+    return RPA_OK;
+}
+
+// S2 + S3 (pair product, pruned 3-D FFT, sphere gather) of the pairs [p0, p0 + pc) of a batch (pair p: band n = n0 + p / mlen,
+// m = m0 + p % mlen) into rows p0 ... of the N buffer; pc <= L.sub_pairs.  win: the rows of the N buffer when the pairs are a window of a
+// larger batch (PdRowWindow, pair_density.cuh).
+int add_pair_densities(rpa_chi0_t *h, const AddArgs &A, int n0, int mlen, int m0, int p0, int pc,
+                       PdRowWindow win = PdRowWindow{INT_MAX, 0, 0}) {
+    ADD_ARGS_LOCALS;
     const int N1 = h->grid[0], N2 = h->grid[1], N3 = h->grid[2];
     const int ng1 = sp.gmax[0] - sp.gmin[0] + 1, ng2 = sp.gmax[1] - sp.gmin[1] + 1, ng3 = sp.gmax[2] - sp.gmin[2] + 1;
-    const int nb2 = ng2 * ng3;
     const double inv_n = 1.0 / ((double)N1 * N2 * N3);
     cd *Nbuf = h->ptr<cd>(L.Nbuf);
-    double *w = h->ptr<double>(L.w);
-
-    for (int n0 = 0; n0 < n_occ; n0 += rows_per_batch) {
-        const int nslots = std::min(rows_per_batch, n_occ - n0);
-        for (int m0 = 0; m0 < n_unocc; m0 += mchunk) {
-            const int mlen = std::min(mchunk, n_unocc - m0);
-            const int K = nslots * mlen;
-            const int Kpad = (int)align_up((size_t)K, K_ALIGN);
-            // rows K..Kpad of the N buffer must be zero (they meet zero weights, but 0 * NaN is NaN)
-            if (Kpad > K) CUDA_TRY(cudaMemsetAsync(Nbuf + (size_t)K * L.ldn, 0, (size_t)(Kpad - K) * L.ldn * sizeof(cd), st));
-
-            // S2 + S3: pair product, pruned 3-D FFT, sphere gather
-            for (int p0 = 0; p0 < K; p0 += L.sub_pairs) {
-                const int pc = std::min(L.sub_pairs, K - p0);
-                if (h->zy_kernel) {
-                    StageTimer tm(h, 0, 1);
-                    PdZyParams P;
-                    P.psi_occ = (const cd *)psi_occ; P.psi_unocc = (const cd *)psi_unocc;
-                    P.I = h->ptr<cd>(L.I);
-                    P.coltab = h->ptr<int32_t>(L.coltab); P.rowtab = h->ptr<int32_t>(L.rowtab); P.ncols = sp.ncols;
-                    P.tw3 = h->ptr<cd>(L.tw3); P.tw2 = h->ptr<cd>(L.tw2);
-                    P.N1 = N1;
-                    P.n0 = n0; P.mlen = mlen; P.m0 = m0;
-                    P.p_begin = p0; P.p_count = pc;
-                    pdzy_plan_units(P, h->zy_G);
-                    P.g2min = sp.gmin[1]; P.ng2 = ng2; P.g3min = sp.gmin[2]; P.ng3 = ng3;
-                    // persistent 1-D grid: one CTA per resident slot, work items (unit, plane) dealt round-robin
-                    const int nctas = std::max(1, std::min(P.n_units * N1, h->n_sm * h->zy_ctas_per_sm));
-                    h->zy_kernel<<<nctas, h->zy_threads, h->zy_smem, st>>>(P);
-                    CUDA_TRY(cudaGetLastError());
-                } else {
-                    StageTimer tm(h, 0, 1);
-                    PdPlaneParams P;
-                    P.psi_occ = (const cd *)psi_occ; P.psi_unocc = (const cd *)psi_unocc;
-                    P.I = h->ptr<cd>(L.I);
-                    P.coltab = h->ptr<int32_t>(L.coltab); P.ncols = sp.ncols;
-                    P.tw3 = h->ptr<cd>(L.tw3); P.tw2 = h->ptr<cd>(L.tw2);
-                    P.N1 = N1; P.N2 = N2; P.N3 = N3;
-                    P.n0 = n0; P.mlen = mlen; P.m0 = m0;
-                    P.p_begin = p0; P.p_count = pc;
-                    P.g2min = sp.gmin[1]; P.ng2 = ng2; P.g3min = sp.gmin[2]; P.ng3 = ng3;
-                    P.RC = h->RC; P.nbuf = h->pd_nbuf; P.pz = h->pz; P.py = h->py;
-                    const int gy = std::max(1, std::min(pc, (148 * 8 + N1 - 1) / N1));
-                    h->pd_kernel<<<dim3(N1, gy), h->pd_threads, h->pd_smem, st>>>(P);
-                    CUDA_TRY(cudaGetLastError());
-                }
-                {
-                    StageTimer tm(h, 1, 1);
-                    const int xslots = pd_xaxis8_slots(N1, sp.gmin[0], ng1);
-                    const int ncols = sp.ncols;   // the x transform runs on the kept (g2, g3) columns only
-                    const int xth = std::min(128, (ncols + 31) / 32 * 32);   // 73 kept columns (configs[2]): 96 threads, not 128
-                    const int xbx = (ncols + xth - 1) / xth;
-                    // short x axes (compile-time N1): blocks walk over the pairs, as many as keep every SM busy with ~8 blocks;
-                    // long axes: one block per (column block, pair) as before (measured: the walk loses 4-5 % there)
-                    const bool xshort = xslots == 2 && (N1 == 24 || N1 == 16);
-                    int xby = pc;
-                    if (xshort) {
-                        // every block resident at once and the same number of pairs for each: ceil(pc xbx / slots) rounds of
-                        // the pair loop (2400 pairs of a configs[2] k-point on 740 slots: 600 blocks x 4 pairs, not 1184 x 2-3 in
-                        // two waves)
-                        int per_sm = 0;
-                        const void *xk = N1 == 24 ? (const void *)pd_xaxis8_kernel<2, 3> : (const void *)pd_xaxis8_kernel<2, 2>;
-                        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, xk, xth, (size_t)N1 * 2 * sizeof(cd)) != cudaSuccess || per_sm < 1)
-                            per_sm = 4;
-                        const int slots = std::max(1, h->n_sm * per_sm / xbx);
-                        const int rounds = (pc + slots - 1) / slots;
-                        xby = (pc + rounds - 1) / rounds;
-                    }
-#define X8_ARGS h->ptr<cd>(L.I), Nbuf, L.ldn, h->ptr<cd>(L.tw1), h->ptr<int32_t>(L.box2s), N1, ncols, sp.gmin[0], ng1, p0, pc, inv_n
-                    if (xslots == 2 && N1 == 24)
-                        pd_xaxis8_kernel<2, 3><<<dim3(xbx, xby), xth, (size_t)N1 * 2 * sizeof(cd), st>>>(X8_ARGS);
-                    else if (xslots == 2 && N1 == 16)
-                        pd_xaxis8_kernel<2, 2><<<dim3(xbx, xby), xth, (size_t)N1 * 2 * sizeof(cd), st>>>(X8_ARGS);
-                    else if (xslots == 2)
-                        pd_xaxis8_kernel<2, 0><<<dim3(xbx, xby), xth, (size_t)N1 * 2 * sizeof(cd), st>>>(X8_ARGS);
-                    else if (xslots == 3)
-                        pd_xaxis8_kernel<3, 0><<<dim3(xbx, xby), xth, (size_t)N1 * 3 * sizeof(cd), st>>>(X8_ARGS);
+    (void)N2; (void)N3;
+    if (h->zy_kernel) {
+        StageTimer tm(h, 0, 1);
+        PdZyParams P;
+        P.psi_occ = (const cd *)psi_occ; P.psi_unocc = (const cd *)psi_unocc;
+        P.I = h->ptr<cd>(L.I);
+        P.coltab = h->ptr<int32_t>(L.coltab); P.rowtab = h->ptr<int32_t>(L.rowtab); P.ncols = sp.ncols;
+        P.tw3 = h->ptr<cd>(L.tw3); P.tw2 = h->ptr<cd>(L.tw2);
+        P.N1 = N1;
+        P.n0 = n0; P.mlen = mlen; P.m0 = m0;
+        P.p_begin = p0; P.p_count = pc;
+        pdzy_plan_units(P, h->zy_G);
+        P.g2min = sp.gmin[1]; P.ng2 = ng2; P.g3min = sp.gmin[2]; P.ng3 = ng3;
+        // persistent 1-D grid: one CTA per resident slot, work items (unit, plane) dealt round-robin
+        const int nctas = std::max(1, std::min(P.n_units * N1, h->n_sm * h->zy_ctas_per_sm));
+        h->zy_kernel<<<nctas, h->zy_threads, h->zy_smem, st>>>(P);
+        CUDA_TRY(cudaGetLastError());
+    } else {
+        StageTimer tm(h, 0, 1);
+        PdPlaneParams P;
+        P.psi_occ = (const cd *)psi_occ; P.psi_unocc = (const cd *)psi_unocc;
+        P.I = h->ptr<cd>(L.I);
+        P.coltab = h->ptr<int32_t>(L.coltab); P.ncols = sp.ncols;
+        P.tw3 = h->ptr<cd>(L.tw3); P.tw2 = h->ptr<cd>(L.tw2);
+        P.N1 = N1; P.N2 = N2; P.N3 = N3;
+        P.n0 = n0; P.mlen = mlen; P.m0 = m0;
+        P.p_begin = p0; P.p_count = pc;
+        P.g2min = sp.gmin[1]; P.ng2 = ng2; P.g3min = sp.gmin[2]; P.ng3 = ng3;
+        P.RC = h->RC; P.nbuf = h->pd_nbuf; P.pz = h->pz; P.py = h->py;
+        const int gy = std::max(1, std::min(pc, (148 * 8 + N1 - 1) / N1));
+        h->pd_kernel<<<dim3(N1, gy), h->pd_threads, h->pd_smem, st>>>(P);
+        CUDA_TRY(cudaGetLastError());
+    }
+    {
+        StageTimer tm(h, 1, 1);
+        const int xslots = pd_xaxis8_slots(N1, sp.gmin[0], ng1);
+        const int ncols = sp.ncols;   // the x transform runs on the kept (g2, g3) columns only
+        const int xth = std::min(128, (ncols + 31) / 32 * 32);   // 73 kept columns (configs[2]): 96 threads, not 128
+        const int xbx = (ncols + xth - 1) / xth;
+        // short x axes (compile-time N1): blocks walk over the pairs, as many as keep every SM busy with ~8 blocks;
+        // long axes: one block per (column block, pair) as before (measured: the walk loses 4-5 % there)
+        const bool xshort = xslots == 2 && (N1 == 24 || N1 == 16);
+        int xby = pc;
+        if (xshort) {
+            // every block resident at once and the same number of pairs for each: ceil(pc xbx / slots) rounds of
+            // the pair loop (2400 pairs of a configs[2] k-point on 740 slots: 600 blocks x 4 pairs, not 1184 x 2-3 in
+            // two waves)
+            int per_sm = 0;
+            const void *xk = N1 == 24 ? (const void *)pd_xaxis8_kernel<2, 3> : (const void *)pd_xaxis8_kernel<2, 2>;
+            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, xk, xth, (size_t)N1 * 2 * sizeof(cd)) != cudaSuccess || per_sm < 1)
+                per_sm = 4;
+            const int slots = std::max(1, h->n_sm * per_sm / xbx);
+            const int rounds = (pc + slots - 1) / slots;
+            xby = (pc + rounds - 1) / rounds;
+        }
+#define X8_ARGS h->ptr<cd>(L.I), Nbuf, L.ldn, h->ptr<cd>(L.tw1), h->ptr<int32_t>(L.box2s), N1, ncols, sp.gmin[0], ng1, p0, pc, inv_n, win
+        if (xslots == 2 && N1 == 24)
+            pd_xaxis8_kernel<2, 3><<<dim3(xbx, xby), xth, (size_t)N1 * 2 * sizeof(cd), st>>>(X8_ARGS);
+        else if (xslots == 2 && N1 == 16)
+            pd_xaxis8_kernel<2, 2><<<dim3(xbx, xby), xth, (size_t)N1 * 2 * sizeof(cd), st>>>(X8_ARGS);
+        else if (xslots == 2)
+            pd_xaxis8_kernel<2, 0><<<dim3(xbx, xby), xth, (size_t)N1 * 2 * sizeof(cd), st>>>(X8_ARGS);
+        else if (xslots == 3)
+            pd_xaxis8_kernel<3, 0><<<dim3(xbx, xby), xth, (size_t)N1 * 3 * sizeof(cd), st>>>(X8_ARGS);
 #undef X8_ARGS
-                    else
-                        pd_xaxis_kernel<<<dim3((ncols + 127) / 128, pc), 128, (size_t)N1 * PD_G1_BLOCK * sizeof(cd), st>>>(
-                            h->ptr<cd>(L.I), Nbuf, L.ldn, h->ptr<cd>(L.tw1), h->ptr<int32_t>(L.box2s), N1, ncols, sp.gmin[0], ng1, p0, inv_n);
-                    CUDA_TRY(cudaGetLastError());
-                }
+        else
+            pd_xaxis_kernel<<<dim3((ncols + 127) / 128, pc), 128, (size_t)N1 * PD_G1_BLOCK * sizeof(cd), st>>>(
+                h->ptr<cd>(L.I), Nbuf, L.ldn, h->ptr<cd>(L.tw1), h->ptr<int32_t>(L.box2s), N1, ncols, sp.gmin[0], ng1, p0, inv_n, win);
+        CUDA_TRY(cudaGetLastError());
+    }
+    return RPA_OK;
+}
+
+// the rest of a batch of K = nslots mlen pairs whose pair densities are in the N buffer: S4 PAW, the optical head, S5 weights,
+// S6 rank-K update of every frequency
+int add_finish_batch(rpa_chi0_t *h, const AddArgs &A, int ptot, int n0, int nslots, int mlen, int m0) {
+    ADD_ARGS_LOCALS;
+    const int K = nslots * mlen;
+    const int Kpad = (int)align_up((size_t)K, K_ALIGN);
+    cd *Nbuf = h->ptr<cd>(L.Nbuf);
+    double *w = h->ptr<double>(L.w);
+    double *band = h->ptr<double>(L.band);
+    double *d_eo = band, *d_fo = band + n_occ, *d_eu = band + 2 * (size_t)n_occ, *d_fu = band + 2 * (size_t)n_occ + n_unocc;
+    // S4: PAW
+    if (ptot > 0) {
+        StageTimer tm(h, 2, 2);
+        paw_T_kernel<<<dim3((ng + 127) / 128, ptot, nslots), 128, 0, st>>>(
+            h->ptr<cd>(L.T), L.ldn, ng, ptot, (const cd *)P_occ, n0, (const cd *)Q, h->ptr<int32_t>(L.aj_atom),
+            h->ptr<int32_t>(L.aj_j), h->ptr<int32_t>(L.atom_poff), h->ptr<int32_t>(L.atom_ni),
+            h->ptr<int64_t>(L.atom_qoff), h->ptr<double>(L.R), h->ptr<double>(L.Kc));
+        CUDA_TRY(cudaGetLastError());
+        const int chunks = (mlen + PAW_PB - 1) / PAW_PB;
+        paw_add_kernel<<<dim3((ng + 127) / 128, nslots * chunks), 128, 0, st>>>(
+            Nbuf, L.ldn, ng, ptot, h->ptr<cd>(L.T), (const cd *)P_unocc, mlen, m0);
+        CUDA_TRY(cudaGetLastError());
+    }
+    // step 10: optical limit, the G = 0 element of every pair density of the batch
+    if (grad) {
+        optical_head_kernel<<<(K + 127) / 128, 128, 0, st>>>(Nbuf, L.ldn, h->idx0, K, n0, mlen, m0, n_occ, n_unocc, d_eo,
+                                                            d_eu, qdir[0], qdir[1], qdir[2], (const cd *)grad);
+        h->launches += 1;
+        CUDA_TRY(cudaGetLastError());
+    }
+    // S5: weights
+    {
+        StageTimer tm(h, 3, 1);
+        weights_kernel<<<dim3((Kpad + 127) / 128, h->n_omega), 128, 0, st>>>(
+            w, L.ldw, K, Kpad, h->ptr<double>(L.omega), h->n_omega, d_eo, d_fo, d_eu, d_fu, n0, mlen, m0, kweight, h->eta);
+        CUDA_TRY(cudaGetLastError());
+    }
+    // S6: rank-K update of every frequency
+    {
+        StageTimer tm(h, 4, 1);
+        bool done_i8 = false;
+        if (h->use_i8 && (h->i8_force || (ng >= I8_MIN_NG && K >= I8_MIN_K))) {
+            int rc = RPA_OK;
+            switch (h->i8_digits) {
+                case 6: rc = i8_batch<6>(h, K, Kpad, &done_i8); break;
+                case 8: rc = i8_batch<8>(h, K, Kpad, &done_i8); break;
+                default: rc = i8_batch<7>(h, K, Kpad, &done_i8); break;
             }
-            // S4: PAW
-            if (ptot > 0) {
-                StageTimer tm(h, 2, 2);
-                paw_T_kernel<<<dim3((ng + 127) / 128, ptot, nslots), 128, 0, st>>>(
-                    h->ptr<cd>(L.T), L.ldn, ng, ptot, (const cd *)P_occ, n0, (const cd *)Q, h->ptr<int32_t>(L.aj_atom),
-                    h->ptr<int32_t>(L.aj_j), h->ptr<int32_t>(L.atom_poff), h->ptr<int32_t>(L.atom_ni),
-                    h->ptr<int64_t>(L.atom_qoff), h->ptr<double>(L.R), h->ptr<double>(L.Kc));
-                CUDA_TRY(cudaGetLastError());
-                const int chunks = (mlen + PAW_PB - 1) / PAW_PB;
-                paw_add_kernel<<<dim3((ng + 127) / 128, nslots * chunks), 128, 0, st>>>(
-                    Nbuf, L.ldn, ng, ptot, h->ptr<cd>(L.T), (const cd *)P_unocc, mlen, m0);
-                CUDA_TRY(cudaGetLastError());
-            }
-            // step 10: optical limit, the G = 0 element of every pair density of the batch
-            if (grad) {
-                optical_head_kernel<<<(K + 127) / 128, 128, 0, st>>>(Nbuf, L.ldn, h->idx0, K, n0, mlen, m0, n_occ, n_unocc, d_eo,
-                                                                    d_eu, qdir[0], qdir[1], qdir[2], (const cd *)grad);
+            if (rc != RPA_OK) return rc;
+        }
+        (done_i8 ? h->i8_batches : h->fp64_batches) += 1;
+        if (done_i8) {
+        } else if (h->use_3m) {
+            // whole waves (one CTA per SM) with full K, then the last partial wave K-sliced so that it fills the GPU too
+            const int ntiles = ntiles_lower(ng, rk3::T), units = ntiles * h->n_omega, nchunks = Kpad / rk3::KC;
+            const int whole = units / h->n_sm * h->n_sm;
+            const int tail = units - whole;
+            auto launch = [&](int off, int count, int ksplit) {
+                rank_k3m_kernel<<<dim3(count, 1, ksplit), rk3::THREADS, rk3::SMEM_BYTES, st>>>(
+                    h->nmap, h->smap, Kpad, w, L.ldw, h->ptr<cd>(L.S), L.ldS, (int64_t)ng * L.ldS, ng, ntiles, off);
+            };
+            // third operand plane of the 3M product: NS = Re N + Im N, one pass over the batch's N
+            rk3_rowsum_kernel<<<dim3(Kpad, (unsigned)((L.ldn + 255) / 256)), 256, 0, st>>>(Nbuf, L.ldn, h->ptr<double>(L.NS));
+            h->launches += 1;
+            double c_single = 0.0, c_tail = 0.0;
+            const int s_single = pick_ksplit(units, nchunks, h->n_sm, &c_single, 512 / rk3::KC);
+            const int s_tail = tail > 0 ? pick_ksplit(tail, nchunks, h->n_sm, &c_tail, 512 / rk3::KC) : 1;
+            // two launches only if the model says they save at least a tenth of an item
+            if (whole > 0 && tail > 0 && whole / h->n_sm + c_tail + 0.1 < c_single) {
+                launch(0, whole, 1);
+                launch(whole, tail, s_tail);
                 h->launches += 1;
-                CUDA_TRY(cudaGetLastError());
+            } else {
+                launch(0, units, s_single);
             }
-            // S5: weights
-            {
-                StageTimer tm(h, 3, 1);
-                weights_kernel<<<dim3((Kpad + 127) / 128, h->n_omega), 128, 0, st>>>(
-                    w, L.ldw, K, Kpad, h->ptr<double>(L.omega), h->n_omega, d_eo, d_fo, d_eu, d_fu, n0, mlen, m0, kweight, h->eta);
-                CUDA_TRY(cudaGetLastError());
-            }
-            // S6: rank-K update of every frequency
-            {
-                StageTimer tm(h, 4, 1);
-                bool done_i8 = false;
-                if (h->use_i8 && (h->i8_force || (ng >= I8_MIN_NG && K >= I8_MIN_K))) {
-                    int rc = RPA_OK;
-                    switch (h->i8_digits) {
-                        case 6: rc = i8_batch<6>(h, K, Kpad, &done_i8); break;
-                        case 8: rc = i8_batch<8>(h, K, Kpad, &done_i8); break;
-                        default: rc = i8_batch<7>(h, K, Kpad, &done_i8); break;
-                    }
-                    if (rc != RPA_OK) return rc;
-                }
-                (done_i8 ? h->i8_batches : h->fp64_batches) += 1;
-                if (done_i8) {
-                } else if (h->use_3m) {
-                    // whole waves (one CTA per SM) with full K, then the last partial wave K-sliced so that it fills the GPU too
-                    const int ntiles = ntiles_lower(ng, rk3::T), units = ntiles * h->n_omega, nchunks = Kpad / rk3::KC;
-                    const int whole = units / h->n_sm * h->n_sm;
-                    const int tail = units - whole;
-                    auto launch = [&](int off, int count, int ksplit) {
-                        rank_k3m_kernel<<<dim3(count, 1, ksplit), rk3::THREADS, rk3::SMEM_BYTES, st>>>(
-                            h->nmap, h->smap, Kpad, w, L.ldw, h->ptr<cd>(L.S), L.ldS, (int64_t)ng * L.ldS, ng, ntiles, off);
-                    };
-                    // third operand plane of the 3M product: NS = Re N + Im N, one pass over the batch's N
-                    rk3_rowsum_kernel<<<dim3(Kpad, (unsigned)((L.ldn + 255) / 256)), 256, 0, st>>>(Nbuf, L.ldn, h->ptr<double>(L.NS));
-                    h->launches += 1;
-                    double c_single = 0.0, c_tail = 0.0;
-                    const int s_single = pick_ksplit(units, nchunks, h->n_sm, &c_single, 512 / rk3::KC);
-                    const int s_tail = tail > 0 ? pick_ksplit(tail, nchunks, h->n_sm, &c_tail, 512 / rk3::KC) : 1;
-                    // two launches only if the model says they save at least a tenth of an item
-                    if (whole > 0 && tail > 0 && whole / h->n_sm + c_tail + 0.1 < c_single) {
-                        launch(0, whole, 1);
-                        launch(whole, tail, s_tail);
-                        h->launches += 1;
-                    } else {
-                        launch(0, units, s_single);
-                    }
-                } else {
-                    const int units = ntiles_lower(ng, rk::T) * ((h->n_omega + rk::Cfg<true>::NW - 1) / rk::Cfg<true>::NW);
-                    const int ksplit = pick_ksplit(units, Kpad / rk::KC, h->n_sm);
-                    rank_k_kernel<true><<<dim3(ntiles_lower(ng, rk::T), (h->n_omega + rk::Cfg<true>::NW - 1) / rk::Cfg<true>::NW, ksplit),
-                                          rk::Cfg<true>::THREADS, rk::Cfg<true>::SMEM_BYTES, st>>>(
-                        Nbuf, L.ldn, 0, Kpad, w, L.ldw, h->ptr<cd>(L.S), L.ldS, (int64_t)ng * L.ldS, ng, 0, h->n_omega, 0, ng);
-                }
-                CUDA_TRY(cudaGetLastError());
-            }
+        } else {
+            const int units = ntiles_lower(ng, rk::T) * ((h->n_omega + rk::Cfg<true>::NW - 1) / rk::Cfg<true>::NW);
+            const int ksplit = pick_ksplit(units, Kpad / rk::KC, h->n_sm);
+            rank_k_kernel<true><<<dim3(ntiles_lower(ng, rk::T), (h->n_omega + rk::Cfg<true>::NW - 1) / rk::Cfg<true>::NW, ksplit),
+                                  rk::Cfg<true>::THREADS, rk::Cfg<true>::SMEM_BYTES, st>>>(
+                Nbuf, L.ldn, 0, Kpad, w, L.ldw, h->ptr<cd>(L.S), L.ldS, (int64_t)ng * L.ldS, ng, 0, h->n_omega, 0, ng);
+        }
+        CUDA_TRY(cudaGetLastError());
+    }
+    return RPA_OK;
+}
+
+// rows K ... Kpad of the N buffer must be zero (they meet zero weights, but 0 * NaN is NaN)
+int add_zero_padding(rpa_chi0_t *h, int K) {
+    const Layout &L = h->L;
+    const int Kpad = (int)align_up((size_t)K, K_ALIGN);
+    if (Kpad > K) CUDA_TRY(cudaMemsetAsync(h->ptr<cd>(L.Nbuf) + (size_t)K * L.ldn, 0, (size_t)(Kpad - K) * L.ldn * sizeof(cd), h->stream));
+    return RPA_OK;
+}
+
+// batches of a call: either several whole occupied rows, or a slice of one row
+void add_batching(const rpa_chi0_t *h, int n_unocc, int *rows_per_batch, int *mchunk) {
+    const int Kmax = h->L.Kmax;
+    *rows_per_batch = 1;
+    *mchunk = n_unocc;
+    if (n_unocc >= Kmax) {
+        const int nch = (n_unocc + Kmax - 1) / Kmax;
+        *mchunk = std::min((int)align_up((size_t)(n_unocc + nch - 1) / nch, K_ALIGN), Kmax);
+    } else {
+        *rows_per_batch = std::max(1, std::min(MAX_SLOTS, Kmax / n_unocc));
+    }
+}
+
+// rpa_chi0_add_kpoint, and rpa_chi0_add_kpoint_optical when grad != NULL (q = 0 handle: G = 0 element replaced)
+int add_kpoint_impl(rpa_chi0_t *h, const AddArgs &A) {
+    if (h && h->pend_open) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_add_kpoint: a streamed k-point is open (rpa_chi0_add_kpoint_end)");
+    int ptot = 0;
+    {
+        const int rc = add_setup(h, A, &ptot);
+        if (rc != RPA_OK) return rc == 1 ? RPA_OK : rc;
+    }
+    int rows_per_batch, mchunk;
+    add_batching(h, A.n_unocc, &rows_per_batch, &mchunk);
+    for (int n0 = 0; n0 < A.n_occ; n0 += rows_per_batch) {
+        const int nslots = std::min(rows_per_batch, A.n_occ - n0);
+        for (int m0 = 0; m0 < A.n_unocc; m0 += mchunk) {
+            const int mlen = std::min(mchunk, A.n_unocc - m0);
+            const int K = nslots * mlen;
+            int rc = add_zero_padding(h, K);
+            for (int p0 = 0; p0 < K && rc == RPA_OK; p0 += h->L.sub_pairs)
+                rc = add_pair_densities(h, A, n0, mlen, m0, p0, std::min(h->L.sub_pairs, K - p0));
+            if (rc == RPA_OK) rc = add_finish_batch(h, A, ptot, n0, nslots, mlen, m0);
+            if (rc != RPA_OK) return rc;
         }
     }
     return RPA_OK;
@@ -976,8 +1044,9 @@ int rpa_chi0_add_kpoint(rpa_chi0_t *h, double kweight, int32_t n_occ, const void
                         const void *psi_unocc, const double *eps_occ, const double *eps_unocc, const double *f_occ,
                         const double *f_unocc, int32_t n_atoms, const int32_t *n_proj, const void *P_occ,
                         const void *P_unocc, const void *Q, const double *R_cart) {
-    return add_kpoint_impl(h, kweight, n_occ, psi_occ, n_unocc, psi_unocc, eps_occ, eps_unocc, f_occ, f_unocc, n_atoms, n_proj,
-                           P_occ, P_unocc, Q, R_cart, nullptr, nullptr);
+    const AddArgs A = {kweight, n_occ, psi_occ, n_unocc, psi_unocc, eps_occ, eps_unocc, f_occ, f_unocc, n_atoms, n_proj,
+                       P_occ, P_unocc, Q, R_cart, nullptr, nullptr};
+    return add_kpoint_impl(h, A);
 }
 
 int rpa_chi0_add_kpoint_optical(rpa_chi0_t *h, double kweight, int32_t n_occ, const void *psi_occ, int32_t n_unocc,
@@ -989,8 +1058,74 @@ int rpa_chi0_add_kpoint_optical(rpa_chi0_t *h, double kweight, int32_t n_occ, co
     const double nrm = sqrt(qdir_cart[0] * qdir_cart[0] + qdir_cart[1] * qdir_cart[1] + qdir_cart[2] * qdir_cart[2]);
     if (!(nrm > 0.0) || !std::isfinite(nrm)) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_add_kpoint_optical: zero direction");
     const double qd[3] = {qdir_cart[0] / nrm, qdir_cart[1] / nrm, qdir_cart[2] / nrm};
-    return add_kpoint_impl(h, kweight, n_occ, psi_occ, n_unocc, psi_unocc, eps_occ, eps_unocc, f_occ, f_unocc, n_atoms, n_proj,
-                           P_occ, P_unocc, Q, R_cart, qd, grad);
+    const AddArgs A = {kweight, n_occ, psi_occ, n_unocc, psi_unocc, eps_occ, eps_unocc, f_occ, f_unocc, n_atoms, n_proj,
+                       P_occ, P_unocc, Q, R_cart, qd, grad};
+    return add_kpoint_impl(h, A);
+}
+
+// rpa_chi0_add_kpoint in three steps, for unoccupied orbitals that are still being produced (include/rpa_chi0.h)
+int rpa_chi0_add_kpoint_begin(rpa_chi0_t *h, double kweight, int32_t n_occ, const void *psi_occ, int32_t n_unocc,
+                              const void *psi_unocc, const double *eps_occ, const double *eps_unocc, const double *f_occ,
+                              const double *f_unocc, int32_t n_atoms, const int32_t *n_proj, const void *P_occ,
+                              const void *P_unocc, const void *Q, const double *R_cart) {
+    if (!h) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_add_kpoint_begin: handle is NULL");
+    if (h->pend_open) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_add_kpoint_begin: the previous streamed k-point was not ended");
+    if (n_occ < 1 || n_unocc < 1) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_add_kpoint_begin: empty band set");
+    int rows_per_batch, mchunk;
+    add_batching(h, n_unocc, &rows_per_batch, &mchunk);
+    if (mchunk < n_unocc || n_occ > rows_per_batch)
+        return fail(RPA_ERR_UNSUPPORTED, "rpa_chi0_add_kpoint_begin: %d x %d transitions are more than one batch (%d, at most %d occupied bands): use rpa_chi0_add_kpoint",
+                    n_occ, n_unocc, h->L.Kmax, MAX_SLOTS);
+    const AddArgs A = {kweight, n_occ, psi_occ, n_unocc, psi_unocc, eps_occ, eps_unocc, f_occ, f_unocc, n_atoms, n_proj,
+                       P_occ, P_unocc, Q, R_cart, nullptr, nullptr};
+    int ptot = 0;
+    {
+        const int rc = add_setup(h, A, &ptot);
+        if (rc != RPA_OK) return rc;
+    }
+    {
+        const int rc = add_zero_padding(h, n_occ * n_unocc);
+        if (rc != RPA_OK) return rc;
+    }
+    h->pend = A;
+    h->pend.eps_occ = h->pend.eps_unocc = h->pend.f_occ = h->pend.f_unocc = h->pend.R_cart = nullptr;   // consumed
+    h->pend.n_proj = nullptr;
+    h->pend_ptot = ptot;
+    h->pend_m_next = 0;
+    h->pend_open = true;
+    return RPA_OK;
+}
+
+int rpa_chi0_add_kpoint_pairs(rpa_chi0_t *h, int32_t m_begin, int32_t m_end) {
+    if (!h) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_add_kpoint_pairs: handle is NULL");
+    if (!h->pend_open) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_add_kpoint_pairs: no streamed k-point is open");
+    const AddArgs &A = h->pend;
+    if (m_begin != h->pend_m_next || m_end < m_begin || m_end > A.n_unocc)
+        return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_add_kpoint_pairs: bands [%d, %d): slices must follow one another from %d up to %d",
+                    m_begin, m_end, h->pend_m_next, A.n_unocc);
+    // the window as a batch of its own -- pair p' = n wl + j is (occupied band n, unoccupied band m_begin + j) -- whose pair
+    // densities go to the rows n n_unocc + m_begin + j of the k-point's batch: one launch for all occupied bands
+    const int wl = m_end - m_begin;
+    if (wl > 0) {
+        const PdRowWindow win = {wl, A.n_unocc, m_begin};
+        const int K = A.n_occ * wl;
+        for (int p0 = 0; p0 < K; p0 += h->L.sub_pairs) {
+            const int rc = add_pair_densities(h, A, 0, wl, m_begin, p0, std::min(h->L.sub_pairs, K - p0), win);
+            if (rc != RPA_OK) return rc;
+        }
+    }
+    h->pend_m_next = m_end;
+    return RPA_OK;
+}
+
+int rpa_chi0_add_kpoint_end(rpa_chi0_t *h) {
+    if (!h) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_add_kpoint_end: handle is NULL");
+    if (!h->pend_open) return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_add_kpoint_end: no streamed k-point is open");
+    h->pend_open = false;   // whatever happens below, the call is over
+    if (h->pend_m_next != h->pend.n_unocc)
+        return fail(RPA_ERR_INVALID_ARG, "rpa_chi0_add_kpoint_end: only %d of %d unoccupied bands were given to rpa_chi0_add_kpoint_pairs; nothing added",
+                    h->pend_m_next, h->pend.n_unocc);
+    return add_finish_batch(h, h->pend, h->pend_ptot, 0, h->pend.n_occ, h->pend.n_unocc, 0);
 }
 
 // Eq. 15 / Eq. 19: gradient matrix elements between occupied and unoccupied bands given on a common plane-wave set.

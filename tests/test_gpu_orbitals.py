@@ -182,6 +182,68 @@ def test_pw_to_grid_index_table_is_kept_and_invalidated():
         h.close()
 
 
+def test_streamed_add_kpoint_is_bitwise_the_single_call():
+    """rpa_chi0_add_kpoint_begin / _pairs / _end with ragged slices against ONE rpa_chi0_add_kpoint call on the same device
+    orbitals: the same pair densities meet in the same rank-K update, so chi0 agrees bit for bit (PAW on).  Then the
+    protocol errors: slices out of order, end before the last band, a second begin, add_kpoint while open, and a band
+    set that is more than one batch."""
+    import torch
+    from paper_1307_8052_b200 import binding as B
+    cfg = W.CONFIGS[0]
+    kd = W.kpoint(cfg, 0)
+    h = _handle(cfg)
+    try:
+        _, K2 = B.rpa_chi0_gvectors(h)
+        Qd = torch.from_numpy(W.paw_Q(cfg, K2)).cuda()
+        R = W.atom_positions(cfg)
+        po, pu = torch.from_numpy(kd.psi_occ).cuda(), torch.from_numpy(kd.psi_unocc).cuda()
+        Po, Pu = torch.from_numpy(kd.P_occ).cuda(), torch.from_numpy(kd.P_unocc).cuda()
+        args = (kd.kweight, po, pu, kd.eps_occ, kd.eps_unocc, kd.f_occ, kd.f_unocc, cfg.n_proj, Po, Pu, Qd, R)
+        B.rpa_chi0_add_kpoint(h, *args)
+        ref = [B.rpa_chi0_get(h, i).clone() for i in range(cfg.n_omega)]
+        n_u = pu.shape[0]
+        for cuts in ([0, n_u], [0, 1, 2, 9, n_u], [0, 5, 5, 20, n_u]):
+            B.rpa_chi0_reset(h)
+            B.rpa_chi0_add_kpoint_begin(h, *args)
+            for a, b in zip(cuts[:-1], cuts[1:]):
+                B.rpa_chi0_add_kpoint_pairs(h, a, b)
+                B.rpa_chi0_get(h, 0)   # other calls are allowed while the k-point is open
+            B.rpa_chi0_add_kpoint_end(h)
+            for i in range(cfg.n_omega):
+                assert torch.equal(B.rpa_chi0_get(h, i), ref[i]), (cuts, i)
+        # protocol errors
+        for call in (lambda: B.rpa_chi0_add_kpoint_pairs(h, 0, 1), lambda: B.rpa_chi0_add_kpoint_end(h)):
+            with pytest.raises(B.RpaError) as ei:   # nothing open
+                call()
+            assert ei.value.code == B.RPA_ERR_INVALID_ARG
+        B.rpa_chi0_reset(h)
+        B.rpa_chi0_add_kpoint_begin(h, *args)
+        for call in (lambda: B.rpa_chi0_add_kpoint_begin(h, *args), lambda: B.rpa_chi0_add_kpoint(h, *args),
+                     lambda: B.rpa_chi0_add_kpoint_pairs(h, 1, 2), lambda: B.rpa_chi0_add_kpoint_pairs(h, 0, n_u + 1)):
+            with pytest.raises(B.RpaError) as ei:
+                call()
+            assert ei.value.code == B.RPA_ERR_INVALID_ARG
+        B.rpa_chi0_add_kpoint_pairs(h, 0, 3)
+        with pytest.raises(B.RpaError) as ei:       # ended early: nothing is added, the k-point is closed
+            B.rpa_chi0_add_kpoint_end(h)
+        assert ei.value.code == B.RPA_ERR_INVALID_ARG
+        assert float(B.rpa_chi0_get(h, 0).abs().max()) == 0.0
+        B.rpa_chi0_add_kpoint(h, *args)
+        assert torch.equal(B.rpa_chi0_get(h, 1), ref[1])
+    finally:
+        h.close()
+    # more than one batch: 4 x 28 transitions on a handle created for 64 per batch
+    om, wt = W.omega_grid(cfg.n_omega)
+    h = B.rpa_chi0_create(cfg.grid, cfg.cell, cfg.q_red, W.tuned_ecut(cfg), om, wt, 64, int(cfg.n_proj.sum()), "cuda:0")
+    try:
+        with pytest.raises(B.RpaError) as ei:
+            B.rpa_chi0_add_kpoint_begin(h, *args)
+        assert ei.value.code == B.RPA_ERR_UNSUPPORTED
+        B.rpa_chi0_add_kpoint(h, *args)             # nothing was left open
+    finally:
+        h.close()
+
+
 def test_add_kpoint_host_pw_in_two_calls_agrees_with_one():
     import torch
     from paper_1307_8052_b200 import binding as B
