@@ -123,7 +123,8 @@ __global__ void __launch_bounds__(128, 3) pw_zy_kernel(const cd *__restrict__ T1
 // TWz[qi3][j < N3/NA3] once; the box is embedded in zero-padded arrays aligned to the radix (position = q - q0,
 // q0 = qmin - (qmin mod NA)), so the inner loops have no bounds tests, no index updates and no conjugations: per term
 // two LDS.128 with immediate offsets and one complex FMA.  The inverse butterfly is the forward one read at -s.
-// Shared memory (cd): TWy[nq2p][NB2] | TWz[nq3p][NB3] | Pp[nq2p][nq3p] | Y[N2][nq3p].
+// Shared memory (cd): TWy[nq2p][NB2] | TWz[nq3p][NB3] | Pp[nq2p][nq3p] | Y[N2][nq3p + 1] (odd pitch in units of 16 bytes: the
+// threads of a warp read the same element of four different rows in the z stage).
 struct PwTabDims {
     int r2, nq2p, r3, nq3p;
     size_t smem;
@@ -134,11 +135,11 @@ static inline PwTabDims pw_tab_dims(int N2, int N3, int na2, int na3, int q2min,
     d.r3 = ((q3min % na3) + na3) % na3;
     d.nq2p = (nq2 + d.r2 + na2 - 1) / na2 * na2;
     d.nq3p = (nq3 + d.r3 + na3 - 1) / na3 * na3;
-    d.smem = ((size_t)d.nq2p * (N2 / na2) + (size_t)d.nq3p * (N3 / na3) + (size_t)d.nq2p * d.nq3p + (size_t)N2 * d.nq3p) * sizeof(cd);
+    d.smem = ((size_t)d.nq2p * (N2 / na2) + (size_t)d.nq3p * (N3 / na3) + (size_t)d.nq2p * d.nq3p + (size_t)N2 * (d.nq3p + 1)) * sizeof(cd);
     return d;
 }
 
-template <int NA2, int NA3>
+template <int NA2, int NA3, int RY, int RZ>
 __global__ void __launch_bounds__(128) pw_zy_tab_kernel(const cd *__restrict__ T1, const cd *__restrict__ tw2,
                                                        const cd *__restrict__ tw3, int N1, int N2, int N3, int q2min, int nq2,
                                                        int q3min, int nq3, int n_items, cd *__restrict__ out) {
@@ -165,7 +166,8 @@ __global__ void __launch_bounds__(128) pw_zy_tab_kernel(const cd *__restrict__ T
         const cd w = tw3[t];
         TWz[i] = cmake(w.x, -w.y);
     }
-    for (int i = tid; i < nq2p * nq3p + N2 * nq3p; i += nth) Pp[i] = cmake(0.0, 0.0);   // Pp and Y: the padding stays zero
+    const int yp = nq3p + 1;
+    for (int i = tid; i < nq2p * nq3p + N2 * yp; i += nth) Pp[i] = cmake(0.0, 0.0);   // Pp and Y: the padding stays zero
     __syncthreads();
     const int ncol = nq2 * nq3;
     for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
@@ -175,36 +177,71 @@ __global__ void __launch_bounds__(128) pw_zy_tab_kernel(const cd *__restrict__ T
             Pp[(r2 + a) * nq3p + r3 + c] = Tp[i];
         }
         __syncthreads();   // Pp complete; every thread has left the z stage of the previous item
-        for (int i = tid; i < NB2 * nq3; i += nth) {
-            const int j = i / nq3, col = r3 + (i - j * nq3);
-            cd z[NA2];
+        // y stage: RY values of j per thread (j, j + ceil(NB2 / RY), ...) share the loads of the box column; the z stage:
+        // RZ rows j2 per thread share the twiddles.  One LDS.128 per operand and term was what bound the kernel (LSU pipe
+        // 85 % busy, profiles/r2a): (1 + R) / R loads per complex multiply-add instead of 2.
+        const int HB2 = (NB2 + RY - 1) / RY;
+        for (int i = tid; i < HB2 * nq3; i += nth) {
+            const int j0 = i / nq3, col = r3 + (i - j0 * nq3);
+            cd z[RY][NA2];
+            const cd *twp[RY];
 #pragma unroll
-            for (int k1 = 0; k1 < NA2; k1++) z[k1] = cmake(0.0, 0.0);
-            const cd *twp = TWy + j, *pp = Pp + col;
+            for (int r = 0; r < RY; r++) {
+                twp[r] = TWy + min(j0 + r * HB2, NB2 - 1);   // a j beyond the axis repeats the last one and is not stored
+#pragma unroll
+                for (int k1 = 0; k1 < NA2; k1++) z[r][k1] = cmake(0.0, 0.0);
+            }
+            const cd *pp = Pp + col;
             for (int base = 0; base < nq2p; base += NA2) {
 #pragma unroll
-                for (int k1 = 0; k1 < NA2; k1++) z[k1] = cfma(twp[(base + k1) * NB2], pp[(base + k1) * nq3p], z[k1]);
-            }
-            Bfly<NA2>::run(z);
+                for (int k1 = 0; k1 < NA2; k1++) {
+                    const cd v = pp[(base + k1) * nq3p];
 #pragma unroll
-            for (int s = 0; s < NA2; s++) Y[(j + NB2 * ((NA2 - s) % NA2)) * nq3p + col] = z[s];
+                    for (int r = 0; r < RY; r++) z[r][k1] = cfma(twp[r][(base + k1) * NB2], v, z[r][k1]);
+                }
+            }
+#pragma unroll
+            for (int r = 0; r < RY; r++) {
+                const int j = j0 + r * HB2;
+                if (j < NB2) {
+                    Bfly<NA2>::run(z[r]);
+#pragma unroll
+                    for (int s = 0; s < NA2; s++) Y[(j + NB2 * ((NA2 - s) % NA2)) * yp + col] = z[r][s];
+                }
+            }
         }
         __syncthreads();
         cd *op = out + (size_t)item * N2 * N3;
-        for (int i = tid; i < N2 * NB3; i += nth) {
+        const int H2 = (N2 + RZ - 1) / RZ;
+        for (int i = tid; i < H2 * NB3; i += nth) {
             const int j2 = i / NB3, j = i - j2 * NB3;
-            cd z[NA3];
+            cd z[RZ][NA3];
+            const cd *yr[RZ];
 #pragma unroll
-            for (int k1 = 0; k1 < NA3; k1++) z[k1] = cmake(0.0, 0.0);
-            const cd *twp = TWz + j, *yr = Y + (size_t)j2 * nq3p;
+            for (int r = 0; r < RZ; r++) {
+                yr[r] = Y + (size_t)min(j2 + r * H2, N2 - 1) * yp;
+#pragma unroll
+                for (int k1 = 0; k1 < NA3; k1++) z[r][k1] = cmake(0.0, 0.0);
+            }
+            const cd *twp = TWz + j;
             for (int base = 0; base < nq3p; base += NA3) {
 #pragma unroll
-                for (int k1 = 0; k1 < NA3; k1++) z[k1] = cfma(twp[(base + k1) * NB3], yr[base + k1], z[k1]);
-            }
-            Bfly<NA3>::run(z);
-            cd *orow = op + (size_t)j2 * N3 + j;
+                for (int k1 = 0; k1 < NA3; k1++) {
+                    const cd w = twp[(base + k1) * NB3];
 #pragma unroll
-            for (int s = 0; s < NA3; s++) orow[NB3 * ((NA3 - s) % NA3)] = z[s];
+                    for (int r = 0; r < RZ; r++) z[r][k1] = cfma(w, yr[r][base + k1], z[r][k1]);
+                }
+            }
+#pragma unroll
+            for (int r = 0; r < RZ; r++) {
+                const int row = j2 + r * H2;
+                if (row < N2) {
+                    Bfly<NA3>::run(z[r]);
+                    cd *orow = op + (size_t)row * N3 + j;
+#pragma unroll
+                    for (int s = 0; s < NA3; s++) orow[NB3 * ((NA3 - s) % NA3)] = z[r][s];
+                }
+            }
         }
     }
 }
@@ -212,10 +249,16 @@ __global__ void __launch_bounds__(128) pw_zy_tab_kernel(const cd *__restrict__ T
 typedef void (*PwZyTabKernel)(const cd *, const cd *, const cd *, int, int, int, int, int, int, int, int, cd *);
 static inline PwZyTabKernel pw_zy_tab_pick(int N2, int N3) {
     const int a2 = pw_pick_na(N2), a3 = pw_pick_na(N3);
-    if (a2 == 12 && a3 == 12) return pw_zy_tab_kernel<12, 12>;
-    if (a2 == 12 && a3 == 8) return pw_zy_tab_kernel<12, 8>;
-    if (a2 == 8 && a3 == 12) return pw_zy_tab_kernel<8, 12>;
-    if (a2 == 8 && a3 == 8) return pw_zy_tab_kernel<8, 8>;
+    // register blocking (2 values of j in the y stage, 4 rows in the z stage) only where a plane still has tasks for
+    // every thread afterwards: on the 24 x 24 planes of configs[2] (72 z tasks) it halves the speed, on 60 x 64 and
+    // 40 x 168 it gains 8 - 15 %
+    const bool blocked = a3 > 0 && N2 * (N3 / a3) >= 256;
+#define PW_TAB_PICK(A2, A3) if (a2 == A2 && a3 == A3) return blocked ? pw_zy_tab_kernel<A2, A3, 2, 4> : pw_zy_tab_kernel<A2, A3, 1, 1>
+    PW_TAB_PICK(12, 12);
+    PW_TAB_PICK(12, 8);
+    PW_TAB_PICK(8, 12);
+    PW_TAB_PICK(8, 8);
+#undef PW_TAB_PICK
     return nullptr;   // an axis without radix 8 or 12: pw_zy_kernel
 }
 
