@@ -31,6 +31,7 @@ constexpr int TILE_BYTES = KC * PITCH;           // 17408
 //                   that frequency's matrix) and K is one panel (32 pairs), so a CTA is mostly prologue (TMA round
 //                   trip) and epilogue (read-modify-write of its tile): 1 frequency per CTA, 4 consumer warps,
 //                   2 stages (= the whole panel), two CTAs per SM so that one computes while the other loads / stores.
+//                   The weights are NOT applied: this instance computes S -= N N^H (w = -1 for every pair).
 template <bool SHARED_N>
 struct Cfg {
     static constexpr int NW = SHARED_N ? 2 : 1;               // frequencies per CTA
@@ -204,7 +205,12 @@ rank_k_kernel(const cd *__restrict__ Nb, int64_t ldn, int64_t strideN, int Kpad,
                     a2[mi] = __hiloint2double(__double2hiint(o) ^ (int)sign_hi, __double2loint(o));
                 }
 #pragma unroll
-                for (int ni = 0; ni < 4; ni++) b[ni] = wv * *reinterpret_cast<const double *>(st + b_off + ko + ni * 128);
+                for (int ni = 0; ni < 4; ni++) {
+                    const double bv = *reinterpret_cast<const double *>(st + b_off + ko + ni * 128);
+                    // the Cholesky update's weight is -1 for every pair: taken as the subtraction in the epilogue, which saves
+                    // the four FP64 multiplications per k-step on the datapath the DMMAs share (same bits: the sums are negated)
+                    b[ni] = SHARED_N ? wv * bv : bv;
+                }
 #pragma unroll
                 for (int mi = 0; mi < 4; mi++)
 #pragma unroll
@@ -269,8 +275,8 @@ rank_k_kernel(const cd *__restrict__ Nb, int64_t ldn, int64_t strideN, int Kpad,
 #pragma unroll
                 for (int e = 0; e < 2; e++)
                     if (cc + e < col_limit && cc + e <= r) {
-                        v[ni][e].x += re[mi][ni][e];
-                        v[ni][e].y += im[mi][ni][e];
+                        v[ni][e].x -= re[mi][ni][e];
+                        v[ni][e].y -= im[mi][ni][e];
                         rowp[cc + e] = v[ni][e];
                     }
             }
