@@ -34,6 +34,8 @@
 // Chunks of 16 pairs in a ring of 5 (213 KB) instead of 32 in a ring of 3: the third plane would not fit otherwise.
 #pragma once
 #include <cuda.h>
+#include <algorithm>
+#include <vector>
 #include "rank_k.cuh"
 
 namespace rk3 {
@@ -66,6 +68,34 @@ struct Operands {
 };
 }  // namespace rk3
 
+// Work of tile t = ti (ti + 1) / 2 + tj in 8-row x 16-column warp blocks, by the rules of rank_k3m_kernel (warps above the
+// diagonal or beyond the matrix idle, diagonal tiles skip their blocks above the diagonal, ragged last rows), and the
+// tiles in order of decreasing work (ties: ascending index, so that neighbours in the triangle stay neighbours).
+static inline int rk3_tile_units(int ti, int tj, int ng) {
+    using namespace rk3;
+    const int row0 = ti * T, col0 = tj * T;
+    int units = 0;
+    for (int w = 0; w < WARPS; w++) {
+        const int rowoff = (w >> 2) * (8 * MI), coloff = (w & 3) * 16;
+        if ((ti == tj && coloff > rowoff + 8 * MI - 1) || row0 + rowoff >= ng || col0 + coloff >= ng) continue;
+        const int mi_valid = std::min(MI, (ng - (row0 + rowoff) + 7) / 8);
+        const int mi_lo = ti == tj ? std::max(0, (coloff - rowoff) / 8) : 0;
+        units += std::max(0, mi_valid - mi_lo);
+    }
+    return units;
+}
+static inline std::vector<int32_t> rk3_tile_order(int ng) {
+    const int nt = (ng + rk3::T - 1) / rk3::T;
+    std::vector<int32_t> order, work;
+    for (int ti = 0; ti < nt; ti++)
+        for (int tj = 0; tj <= ti; tj++) {
+            order.push_back(ti * (ti + 1) / 2 + tj);
+            work.push_back(rk3_tile_units(ti, tj, ng));
+        }
+    std::stable_sort(order.begin(), order.end(), [&](int32_t a, int32_t b) { return work[a] > work[b]; });
+    return order;
+}
+
 // 2-D tiled bulk tensor copy global -> shared (TMA, UTMALDG in SASS): box of the tensor map at element coordinates (x, y)
 __device__ __forceinline__ void tma_load_2d(void *dst_smem, const CUtensorMap *map, int x, int y, uint64_t *bar) {
     asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
@@ -84,20 +114,25 @@ __global__ void __launch_bounds__(256) rk3_rowsum_kernel(const cd *__restrict__ 
 // Nb[Kpad][ldn] (rows >= K zero) through nmap: a 2-D FP64 tensor map over it, dims (2 ldn, Kmax), box (132, 16); its row
 // sums NS[Kpad][ldn] through smap: dims (ldn, Kmax), box (68, 16);
 // w[n_omega][ldw], S[n_omega][ng][ldS] (lower triangle accumulated), Kpad % 16 == 0.
-// Work items (tile, frequency) are numbered item = iw * ntiles + tile; grid = (n_items_of_this_launch, 1, ksplit), the
+// Work items (tile, frequency) are numbered item = slot * n_omega + iw, tile = order[slot]; grid = (n_items_of_this_launch, 1, ksplit), the
 // launch covers items item_off .. item_off + gridDim.x - 1; ksplit as in rank_k_kernel (atomic tile adds when > 1).
 // The host issues the whole waves with ksplit = 1 and the last partial wave K-sliced so that it also fills the GPU.
 __global__ void __launch_bounds__(rk3::THREADS, 1)
 rank_k3m_kernel(const __grid_constant__ CUtensorMap nmap, const __grid_constant__ CUtensorMap smap, int Kpad,
                 const double *__restrict__ w, int64_t ldw,
-                cd *__restrict__ S, int64_t ldS, int64_t strideS, int ng, int ntiles, int item_off) {
+                cd *__restrict__ S, int64_t ldS, int64_t strideS, int ng, int n_omega, int item_off,
+                const int32_t *__restrict__ order) {
     using namespace rk3;
     extern __shared__ __align__(128) unsigned char rk_smem[];
     uint64_t *full = reinterpret_cast<uint64_t *>(rk_smem + STAGES * STAGE_BYTES);
     uint64_t *empty = full + STAGES;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int item = item_off + (int)blockIdx.x;
-    const int iw = item / ntiles, t = item - iw * ntiles;
+    // tile-major, heaviest tiles first (order[] from rk3_tile_order): the grid's CTAs start in item order, so the light
+    // tiles of the diagonal and of the ragged last row fill the end of the launch instead of leaving SMs idle behind full
+    // tiles, and the n_omega CTAs of a tile run together and share its operand tiles in L2
+    const int slot = item / n_omega, iw = item - slot * n_omega;
+    const int t = order[slot];
     int ti = (int)((sqrt(8.0 * (double)t + 1.0) - 1.0) * 0.5);
     while ((ti + 1) * (ti + 2) / 2 <= t) ti++;
     while (ti * (ti + 1) / 2 > t) ti--;

@@ -142,7 +142,7 @@ void build_sphere(const int32_t grid[3], const double B[9], const double q[3], d
 
 struct Layout {
     size_t S, Nbuf, NS, w, I, T, M, Lt, wneg, tw1, tw2, tw3, box2s, coltab, rowtab, Kc, omega, wt, band, R, aj_atom, aj_j, atom_poff, atom_ni,
-        atom_qoff, v, e, tr, logdet, flag, ec, pwtab, total;
+        atom_qoff, v, e, tr, logdet, flag, ec, pwtab, rkorder, total;
     int64_t ldS, ldn, ldw;
     int Kmax, sub_pairs, ec_group;
     size_t I_pair_bytes;
@@ -207,6 +207,7 @@ void make_layout(const int32_t grid[3], const Sphere &sp, int n_omega, int max_b
     L->flag = take((size_t)EC_GROUP * sizeof(int));
     L->ec = take(sizeof(double));
     L->pwtab = take((size_t)grid[0] * grid[1] * grid[2] * sizeof(int32_t));   // plane-wave box -> coefficient index (rpa_pw_to_grid), kept between calls
+    L->rkorder = take((size_t)((ng + rk3::T - 1) / rk3::T) * ((ng + rk3::T - 1) / rk3::T + 1) / 2 * sizeof(int32_t));   // rank_k3m_kernel: tiles, heaviest first
     L->total = off;
 }
 
@@ -648,6 +649,8 @@ int create_impl(rpa_chi0_t **out, const int32_t grid[3], const double cell[9], c
     CREATE_TRY(cudaMemcpyAsync(h->ws + L.Kc, sp.Kc.data(), sp.Kc.size() * sizeof(double), cudaMemcpyHostToDevice, h->stream));
     CREATE_TRY(cudaMemcpyAsync(h->ws + L.omega, h->omega.data(), n_omega * sizeof(double), cudaMemcpyHostToDevice, h->stream));
     CREATE_TRY(cudaMemcpyAsync(h->ws + L.wt, h->wt.data(), n_omega * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+    const std::vector<int32_t> rkorder = rk3_tile_order(sp.ng);
+    CREATE_TRY(cudaMemcpyAsync(h->ws + L.rkorder, rkorder.data(), rkorder.size() * sizeof(int32_t), cudaMemcpyHostToDevice, h->stream));
     {
         std::vector<double> wneg((size_t)L.ec_group * CH_P * CH_NB, -1.0);   // weight of the Cholesky trailing update
         CREATE_TRY(cudaMemcpyAsync(h->ws + L.wneg, wneg.data(), wneg.size() * sizeof(double), cudaMemcpyHostToDevice, h->stream));
@@ -963,7 +966,7 @@ int add_finish_batch(rpa_chi0_t *h, const AddArgs &A, int ptot, int n0, int nslo
             const int tail = units - whole;
             auto launch = [&](int off, int count, int ksplit) {
                 rank_k3m_kernel<<<dim3(count, 1, ksplit), rk3::THREADS, rk3::SMEM_BYTES, st>>>(
-                    h->nmap, h->smap, Kpad, w, L.ldw, h->ptr<cd>(L.S), L.ldS, (int64_t)ng * L.ldS, ng, ntiles, off);
+                    h->nmap, h->smap, Kpad, w, L.ldw, h->ptr<cd>(L.S), L.ldS, (int64_t)ng * L.ldS, ng, h->n_omega, off, h->ptr<int32_t>(L.rkorder));
             };
             // third operand plane of the 3M product: NS = Re N + Im N, one pass over the batch's N
             rk3_rowsum_kernel<<<dim3(Kpad, (unsigned)((L.ldn + 255) / 256)), 256, 0, st>>>(Nbuf, L.ldn, h->ptr<double>(L.NS));
