@@ -40,7 +40,7 @@ MIN_WARMUP = 3   # timing rule of the bench contract: at least 3 untimed steps
 # dram__bytes_read.sum + dram__bytes_write.sum of rank_k3m_kernel from the ncu --set full capture named beside it: one
 # batch of configs[1] (7200 transitions x 16 omega) = its whole-wave launch + its K-sliced tail launch.  A constant
 # copied from that profile, NOT measured in the run that prints it: `traffic_from` says so in the JSON.
-RANK_K_DRAM_TRAFFIC = {1: (4436.7e6, "profiles/r2c_rank_k3m.md")}
+RANK_K_DRAM_TRAFFIC = {1: (2188.7e6, "profiles/r2h_rank_k3m.md")}
 RANK_K_I8_DRAM_TRAFFIC = {1: (4455.9e6, "profiles/r1i_bench_cfg1.md")}
 
 
