@@ -351,13 +351,14 @@ int ntiles_lower(int n, int t) {
 
 // K slices of the rank-K launch: one CTA per SM, `units` equal work items (tile x frequency pair).  With s slices
 // the grid needs ceil(units s / n_sm) rounds of 1/s of an item each; take the s that minimises that time, charging
-// 1 % per extra slice for its prologue / atomic epilogue, and keep at least min_chunks chunks (512 pairs) per slice.
+// 3 % per extra slice for its prologue / atomic epilogue (measured on the 448 items of configs[2], K = 2400: 2 / 3 / 4
+// slices 0.787 / 0.781 / 0.807 ms, one 0.869), and keep at least min_chunks chunks (512 pairs) per slice.
 int pick_ksplit(int units, int nchunks, int n_sm, double *cost_out = nullptr, int min_chunks = 16) {
     int best = 1;
     double best_cost = 1e300;
     for (int s = 1; s <= 8 && nchunks / s >= min_chunks; s++) {
         const double rounds = (double)(((int64_t)units * s + n_sm - 1) / n_sm) / s;
-        const double cost = rounds * (1.0 + 0.01 * (s - 1));
+        const double cost = rounds * (1.0 + 0.03 * (s - 1));
         if (cost < best_cost * (1.0 - 1e-9)) { best_cost = cost; best = s; }
     }
     if (cost_out) *cost_out = best_cost;   // in units of one full-K item
@@ -974,8 +975,10 @@ int add_finish_batch(rpa_chi0_t *h, const AddArgs &A, int ptot, int n0, int nslo
             double c_single = 0.0, c_tail = 0.0;
             const int s_single = pick_ksplit(units, nchunks, h->n_sm, &c_single, 512 / rk3::KC);
             const int s_tail = tail > 0 ? pick_ksplit(tail, nchunks, h->n_sm, &c_tail, 512 / rk3::KC) : 1;
-            // two launches only if the model says they save at least a tenth of an item
-            if (whole > 0 && tail > 0 && whole / h->n_sm + c_tail + 0.1 < c_single) {
+            // two launches only if the model says they save at least a tenth of an item, and only behind at least eight waves:
+            // the first launch ends ragged (tiles differ in work) and the second waits for its last CTA, which on the three
+            // waves of configs[2] costs more than the sliced remainder saves (0.871 against 0.781 ms per k-point)
+            if (whole >= 8 * h->n_sm && tail > 0 && whole / h->n_sm + c_tail + 0.1 < c_single) {
                 launch(0, whole, 1);
                 launch(whole, tail, s_tail);
                 h->launches += 1;
