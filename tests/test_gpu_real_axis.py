@@ -123,3 +123,29 @@ def test_config1_real_axis_full_size_sampled():
     for j, i in enumerate((1, 3, 7)):
         assert rel_fro(chi_sel[i], chi_o[j]) <= CHI_TOL, (i, rel_fro(chi_sel[i], chi_o[j]))
     assert rel_fro(chi_sel[7], chi_sel[3].conj().T) <= 1e-12
+
+
+def test_real_axis_streamed_kpoint_is_bitwise_the_single_call():
+    """rpa_chi0_add_kpoint_begin / _pairs / _end on a real-axis handle (two accumulator slots per frequency): the same
+    kernels in the same order as one rpa_chi0_add_kpoint call, so every slot agrees bit for bit."""
+    import torch
+    from paper_1307_8052_b200 import binding as B
+    cfg = W.CONFIGS[0]
+    kd = W.kpoint(cfg, 0)
+    om = np.array([0.0, 0.4, -1.3])
+    for h, g, K2 in _gpu_real_axis(cfg, [], om, ETA):
+        Qd = torch.from_numpy(W.paw_Q(cfg, K2)).to("cuda:0")
+        dv = {k: torch.from_numpy(getattr(kd, k)).to("cuda:0") for k in ("psi_occ", "psi_unocc", "P_occ", "P_unocc")}
+        args = (kd.kweight, dv["psi_occ"], dv["psi_unocc"], kd.eps_occ, kd.eps_unocc, kd.f_occ, kd.f_unocc, cfg.n_proj,
+                dv["P_occ"], dv["P_unocc"], Qd, W.atom_positions(cfg))
+        B.rpa_chi0_add_kpoint(h, *args)
+        ref = [B.rpa_chi0_get(h, i).clone() for i in range(len(om))]
+        B.rpa_chi0_reset(h)
+        B.rpa_chi0_add_kpoint_begin(h, *args)
+        n_u = dv["psi_unocc"].shape[0]
+        for a, b in ((0, 7), (7, 8), (8, n_u)):
+            B.rpa_chi0_add_kpoint_pairs(h, a, b)
+        B.rpa_chi0_add_kpoint_end(h)
+        for i in range(len(om)):
+            assert torch.equal(B.rpa_chi0_get(h, i), ref[i]), i
+        assert float(ref[1].abs().max()) > 0.0
