@@ -40,3 +40,17 @@ def test_work_item_map_of_the_pair_density_kernel_matches_a_plain_walk(tmp_path)
     out = subprocess.run([exe], capture_output=True, text=True)
     cases, bad = (int(x) for x in out.stdout.split())
     assert out.returncode == 0 and bad == 0 and cases == 60000, out.stdout
+
+
+@pytest.mark.skipif(not (os.path.exists(NVCC) or shutil.which("nvcc")), reason="nvcc not available")
+def test_tile_order_of_the_rank_k_kernel_is_a_permutation_sorted_by_work(tmp_path):
+    """rk3_tile_order / rk3_tile_units (csrc/rank_k3m.cuh): every lower-triangle tile exactly once, work never increasing,
+    the block count of a tile never below a plain walk over its elements; matrix sizes 1 ... 700 and those of the configs."""
+    exe = str(tmp_path / "tile_order_check")
+    src = os.path.join(HERE, "host", "tile_order_check.cu")
+    r = subprocess.run([NVCC, "-O1", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-diag-suppress", "20208", "-o", exe, src],
+                       capture_output=True, text=True)
+    assert r.returncode == 0, r.stderr
+    out = subprocess.run([exe], capture_output=True, text=True)
+    sizes, bad = (int(x) for x in out.stdout.split())
+    assert out.returncode == 0 and bad == 0 and sizes == 705, out.stdout
