@@ -324,3 +324,48 @@ def test_nothing_is_written_outside_the_workspace_and_the_outputs():
             check(psi_buf, psi_off, cfg.n_occ * N * 16, "psi_out of rpa_symmetry_remap")
         finally:
             h.close()
+
+
+@pytest.mark.parametrize("ng_target", [20, 33, 64, 97, 129, 160, 257, 300, 385, 520, 777])
+def test_ec_q_on_synthetic_accumulators_of_many_sizes(ng_target):
+    """The factorisation of rpa_ec_q by itself -- ec_build / ec_trace / chol_panel / the strips and look-ahead columns in
+    32 x 32 tiles / the big updates in 64 x 64 tiles -- on spheres whose size sits on and around the panel (32), tile (64)
+    and block (128) edges: the accumulators are filled directly with a Hermitian negative semi-definite matrix per frequency
+    (skewed cell, no pair densities involved), chi0 is read back with rpa_chi0_get, and e(omega), E_c(q) must agree with the
+    oracle's unblocked Cholesky of the same chi0; the lane / tile-shape variants must agree with each other bit for bit."""
+    import oracle
+    import torch
+    from paper_1307_8052_b200 import binding as B
+    cell = np.array([[7.0, 0.3, 0.0], [0.2, 7.5, 0.1], [0.0, -0.4, 8.0]])
+    cfg = W.custom_config(200 + ng_target, cell, (20, 20, 20), (0.25, 0.1, 0.0), 1, 1, ng_target, 3, 1, 1)
+    h = _handle(cfg, ptot=0)
+    try:
+        ng = B.rpa_chi0_ng(h)
+        assert ng == ng_target
+        _, K2 = B.rpa_chi0_gvectors(h)
+        v = W.coulomb(K2)
+        S = B.rpa_chi0_accumulators(h).view(cfg.n_omega, ng, ng)
+        rng = np.random.default_rng([77, ng])
+        for i in range(cfg.n_omega):
+            r = max(1, ng // 3)
+            A = (rng.standard_normal((ng, r)) + 1j * rng.standard_normal((ng, r))) / np.sqrt(2.0 * r)
+            M = -(A * rng.uniform(0.01, 2.0, r)) @ A.conj().T / np.sqrt(np.outer(v, v))   # v^1/2 chi0 v^1/2 of order one
+            M = np.tril(M)                                                                # the library keeps one triangle
+            M[np.diag_indices(ng)] = M.diagonal().real
+            S[i].copy_(torch.from_numpy(M))
+        chi = np.stack([B.rpa_chi0_get(h, i).cpu().numpy() for i in range(cfg.n_omega)])
+        assert np.array_equal(chi, chi.conj().transpose(0, 2, 1))
+        om, wt = W.omega_grid(cfg.n_omega)
+        ec_o, e_o = oracle.ec_q(chi, v, wt)
+        ref = None
+        for lanes in (2, 1, 3, 2 | B.RPA_EC_FLAG_WIDE_TILES):
+            B.rpa_chi0_set_ec_lanes(h, lanes)
+            ec, e = B.rpa_ec_q(h, v)
+            if ref is None:
+                ref = (ec, e)
+                assert np.all(np.abs(e - e_o) <= 1e-10 * np.abs(e_o)), (e, e_o)
+                assert abs(ec - ec_o) <= 1e-10 * abs(ec_o)
+            else:
+                assert ec == ref[0] and np.array_equal(e, ref[1]), lanes
+    finally:
+        h.close()
