@@ -37,6 +37,18 @@ def test_tiny_skewed_cell_ragged(tiny_cfg):
     _compare(tiny_cfg, [W.kpoint(tiny_cfg, 0)])
 
 
+@pytest.mark.parametrize("ng_target", [63, 64, 65, 127, 129, 191, 193, 257])
+def test_sphere_sizes_around_the_tile_edges(ng_target):
+    """nG on and next to multiples of the rank-K tile (64) and of its 8-row warp blocks: one or two rows / columns in the
+    last tile, a full last tile, a diagonal tile that is the ragged one -- every element of chi0 and E_c(q) against the
+    oracle (skewed cell, 20^3 grid, 3 x 11 bands in batches of 32 so that several ragged batches add up, PAW on)."""
+    cell = np.array([[7.0, 0.3, 0.0], [0.2, 7.5, 0.1], [0.0, -0.4, 8.0]])
+    cfg = W.custom_config(300 + ng_target, cell, (20, 20, 20), (0.25, 0.1, 0.0), n_occ=3, n_unocc=11, ng_target=ng_target,
+                          n_omega=3, n_atoms=2, n_proj_per_atom=2, orb_ecut_ha=3.0)
+    chi = _compare(cfg, [W.kpoint(cfg, 0)], max_batch_pairs=32)
+    assert chi.shape[1] == ng_target
+
+
 def test_config0_toy_full():
     cfg = W.CONFIGS[0]
     chi = _compare(cfg, [W.kpoint(cfg, 0)])
